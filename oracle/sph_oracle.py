@@ -1,0 +1,210 @@
+"""ctypes front end of oracle/sph_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs
+import this module.  It holds no arithmetic of the method: it promotes the caller's FP32
+arrays to FP64 exactly, calls the C functions and hands back numpy arrays.  The equations
+and their PAPER.md citations are in sph_oracle.c.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from dataclasses import dataclass
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "sph_oracle.c")
+_LIB = os.path.join(_HERE, "liboracle.so")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile sph_oracle.c with gcc (OpenMP) into oracle/liboracle.so."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + f".{os.getpid()}.tmp"
+        subprocess.check_call(
+            ["gcc", "-O2", "-fopenmp", "-fPIC", "-shared", "-o", tmp, _SRC, "-lm"])
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+class _Box(C.Structure):
+    _fields_ = [("lo", C.c_double * 3), ("len", C.c_double * 3), ("periodic", C.c_int32 * 3)]
+
+
+class _Params(C.Structure):
+    _fields_ = [("kernel", C.c_int32), ("n_ngb", C.c_double), ("gamma", C.c_double),
+                ("av_alpha", C.c_double), ("av_beta", C.c_double), ("av_eps", C.c_double),
+                ("eta_cfl", C.c_double), ("eta_acc", C.c_double)]
+
+
+@dataclass
+class Params:
+    kernel: int = 1          # Wendland C2
+    n_ngb: float = 64.0
+    gamma: float = 5.0 / 3.0
+    av_alpha: float = 1.0
+    av_beta: float = 2.0
+    av_eps: float = 0.01
+    eta_cfl: float = 0.3
+    eta_acc: float = 0.2
+
+    def c(self) -> _Params:
+        return _Params(self.kernel, self.n_ngb, self.gamma, self.av_alpha, self.av_beta,
+                       self.av_eps, self.eta_cfl, self.eta_acc)
+
+
+@dataclass
+class Box:
+    lo: tuple = (0.0, 0.0, 0.0)
+    len: tuple = (1.0, 1.0, 1.0)
+    periodic: tuple = (1, 1, 1)
+
+    def c(self) -> _Box:
+        b = _Box()
+        for d in range(3):
+            # FP32 box values are promoted exactly, like every other input
+            b.lo[d] = float(np.float32(self.lo[d]))
+            b.len[d] = float(np.float32(self.len[d]))
+            b.periodic[d] = int(self.periodic[d])
+        return b
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        build()
+        _lib = C.CDLL(_LIB)
+        _lib.orc_w.restype = C.c_double
+        _lib.orc_w.argtypes = [C.c_int, C.c_double]
+        _lib.orc_dw.restype = C.c_double
+        _lib.orc_dw.argtypes = [C.c_int, C.c_double]
+        _lib.orc_dist2.restype = C.c_double
+    return _lib
+
+
+def num_threads() -> int:
+    return int(lib().orc_num_threads())
+
+
+def _d(a):
+    """Exact promotion to a contiguous FP64 array."""
+    return np.ascontiguousarray(np.asarray(a), dtype=np.float64)
+
+
+def _p(a, t=C.c_double):
+    return a.ctypes.data_as(C.POINTER(t)) if a is not None else None
+
+
+def _targets(n, targets):
+    if targets is None:
+        return n, None
+    t = np.ascontiguousarray(np.asarray(targets), dtype=np.int64)
+    return len(t), t
+
+
+def w(kernel: int, q: float) -> float:
+    return lib().orc_w(int(kernel), float(q))
+
+
+def dw(kernel: int, q: float) -> float:
+    return lib().orc_dw(int(kernel), float(q))
+
+
+def density(x, y, z, m, h_hint, box: Box, par: Params, targets=None, cells: bool = False,
+            cell_side: float | None = None):
+    """h (root of Eq. 6), rho (Eq. 5), Omega (Eq. 7), n_i.  Brute force unless cells=True."""
+    x, y, z, m, hh = map(_d, (x, y, z, m, h_hint))
+    n = len(x)
+    b, p = box.c(), par.c()
+    if cells:
+        assert targets is None
+        h = np.empty(n); rho = np.empty(n); om = np.empty(n); nn = np.empty(n, np.int32)
+        nfb = C.c_int64(0)
+        side = float(cell_side if cell_side is not None else 2.0 * 1.3 * hh.max())
+        rc = lib().orc_density_cells(C.c_int64(n), _p(x), _p(y), _p(z), _p(m), _p(hh), C.byref(b),
+                                     C.byref(p), C.c_double(side), _p(h), _p(rho), _p(om),
+                                     _p(nn, C.c_int32), C.byref(nfb))
+        if rc:
+            raise RuntimeError(f"orc_density_cells failed: {rc}")
+        return h, rho, om, nn
+    nt, t = _targets(n, targets)
+    h = np.empty(nt); rho = np.empty(nt); om = np.empty(nt); nn = np.empty(nt, np.int32)
+    rc = lib().orc_density_brute(C.c_int64(n), _p(x), _p(y), _p(z), _p(m), _p(hh), C.byref(b),
+                                 C.byref(p), C.c_int64(nt), _p(t, C.c_int64), _p(h), _p(rho),
+                                 _p(om), _p(nn, C.c_int32))
+    if rc:
+        raise RuntimeError(f"orc_density_brute failed: {rc}")
+    return h, rho, om, nn
+
+
+def density_at_h(x, y, z, m, h, box: Box, par: Params, targets=None):
+    """rho, Omega, n_i and the relative residual of Eq. (6) at a PRESCRIBED h (brute force)."""
+    x, y, z, m, h = map(_d, (x, y, z, m, h))
+    n = len(x)
+    b, p = box.c(), par.c()
+    nt, t = _targets(n, targets)
+    rho = np.empty(nt); om = np.empty(nt); nn = np.empty(nt, np.int32); res = np.empty(nt)
+    lib().orc_density_at_h_brute(C.c_int64(n), _p(x), _p(y), _p(z), _p(m), _p(h), C.byref(b),
+                                 C.byref(p), C.c_int64(nt), _p(t, C.c_int64), _p(rho), _p(om),
+                                 _p(nn, C.c_int32), _p(res))
+    return rho, om, nn, res
+
+
+def neighbors(x, y, z, h, box: Box, mode: int = 0, targets=None):
+    """CSR neighbour lists at a prescribed h. mode 0 gather (self incl.), 1 gather-or-scatter."""
+    x, y, z, h = map(_d, (x, y, z, h))
+    n = len(x)
+    b = box.c()
+    nt, t = _targets(n, targets)
+    off = np.zeros(nt + 1, np.int64)
+    args = [C.c_int64(n), _p(x), _p(y), _p(z), _p(h), C.byref(b), C.c_int(mode), C.c_int64(nt),
+            _p(t, C.c_int64), _p(off, C.c_int64)]
+    lib().orc_neighbors_brute(*args, None)
+    idx = np.empty(int(off[-1]), np.int64)
+    lib().orc_neighbors_brute(*args, _p(idx, C.c_int64))
+    return off, idx
+
+
+def forces(x, y, z, m, vx, vy, vz, u, rho, h, omega, box: Box, par: Params, targets=None,
+           cells: bool = False):
+    """a, du/dt, mu_min and the normalisers Sa, Su (Eqs. 13-18). Returns a dict."""
+    arrs = list(map(_d, (x, y, z, m, vx, vy, vz, u, rho, h, omega)))
+    n = len(arrs[0])
+    b, p = box.c(), par.c()
+    nt, t = (n, None) if cells else _targets(n, targets)
+    out = {k: np.empty(nt) for k in ("ax", "ay", "az", "dudt", "mu_min", "Sa", "Su")}
+    npairs = np.empty(nt, np.int32)
+    ptrs = [_p(a) for a in arrs]
+    outs = [_p(out[k]) for k in ("ax", "ay", "az", "dudt", "mu_min", "Sa", "Su")]
+    if cells:
+        assert targets is None
+        rc = lib().orc_forces_cells(C.c_int64(n), *ptrs, C.byref(b), C.byref(p),
+                                    C.c_double(2.0 * float(arrs[9].max())), *outs,
+                                    _p(npairs, C.c_int32))
+    else:
+        rc = lib().orc_forces_brute(C.c_int64(n), *ptrs, C.byref(b), C.byref(p), C.c_int64(nt),
+                                    _p(t, C.c_int64), *outs, _p(npairs, C.c_int32))
+    if rc:
+        raise RuntimeError(f"orc_forces failed: {rc}")
+    out["n_pairs"] = npairs
+    return out
+
+
+def eos(rho, u, gamma):
+    rho, u = _d(rho), _d(u)
+    P = np.empty_like(rho); c = np.empty_like(rho)
+    lib().orc_eos(C.c_int64(len(rho)), _p(rho), _p(u), C.c_double(gamma), _p(P), _p(c))
+    return P, c
+
+
+def timestep(h, c, ax, ay, az, mu_min, par: Params):
+    h, c, ax, ay, az, mu = map(_d, (h, c, ax, ay, az, mu_min))
+    p = par.c()
+    dti = np.empty_like(h)
+    dtm = C.c_double(0)
+    lib().orc_timestep(C.c_int64(len(h)), _p(h), _p(c), _p(ax), _p(ay), _p(az), _p(mu),
+                       C.byref(p), _p(dti), C.byref(dtm))
+    return dti, dtm.value
