@@ -1,0 +1,155 @@
+/*
+ * sph.h -- C-ABI of the B200-native SPH interaction sweep (arxiv/paper_2511_11425,
+ * "SPH in pkdgrav3 for Shock Physics Simulations. I. Hydrodynamics").
+ *
+ * The library computes, on ONE GPU (sm_100a), the data-parallel hot path of the paper's
+ * SPH method: neighbour search within the kernel support 2h (Section
+ * 2.3.2), the density / smoothing-length solve (Eqs. 5-7), the hydro
+ * force pass with Monaghan artificial viscosity and the ideal-gas EOS (PAPER.md:186-219,
+ * Eqs. 13-18) and the time-step criteria (Eq. 26).
+ *
+ * Conventions for every call
+ *   - All array pointers are DEVICE pointers to FP32 (or int32 / int64 where stated)
+ *     arrays of length n in the CALLER'S particle order, both for inputs and outputs.
+ *     The spatial sort is internal.  The caller owns every array it passes; the context
+ *     owns its sorted copies, cell table and scratch, all allocated in sph_create.
+ *   - Work is enqueued on the CUDA stream given to sph_create; calls do not synchronise
+ *     unless stated (sph_stats, sph_neighbors, sph_fp32_peak do).
+ *   - Return value: SPH_OK (0) or a negative error code.  No exceptions, no exit, no
+ *     printing.  sph_last_error gives a text for the last failure of a context.
+ *   - Call order: sph_build_cells -> sph_density_h -> sph_forces -> sph_timestep.
+ *     sph_forces / sph_neighbors may be fed rho, h, Omega from elsewhere as long as
+ *     sph_build_cells ran on the same positions (else SPH_ESTALE).
+ *   - Kernel: Wendland C2 with support radius 2h (readings R2, R3)
+ *       W(r,h) = h^-3 (21/(16 pi)) (1-q/2)^4 (1+2q),  q = r/h < 2.
+ */
+#ifndef SPH_B200_H
+#define SPH_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+    SPH_OK      = 0,
+    SPH_EINVAL  = -1, /* null pointer, n <= 0, n > n_max, bad parameter                  */
+    SPH_EBOX    = -2, /* a periodic side is shorter than 2 x the search diameter, so the  */
+                      /* minimum image is not unique; reported by sph_stats */
+    SPH_ENOMEM  = -3, /* device allocation failed                                         */
+    SPH_ECUDA   = -4, /* CUDA runtime error (text in sph_last_error)                      */
+    SPH_ESTALE  = -5, /* sph_build_cells has not run for this n                           */
+    SPH_ENOSPC  = -6  /* sph_neighbors: `capacity` too small; *needed holds the size      */
+};
+
+typedef struct {
+    float   lo[3];        /* lower corner                                                  */
+    float   len[3];       /* side lengths (> 0)                                            */
+    int32_t periodic[3];  /* 1: periodic in that dimension (minimum image)    */
+} sph_box;
+
+typedef struct {
+    int32_t kernel;       /* 1 = Wendland C2 (the only one built)            */
+    float   n_ngb;        /* kernel mass in units of m_i, Eq. (6) with R_kernel = 2h       */
+    float   gamma;        /* ideal gas P = (gamma-1) rho u                  */
+    float   av_alpha;     /* Eq. (15) alpha                                                */
+    float   av_beta;      /* Eq. (15) beta                                                 */
+    float   av_eps;       /* Eq. (16) epsilon (0.01, Monaghan 1992)                        */
+    float   eta_cfl;      /* Eq. (26) Courant parameter eta_C                              */
+    float   eta_acc;      /* eta_a = 0.2                                    */
+    float   h_tol;        /* Newton stop |dh|/h (<= 0: default 1e-6)                       */
+    int32_t h_max_iter;   /* Newton sweep cap per particle (<= 0: default 40)              */
+    float   search_slack; /* density search radius = 2 h_guess x this (<= 1: default 1.1);  */
+                          /* PAPER.md:152 "slightly larger kernel"; results do not depend   */
+                          /* on it                                                         */
+    float   cell_div_x;   /* cells per minimum search radius along x (<= 0: default 4)     */
+    float   cell_div_yz;  /* ... along y and z (<= 0: default 1.5)                         */
+} sph_params;
+
+/* 64-bit counters accumulated on the device since the last sph_stats_reset.             */
+typedef struct {
+    int64_t dens_tested;      /* candidate pairs distance-tested by sph_density_h          */
+    int64_t dens_listed;      /* pairs kept in the per-target lists (within the slack ball) */
+    int64_t dens_pairs;       /* sum_i n_i at the final h (self included)                  */
+    int64_t dens_sweeps;      /* Newton sweeps summed over particles                       */
+    int64_t dens_recollect;   /* targets whose search ball had to be rebuilt larger        */
+    int64_t dens_overflow;    /* targets that fell back to the streaming (list-free) path  */
+    int64_t dens_nonconv;     /* particles not converged within h_max_iter                 */
+    int64_t dens_recheck;     /* borderline pairs re-evaluated in FP64                     */
+    int64_t force_tested;     /* candidate pairs distance-tested by sph_forces             */
+    int64_t force_pairs;      /* pairs with 0 < r < 2 max(h_i,h_j) (FP32 test)             */
+    int64_t force_av_pairs;   /* of those, approaching pairs (v_ij . r_ij < 0)             */
+    int64_t n_cells;          /* cells in the index of the last sph_build_cells            */
+    int64_t grid_flags;       /* bit 0: SPH_EBOX condition met; bit 1: cell table clipped   */
+    int64_t reserved[3];
+} sph_stats_t;
+
+typedef struct sph_ctx sph_ctx;
+
+/* Create a context for up to n_max particles on the current CUDA device.
+ * cuda_stream: a cudaStream_t (NULL = legacy default stream).  Allocates all scratch.    */
+int  sph_create(sph_ctx** out, const sph_params* params, const sph_box* box, int64_t n_max,
+                void* cuda_stream);
+void sph_destroy(sph_ctx* ctx);
+
+/* Steps a1-a3: spatial index standing in for the tree of PAPER.md:66-68,
+ * 121-127.  Bins the n particles into a uniform grid whose cell sides derive from
+ * min(h) (device-side, no host round trip), counting-sorts them so that every x-row of
+ * cells is one contiguous particle range, and keeps the permutation.  h is the caller's
+ * current guess of the smoothing lengths (> 0); it only sizes the cells.                 */
+int  sph_build_cells(sph_ctx* ctx, int64_t n, const float* x, const float* y, const float* z,
+                     const float* h);
+
+/* Steps a4-a6: Eqs. (5)-(7).  For every particle finds h_i with
+ * (32 pi/3) sum_j m_j w(r_ij/h_i) = n_ngb m_i (gather, self included) by safeguarded
+ * Newton-Raphson on a per-target neighbour list, then writes
+ *   h_inout (in: guess, out: solution), rho = sum_j m_j W_ij(h_i), omega (Eq. 7),
+ *   n_ngb_out = #{j : r_ij < 2 h_i} (borderline pairs decided in FP64).                  */
+int  sph_density_h(sph_ctx* ctx, const float* m, float* h_inout, float* rho, float* omega,
+                   int32_t* n_ngb_out);
+
+/* Steps a7-a9: Eqs. (13)-(18), with P = (gamma-1) rho u, c = sqrt(gamma
+ * P/rho).  Pair set: 0 < r_ij < 2 max(h_i,h_j) (gather and scatter).
+ * Outputs: acceleration a, du/dt = Eq. (14) + Eq. (18), mu_min_i = min(0, min_j mu_ij),
+ * and the EOS values P, c.  v and u are whatever the caller wants used (the "predicted"
+ * values of PAPER.md:232-240).                                                           */
+int  sph_forces(sph_ctx* ctx, const float* m, const float* vx, const float* vy, const float* vz,
+                const float* u, const float* rho, const float* h, const float* omega,
+                float* ax, float* ay, float* az, float* dudt, float* mu_min, float* P,
+                float* c);
+
+/* Steps a10-a11: PAPER.md:263-268.  dt_a = eta_a sqrt(2h/|a|) (no limit if a = 0),
+ * dt_CFL = eta_C h/((1+0.6 alpha) c + 0.6 beta |mu_min|), dt_i = min of the two,
+ * *dt_min_device = min_i dt_i (one float in device memory).                              */
+int  sph_timestep(sph_ctx* ctx, const float* h, const float* c, const float* ax, const float* ay,
+                  const float* az, const float* mu_min, float* dt_i, float* dt_min_device);
+
+/* Diagnostic: CSR neighbour lists at a prescribed h, caller indices; a list is a set, the
+ * order inside it is unspecified.
+ * mode 0: j with r_ij < 2 h_i (self included); mode 1: j != i with r_ij < 2 max(h_i,h_j).
+ * Borderline pairs are decided in FP64 on the FP32 inputs, so the sets equal the exact
+ * ones.  offsets: n+1 int64 (device).  indices: `capacity` int32 (device, may be NULL if
+ * capacity = 0).  *needed (host) receives the total length.  Synchronises the stream.    */
+int  sph_neighbors(sph_ctx* ctx, const float* h, int32_t mode, int64_t* offsets, int32_t* indices,
+                   int64_t capacity, int64_t* needed);
+
+/* Copies the device counters to *out (host).  Synchronises the stream.                   */
+int  sph_stats(sph_ctx* ctx, sph_stats_t* out);
+int  sph_stats_reset(sph_ctx* ctx);
+
+/* perm_out[p] = caller index of the particle at sorted position p (device, n int32).     */
+int  sph_permutation(sph_ctx* ctx, int32_t* perm_out);
+
+/* Measures the FP32 FMA rate of the device with a register-resident FFMA kernel running
+ * for about `seconds`; *tflops (host) = 2 x FMAs / time.  The ALU roofline denominator of
+ * bench.py.  Synchronises.                                                               */
+int  sph_fp32_peak(void* cuda_stream, float seconds, double* tflops);
+
+const char* sph_strerror(int code);
+const char* sph_last_error(const sph_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SPH_B200_H */

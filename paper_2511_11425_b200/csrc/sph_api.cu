@@ -1,0 +1,212 @@
+// sph_api.cu -- the extern "C" boundary of include/sph.h: context life cycle, argument
+// checks, error text, counters.  All compute is in the sph_*.cu kernels it dispatches to.
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include "sph_internal.cuh"
+
+static void fill_defaults(sph_params& p) {
+    if (p.kernel == 0) p.kernel = 1;
+    if (!(p.n_ngb > 0.0f)) p.n_ngb = 64.0f;
+    if (!(p.gamma > 1.0f)) p.gamma = 5.0f / 3.0f;
+    if (!(p.av_eps > 0.0f)) p.av_eps = 0.01f;
+    if (!(p.eta_cfl > 0.0f)) p.eta_cfl = 0.3f;
+    if (!(p.eta_acc > 0.0f)) p.eta_acc = 0.2f;
+    if (!(p.h_tol > 0.0f)) p.h_tol = 1e-6f;
+    if (p.h_max_iter <= 0) p.h_max_iter = 40;
+    if (!(p.search_slack > 1.0f)) p.search_slack = 1.1f;
+    if (!(p.cell_div_x > 0.0f)) p.cell_div_x = 4.0f;
+    if (!(p.cell_div_yz > 0.0f)) p.cell_div_yz = 1.5f;
+}
+
+template <class T>
+static cudaError_t dalloc(T** p, size_t count) {
+    return cudaMalloc((void**)p, count * sizeof(T));
+}
+
+extern "C" int sph_create(sph_ctx** out, const sph_params* params, const sph_box* box,
+                          int64_t n_max, void* cuda_stream) {
+    if (!out || !params || !box || n_max <= 0 || n_max > (int64_t)0x7fffff00) return SPH_EINVAL;
+    if (params->kernel != 0 && params->kernel != 1) return SPH_EINVAL;
+    if (params->n_ngb > 0.0f && params->n_ngb <= 14.0f) return SPH_EINVAL;  // root must exist
+    for (int d = 0; d < 3; ++d)
+        if (!(box->len[d] > 0.0f)) return SPH_EINVAL;
+    sph_ctx* c = new (std::nothrow) sph_ctx;
+    if (!c) return SPH_ENOMEM;
+    memset(c, 0, sizeof(*c));
+    c->par = *params;
+    fill_defaults(c->par);
+    c->box    = *box;
+    c->n_max  = n_max;
+    c->stream = (cudaStream_t)cuda_stream;
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
+        delete c;
+        return SPH_ECUDA;
+    }
+    // cell table: a few cells per particle is the working point; vacuum around free
+    // surfaces needs more, hence the generous cap (4 B per cell)
+    c->cap_cells = 8 * n_max + (1 << 20);
+    if (c->cap_cells > ((int64_t)1 << 30)) c->cap_cells = (int64_t)1 << 30;
+    bool ok = true;
+    ok = ok && dalloc(&c->grid, 1) == cudaSuccess;
+    ok = ok && dalloc(&c->red, 8) == cudaSuccess;
+    ok = ok && dalloc(&c->cell_cnt, (size_t)c->cap_cells + 1) == cudaSuccess;
+    ok = ok && dalloc(&c->cell_start, (size_t)c->cap_cells + 1) == cudaSuccess;
+    ok = ok && dalloc(&c->key, (size_t)n_max) == cudaSuccess;
+    ok = ok && dalloc(&c->rank, (size_t)n_max) == cudaSuccess;
+    ok = ok && dalloc(&c->perm, (size_t)n_max) == cudaSuccess;
+    ok = ok && dalloc(&c->inv_perm, (size_t)n_max) == cudaSuccess;
+    ok = ok && dalloc(&c->scan_part, (size_t)SPH_SCAN_BLOCKS + 1) == cudaSuccess;
+    ok = ok && dalloc(&c->pos_h, (size_t)n_max) == cudaSuccess;
+    ok = ok && dalloc(&c->pos_m, (size_t)n_max) == cudaSuccess;
+    ok = ok && dalloc(&c->vel_m, (size_t)n_max) == cudaSuccess;
+    ok = ok && dalloc(&c->rcak, (size_t)n_max) == cudaSuccess;
+    ok = ok && dalloc(&c->stats, (size_t)ST_NCOUNTERS) == cudaSuccess;
+    ok = ok && dalloc(&c->dt_part, (size_t)1024) == cudaSuccess;
+    ok = ok && dalloc(&c->nb_total, (size_t)2) == cudaSuccess;
+    if (ok) ok = cudaMemsetAsync(c->stats, 0, ST_NCOUNTERS * sizeof(unsigned long long),
+                                 c->stream) == cudaSuccess;
+    if (ok) ok = cudaMemsetAsync(c->grid, 0, sizeof(SphGrid), c->stream) == cudaSuccess;
+    if (!ok) {
+        cudaGetLastError();
+        sph_destroy(c);
+        return SPH_ENOMEM;
+    }
+    *out = c;
+    return SPH_OK;
+}
+
+extern "C" void sph_destroy(sph_ctx* c) {
+    if (!c) return;
+    cudaStreamSynchronize(c->stream);
+    cudaFree(c->grid);      cudaFree(c->red);       cudaFree(c->cell_cnt);
+    cudaFree(c->cell_start); cudaFree(c->key);      cudaFree(c->rank);
+    cudaFree(c->perm);      cudaFree(c->inv_perm);  cudaFree(c->scan_part);
+    cudaFree(c->pos_h);     cudaFree(c->pos_m);     cudaFree(c->vel_m);
+    cudaFree(c->rcak);      cudaFree(c->stats);     cudaFree(c->dt_part);
+    cudaFree(c->nb_total);
+    delete c;
+}
+
+static int fail(sph_ctx* c, int code, const char* what) {
+    if (c) snprintf(c->err, sizeof(c->err), "%s: %s", sph_strerror(code), what);
+    return code;
+}
+
+extern "C" int sph_build_cells(sph_ctx* c, int64_t n, const float* x, const float* y,
+                               const float* z, const float* h) {
+    if (!c) return SPH_EINVAL;
+    if (!x || !y || !z || !h) return fail(c, SPH_EINVAL, "sph_build_cells: null array");
+    if (n <= 0 || n > c->n_max) return fail(c, SPH_EINVAL, "sph_build_cells: n out of range");
+    c->built = false;
+    int rc = sph_launch_build(c, n, x, y, z, h);
+    if (rc == SPH_OK) {
+        c->n     = n;
+        c->built = true;
+    }
+    return rc;
+}
+
+extern "C" int sph_density_h(sph_ctx* c, const float* m, float* h, float* rho, float* omega,
+                             int32_t* nn) {
+    if (!c) return SPH_EINVAL;
+    if (!m || !h || !rho || !omega || !nn) return fail(c, SPH_EINVAL, "sph_density_h: null array");
+    if (!c->built) return fail(c, SPH_ESTALE, "sph_density_h before sph_build_cells");
+    return sph_launch_density(c, m, h, rho, omega, nn);
+}
+
+extern "C" int sph_forces(sph_ctx* c, const float* m, const float* vx, const float* vy,
+                          const float* vz, const float* u, const float* rho, const float* h,
+                          const float* omega, float* ax, float* ay, float* az, float* dudt,
+                          float* mu_min, float* P, float* cs) {
+    if (!c) return SPH_EINVAL;
+    if (!m || !vx || !vy || !vz || !u || !rho || !h || !omega || !ax || !ay || !az || !dudt ||
+        !mu_min || !P || !cs)
+        return fail(c, SPH_EINVAL, "sph_forces: null array");
+    if (!c->built) return fail(c, SPH_ESTALE, "sph_forces before sph_build_cells");
+    return sph_launch_forces(c, m, vx, vy, vz, u, rho, h, omega, ax, ay, az, dudt, mu_min, P, cs);
+}
+
+extern "C" int sph_timestep(sph_ctx* c, const float* h, const float* cs, const float* ax,
+                            const float* ay, const float* az, const float* mu_min, float* dt_i,
+                            float* dt_min) {
+    if (!c) return SPH_EINVAL;
+    if (!h || !cs || !ax || !ay || !az || !mu_min || !dt_i || !dt_min)
+        return fail(c, SPH_EINVAL, "sph_timestep: null array");
+    if (c->n <= 0) return fail(c, SPH_ESTALE, "sph_timestep before sph_build_cells");
+    return sph_launch_timestep(c, h, cs, ax, ay, az, mu_min, dt_i, dt_min);
+}
+
+extern "C" int sph_neighbors(sph_ctx* c, const float* h, int32_t mode, int64_t* offsets,
+                             int32_t* indices, int64_t capacity, int64_t* needed) {
+    if (!c) return SPH_EINVAL;
+    if (!h || !offsets || !needed || (mode != 0 && mode != 1) || capacity < 0 ||
+        (capacity > 0 && !indices))
+        return fail(c, SPH_EINVAL, "sph_neighbors: bad argument");
+    if (!c->built) return fail(c, SPH_ESTALE, "sph_neighbors before sph_build_cells");
+    return sph_launch_neighbors(c, h, mode, offsets, indices, capacity, needed);
+}
+
+extern "C" int sph_stats(sph_ctx* c, sph_stats_t* out) {
+    if (!c || !out) return SPH_EINVAL;
+    unsigned long long v[ST_NCOUNTERS];
+    SphGrid g;
+    SPH_CUDA_CHECK(c, cudaMemcpyAsync(v, c->stats, sizeof(v), cudaMemcpyDeviceToHost, c->stream));
+    SPH_CUDA_CHECK(c, cudaMemcpyAsync(&g, c->grid, sizeof(g), cudaMemcpyDeviceToHost, c->stream));
+    SPH_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));
+    memset(out, 0, sizeof(*out));
+    out->dens_tested    = (int64_t)v[ST_DENS_TESTED];
+    out->dens_listed    = (int64_t)v[ST_DENS_LISTED];
+    out->dens_pairs     = (int64_t)v[ST_DENS_PAIRS];
+    out->dens_sweeps    = (int64_t)v[ST_DENS_SWEEPS];
+    out->dens_recollect = (int64_t)v[ST_DENS_RECOLLECT];
+    out->dens_overflow  = (int64_t)v[ST_DENS_OVERFLOW];
+    out->dens_nonconv   = (int64_t)v[ST_DENS_NONCONV];
+    out->dens_recheck   = (int64_t)v[ST_DENS_RECHECK];
+    out->force_tested   = (int64_t)v[ST_FORCE_TESTED];
+    out->force_pairs    = (int64_t)v[ST_FORCE_PAIRS];
+    out->force_av_pairs = (int64_t)v[ST_FORCE_AV];
+    out->n_cells        = g.ncells;
+    out->grid_flags     = g.flags;
+    out->reserved[0]    = g.nx;
+    out->reserved[1]    = g.ny;
+    out->reserved[2]    = g.nz;
+    return SPH_OK;
+}
+
+extern "C" int sph_stats_reset(sph_ctx* c) {
+    if (!c) return SPH_EINVAL;
+    SPH_CUDA_CHECK(c, cudaMemsetAsync(c->stats, 0, ST_NCOUNTERS * sizeof(unsigned long long),
+                                      c->stream));
+    return SPH_OK;
+}
+
+extern "C" int sph_permutation(sph_ctx* c, int32_t* perm_out) {
+    if (!c || !perm_out) return SPH_EINVAL;
+    if (!c->built) return fail(c, SPH_ESTALE, "sph_permutation before sph_build_cells");
+    SPH_CUDA_CHECK(c, cudaMemcpyAsync(perm_out, c->perm, (size_t)c->n * sizeof(int32_t),
+                                      cudaMemcpyDeviceToDevice, c->stream));
+    return SPH_OK;
+}
+
+extern "C" int sph_fp32_peak(void* cuda_stream, float seconds, double* tflops) {
+    if (!tflops || !(seconds > 0.0f)) return SPH_EINVAL;
+    return sph_launch_fp32_peak((cudaStream_t)cuda_stream, seconds, tflops);
+}
+
+extern "C" const char* sph_strerror(int code) {
+    switch (code) {
+    case SPH_OK:     return "ok";
+    case SPH_EINVAL: return "invalid argument";
+    case SPH_EBOX:   return "periodic box too small for the kernel support";
+    case SPH_ENOMEM: return "out of device memory";
+    case SPH_ECUDA:  return "CUDA error";
+    case SPH_ESTALE: return "index not built";
+    case SPH_ENOSPC: return "output capacity too small";
+    }
+    return "unknown error";
+}
+
+extern "C" const char* sph_last_error(const sph_ctx* c) { return c ? c->err : ""; }

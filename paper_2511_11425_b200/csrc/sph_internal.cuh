@@ -1,0 +1,253 @@
+// sph_internal.cuh -- context, device-resident grid descriptor and the warp-level
+// neighbour-row enumeration shared by the sweeps.  Internal to the CUDA library; the public
+// boundary is include/sph.h.  Shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "../../include/sph.h"
+
+// ---------------------------------------------------------------------------------------
+// Spatial index.  Uniform grid, cell = (cz*ny + cy)*nx + cx, so that
+// a run of cells along x is ONE contiguous range of the sorted particle arrays
+// (the paper's "particles of a cell are contiguous", applied to rows).
+// The descriptor lives in device memory and is written by a kernel from min(h): no host
+// round trip between sph_build_cells and the sweeps.
+// ---------------------------------------------------------------------------------------
+struct SphGrid {
+    int   nx, ny, nz, ncells;
+    float sx, sy, sz;          // cell sides
+    float isx, isy, isz;       // inverse cell sides
+    float lo[3], len[3];
+    int   per[3];
+    float hmin, hmax;          // of the h given to sph_build_cells
+    float xext;                // largest |coordinate| that enters a displacement
+    int   flags;               // bit0: periodic side too short; bit1: cell table clipped
+    unsigned force_hmax_bits;  // max h given to sph_forces (float bits, atomicMax)
+    int   pad[3];
+};
+
+enum {  // indices into the device counter block (uint64 each), mirrors sph_stats_t
+    ST_DENS_TESTED = 0, ST_DENS_LISTED, ST_DENS_PAIRS, ST_DENS_SWEEPS, ST_DENS_RECOLLECT,
+    ST_DENS_OVERFLOW, ST_DENS_NONCONV, ST_DENS_RECHECK, ST_FORCE_TESTED, ST_FORCE_PAIRS,
+    ST_FORCE_AV, ST_NCOUNTERS
+};
+
+struct sph_ctx {
+    sph_params   par;
+    sph_box      box;
+    int64_t      n_max, n;
+    int64_t      cap_cells;
+    cudaStream_t stream;
+    bool         built;
+    int          sm_count;
+    // device memory
+    SphGrid*     grid;
+    unsigned*    red;          // [8] uint: hmin bits, hmax bits, max|x| bits ...
+    uint32_t*    cell_cnt;     // cap_cells + 1
+    uint32_t*    cell_start;   // cap_cells + 1
+    uint32_t*    key;          // n_max
+    uint32_t*    rank;         // n_max
+    int32_t*     perm;         // n_max: sorted position -> caller index
+    int32_t*     inv_perm;     // n_max: caller index -> sorted position
+    uint32_t*    scan_part;    // SCAN_BLOCKS + 1
+    float4*      pos_h;        // sorted (x, y, z, h)
+    float4*      pos_m;        // sorted (x, y, z, m)
+    float4*      vel_m;        // sorted (vx, vy, vz, m)
+    float4*      rcak;         // sorted (rho, c, A = P/(Omega rho^2), K = 5 sigma / h^5)
+    unsigned long long* stats; // ST_NCOUNTERS
+    float*       dt_part;      // per-block minima of the time-step reduction
+    int64_t*     nb_total;     // neighbour-list total (device) + pinned mirror
+    char         err[256];
+};
+
+#define SPH_SCAN_BLOCKS 1024
+
+#define SPH_CUDA_CHECK(ctx, call)                                                          \
+    do {                                                                                   \
+        cudaError_t e_ = (call);                                                           \
+        if (e_ != cudaSuccess) {                                                           \
+            snprintf((ctx)->err, sizeof((ctx)->err), "%s:%d %s: %s", __FILE__, __LINE__,   \
+                     #call, cudaGetErrorString(e_));                                       \
+            return SPH_ECUDA;                                                              \
+        }                                                                                  \
+    } while (0)
+
+#ifdef __CUDACC__
+
+#define SPH_FULL 0xffffffffu
+
+// Wendland C2, support 2h: w(q) = SIGMA (1-q/2)^4 (1+2q); (32 pi/3) SIGMA = 14.
+#define SPH_SIGMA 0.41778172561566733f   /* 21/(16 pi) */
+
+__device__ __forceinline__ int sph_fdiv(int u, int n) {   // floor(u / n), n > 0
+    return (u >= 0) ? (u / n) : -((-u + n - 1) / n);
+}
+
+__device__ __forceinline__ int sph_cell_coord(float x, float lo, float is, int n) {
+    float c = floorf((x - lo) * is);
+    c = fminf(fmaxf(c, 0.0f), (float)(n - 1));
+    return (int)c;   // NaN -> 0 through fmaxf
+}
+
+// Range of (unwrapped) cell coordinates that can hold a particle within R of x.
+__device__ __forceinline__ void sph_axis_range(float x, float R, float lo, float is, int n,
+                                               int per, int& u0, int& u1) {
+    float a = floorf((x - lo - R) * is - 1e-3f);
+    float b = floorf((x - lo + R) * is + 1e-3f);
+    a = fminf(fmaxf(a, -1.0e9f), 1.0e9f);
+    b = fminf(fmaxf(b, -1.0e9f), 1.0e9f);
+    u0 = (int)a;
+    u1 = (int)b;
+    if (per) {
+        if (u1 - u0 + 1 > n) {   // whole axis: every cell once, image nearest to the target
+            int c = (int)fminf(fmaxf(floorf((x - lo) * is), -1.0e9f), 1.0e9f);
+            u0 = c - (n - 1) / 2;
+            u1 = u0 + n - 1;
+        }
+    } else {
+        u0 = min(max(u0, 0), n - 1);
+        u1 = min(max(u1, 0), n - 1);
+    }
+}
+
+// One contiguous run of candidate sources: sorted positions [start, end), and the target's
+// coordinates shifted by the periodic image of the run, so that d = s - x_j.
+struct RowRec {
+    uint32_t start, end;
+    float    sx, sy, sz;
+};
+#define SPH_RCAP 64   // two x segments for each of 32 rows built per batch
+
+// Squared distance from coordinate y to the slab [u*s, (u+1)*s) + lo; edge cells of a
+// non-periodic axis extend to infinity (particles outside the box are binned there).
+__device__ __forceinline__ float sph_slab_dist(float y, int u, float lo, float s, int n, int per) {
+    float a = lo + (float)u * s;
+    float below = a - y;           // > 0: y is below the slab
+    float above = y - (a + s);     // > 0: y is above the slab
+    if (!per) {
+        if (u <= 0) below = 0.0f;
+        if (u >= n - 1) above = 0.0f;
+    }
+    float d = fmaxf(fmaxf(below, above) - 1e-3f * s, 0.0f);
+    return d;
+}
+
+// Warp-collective.  Calls body(const RowRec&) for every non-empty row segment whose cells
+// can hold a particle within R of (xi, yi, zi).  `rows` is SPH_RCAP records of this warp's
+// shared memory.  All 32 lanes must call with identical arguments.
+template <class Body>
+__device__ __forceinline__ void sph_for_each_row(const SphGrid& g,
+                                                 const uint32_t* __restrict__ cell_start,
+                                                 float xi, float yi, float zi, float R,
+                                                 RowRec* rows, int lane, Body&& body) {
+    int x0, x1, y0, y1, z0, z1;
+    sph_axis_range(xi, R, g.lo[0], g.isx, g.nx, g.per[0], x0, x1);
+    sph_axis_range(yi, R, g.lo[1], g.isy, g.ny, g.per[1], y0, y1);
+    sph_axis_range(zi, R, g.lo[2], g.isz, g.nz, g.per[2], z0, z1);
+    const int   kx0  = sph_fdiv(x0, g.nx);
+    const int   c0   = x0 - kx0 * g.nx;
+    const int   span = x1 - x0;
+    const int   a_c1 = min(c0 + span, g.nx - 1);
+    const bool  two  = (c0 + span > g.nx - 1);
+    const int   b_c1 = c0 + span - g.nx;
+    const float sxA  = xi - (float)kx0 * g.len[0];
+    const float sxB  = xi - (float)(kx0 + 1) * g.len[0];
+    const int   nyr  = y1 - y0 + 1, nzr = z1 - z0 + 1, nrow = nyr * nzr;
+    const float R2   = R * R * (1.0f + 1e-5f);
+    const unsigned lt = (1u << lane) - 1u;
+
+    for (int base = 0; base < nrow; base += 32) {
+        const int r  = base + lane;
+        bool      ok = r < nrow;
+        const int iz = r / nyr, iy = r - iz * nyr;
+        const int uy = y0 + iy, uz = z0 + iz;
+        uint32_t  a0 = 0, a1 = 0, b0 = 0, b1 = 0;
+        float     sy = yi, sz = zi;
+        if (ok) {
+            float dy = sph_slab_dist(yi, uy, g.lo[1], g.sy, g.ny, g.per[1]);
+            float dz = sph_slab_dist(zi, uz, g.lo[2], g.sz, g.nz, g.per[2]);
+            ok = (dy * dy + dz * dz <= R2);
+        }
+        if (ok) {
+            const int ky = sph_fdiv(uy, g.ny), cy = uy - ky * g.ny;
+            const int kz = sph_fdiv(uz, g.nz), cz = uz - kz * g.nz;
+            sy = yi - (float)ky * g.len[1];
+            sz = zi - (float)kz * g.len[2];
+            const uint32_t rb = (uint32_t)(cz * g.ny + cy) * (uint32_t)g.nx;
+            a0 = __ldg(cell_start + rb + c0);
+            a1 = __ldg(cell_start + rb + a_c1 + 1);
+            if (two) {
+                b0 = __ldg(cell_start + rb);
+                b1 = __ldg(cell_start + rb + b_c1 + 1);
+            }
+        }
+        const bool     va = ok && (a1 > a0), vb = ok && (b1 > b0);
+        const unsigned ma = __ballot_sync(SPH_FULL, va), mb = __ballot_sync(SPH_FULL, vb);
+        const int      na = __popc(ma);
+        if (va) {
+            RowRec rr{a0, a1, sxA, sy, sz};
+            rows[__popc(ma & lt)] = rr;
+        }
+        if (vb) {
+            RowRec rr{b0, b1, sxB, sy, sz};
+            rows[na + __popc(mb & lt)] = rr;
+        }
+        __syncwarp();
+        const int cnt = na + __popc(mb);
+        for (int q = 0; q < cnt; ++q) {
+            const RowRec rr = rows[q];
+            body(rr);
+        }
+        __syncwarp();
+    }
+}
+
+// Exact (FP64) squared distance of two particles under the minimum-image convention,
+// evaluated on the FP32 inputs -- the definition the neighbour sets are tested against
+// (reading R7).  Rare: only pairs within a relative band tau of the support edge.
+__device__ __forceinline__ double sph_r2_exact(const SphGrid& g, float ax, float ay, float az,
+                                               float bx, float by, float bz) {
+    double dx = (double)ax - (double)bx, dy = (double)ay - (double)by, dz = (double)az - (double)bz;
+    if (g.per[0]) { double L = (double)g.len[0]; dx -= L * rint(dx / L); }
+    if (g.per[1]) { double L = (double)g.len[1]; dy -= L * rint(dy / L); }
+    if (g.per[2]) { double L = (double)g.len[2]; dz -= L * rint(dz / L); }
+    return dx * dx + dy * dy + dz * dz;
+}
+
+// Relative half-width of the band around r^2 = 4h^2 inside which the FP32 distance cannot
+// be trusted: |delta r^2| / r^2 <= 2 sqrt(3) 2^-24 xext / r + O(2^-22).
+__device__ __forceinline__ float sph_band(const SphGrid& g, float h) {
+    return 1e-6f + 2.5e-7f * g.xext / h;
+}
+
+__device__ __forceinline__ float sph_warp_sum(float v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(SPH_FULL, v, o);
+    return v;
+}
+__device__ __forceinline__ float sph_warp_min(float v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fminf(v, __shfl_xor_sync(SPH_FULL, v, o));
+    return v;
+}
+__device__ __forceinline__ int sph_warp_sum_int(int v) {
+    return __reduce_add_sync(SPH_FULL, v);
+}
+
+#endif  // __CUDACC__
+
+// host-side launch helpers implemented across the .cu files
+int sph_launch_build(sph_ctx* c, int64_t n, const float* x, const float* y, const float* z,
+                     const float* h);
+int sph_launch_density(sph_ctx* c, const float* m, float* h, float* rho, float* omega,
+                       int32_t* nn);
+int sph_launch_forces(sph_ctx* c, const float* m, const float* vx, const float* vy,
+                      const float* vz, const float* u, const float* rho, const float* h,
+                      const float* omega, float* ax, float* ay, float* az, float* dudt,
+                      float* mu_min, float* P, float* cs);
+int sph_launch_timestep(sph_ctx* c, const float* h, const float* cs, const float* ax,
+                        const float* ay, const float* az, const float* mu_min, float* dt_i,
+                        float* dt_min);
+int sph_launch_neighbors(sph_ctx* c, const float* h, int32_t mode, int64_t* offsets,
+                         int32_t* indices, int64_t capacity, int64_t* needed);
+int sph_launch_fp32_peak(cudaStream_t s, float seconds, double* tflops);

@@ -1,0 +1,255 @@
+"""Thin ctypes binding of the C-ABI CUDA library declared in include/sph.h.
+
+Argument marshalling only: every step of the path runs in the library's kernels.  Torch is
+used for device memory and the stream.  There is no CPU fallback: if the library is missing
+or no CUDA device is present, the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass, field
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libsph_b200.so")
+
+SPH_OK, SPH_EINVAL, SPH_EBOX, SPH_ENOMEM, SPH_ECUDA, SPH_ESTALE, SPH_ENOSPC = 0, -1, -2, -3, -4, -5, -6
+
+# every symbol include/sph.h declares (tests check the library exports exactly these)
+SYMBOLS = ["sph_create", "sph_destroy", "sph_build_cells", "sph_density_h", "sph_forces",
+           "sph_timestep", "sph_neighbors", "sph_stats", "sph_stats_reset", "sph_permutation",
+           "sph_fp32_peak", "sph_strerror", "sph_last_error"]
+
+
+class SphError(RuntimeError):
+    def __init__(self, code, text):
+        super().__init__(f"sph error {code}: {text}")
+        self.code = code
+
+
+class _Box(C.Structure):
+    _fields_ = [("lo", C.c_float * 3), ("len", C.c_float * 3), ("periodic", C.c_int32 * 3)]
+
+
+class _Params(C.Structure):
+    _fields_ = [("kernel", C.c_int32), ("n_ngb", C.c_float), ("gamma", C.c_float),
+                ("av_alpha", C.c_float), ("av_beta", C.c_float), ("av_eps", C.c_float),
+                ("eta_cfl", C.c_float), ("eta_acc", C.c_float), ("h_tol", C.c_float),
+                ("h_max_iter", C.c_int32), ("search_slack", C.c_float),
+                ("cell_div_x", C.c_float), ("cell_div_yz", C.c_float)]
+
+
+class _Stats(C.Structure):
+    _fields_ = [(k, C.c_int64) for k in (
+        "dens_tested", "dens_listed", "dens_pairs", "dens_sweeps", "dens_recollect",
+        "dens_overflow", "dens_nonconv", "dens_recheck", "force_tested", "force_pairs",
+        "force_av_pairs", "n_cells", "grid_flags")] + [("reserved", C.c_int64 * 3)]
+
+
+@dataclass
+class Params:
+    kernel: int = 1
+    n_ngb: float = 64.0
+    gamma: float = 5.0 / 3.0
+    av_alpha: float = 1.0
+    av_beta: float = 2.0
+    av_eps: float = 0.01
+    eta_cfl: float = 0.3
+    eta_acc: float = 0.2
+    h_tol: float = 0.0          # 0 -> library default
+    h_max_iter: int = 0
+    search_slack: float = 0.0
+    cell_div_x: float = 0.0
+    cell_div_yz: float = 0.0
+
+    def c(self) -> _Params:
+        return _Params(self.kernel, self.n_ngb, self.gamma, self.av_alpha, self.av_beta,
+                       self.av_eps, self.eta_cfl, self.eta_acc, self.h_tol, self.h_max_iter,
+                       self.search_slack, self.cell_div_x, self.cell_div_yz)
+
+
+@dataclass
+class Box:
+    lo: tuple = (0.0, 0.0, 0.0)
+    len: tuple = (1.0, 1.0, 1.0)
+    periodic: tuple = (1, 1, 1)
+
+    def c(self) -> _Box:
+        b = _Box()
+        for d in range(3):
+            b.lo[d], b.len[d], b.periodic[d] = float(self.lo[d]), float(self.len[d]), int(self.periodic[d])
+        return b
+
+
+_lib = None
+
+
+def load():
+    """dlopen the library (building it is __graft_entry__.build / python -m ...build)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise SphError(SPH_EINVAL, f"{LIB_PATH} missing: run `python -m paper_2511_11425_b200.build`")
+    lib = C.CDLL(LIB_PATH)
+    vp, i64, i32, fp = C.c_void_p, C.c_int64, C.c_int32, C.c_void_p  # device pointers as void*
+    lib.sph_create.argtypes = [C.POINTER(vp), C.POINTER(_Params), C.POINTER(_Box), i64, vp]
+    lib.sph_destroy.argtypes = [vp]
+    lib.sph_destroy.restype = None
+    lib.sph_build_cells.argtypes = [vp, i64, fp, fp, fp, fp]
+    lib.sph_density_h.argtypes = [vp] + [fp] * 5
+    lib.sph_forces.argtypes = [vp] + [fp] * 15
+    lib.sph_timestep.argtypes = [vp] + [fp] * 8
+    lib.sph_neighbors.argtypes = [vp, fp, i32, fp, fp, i64, C.POINTER(i64)]
+    lib.sph_stats.argtypes = [vp, C.POINTER(_Stats)]
+    lib.sph_stats_reset.argtypes = [vp]
+    lib.sph_permutation.argtypes = [vp, fp]
+    lib.sph_fp32_peak.argtypes = [vp, C.c_float, C.POINTER(C.c_double)]
+    lib.sph_strerror.argtypes = [C.c_int]
+    lib.sph_strerror.restype = C.c_char_p
+    lib.sph_last_error.argtypes = [vp]
+    lib.sph_last_error.restype = C.c_char_p
+    for name in SYMBOLS:
+        if name not in ("sph_destroy", "sph_strerror", "sph_last_error"):
+            getattr(lib, name).restype = C.c_int
+    _lib = lib
+    return lib
+
+
+def _ptr(t: torch.Tensor, dtype, n=None):
+    if not t.is_cuda or t.dtype != dtype or not t.is_contiguous():
+        raise SphError(SPH_EINVAL, f"expected a contiguous CUDA tensor of {dtype}")
+    if n is not None and t.numel() != n:
+        raise SphError(SPH_EINVAL, f"expected {n} elements, got {t.numel()}")
+    return C.c_void_p(t.data_ptr())
+
+
+def fp32_peak(seconds: float = 1.0) -> float:
+    """Measured FP32 FMA rate of the current device in TFLOP/s (sph_fp32_peak)."""
+    if not torch.cuda.is_available():
+        raise SphError(SPH_ECUDA, "no CUDA device")
+    out = C.c_double(0.0)
+    rc = load().sph_fp32_peak(C.c_void_p(torch.cuda.current_stream().cuda_stream), seconds,
+                              C.byref(out))
+    if rc:
+        raise SphError(rc, load().sph_strerror(rc).decode())
+    return out.value
+
+
+class Sph:
+    """One sph_ctx.  All tensors: CUDA, contiguous, length n, caller order."""
+
+    def __init__(self, params: Params, box: Box, n_max: int, stream: torch.cuda.Stream | None = None):
+        if not torch.cuda.is_available():
+            raise SphError(SPH_ECUDA, "no CUDA device: the SPH path has no CPU fallback")
+        self.lib = load()
+        self.stream = stream if stream is not None else torch.cuda.current_stream()
+        self.n_max = int(n_max)
+        self.n = 0
+        self._ctx = C.c_void_p()
+        p, b = params.c(), box.c()
+        rc = self.lib.sph_create(C.byref(self._ctx), C.byref(p), C.byref(b), self.n_max,
+                                 C.c_void_p(self.stream.cuda_stream))
+        if rc:
+            raise SphError(rc, self.lib.sph_strerror(rc).decode())
+
+    def close(self):
+        if getattr(self, "_ctx", None) is not None and self._ctx.value:
+            self.lib.sph_destroy(self._ctx)
+            self._ctx = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, rc):
+        if rc:
+            raise SphError(rc, self.lib.sph_last_error(self._ctx).decode() or
+                           self.lib.sph_strerror(rc).decode())
+
+    # ---- the four calls of the hot path -------------------------------------------------
+    def build_cells(self, x, y, z, h):
+        n = x.numel()
+        f = torch.float32
+        self._check(self.lib.sph_build_cells(self._ctx, n, _ptr(x, f, n), _ptr(y, f, n),
+                                             _ptr(z, f, n), _ptr(h, f, n)))
+        self.n = n
+
+    def density_h(self, m, h_inout, rho, omega, n_ngb):
+        n, f = self.n, torch.float32
+        self._check(self.lib.sph_density_h(self._ctx, _ptr(m, f, n), _ptr(h_inout, f, n),
+                                           _ptr(rho, f, n), _ptr(omega, f, n),
+                                           _ptr(n_ngb, torch.int32, n)))
+
+    def forces(self, m, vx, vy, vz, u, rho, h, omega, ax, ay, az, dudt, mu_min, P, c):
+        n, f = self.n, torch.float32
+        args = [_ptr(t, f, n) for t in (m, vx, vy, vz, u, rho, h, omega, ax, ay, az, dudt,
+                                        mu_min, P, c)]
+        self._check(self.lib.sph_forces(self._ctx, *args))
+
+    def timestep(self, h, c, ax, ay, az, mu_min, dt_i, dt_min):
+        n, f = self.n, torch.float32
+        args = [_ptr(t, f, n) for t in (h, c, ax, ay, az, mu_min, dt_i)]
+        self._check(self.lib.sph_timestep(self._ctx, *args, _ptr(dt_min, f, 1)))
+
+    # ---- diagnostics --------------------------------------------------------------------
+    def neighbors(self, h, mode=0):
+        """CSR lists (offsets int64[n+1], indices int32) at the prescribed h."""
+        n = self.n
+        off = torch.empty(n + 1, dtype=torch.int64, device=h.device)
+        need = C.c_int64(0)
+        self._check(self.lib.sph_neighbors(self._ctx, _ptr(h, torch.float32, n), mode,
+                                           _ptr(off, torch.int64), None, 0, C.byref(need)))
+        idx = torch.empty(max(need.value, 1), dtype=torch.int32, device=h.device)
+        self._check(self.lib.sph_neighbors(self._ctx, _ptr(h, torch.float32, n), mode,
+                                           _ptr(off, torch.int64), _ptr(idx, torch.int32),
+                                           need.value, C.byref(need)))
+        return off, idx[:need.value]
+
+    def stats(self) -> dict:
+        s = _Stats()
+        self._check(self.lib.sph_stats(self._ctx, C.byref(s)))
+        d = {k: int(getattr(s, k)) for k, _ in _Stats._fields_ if k != "reserved"}
+        d["grid_dims"] = tuple(int(v) for v in s.reserved)
+        return d
+
+    def stats_reset(self):
+        self._check(self.lib.sph_stats_reset(self._ctx))
+
+    def permutation(self):
+        p = torch.empty(self.n, dtype=torch.int32, device="cuda")
+        self._check(self.lib.sph_permutation(self._ctx, _ptr(p, torch.int32, self.n)))
+        return p
+
+
+@dataclass
+class StepBuffers:
+    """Device arrays of one density + force step, allocated once."""
+    n: int
+    device: str = "cuda"
+    t: dict = field(default_factory=dict)
+
+    def __post_init__(self):
+        f = dict(dtype=torch.float32, device=self.device)
+        for k in ("rho", "omega", "ax", "ay", "az", "dudt", "mu_min", "P", "c", "dt_i"):
+            self.t[k] = torch.empty(self.n, **f)
+        self.t["n_ngb"] = torch.empty(self.n, dtype=torch.int32, device=self.device)
+        self.t["dt_min"] = torch.empty(1, **f)
+
+    def __getitem__(self, k):
+        return self.t[k]
+
+
+def step(ctx: Sph, w: dict, out: StepBuffers, h: torch.Tensor):
+    """One pass of the whole hot path: build_cells -> density_h -> forces -> timestep.
+    `w` holds the device tensors x, y, z, m, vx, vy, vz, u; `h` is updated in place."""
+    ctx.build_cells(w["x"], w["y"], w["z"], h)
+    ctx.density_h(w["m"], h, out["rho"], out["omega"], out["n_ngb"])
+    ctx.forces(w["m"], w["vx"], w["vy"], w["vz"], w["u"], out["rho"], h, out["omega"],
+               out["ax"], out["ay"], out["az"], out["dudt"], out["mu_min"], out["P"], out["c"])
+    ctx.timestep(h, out["c"], out["ax"], out["ay"], out["az"], out["mu_min"], out["dt_i"],
+                 out["dt_min"])

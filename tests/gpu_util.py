@@ -1,0 +1,87 @@
+"""Helpers of the GPU parity tests: move a workload to the device, run the C-ABI calls,
+and compare with the oracle.  Test infrastructure only."""
+from __future__ import annotations
+
+import numpy as np
+import torch
+
+from oracle import sph_oracle as orc
+from paper_2511_11425_b200 import sph
+
+F_KEYS = ("x", "y", "z", "m", "vx", "vy", "vz", "u", "h")
+
+
+def to_device(w):
+    return {k: torch.from_numpy(np.ascontiguousarray(w[k])).cuda() for k in F_KEYS}
+
+
+def make_params(w, **kw):
+    gp = sph.Params(gamma=float(w["gamma"]), av_alpha=float(w["av_alpha"]),
+                    av_beta=float(w["av_beta"]), **kw)
+    op = orc.Params(gamma=float(np.float32(w["gamma"])), av_alpha=float(np.float32(w["av_alpha"])),
+                    av_beta=float(np.float32(w["av_beta"])), av_eps=float(np.float32(0.01)),
+                    eta_cfl=float(np.float32(0.3)), eta_acc=float(np.float32(0.2)))
+    return gp, op
+
+
+def make_boxes(w):
+    return (sph.Box(w["box_lo"], w["box_len"], w["periodic"]),
+            orc.Box(w["box_lo"], w["box_len"], w["periodic"]))
+
+
+def make_ctx(w, **kw):
+    gp, _ = make_params(w, **kw)
+    gb, _ = make_boxes(w)
+    return sph.Sph(gp, gb, int(w["n"]))
+
+
+def run_density(ctx, d, h0=None):
+    n = d["x"].numel()
+    h = (d["h"] if h0 is None else h0).clone()
+    rho = torch.empty(n, device="cuda")
+    om = torch.empty(n, device="cuda")
+    nn = torch.empty(n, dtype=torch.int32, device="cuda")
+    ctx.build_cells(d["x"], d["y"], d["z"], h)
+    ctx.density_h(d["m"], h, rho, om, nn)
+    torch.cuda.synchronize()
+    return h, rho, om, nn
+
+
+def run_forces(ctx, d, rho, h, om):
+    n = d["x"].numel()
+    o = {k: torch.empty(n, device="cuda") for k in ("ax", "ay", "az", "dudt", "mu_min", "P", "c")}
+    ctx.forces(d["m"], d["vx"], d["vy"], d["vz"], d["u"], rho, h, om, o["ax"], o["ay"], o["az"],
+               o["dudt"], o["mu_min"], o["P"], o["c"])
+    torch.cuda.synchronize()
+    return o
+
+
+def run_timestep(ctx, h, o):
+    n = h.numel()
+    dti = torch.empty(n, device="cuda")
+    dtm = torch.empty(1, device="cuda")
+    ctx.timestep(h, o["c"], o["ax"], o["ay"], o["az"], o["mu_min"], dti, dtm)
+    torch.cuda.synchronize()
+    return dti, dtm
+
+
+def np64(t):
+    return t.detach().cpu().numpy().astype(np.float64)
+
+
+def csr_sets(off, idx, k):
+    off = np.asarray(off)
+    idx = np.asarray(idx)
+    return np.sort(idx[off[k]:off[k + 1]])
+
+
+def force_errors(g, o, sel=None):
+    """Errors normalised by the sum of pairwise term magnitudes (BASELINE.json north_star)."""
+    gx, gy, gz, gu = (np64(g[k]) for k in ("ax", "ay", "az", "dudt"))
+    if sel is not None:
+        gx, gy, gz, gu = gx[sel], gy[sel], gz[sel], gu[sel]
+    da = np.sqrt((gx - o["ax"]) ** 2 + (gy - o["ay"]) ** 2 + (gz - o["az"]) ** 2)
+    ea = da / np.maximum(o["Sa"], 1e-300)
+    eu = np.abs(gu - o["dudt"]) / np.maximum(o["Su"], 1e-300)
+    eu = np.where(o["Su"] > 0, eu, np.abs(gu - o["dudt"]))
+    return ea, eu
