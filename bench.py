@@ -47,6 +47,9 @@ def parse():
     ap.add_argument("--ref-nside", type=int, default=64,
                     help="lattice side of the bounded sample the CPU oracle is timed on")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--slack", type=float, default=0.0, help="sph_params.search_slack (0: default)")
+    ap.add_argument("--cell-div-x", type=float, default=0.0, help="sph_params.cell_div_x (0: default)")
+    ap.add_argument("--cell-div-yz", type=float, default=0.0, help="sph_params.cell_div_yz (0: default)")
     ap.add_argument("--v-sigma", type=float, default=0.0,
                     help="> 0: Sedov variant with random velocities (AV branch exercised)")
     return ap.parse_args()
@@ -175,7 +178,9 @@ def run_gpu(a):
     keys = ("x", "y", "z", "m", "vx", "vy", "vz", "u", "h")
     host = {k: torch.from_numpy(w[k]).pin_memory() for k in keys}
     d = {k: host[k].cuda() for k in keys}
-    ctx = sph.Sph(sph.Params(gamma=w["gamma"], av_alpha=w["av_alpha"], av_beta=w["av_beta"]),
+    ctx = sph.Sph(sph.Params(gamma=w["gamma"], av_alpha=w["av_alpha"], av_beta=w["av_beta"],
+                             search_slack=a.slack, cell_div_x=a.cell_div_x,
+                             cell_div_yz=a.cell_div_yz),
                   sph.Box(w["box_lo"], w["box_len"], w["periodic"]), n)
     out = sph.StepBuffers(n)
     h = torch.empty_like(d["h"])

@@ -2,9 +2,11 @@
 // scatter neighbour search and the hydro force sweep, PAPER.md:186-219 (Section 2.3.5),
 // Eqs. (13)-(18), ideal gas of PAPER.md:111.
 //
-// One warp per target.  Lanes distance-test 32 consecutive candidates of a row, accepted
-// pairs (0 < r < 2 max(h_i,h_j)) go through a 64-entry ring in shared memory
-// so that the pair arithmetic always runs with 32 busy lanes.
+// G = 8 lanes per target, four targets per warp.  Phase 1: the lanes of a group distance-
+// test the candidates of the rows in reach (0 < r < 2 max(h_i,h_j), gather and scatter,
+// PAPER.md:191) and each lane notes the indices it accepted in a private column of a
+// shared-memory list.  Phase 2: every lane works through its own column -- the pair
+// arithmetic runs without divergence between accepted and rejected candidates.
 //
 // Pair arithmetic (d = x_i - x_j, r = |d|, q_a = r/h_a, g_a = K_a (1-q_a/2)_+^3 with
 // K_a = 5 SIGMA / h_a^5, so that dW/dr(r,h_a) = -g_a r):
@@ -17,19 +19,20 @@
 
 namespace {
 
-constexpr int F_WARPS   = 8;
-constexpr int F_TPB     = F_WARPS * 32;
-constexpr int F_TARGETS = 64;
-constexpr int RING      = 64;
+constexpr int F_G      = 8;
+constexpr int F_NT     = 32 / F_G;
+constexpr int F_WARPS  = 4;
+constexpr int F_TPB    = F_WARPS * 32;
+constexpr int F_ROUNDS = 2;
+constexpr int F_TARGETS = F_WARPS * F_NT * F_ROUNDS;
+constexpr int F_SLOTS  = 26;   // list entries per lane
 
 struct ForcePar {
     float alpha, beta, eps;
 };
 
-struct FWarpSmem {
-    uint32_t j[RING];
-    float    dx[RING], dy[RING], dz[RING], r2[RING], hj[RING];
-    RowRec   rows[SPH_RCAP];
+struct FWarpList {
+    uint32_t j[F_SLOTS][32];
 };
 
 // a7: EOS and the per-particle factors, written in sorted order (scattered 16-byte stores)
@@ -64,123 +67,128 @@ __global__ void k_force_prep(int64_t n, const int32_t* __restrict__ inv_perm,
 
 __global__ void k_zero_hmax(SphGrid* g) { g->force_hmax_bits = 0u; }
 
-__global__ __launch_bounds__(F_TPB) void k_forces(int n, const SphGrid* __restrict__ gp,
-                                                  const uint32_t* __restrict__ cell_start,
-                                                  const float4* __restrict__ pos_h,
-                                                  const float4* __restrict__ vel_m,
-                                                  const float4* __restrict__ rcak,
-                                                  const int32_t* __restrict__ perm, ForcePar par,
-                                                  float* ax, float* ay, float* az, float* dudt,
-                                                  float* mu_min, unsigned long long* stats) {
-    __shared__ FWarpSmem sm_all[F_WARPS];
+__global__ __launch_bounds__(F_TPB, SPH_MINB) void k_forces(int n, const SphGrid* __restrict__ gp,
+                                                     const uint32_t* __restrict__ cell_start,
+                                                     const float4* __restrict__ pos_h,
+                                                     const float4* __restrict__ vel_m,
+                                                     const float4* __restrict__ rcak,
+                                                     const int32_t* __restrict__ perm,
+                                                     ForcePar par, float* ax, float* ay, float* az,
+                                                     float* dudt, float* mu_min,
+                                                     unsigned long long* stats) {
+    __shared__ FWarpList lists[F_WARPS];
     __shared__ SphGrid   g;
-    __shared__ unsigned long long st_sh[3];
+    __shared__ unsigned  st_sh[3];
     if (threadIdx.x < sizeof(SphGrid) / 4)
         ((int*)&g)[threadIdx.x] = ((const int*)gp)[threadIdx.x];
-    if (threadIdx.x < 3) st_sh[threadIdx.x] = 0ull;
+    if (threadIdx.x < 3) st_sh[threadIdx.x] = 0u;
     __syncthreads();
 
-    const int      wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const unsigned lt  = (1u << lane) - 1u;
-    FWarpSmem&     sm  = sm_all[wid];
-    const float    hmax_all = __uint_as_float(g.force_hmax_bits);
+    const int   wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int   gq  = lane / F_G;
+    FWarpList&  L   = lists[wid];
+    const float hmax_all = __uint_as_float(g.force_hmax_bits);
+    const float iLx = g.per[0] ? 1.0f / g.len[0] : 0.0f, Lx = g.per[0] ? g.len[0] : 0.0f;
+    const float iLy = g.per[1] ? 1.0f / g.len[1] : 0.0f, Ly = g.per[1] ? g.len[1] : 0.0f;
+    const float iLz = g.per[2] ? 1.0f / g.len[2] : 0.0f, Lz = g.per[2] ? g.len[2] : 0.0f;
 
-    unsigned long long c_tested = 0;
-    unsigned c_pairs = 0, c_av = 0;
+    unsigned c_tested = 0, c_pairs = 0, c_av = 0;
 
-    for (int t = wid; t < F_TARGETS; t += F_WARPS) {
-        const int p = blockIdx.x * F_TARGETS + t;
-        if (p >= n) break;
-        const float4 pi = pos_h[p];
-        const float4 vi = vel_m[p];
-        const float4 ri = rcak[p];
-        const float  hi = pi.w, ihi = 1.0f / hi;
-        const float  rho_i = ri.x, c_i = ri.y, A_i = ri.z, K_i = ri.w;
+    for (int round = 0; round < F_ROUNDS; ++round) {
+        const int  p      = (blockIdx.x * F_ROUNDS + round) * (F_WARPS * F_NT) + wid * F_NT + gq;
+        const bool tvalid = p < n;
+        float4 pi = make_float4(0.f, 0.f, 0.f, 1.f), vi = pi, ri = make_float4(1.f, 1.f, 0.f, 0.f);
+        if (tvalid) {
+            pi = pos_h[p];
+            vi = vel_m[p];
+            ri = rcak[p];
+        }
+        const float hi = pi.w, ihi = __fdividef(1.0f, hi);
+        const float rho_i = ri.x, c_i = ri.y, A_i = ri.z, K_i = ri.w;
         // scatter neighbours can be as far as 2 h_j: search with the largest h in use
         const float R = 2.0f * fmaxf(hi, hmax_all) * (1.0f + 1e-5f);
         const float hi2x4 = 4.0f * hi * hi;
 
         float acx = 0.0f, acy = 0.0f, acz = 0.0f, du = 0.0f, mumin = 0.0f;
-        int   head = 0, fill = 0;  // ring state (warp-uniform)
 
-        auto process = [&](int k, bool active) {
-            // one pair per lane: ring entry k
-            if (active) {
-                const uint32_t j  = sm.j[k];
-                const float    dx = sm.dx[k], dy = sm.dy[k], dz = sm.dz[k], r2 = sm.r2[k];
-                const float    hj = sm.hj[k];
-                const float4   vj = __ldg(vel_m + j);
-                const float4   rj = __ldg(rcak + j);
-                const float r  = sqrtf(r2);
-                const float ti = fmaxf(1.0f - 0.5f * r * ihi, 0.0f);
-                const float tj = fmaxf(1.0f - 0.5f * __fdividef(r, hj), 0.0f);
-                const float gi = K_i * ti * ti * ti;
-                const float gj = rj.w * tj * tj * tj;
-                const float vdx = vi.x - vj.x, vdy = vi.y - vj.y, vdz = vi.z - vj.z;
-                const float vr = vdx * dx + vdy * dy + vdz * dz;   // v_ij . r_ij
-                float pig = 0.0f;                                   // Pi_ij * gbar
-                if (vr < 0.0f) {
-                    const float hb  = 0.5f * (hi + hj);
-                    const float mu  = hb * vr / (r2 + par.eps * hb * hb);
-                    const float cb  = 0.5f * (c_i + rj.y);
-                    const float rb  = 0.5f * (rho_i + rj.x);
-                    const float Pij = mu * (par.beta * mu - par.alpha * cb) / rb;
-                    pig   = Pij * 0.5f * (gi + gj);
-                    mumin = fminf(mumin, mu);
-                    ++c_av;
-                }
-                const float Ag = A_i * gi;
-                const float ca = vj.w * (Ag + rj.z * gj + pig);
-                acx += ca * dx;
-                acy += ca * dy;
-                acz += ca * dz;
-                du -= vj.w * (Ag + 0.5f * pig) * vr;
+        // one pair: source j at displacement (dx, dy, dz), smoothing length hj
+        auto pair = [&](uint32_t j, float dx, float dy, float dz, float r2, float hj) {
+            const float4 vj = __ldg(vel_m + j);
+            const float4 rj = __ldg(rcak + j);
+            const float r  = r2 * rsqrtf(r2);
+            const float ti = fmaxf(1.0f - 0.5f * r * ihi, 0.0f);
+            const float tj = fmaxf(1.0f - 0.5f * __fdividef(r, hj), 0.0f);
+            const float gi = K_i * ti * ti * ti;
+            const float gj = rj.w * tj * tj * tj;
+            const float vdx = vi.x - vj.x, vdy = vi.y - vj.y, vdz = vi.z - vj.z;
+            const float vr = vdx * dx + vdy * dy + vdz * dz;   // v_ij . r_ij
+            float pig = 0.0f;                                   // Pi_ij * gbar
+            if (vr < 0.0f) {
+                const float hb  = 0.5f * (hi + hj);
+                const float mu  = __fdividef(hb * vr, r2 + par.eps * hb * hb);
+                const float cb  = 0.5f * (c_i + rj.y);
+                const float rb  = 0.5f * (rho_i + rj.x);
+                const float Pij = __fdividef(mu * (par.beta * mu - par.alpha * cb), rb);
+                pig   = Pij * 0.5f * (gi + gj);
+                mumin = fminf(mumin, mu);
+                ++c_av;
             }
+            const float Ag = A_i * gi;
+            const float ca = vj.w * (Ag + rj.z * gj + pig);
+            acx += ca * dx;
+            acy += ca * dy;
+            acz += ca * dz;
+            du -= vj.w * (Ag + 0.5f * pig) * vr;
+            ++c_pairs;
         };
 
-        sph_for_each_row(g, cell_start, pi.x, pi.y, pi.z, R, sm.rows, lane, [&](const RowRec& rr) {
-            for (uint32_t k0 = rr.start; k0 < rr.end; k0 += 32) {
-                const uint32_t j = k0 + lane;
-                const bool     v = j < rr.end;
-                float4 pj = make_float4(3.0e18f, 3.0e18f, 3.0e18f, 0.0f);
-                if (v) pj = __ldg(pos_h + j);
-                const float dx = rr.sx - pj.x, dy = rr.sy - pj.y, dz = rr.sz - pj.z;
-                const float r2 = dx * dx + dy * dy + dz * dz;
-                const float Hm = fmaxf(hi2x4, 4.0f * pj.w * pj.w);
-                const bool  acc = v && (r2 < Hm) && (r2 > 0.0f);
-                const unsigned mk = __ballot_sync(SPH_FULL, acc);
-                if (acc) {
-                    const int slot = (head + fill + __popc(mk & lt)) & (RING - 1);
-                    sm.j[slot]  = j;
-                    sm.dx[slot] = dx;
-                    sm.dy[slot] = dy;
-                    sm.dz[slot] = dz;
-                    sm.r2[slot] = r2;
-                    sm.hj[slot] = pj.w;
-                }
-                fill += __popc(mk);
-                c_tested += min(32u, rr.end - k0);
-                __syncwarp();
-                if (fill >= 32) {
-                    process((head + lane) & (RING - 1), true);
-                    head = (head + 32) & (RING - 1);
-                    fill -= 32;
-                    c_pairs += 32;
-                    __syncwarp();
-                }
+        // ---- phase 1: lane-private index lists
+        int      cnt = 0;
+        unsigned rot = 0;
+        sph_group_rows<F_G>(g, cell_start, pos_h, pi.x, pi.y, pi.z, R, tvalid, lane, rot, c_tested,
+                            [&](uint32_t j, const float4 pj, float sx, float sy, float sz) {
+            const float dx = sx - pj.x, dy = sy - pj.y, dz = sz - pj.z;
+            const float r2 = dx * dx + dy * dy + dz * dz;
+            const float Hm = fmaxf(hi2x4, 4.0f * pj.w * pj.w);
+            if (r2 < Hm && r2 > 0.0f) {
+                if (cnt < F_SLOTS) L.j[cnt][lane] = j;
+                ++cnt;
             }
         });
-        __syncwarp();
-        if (fill > 0) {
-            process((head + lane) & (RING - 1), lane < fill);
-            c_pairs += fill;
+        const bool ovf = sph_group_any<F_G>(cnt > F_SLOTS, lane);
+
+        // ---- phase 2: the pairs of this lane's column
+        const int mycnt  = ovf ? 0 : cnt;
+        const int maxcnt = __reduce_max_sync(SPH_FULL, mycnt);
+        for (int k = 0; k < maxcnt; ++k) {
+            if (k < mycnt) {
+                const uint32_t j  = L.j[k][lane];
+                const float4   pj = __ldg(pos_h + j);
+                float dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;
+                dx -= Lx * rintf(dx * iLx);   // minimum image (no-op on open axes)
+                dy -= Ly * rintf(dy * iLy);
+                dz -= Lz * rintf(dz * iLz);
+                const float r2 = dx * dx + dy * dy + dz * dz;
+                pair(j, dx, dy, dz, r2, pj.w);
+            }
         }
-        acx = sph_warp_sum(acx);
-        acy = sph_warp_sum(acy);
-        acz = sph_warp_sum(acz);
-        du  = sph_warp_sum(du);
-        mumin = sph_warp_min(mumin);
-        if (lane == 0) {
+        // a column overflowed (very crowded neighbourhood): redo the group without lists
+        if (__any_sync(SPH_FULL, ovf)) {
+            sph_group_rows<F_G>(g, cell_start, pos_h, pi.x, pi.y, pi.z, R, tvalid && ovf, lane, rot,
+                                c_tested,
+                                [&](uint32_t j, const float4 pj, float sx, float sy, float sz) {
+                const float dx = sx - pj.x, dy = sy - pj.y, dz = sz - pj.z;
+                const float r2 = dx * dx + dy * dy + dz * dz;
+                const float Hm = fmaxf(hi2x4, 4.0f * pj.w * pj.w);
+                if (r2 < Hm && r2 > 0.0f) pair(j, dx, dy, dz, r2, pj.w);
+            });
+        }
+        acx = sph_group_sum<F_G>(acx);
+        acy = sph_group_sum<F_G>(acy);
+        acz = sph_group_sum<F_G>(acz);
+        du  = sph_group_sum<F_G>(du);
+        mumin = sph_group_min<F_G>(mumin);
+        if (tvalid && (lane & (F_G - 1)) == 0) {
             const int i = perm[p];
             ax[i] = acx; ay[i] = acy; az[i] = acz;
             dudt[i]   = du;
@@ -189,15 +197,15 @@ __global__ __launch_bounds__(F_TPB) void k_forces(int n, const SphGrid* __restri
         __syncwarp();
     }
 
-    c_av = __reduce_add_sync(SPH_FULL, c_av);
-    if (lane == 0) {
-        atomicAdd(&st_sh[0], c_tested);
-        atomicAdd(&st_sh[1], (unsigned long long)c_pairs);
-        atomicAdd(&st_sh[2], (unsigned long long)c_av);
+    unsigned v[3] = {c_tested, c_pairs, c_av};
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        const unsigned t = __reduce_add_sync(SPH_FULL, v[k]);
+        if (lane == 0 && t) atomicAdd(&st_sh[k], t);
     }
     __syncthreads();
-    if (threadIdx.x < 3 && st_sh[threadIdx.x] != 0ull)
-        atomicAdd(stats + ST_FORCE_TESTED + threadIdx.x, st_sh[threadIdx.x]);
+    if (threadIdx.x < 3 && st_sh[threadIdx.x] != 0u)
+        atomicAdd(stats + ST_FORCE_TESTED + threadIdx.x, (unsigned long long)st_sh[threadIdx.x]);
 }
 
 }  // namespace

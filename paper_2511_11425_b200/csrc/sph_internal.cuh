@@ -75,6 +75,12 @@ struct sph_ctx {
 #ifdef __CUDACC__
 
 #define SPH_FULL 0xffffffffu
+#ifndef SPH_UNROLL
+#define SPH_UNROLL 1   // candidate windows loaded ahead per lane
+#endif
+#ifndef SPH_MINB
+#define SPH_MINB 8     // resident blocks per SM the sweeps are compiled for
+#endif
 
 // Wendland C2, support 2h: w(q) = SIGMA (1-q/2)^4 (1+2q); (32 pi/3) SIGMA = 14.
 #define SPH_SIGMA 0.41778172561566733f   /* 21/(16 pi) */
@@ -200,6 +206,136 @@ __device__ __forceinline__ void sph_for_each_row(const SphGrid& g,
         }
         __syncwarp();
     }
+}
+
+// ---------------------------------------------------------------------------------------
+// Sub-warp enumeration: the warp holds 32/G targets, G consecutive lanes each.  All loops
+// have warp-uniform trip counts (maxima over the groups), groups that have nothing to do
+// are predicated off, so the warp never splits.
+// ---------------------------------------------------------------------------------------
+__device__ __forceinline__ int sph_wrap(int u, int n, int& k) {   // u = c + k n, 0 <= c < n
+    if (n >= 8) k = (u < 0) ? -1 : ((u >= n) ? 1 : 0);
+    else        k = sph_fdiv(u, n);
+    int c = u - k * n;
+    return min(max(c, 0), n - 1);   // memory-safe even for coordinates outside a periodic box
+}
+
+// Calls test(j, pj, sx, sy, sz) on ONE lane for every candidate source j of that lane's
+// target: pj = pos[j], and d = (sx - pj.x, sy - pj.y, sz - pj.z) is the displacement to the
+// right periodic image.  `active` (uniform in a group) switches a group off.  `rot`
+// (uniform in a group) rotates the lane a row starts on, so that candidates -- and with them
+// the lane-private lists built from them -- spread evenly over the G lanes.  `tested` is
+// advanced by the number of candidates on the group's first lane.
+template <int G, class Test>
+__device__ __forceinline__ void sph_group_rows(const SphGrid& g,
+                                               const uint32_t* __restrict__ cell_start,
+                                               const float4* __restrict__ pos, float xi, float yi,
+                                               float zi, float R, bool active, int lane,
+                                               unsigned& rot, unsigned& tested, Test&& test) {
+    constexpr unsigned GM = (G == 32) ? 0xffffffffu : ((1u << G) - 1u);
+    const int sl = lane & (G - 1);
+    const int g0 = lane & ~(G - 1);
+    int x0, x1, y0, y1, z0, z1;
+    sph_axis_range(xi, R, g.lo[0], g.isx, g.nx, g.per[0], x0, x1);
+    sph_axis_range(yi, R, g.lo[1], g.isy, g.ny, g.per[1], y0, y1);
+    sph_axis_range(zi, R, g.lo[2], g.isz, g.nz, g.per[2], z0, z1);
+    int         kx0;
+    const int   c0   = sph_wrap(x0, g.nx, kx0);
+    const int   span = x1 - x0;
+    const int   a_c1 = min(c0 + span, g.nx - 1);
+    const bool  two  = (c0 + span > g.nx - 1);
+    const int   b_c1 = min(c0 + span - g.nx, g.nx - 1);
+    const float sxA  = xi - (float)kx0 * g.len[0];
+    const float sxB  = xi - (float)(kx0 + 1) * g.len[0];
+    const int   nyr  = y1 - y0 + 1, nzr = z1 - z0 + 1;
+    const int   nrow = active ? nyr * nzr : 0;
+    const float inv_nyr = __fdividef(1.0f, (float)nyr);
+    const float R2   = R * R * (1.0f + 1e-5f);
+    const int   nrow_max = __reduce_max_sync(SPH_FULL, nrow);
+
+    for (int rb = 0; rb < nrow_max; rb += G) {
+        const int r  = rb + sl;
+        bool      ok = r < nrow;
+        const int iz = (int)(((float)r + 0.5f) * inv_nyr), iy = r - iz * nyr;
+        const int uy = y0 + iy, uz = z0 + iz;
+        uint32_t  a0 = 0, a1 = 0, b0 = 0, b1 = 0;
+        float     sy = yi, sz = zi;
+        if (ok) {
+            const float dy = sph_slab_dist(yi, uy, g.lo[1], g.sy, g.ny, g.per[1]);
+            const float dz = sph_slab_dist(zi, uz, g.lo[2], g.sz, g.nz, g.per[2]);
+            ok = (dy * dy + dz * dz <= R2);
+        }
+        if (ok) {
+            int ky, kz;
+            const int cy = sph_wrap(uy, g.ny, ky), cz = sph_wrap(uz, g.nz, kz);
+            sy = yi - (float)ky * g.len[1];
+            sz = zi - (float)kz * g.len[2];
+            const uint32_t rq = (uint32_t)(cz * g.ny + cy) * (uint32_t)g.nx;
+            a0 = __ldg(cell_start + rq + c0);
+            a1 = __ldg(cell_start + rq + a_c1 + 1);
+            if (two) {
+                b0 = __ldg(cell_start + rq);
+                b1 = __ldg(cell_start + rq + b_c1 + 1);
+            }
+        }
+        const int nseg = __any_sync(SPH_FULL, b1 > b0) ? 2 : 1;
+        for (int seg = 0; seg < nseg; ++seg) {
+            const uint32_t s0 = seg ? b0 : a0, s1 = seg ? b1 : a1;
+            const float    sxx = seg ? sxB : sxA;
+            unsigned gm = (__ballot_sync(SPH_FULL, s1 > s0) >> g0) & GM;
+            const int nk = __reduce_max_sync(SPH_FULL, __popc(gm));
+            for (int k = 0; k < nk; ++k) {
+                const bool have = gm != 0u;
+                const int  src  = g0 + (have ? (__ffs(gm) - 1) : 0);
+                gm &= gm - 1u;
+                uint32_t       rs  = __shfl_sync(SPH_FULL, s0, src);
+                uint32_t       re  = __shfl_sync(SPH_FULL, s1, src);
+                const float    rsy = __shfl_sync(SPH_FULL, sy, src);
+                const float    rsz = __shfl_sync(SPH_FULL, sz, src);
+                if (!have) re = rs;
+                uint32_t c = rs + ((sl - rot) & (G - 1));
+                rot = (rot + (re - rs)) & (G - 1);
+                if (sl == 0) tested += re - rs;
+                do {   // SPH_UNROLL windows per trip: as many independent loads in flight
+                    bool   vv[SPH_UNROLL];
+                    float4 pp[SPH_UNROLL];
+#pragma unroll
+                    for (int u = 0; u < SPH_UNROLL; ++u) {
+                        vv[u] = c + u * G < re;
+                        if (vv[u]) pp[u] = __ldg(pos + c + u * G);
+                    }
+#pragma unroll
+                    for (int u = 0; u < SPH_UNROLL; ++u)
+                        if (vv[u]) test(c + u * G, pp[u], sxx, rsy, rsz);
+                    c += SPH_UNROLL * G;
+                } while (__any_sync(SPH_FULL, c < re));
+            }
+        }
+    }
+}
+
+template <int G>
+__device__ __forceinline__ float sph_group_sum(float v) {
+#pragma unroll
+    for (int o = G / 2; o > 0; o >>= 1) v += __shfl_xor_sync(SPH_FULL, v, o);
+    return v;
+}
+template <int G>
+__device__ __forceinline__ float sph_group_min(float v) {
+#pragma unroll
+    for (int o = G / 2; o > 0; o >>= 1) v = fminf(v, __shfl_xor_sync(SPH_FULL, v, o));
+    return v;
+}
+template <int G>
+__device__ __forceinline__ int sph_group_sum_int(int v) {
+#pragma unroll
+    for (int o = G / 2; o > 0; o >>= 1) v += __shfl_xor_sync(SPH_FULL, v, o);
+    return v;
+}
+template <int G>
+__device__ __forceinline__ bool sph_group_any(bool p, int lane) {
+    constexpr unsigned GM = (G == 32) ? 0xffffffffu : ((1u << G) - 1u);
+    return ((__ballot_sync(SPH_FULL, p) >> (lane & ~(G - 1))) & GM) != 0u;
 }
 
 // Exact (FP64) squared distance of two particles under the minimum-image convention,

@@ -13,7 +13,7 @@ from dataclasses import dataclass, field
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libsph_b200.so")
+LIB_PATH = os.environ.get("SPH_B200_LIB") or os.path.join(_HERE, "libsph_b200.so")
 
 SPH_OK, SPH_EINVAL, SPH_EBOX, SPH_ENOMEM, SPH_ECUDA, SPH_ESTALE, SPH_ENOSPC = 0, -1, -2, -3, -4, -5, -6
 
