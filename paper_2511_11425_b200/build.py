@@ -61,7 +61,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     with ThreadPoolExecutor(max_workers=len(SOURCES)) as ex:
         objs = list(ex.map(one, SOURCES))
     tmp = LIB + f".{os.getpid()}.tmp"
-    subprocess.check_call([nvcc, "-shared", "-o", tmp, *objs, "-lcudart"])
+    subprocess.check_call([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", tmp,
+                           *objs, "-lcudart"])
     os.replace(tmp, LIB)
     return LIB
 

@@ -166,3 +166,124 @@ def test_c1_zero_jitter_lattice_values(gu):
     assert np.abs(gu.np64(rho) / 1.014620121305 - 1).max() <= TOL_H
     assert np.abs(gu.np64(om) / 0.966619609416 - 1).max() <= TOL_H
     assert (nn == 81).all()
+
+
+# ------------------------------------------------------------------------------------------
+# Larger configurations: the oracle's cell-list variant (pinned against the brute force in
+# tests/test_oracle_pins.py) for every particle, the brute force itself on a seeded sample.
+# ------------------------------------------------------------------------------------------
+def _sample(n, k, seed):
+    return np.sort(np.random.default_rng(seed).choice(n, size=k, replace=False))
+
+
+def _full_step(gu, w, **kw):
+    from paper_2511_11425_b200 import sph
+    d = gu.to_device(w)
+    ctx = gu.make_ctx(w, **kw)
+    out = sph.StepBuffers(int(w["n"]))
+    h = d["h"].clone()
+    sph.step(ctx, d, out, h)
+    torch.cuda.synchronize()
+    return ctx, d, out, h
+
+
+def _check_sample(gu, w, ctx, out, h, sel, op, ob):
+    """Brute-force oracle on the targets `sel` against ALL particles."""
+    oh, orho, oom, _ = orc.density(w["x"], w["y"], w["z"], w["m"], w["h"], ob, op, targets=sel)
+    assert _rel(gu.np64(h)[sel], oh).max() <= TOL_H
+    assert _rel(gu.np64(out["rho"])[sel], orho).max() <= TOL_H
+    assert _rel(gu.np64(out["omega"])[sel], oom).max() <= TOL_H
+    hg = h.cpu().numpy()
+    _, _, onn, _ = orc.density_at_h(w["x"], w["y"], w["z"], w["m"], hg, ob, op, targets=sel)
+    assert np.array_equal(out["n_ngb"].cpu().numpy()[sel], onn)
+    # forces, stage-isolated at full size: the device's own rho, h, Omega into the oracle
+    rg, og = out["rho"].cpu().numpy(), out["omega"].cpu().numpy()
+    o = orc.forces(w["x"], w["y"], w["z"], w["m"], w["vx"], w["vy"], w["vz"], w["u"], rg, hg, og,
+                   ob, op, targets=sel)
+    ea, eu = gu.force_errors(out.t, o, sel)
+    assert ea.max() <= TOL_F, ea.max()
+    assert eu.max() <= TOL_F, eu.max()
+    scale = max(np.abs(o["mu_min"]).max(), 1e-300)
+    assert np.abs(gu.np64(out["mu_min"])[sel] - o["mu_min"]).max() <= 1e-5 * scale
+    # time step, stage-isolated
+    odti, _ = orc.timestep(hg, out["c"].cpu().numpy(), out["ax"].cpu().numpy(),
+                           out["ay"].cpu().numpy(), out["az"].cpu().numpy(),
+                           out["mu_min"].cpu().numpy(), op)
+    assert _rel(gu.np64(out["dt_i"]), odti).max() <= TOL_DT
+    assert abs(float(out["dt_min"].item()) - odti.min()) <= TOL_DT * odti.min()
+
+
+def test_c2_sod_tube_variable_h(gu):
+    """Config 2: 8:1 density jump, h differs by 2x across the interface, so the scatter half
+    of the force pair set and the variable reach of the search are exercised."""
+    w = workloads.sod_tube(h_start="warm")
+    _, op = gu.make_params(w)
+    _, ob = gu.make_boxes(w)
+    ctx, d, out, h = _full_step(gu, w)
+    st = ctx.stats()
+    assert st["dens_nonconv"] == 0 and st["grid_flags"] & 1 == 0, st
+    # every particle against the cell-list oracle
+    oh, orho, oom, onn = orc.density(w["x"], w["y"], w["z"], w["m"], w["h"], ob, op, cells=True)
+    assert _rel(gu.np64(h), oh).max() <= TOL_H
+    assert _rel(gu.np64(out["rho"]), orho).max() <= TOL_H
+    assert _rel(gu.np64(out["omega"]), oom).max() <= TOL_H
+    o = orc.forces(w["x"], w["y"], w["z"], w["m"], w["vx"], w["vy"], w["vz"], w["u"], orho, oh, oom,
+                   ob, op, cells=True)
+    ea, eu = gu.force_errors(out.t, o)
+    assert ea.max() <= TOL_F, ea.max()
+    assert eu.max() <= TOL_F, eu.max()
+    assert abs(st["force_pairs"] - int(o["n_pairs"].sum())) <= 1e-6 * o["n_pairs"].sum()
+    # a sample straddling the interface against the brute force
+    near = np.flatnonzero(np.abs(w["x"] - 0.5) < 0.03)
+    sel = np.sort(np.concatenate([_sample(w["n"], 192, 21), near[_sample(len(near), 192, 22)]]))
+    _check_sample(gu, w, ctx, out, h, np.unique(sel), op, ob)
+    # neighbour lists at the device's h, gather-or-scatter mode, on the interface sample
+    off, idx = ctx.neighbors(h, 1)
+    off, idx = off.cpu().numpy(), idx.cpu().numpy()
+    selu = np.unique(sel)
+    ooff, oidx = orc.neighbors(w["x"], w["y"], w["z"], h.cpu().numpy(), ob, 1, targets=selu)
+    for k, i in enumerate(selu):
+        assert np.array_equal(np.sort(idx[off[i]:off[i + 1]]), oidx[ooff[k]:ooff[k + 1]]), i
+
+
+def test_c3_sedov_full_size_sampled(gu):
+    """Config 3 at BASELINE.json's full size (128^3 = 2 097 152 particles), in the launch
+    configuration bench.py times; 256 seeded targets plus the 64 particles nearest the blast
+    centre (where u varies by 10 orders of magnitude) against the brute-force oracle."""
+    w = workloads.sedov(nside=128, h_start="warm")
+    _, op = gu.make_params(w)
+    _, ob = gu.make_boxes(w)
+    ctx, d, out, h = _full_step(gu, w)
+    st = ctx.stats()
+    assert st["dens_nonconv"] == 0 and st["dens_overflow"] == 0, st
+    r2c = (w["x"] - 0.5) ** 2 + (w["y"] - 0.5) ** 2 + (w["z"] - 0.5) ** 2
+    sel = np.unique(np.concatenate([_sample(w["n"], 256, 31), np.argsort(r2c)[:64]]))
+    _check_sample(gu, w, ctx, out, h, sel, op, ob)
+    # properties that hold at any size
+    assert int(out["n_ngb"].sum().item()) == st["dens_pairs"]
+    m = w["m"].astype(np.float64)
+    a = np.stack([gu.np64(out[k]) for k in ("ax", "ay", "az")])
+    assert np.abs((m * a).sum(axis=1)).max() <= 1e-5 * (m * np.linalg.norm(a, axis=0)).sum()
+    assert torch.isfinite(out["dudt"]).all() and (out["dt_i"] > 0).all()
+
+
+def test_edge_cases_small_and_open_box(gu):
+    """n not a multiple of the 32 targets per block, an open (non-periodic) box with free
+    surfaces, unequal masses, particles outside the nominal box."""
+    rng = np.random.default_rng(41)
+    n = 1000 + 7
+    w = dict(x=rng.uniform(-0.1, 1.1, n), y=rng.uniform(0, 1, n), z=rng.uniform(0, 1, n),
+             m=rng.uniform(0.5, 1.5, n) / n, vx=rng.normal(0, 0.1, n), vy=rng.normal(0, 0.1, n),
+             vz=rng.normal(0, 0.1, n), u=rng.uniform(0.5, 2.0, n), h=np.full(n, 0.2), n=n,
+             box_lo=(0.0, 0.0, 0.0), box_len=(1.0, 1.0, 1.0), periodic=(0, 0, 0),
+             gamma=1.4, av_alpha=1.5, av_beta=3.0)
+    for k in gu.F_KEYS:
+        w[k] = np.ascontiguousarray(w[k], np.float32)
+    _, op = gu.make_params(w)
+    _, ob = gu.make_boxes(w)
+    ctx, d, out, h = _full_step(gu, w)
+    assert ctx.stats()["dens_nonconv"] == 0
+    _check_sample(gu, w, ctx, out, h, np.arange(n), op, ob)
+    off, idx = ctx.neighbors(h, 0)
+    ooff, oidx = orc.neighbors(w["x"], w["y"], w["z"], h.cpu().numpy(), ob, 0)
+    assert np.array_equal(off.cpu().numpy(), ooff)
