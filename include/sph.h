@@ -74,7 +74,8 @@ typedef struct {
     int64_t dens_pairs;       /* sum_i n_i at the final h (self included)                  */
     int64_t dens_sweeps;      /* Newton sweeps summed over particles                       */
     int64_t dens_recollect;   /* targets whose search ball had to be rebuilt larger        */
-    int64_t dens_overflow;    /* targets that fell back to the streaming (list-free) path  */
+    int64_t dens_overflow;    /* targets finished by the robust list-free kernel (a list   */
+                              /* column overflowed, or an entry sat in the FP64 band)      */
     int64_t dens_nonconv;     /* particles not converged within h_max_iter                 */
     int64_t dens_recheck;     /* borderline pairs re-evaluated in FP64                     */
     int64_t force_tested;     /* candidate pairs distance-tested by sph_forces             */

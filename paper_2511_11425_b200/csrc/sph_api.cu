@@ -64,6 +64,9 @@ extern "C" int sph_create(sph_ctx** out, const sph_params* params, const sph_box
     ok = ok && dalloc(&c->vel_m, (size_t)n_max) == cudaSuccess;
     ok = ok && dalloc(&c->rcak, (size_t)n_max) == cudaSuccess;
     ok = ok && dalloc(&c->stats, (size_t)ST_NCOUNTERS) == cudaSuccess;
+    ok = ok && dalloc(&c->coarse_hmax, (size_t)SPH_COARSE_MAX) == cudaSuccess;
+    ok = ok && dalloc(&c->fix_list, (size_t)n_max) == cudaSuccess;
+    ok = ok && dalloc(&c->fix_cnt, (size_t)2) == cudaSuccess;
     ok = ok && dalloc(&c->dt_part, (size_t)1024) == cudaSuccess;
     ok = ok && dalloc(&c->nb_total, (size_t)2) == cudaSuccess;
     if (ok) ok = cudaMemsetAsync(c->stats, 0, ST_NCOUNTERS * sizeof(unsigned long long),
@@ -86,7 +89,8 @@ extern "C" void sph_destroy(sph_ctx* c) {
     cudaFree(c->perm);      cudaFree(c->inv_perm);  cudaFree(c->scan_part);
     cudaFree(c->pos_h);     cudaFree(c->pos_m);     cudaFree(c->vel_m);
     cudaFree(c->rcak);      cudaFree(c->stats);     cudaFree(c->dt_part);
-    cudaFree(c->nb_total);
+    cudaFree(c->nb_total);  cudaFree(c->fix_list);  cudaFree(c->fix_cnt);
+    cudaFree(c->coarse_hmax);
     delete c;
 }
 

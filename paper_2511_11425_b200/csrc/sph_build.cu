@@ -94,6 +94,19 @@ __global__ void k_grid_setup(SphGrid* g, const unsigned* red, sph_box box, float
     }
     g->hmin = hmin; g->hmax = hmax; g->xext = ext; g->flags = flags;
     g->force_hmax_bits = 0u;
+    // coarse max-h map: cells of about 8 h_min, at most SPH_COARSE_MAX of them
+    float cs = 8.0f * hmin * slack;
+    for (int it = 0; it < 64; ++it) {
+        double prod = 1.0;
+        for (int d = 0; d < 3; ++d) {
+            float fn = fminf(fmaxf(box.len[d] / cs, 1.0f), 1.0e6f);
+            g->cn[d] = max((int)floorf(fn), 1);
+            prod *= (double)g->cn[d];
+        }
+        if (prod <= (double)SPH_COARSE_MAX) break;
+        cs *= (float)fmax(cbrt(prod / (double)SPH_COARSE_MAX) * 1.02, 1.05);
+    }
+    for (int d = 0; d < 3; ++d) g->ics[d] = (float)g->cn[d] / box.len[d];
 }
 
 __global__ void k_zero_cells(const SphGrid* __restrict__ g, uint32_t* cnt) {

@@ -5,7 +5,10 @@
 // candidate rows of the cell grid (coalesced float4 loads), every lane keeps the candidates
 // it accepted in a private column of a shared-memory list (r, m) -- the paper's "we keep the
 // precomputed interaction list", built for a "slightly larger kernel" -- and
-// the root of Eq. (6) is then found on that list alone.
+// the root of Eq. (6) is then found on that list alone.  Targets the lean kernel cannot
+// finish (a list column overflows, an entry sits in the FP32-uncertain band around 2h, the
+// iteration does not converge) are queued for k_density_fix, which re-walks the rows in
+// every sweep with one warp per target and decides borderline neighbours in FP64.
 //
 // With w(q) = SIGMA wt(q), wt = (1-q/2)^4 (1+2q), t = 1-q/2, and per target
 //   S = sum_j m_j wt(q_j),  E = sum_j m_j 5 q^2 t^3,  F = sum_j m_j q^2 t^2 (10 t - 7.5 q):
@@ -26,8 +29,8 @@ constexpr int   D_G      = 8;             // lanes per target
 constexpr int   D_NT     = 32 / D_G;      // targets per warp
 constexpr int   D_WARPS  = 4;
 constexpr int   D_TPB    = D_WARPS * 32;
-constexpr int   D_ROUNDS = 2;             // target quads per warp
-constexpr int   D_TARGETS = D_WARPS * D_NT * D_ROUNDS;
+constexpr int   D_QUADS  = 16;            // target quads per block, handed out dynamically
+constexpr int   D_TARGETS = D_NT * D_QUADS;
 constexpr int   D_SLOTS  = 28;            // list entries per lane
 constexpr float D_ACCEPT = 3.0e-4f;
 
@@ -51,38 +54,76 @@ __global__ void k_pack_pos_m(int64_t n, const float4* __restrict__ pos_h,
     pos_m[p] = a;
 }
 
-__global__ __launch_bounds__(D_TPB, SPH_MINB) void k_density(int n, const SphGrid* __restrict__ gp,
-                                                      const uint32_t* __restrict__ cell_start,
-                                                      const float4* __restrict__ pos_m,
-                                                      const int32_t* __restrict__ perm,
-                                                      DensPar par, float* h_io, float* rho,
-                                                      float* omega, int32_t* nn,
-                                                      unsigned long long* stats) {
-    __shared__ WarpList lists[D_WARPS];
-    __shared__ SphGrid g;
-    __shared__ unsigned st_sh[8];
-    if (threadIdx.x < sizeof(SphGrid) / 4)
-        ((int*)&g)[threadIdx.x] = ((const int*)gp)[threadIdx.x];
-    if (threadIdx.x < 8) st_sh[threadIdx.x] = 0u;
-    __syncthreads();
-
-    const int   wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int   gq  = lane / D_G;
-    WarpList&   L   = lists[wid];
+// One safeguarded Halley step from the sums at h.  Returns true if the step is accepted as
+// final; hn is the next iterate either way, Sn / En the sums carried to hn.
+__device__ __forceinline__ bool halley_step(float s, float e, float f2, float T, float h, float ih,
+                                            float hcap, float tol, float& hlo, float& hhi,
+                                            float& hn, float& Sn, float& En, bool& conv) {
     const float INF = __int_as_float(0x7f800000);
+    const float f = s - T;
+    if (f < 0.0f) hlo = h; else hhi = h;
+    const float den = 2.0f * e * e + f * (e + f2);
+    float dh;
+    bool  genuine = true;
+    if (e > 0.0f && den > 0.0f)  dh = __fdividef(-2.0f * f * e * h, den);
+    else if (e > 0.0f)           dh = __fdividef(-f * h, e);
+    else                       { dh = h; genuine = false; }
+    hn = h + dh;
+    if (!(hn >= 0.5f * h)) { hn = 0.5f * h; genuine = false; }
+    if (!(hn <= 2.0f * h)) { hn = 2.0f * h; genuine = false; }
+    if (hhi < INF && !(hn >= hlo && hn <= hhi)) { hn = 0.5f * (hlo + hhi); genuine = false; }
+    if (hn > hcap) { hn = hcap; genuine = false; }
+    dh = hn - h;
+    const float x = dh * ih;
+    Sn = s + x * (e - 0.5f * x * (e + f2));   // Taylor: S' = E/h, S'' = -(E+F)/h^2
+    En = e - x * f2;                          //         E' = -F/h
+    const bool small  = fabsf(dh) <= D_ACCEPT * h;
+    const bool tight  = (hhi - hlo) <= tol * h;      // bracket closed to the tolerance
+    const bool capped = (hn >= hcap && h >= hcap);
+    conv = !(capped && f < 0.0f);
+    return (genuine && small) || tight || capped;
+}
 
-    // largest h the search may use: keeps 2 h slack below half the shortest periodic side
+__device__ __forceinline__ float density_hcap(const SphGrid& g) {
+    // largest h the search may use: keeps 2 h x 1.25 below half the shortest periodic side
     float hcap = 3.0e37f;
     for (int d = 0; d < 3; ++d)
         if (g.per[d]) hcap = fminf(hcap, g.len[d] / (4.0f * 1.25f) * 0.999f);
         else          hcap = fminf(hcap, 4.0f * fmaxf(g.len[0], fmaxf(g.len[1], g.len[2])));
-    const float band_c = 2.5e-7f * g.xext;   // sph_band(h) = 1e-6 + band_c / h
+    return hcap;
+}
 
-    unsigned c_tested = 0, c_listed = 0, c_pairs = 0, c_sweeps = 0;
-    unsigned c_recollect = 0, c_overflow = 0, c_nonconv = 0, c_recheck = 0;
+__global__ __launch_bounds__(D_TPB, SPH_MINB) void k_density(
+    int n, const SphGrid* __restrict__ gp, const uint32_t* __restrict__ cell_start,
+    const float4* __restrict__ pos_m, const int32_t* __restrict__ perm, DensPar par, float* h_io,
+    float* rho, float* omega, int32_t* nn, int32_t* fix_list, unsigned* fix_cnt,
+    unsigned long long* stats) {
+    __shared__ WarpList lists[D_WARPS];
+    __shared__ SphGrid  g;
+    __shared__ unsigned st_sh[5];
+    __shared__ int      next_quad;
+    if (threadIdx.x < sizeof(SphGrid) / 4)
+        ((int*)&g)[threadIdx.x] = ((const int*)gp)[threadIdx.x];
+    if (threadIdx.x < 5) st_sh[threadIdx.x] = 0u;
+    if (threadIdx.x == 0) next_quad = 0;
+    __syncthreads();
 
-    for (int round = 0; round < D_ROUNDS; ++round) {
-        const int  p      = (blockIdx.x * D_ROUNDS + round) * (D_WARPS * D_NT) + wid * D_NT + gq;
+    const int   wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int   gq  = lane / D_G;
+    const bool  leader = (lane & (D_G - 1)) == 0;
+    float* const lr = &lists[wid].r[0][lane];   // this lane's column, slot stride 32 floats
+    float* const lm = &lists[wid].m[0][lane];
+    const float hcap   = density_hcap(g);
+    const float band_c = 2.5e-7f * g.xext;      // sph_band(h) = 1e-6 + band_c / h
+
+    unsigned c_tested = 0, c_listed = 0, c_pairs = 0, c_sweeps = 0, c_recollect = 0;
+
+    for (;;) {
+        int quad = 0;
+        if (lane == 0) quad = atomicAdd(&next_quad, 1);
+        quad = __shfl_sync(SPH_FULL, quad, 0);
+        if (quad >= D_QUADS) break;
+        const int  p      = (blockIdx.x * D_QUADS + quad) * D_NT + gq;
         const bool tvalid = p < n;
         float4 pi = make_float4(0.f, 0.f, 0.f, 1.f);
         int    i  = 0;
@@ -95,12 +136,11 @@ __global__ __launch_bounds__(D_TPB, SPH_MINB) void k_density(int n, const SphGri
         if (!(h > 0.0f) || !(h < 3.0e38f)) h = g.hmin;
         h = fminf(h, hcap);
         const float T = par.n_ngb * pi.w * (1.0f / 14.0f);
-        float    hlo = 0.0f, hhi = INF;
+        float    hlo = 0.0f, hhi = __int_as_float(0x7f800000);
         float    Rc = 0.0f;         // radius the list is complete for
         int      cnt = 0;           // entries in this lane's column
         unsigned rot = 0;
-        bool     stream = false;    // list overflowed: evaluate by re-enumeration
-        bool     first = true, done = !tvalid, conv = false;
+        bool     first = true, done = !tvalid, fix = false;
         float    S = 0.0f, E = 0.0f;
         int      sweeps = 0;
 
@@ -108,46 +148,41 @@ __global__ __launch_bounds__(D_TPB, SPH_MINB) void k_density(int n, const SphGri
             const float ih  = __fdividef(1.0f, h);
             const float tau = 1e-6f + band_c * ih;
             // ---- (re)build the lists of the groups whose ball outgrew them
-            const bool need = !done && !stream && (2.0f * h * (1.0f + 2.0f * tau) > Rc);
+            const bool need = !done && (2.0f * h * (1.0f + 2.0f * tau) > Rc);
             if (__any_sync(SPH_FULL, need)) {
                 if (need) {
                     Rc = 2.0f * h * (first ? par.slack : fmaxf(par.slack, 1.25f));
-                    if (!first && (lane & (D_G - 1)) == 0) ++c_recollect;
+                    if (!first && leader) ++c_recollect;
                     first = false;
                     cnt   = 0;
                 }
                 const float Rc2 = Rc * Rc;
-                sph_group_rows<D_G>(g, cell_start, pos_m, pi.x, pi.y, pi.z, Rc, need, lane, rot, c_tested,
+                sph_group_rows<D_G>(g, cell_start, pos_m, pi.x, pi.y, pi.z, Rc, need, lane, rot,
+                                    c_tested,
                                     [&](uint32_t j, const float4 pj, float sx, float sy, float sz) {
                     const float dx = sx - pj.x, dy = sy - pj.y, dz = sz - pj.z;
                     const float r2 = dx * dx + dy * dy + dz * dz;
                     if (r2 < Rc2) {
                         if (cnt < D_SLOTS) {
-                            L.r[cnt][lane] = r2 * rsqrtf(fmaxf(r2, 1e-35f));
-                            L.m[cnt][lane] = pj.w;
+                            lr[cnt * 32] = r2 * rsqrtf(fmaxf(r2, 1e-35f));
+                            lm[cnt * 32] = pj.w;
                         }
                         ++cnt;
                     }
                 });
-                const bool ovf = sph_group_any<D_G>(need && cnt > D_SLOTS, lane);
-                if (need) {
-                    if (ovf) {
-                        stream = true;
-                        if ((lane & (D_G - 1)) == 0) ++c_overflow;
-                    } else {
-                        c_listed += cnt;
-                    }
+                if (sph_group_any<D_G>(need && cnt > D_SLOTS, lane) && need) {
+                    done = true;     // a column overflowed: leave the target to k_density_fix
+                    fix  = true;
                 }
             }
-            // ---- one sweep: S(h), E(h), F(h)
+            // ---- one sweep over the lists: S(h), E(h), F(h)
             float s = 0.0f, e = 0.0f, f2 = 0.0f;
-            const bool use_list = !done && !stream;
-            const int  mycnt    = use_list ? cnt : 0;
-            const int  maxcnt   = __reduce_max_sync(SPH_FULL, mycnt);
+            const int mycnt  = done ? 0 : cnt;
+            const int maxcnt = __reduce_max_sync(SPH_FULL, mycnt);
             for (int k = 0; k < maxcnt; ++k) {
                 if (k < mycnt) {
-                    const float q  = L.r[k][lane] * ih;
-                    const float mj = L.m[k][lane];
+                    const float q  = lr[k * 32] * ih;
+                    const float mj = lm[k * 32];
                     const float tt = fmaxf(1.0f - 0.5f * q, 0.0f);
                     const float t2 = tt * tt, q2 = q * q;
                     s  += mj * (t2 * t2 * (1.0f + 2.0f * q));
@@ -155,125 +190,178 @@ __global__ __launch_bounds__(D_TPB, SPH_MINB) void k_density(int n, const SphGri
                     f2 += mj * (q2 * t2 * (10.0f * tt - 7.5f * q));
                 }
             }
-            const bool sgroup = stream && !done;
-            if (__any_sync(SPH_FULL, sgroup)) {
-                const float H2 = 4.0f * h * h;
-                sph_group_rows<D_G>(g, cell_start, pos_m, pi.x, pi.y, pi.z, 2.0f * h, sgroup, lane,
-                                    rot, c_tested,
-                                    [&](uint32_t j, const float4 pj, float sx, float sy, float sz) {
-                    const float dx = sx - pj.x, dy = sy - pj.y, dz = sz - pj.z;
-                    const float r2 = dx * dx + dy * dy + dz * dz;
-                    if (r2 < H2) {
-                        const float q  = r2 * rsqrtf(fmaxf(r2, 1e-35f)) * ih;
-                        const float tt = fmaxf(1.0f - 0.5f * q, 0.0f);
-                        const float t2 = tt * tt, q2 = q * q;
-                        s  += pj.w * (t2 * t2 * (1.0f + 2.0f * q));
-                        e  += pj.w * (5.0f * q2 * t2 * tt);
-                        f2 += pj.w * (q2 * t2 * (10.0f * tt - 7.5f * q));
-                    }
-                });
-            }
             s  = sph_group_sum<D_G>(s);
             e  = sph_group_sum<D_G>(e);
             f2 = sph_group_sum<D_G>(f2);
             if (done) continue;
             ++sweeps;
-            // ---- safeguarded Halley step
-            const float f = s - T;
-            if (f < 0.0f) hlo = h; else hhi = h;
-            const float den = 2.0f * e * e + f * (e + f2);
-            float dh;
-            bool  genuine = true;
-            if (e > 0.0f && den > 0.0f)  dh = -2.0f * f * e * h / den;
-            else if (e > 0.0f)           dh = -f * h / e;
-            else                       { dh = h; genuine = false; }
-            float hn = h + dh;
-            if (!(hn >= 0.5f * h)) { hn = 0.5f * h; genuine = false; }
-            if (!(hn <= 2.0f * h)) { hn = 2.0f * h; genuine = false; }
-            if (hhi < INF && !(hn >= hlo && hn <= hhi)) { hn = 0.5f * (hlo + hhi); genuine = false; }
-            if (hn > hcap) { hn = hcap; genuine = false; }
-            dh = hn - h;
-            const bool small = fabsf(dh) <= D_ACCEPT * h;
-            const bool tight = (hhi - hlo) <= par.tol * h;   // bracket closed to the tolerance
-            if ((genuine && small) || tight || (hn >= hcap && h >= hcap)) {
-                // carry S and E to hn; the list must cover the ball of hn (+ band) as well
-                const float x = dh * ih;
-                const float Sn = s + x * (e - 0.5f * x * (e + f2));
-                const float En = e - x * f2;
-                if (stream || 2.0f * hn * (1.0f + 2.0f * (1e-6f + band_c / hn)) <= Rc) {
-                    S = Sn; E = En; h = hn;
-                    done = true;
-                    conv = !(hn >= hcap && f < 0.0f);
-                    continue;
-                }
-            }
-            if (sweeps >= par.max_iter) {
-                S = s; E = e;
+            float hn, Sn, En;
+            bool  conv;
+            const bool acc = halley_step(s, e, f2, T, h, ih, hcap, par.tol, hlo, hhi, hn, Sn, En, conv);
+            if (acc && 2.0f * hn * (1.0f + 2.0f * (1e-6f + band_c * __fdividef(1.0f, hn))) <= Rc) {
+                S = Sn; E = En; h = hn;   // the list covers the ball of hn (+ band) as well
                 done = true;
+                fix  = !conv;
                 continue;
             }
             h = hn;
-        }
-        if (tvalid && (lane & (D_G - 1)) == 0) {
-            if (!conv) ++c_nonconv;
-            c_sweeps += sweeps;
+            if (sweeps >= par.max_iter) { done = true; fix = true; }
         }
 
-        // ---- n_i = #{j : r_ij < 2h}.  From the list; if an entry sits in the FP32-uncertain
-        // band around 2h (or there is no list), recount with the FP64 test on the candidates.
-        const float  H   = 2.0f * h;
-        const float  tau = 1e-6f + band_c / h;
+        // ---- n_i = #{j : r_ij < 2h} from the list; an entry inside the FP32-uncertain band
+        // around 2h sends the target to the exact recount of k_density_fix.
+        const float H = 2.0f * h, tauH = (1e-6f + band_c / h) * H;
         int  ni = 0;
         bool edge = false;
-        if (tvalid && !stream) {
+        if (tvalid && !fix) {
             for (int k = 0; k < cnt; ++k) {
-                const float r = L.r[k][lane];
+                const float r = lr[k * 32];
                 ni += (r < H) ? 1 : 0;
-                edge |= fabsf(r - H) <= tau * H;
+                edge |= fabsf(r - H) <= tauH;
             }
         }
-        const bool any_edge = sph_group_any<D_G>(edge, lane);
-        const bool exact    = tvalid && (stream || any_edge);
-        if (__any_sync(SPH_FULL, exact)) {
-            if (exact) ni = 0;
-            const float  H2  = H * H;
-            const double H2e = 4.0 * (double)h * (double)h;
-            sph_group_rows<D_G>(g, cell_start, pos_m, pi.x, pi.y, pi.z, H * (1.0f + 2.0f * tau),
-                                exact, lane, rot, c_tested,
-                                [&](uint32_t j, const float4 pj, float sx, float sy, float sz) {
-                const float dx = sx - pj.x, dy = sy - pj.y, dz = sz - pj.z;
-                const float r2 = dx * dx + dy * dy + dz * dz;
-                bool in = r2 < H2;
-                if (fabsf(r2 - H2) <= 2.0f * tau * H2) {
-                    in = sph_r2_exact(g, pi.x, pi.y, pi.z, pj.x, pj.y, pj.z) < H2e;
-                    ++c_recheck;
-                }
-                ni += in ? 1 : 0;
-            });
-        }
+        const bool recount = sph_group_any<D_G>(edge, lane) && !fix;   // h, rho, Omega stand
         ni = sph_group_sum_int<D_G>(ni);
-        if (tvalid && (lane & (D_G - 1)) == 0) {
-            const float ih = 1.0f / h;
-            h_io[i]  = h;
-            rho[i]   = SPH_SIGMA * S * ih * ih * ih;
-            omega[i] = E / (3.0f * S);
-            nn[i]    = ni;
-            c_pairs += ni;
+        if (tvalid) c_listed += cnt;
+        if (tvalid && leader) {
+            h_io[i] = h;   // final, or the best iterate for the fix kernel to start from
+            c_sweeps += sweeps;
+            if (!fix) {
+                const float ih = 1.0f / h;
+                rho[i]   = SPH_SIGMA * S * ih * ih * ih;
+                omega[i] = E / (3.0f * S);
+                nn[i]    = ni;
+            }
+            if (fix)          fix_list[atomicAdd(fix_cnt, 1u)] = p;
+            else if (recount) fix_list[atomicAdd(fix_cnt, 1u)] = p | (int32_t)0x80000000;
+            else              c_pairs += ni;
         }
         __syncwarp();
     }
 
     // ---- counters: lanes -> warp -> block -> one atomic per block and counter
-    unsigned v[8] = {c_tested, c_listed, c_pairs, c_sweeps, c_recollect, c_overflow, c_nonconv,
-                     c_recheck};
+    unsigned v[5] = {c_tested, c_listed, c_pairs, c_sweeps, c_recollect};
 #pragma unroll
-    for (int k = 0; k < 8; ++k) {
+    for (int k = 0; k < 5; ++k) {
         const unsigned t = __reduce_add_sync(SPH_FULL, v[k]);
         if (lane == 0 && t) atomicAdd(&st_sh[k], t);
     }
     __syncthreads();
-    if (threadIdx.x < 8 && st_sh[threadIdx.x] != 0u)
+    if (threadIdx.x < 5 && st_sh[threadIdx.x] != 0u)
         atomicAdd(stats + ST_DENS_TESTED + threadIdx.x, (unsigned long long)st_sh[threadIdx.x]);
+}
+
+// The robust path: one warp per queued target, no list.  Every sweep re-walks the candidate
+// rows (32 lanes over each row), so neither crowding nor a growing h can break it, and the
+// final count decides neighbours inside the FP32-uncertain band in FP64.
+__global__ __launch_bounds__(256) void k_density_fix(
+    const SphGrid* __restrict__ gp, const uint32_t* __restrict__ cell_start,
+    const float4* __restrict__ pos_m, const int32_t* __restrict__ perm, DensPar par,
+    const int32_t* __restrict__ fix_list, const unsigned* __restrict__ fix_cnt, float* h_io,
+    float* rho, float* omega, int32_t* nn, unsigned long long* stats) {
+    __shared__ RowRec  rows_all[8][SPH_RCAP];
+    __shared__ SphGrid g;
+    if (threadIdx.x < sizeof(SphGrid) / 4)
+        ((int*)&g)[threadIdx.x] = ((const int*)gp)[threadIdx.x];
+    __syncthreads();
+    const int      wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    RowRec*        rows = rows_all[wid];
+    const unsigned nfix = *fix_cnt;
+    const float    hcap = density_hcap(g);
+    unsigned long long c_tested = 0, c_pairs = 0, c_sweeps = 0;
+    unsigned c_nonconv = 0, c_recheck = 0, c_targets = 0;
+
+    for (unsigned t = blockIdx.x * 8 + wid; t < nfix; t += gridDim.x * 8) {
+        const int    pq = fix_list[t];
+        const bool   count_only = pq < 0;   // h, rho, Omega are final: exact n_i only
+        const int    p  = pq & 0x7fffffff;
+        const float4 pi = pos_m[p];
+        const int    i  = perm[p];
+        const float  T  = par.n_ngb * pi.w * (1.0f / 14.0f);
+        float h = fminf(h_io[i], hcap);
+        float hlo = 0.0f, hhi = __int_as_float(0x7f800000);
+        float S = 0.0f, E = 0.0f;
+        bool  conv = count_only;
+        int   sweeps = 0;
+        while (!count_only) {
+            const float ih = 1.0f / h, H2 = 4.0f * h * h;
+            float s = 0.0f, e = 0.0f, f2 = 0.0f;
+            sph_for_each_row(g, cell_start, pi.x, pi.y, pi.z, 2.0f * h, rows, lane,
+                             [&](const RowRec& rr) {
+                for (uint32_t k0 = rr.start; k0 < rr.end; k0 += 32) {
+                    const uint32_t j = k0 + lane;
+                    if (j < rr.end) {
+                        const float4 pj = __ldg(pos_m + j);
+                        const float dx = rr.sx - pj.x, dy = rr.sy - pj.y, dz = rr.sz - pj.z;
+                        const float r2 = dx * dx + dy * dy + dz * dz;
+                        if (r2 < H2) {
+                            const float q  = sqrtf(r2) * ih;
+                            const float tt = fmaxf(1.0f - 0.5f * q, 0.0f);
+                            const float t2 = tt * tt, q2 = q * q;
+                            s  += pj.w * (t2 * t2 * (1.0f + 2.0f * q));
+                            e  += pj.w * (5.0f * q2 * t2 * tt);
+                            f2 += pj.w * (q2 * t2 * (10.0f * tt - 7.5f * q));
+                        }
+                    }
+                    c_tested += min(32u, rr.end - k0);
+                }
+            });
+            s  = sph_warp_sum(s);
+            e  = sph_warp_sum(e);
+            f2 = sph_warp_sum(f2);
+            ++sweeps;
+            float hn, Sn, En;
+            const bool acc = halley_step(s, e, f2, T, h, ih, hcap, par.tol, hlo, hhi, hn, Sn, En, conv);
+            if (acc) { S = Sn; E = En; h = hn; break; }
+            if (sweeps >= par.max_iter) { S = s; E = e; conv = false; break; }
+            h = hn;
+        }
+        // ---- exact neighbour count at the final h
+        const float  tau = sph_band(g, h), H = 2.0f * h, H2 = H * H;
+        const double H2e = 4.0 * (double)h * (double)h;
+        int ni = 0;
+        sph_for_each_row(g, cell_start, pi.x, pi.y, pi.z, H * (1.0f + 2.0f * tau), rows, lane,
+                         [&](const RowRec& rr) {
+            for (uint32_t k0 = rr.start; k0 < rr.end; k0 += 32) {
+                const uint32_t j = k0 + lane;
+                if (j < rr.end) {
+                    const float4 pj = __ldg(pos_m + j);
+                    const float dx = rr.sx - pj.x, dy = rr.sy - pj.y, dz = rr.sz - pj.z;
+                    const float r2 = dx * dx + dy * dy + dz * dz;
+                    bool in = r2 < H2;
+                    if (fabsf(r2 - H2) <= 2.0f * tau * H2) {
+                        in = sph_r2_exact(g, pi.x, pi.y, pi.z, pj.x, pj.y, pj.z) < H2e;
+                        ++c_recheck;
+                    }
+                    ni += in ? 1 : 0;
+                }
+            }
+        });
+        ni = sph_warp_sum_int(ni);
+        if (lane == 0) {
+            nn[i] = ni;
+            if (!count_only) {
+                const float ih = 1.0f / h;
+                h_io[i]  = h;
+                rho[i]   = SPH_SIGMA * S * ih * ih * ih;
+                omega[i] = E / (3.0f * S);
+            }
+        }
+        c_pairs += ni;
+        c_sweeps += sweeps;
+        c_targets += 1;
+        if (!conv) ++c_nonconv;
+        __syncwarp();
+    }
+    c_recheck = __reduce_add_sync(SPH_FULL, c_recheck);
+    if (lane == 0 && c_targets) {
+        atomicAdd(stats + ST_DENS_TESTED, c_tested);
+        atomicAdd(stats + ST_DENS_PAIRS, c_pairs);
+        atomicAdd(stats + ST_DENS_SWEEPS, c_sweeps);
+        atomicAdd(stats + ST_DENS_OVERFLOW, (unsigned long long)c_targets);
+        atomicAdd(stats + ST_DENS_NONCONV, (unsigned long long)c_nonconv);
+        atomicAdd(stats + ST_DENS_RECHECK, (unsigned long long)c_recheck);
+    }
 }
 
 }  // namespace
@@ -283,10 +371,14 @@ int sph_launch_density(sph_ctx* c, const float* m, float* h, float* rho, float* 
     cudaStream_t  s = c->stream;
     const int64_t n = c->n;
     k_pack_pos_m<<<(int)((n + 255) / 256), 256, 0, s>>>(n, c->pos_h, c->perm, m, c->pos_m);
+    SPH_CUDA_CHECK(c, cudaMemsetAsync(c->fix_cnt, 0, sizeof(unsigned), s));
     DensPar par{c->par.n_ngb, c->par.h_tol, c->par.search_slack, c->par.h_max_iter};
-    const int    nblk = (int)((n + D_TARGETS - 1) / D_TARGETS);
-    k_density<<<nblk, D_TPB, 0, s>>>((int)n, c->grid, c->cell_start, c->pos_m, c->perm, par, h,
-                                       rho, omega, nn, c->stats);
+    const int nblk = (int)((n + D_TARGETS - 1) / D_TARGETS);
+    k_density<<<nblk, D_TPB, 0, s>>>((int)n, c->grid, c->cell_start, c->pos_m, c->perm, par, h, rho,
+                                     omega, nn, c->fix_list, c->fix_cnt, c->stats);
+    k_density_fix<<<c->sm_count * 4, 256, 0, s>>>(c->grid, c->cell_start, c->pos_m, c->perm, par,
+                                                  c->fix_list, c->fix_cnt, h, rho, omega, nn,
+                                                  c->stats);
     SPH_CUDA_CHECK(c, cudaGetLastError());
     return SPH_OK;
 }

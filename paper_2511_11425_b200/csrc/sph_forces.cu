@@ -6,7 +6,8 @@
 // test the candidates of the rows in reach (0 < r < 2 max(h_i,h_j), gather and scatter,
 // PAPER.md:191) and each lane notes the indices it accepted in a private column of a
 // shared-memory list.  Phase 2: every lane works through its own column -- the pair
-// arithmetic runs without divergence between accepted and rejected candidates.
+// arithmetic runs without divergence between accepted and rejected candidates.  A group
+// whose column overflows is queued for k_forces_fix (one warp per target, no list).
 //
 // Pair arithmetic (d = x_i - x_j, r = |d|, q_a = r/h_a, g_a = K_a (1-q_a/2)_+^3 with
 // K_a = 5 SIGMA / h_a^5, so that dW/dr(r,h_a) = -g_a r):
@@ -23,8 +24,8 @@ constexpr int F_G      = 8;
 constexpr int F_NT     = 32 / F_G;
 constexpr int F_WARPS  = 4;
 constexpr int F_TPB    = F_WARPS * 32;
-constexpr int F_ROUNDS = 2;
-constexpr int F_TARGETS = F_WARPS * F_NT * F_ROUNDS;
+constexpr int F_QUADS  = 16;   // target quads per block, handed out dynamically
+constexpr int F_TARGETS = F_NT * F_QUADS;
 constexpr int F_SLOTS  = 26;   // list entries per lane
 
 struct ForcePar {
@@ -43,8 +44,8 @@ __global__ void k_force_prep(int64_t n, const int32_t* __restrict__ inv_perm,
                              const float* __restrict__ rho, const float* __restrict__ h,
                              const float* __restrict__ omega, float gamma, float4* pos_h,
                              float4* vel_m, float4* rcak, float* P, float* cs, SphGrid* g) {
-    int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    float   hi = 0.0f;
+    int64_t  i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    float    hi = 0.0f;
     if (i < n) {
         const int p = inv_perm[i];
         hi = h[i];
@@ -62,31 +63,102 @@ __global__ void k_force_prep(int64_t n, const int32_t* __restrict__ inv_perm,
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) hi = fmaxf(hi, __shfl_xor_sync(SPH_FULL, hi, o));
-    if ((threadIdx.x & 31) == 0 && hi > 0.0f) atomicMax(&g->force_hmax_bits, __float_as_uint(hi));
+    if ((threadIdx.x & 31) == 0 && hi > 0.0f &&
+        *(volatile unsigned*)&g->force_hmax_bits < __float_as_uint(hi))
+        atomicMax(&g->force_hmax_bits, __float_as_uint(hi));
+}
+
+// a6: max h per coarse cell, the bound of the scatter reach.  Runs over the SORTED records, so
+// the 32 particles of a warp almost always share one coarse cell: one atomic per warp.
+__global__ void k_coarse_hmax(int64_t n, const SphGrid* __restrict__ g,
+                              const float4* __restrict__ pos_h, unsigned* coarse) {
+    int64_t  p  = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    unsigned cc = 0xffffffffu, hb = 0u;
+    if (p < n) {
+        const float4 a = pos_h[p];
+        if (a.w > 0.0f) {
+            const int cx = sph_cell_coord(a.x, g->lo[0], g->ics[0], g->cn[0]);
+            const int cy = sph_cell_coord(a.y, g->lo[1], g->ics[1], g->cn[1]);
+            const int cz = sph_cell_coord(a.z, g->lo[2], g->ics[2], g->cn[2]);
+            cc = (unsigned)((cz * g->cn[1] + cy) * g->cn[0] + cx);
+            hb = __float_as_uint(a.w);
+        }
+    }
+    const unsigned cc0 = __shfl_sync(SPH_FULL, cc, 0);
+    if (__all_sync(SPH_FULL, cc == cc0)) {
+        const unsigned mx = __reduce_max_sync(SPH_FULL, hb);
+        if ((threadIdx.x & 31) == 0 && cc != 0xffffffffu && __ldcg(coarse + cc) < mx)
+            atomicMax(coarse + cc, mx);
+    } else if (cc != 0xffffffffu && __ldcg(coarse + cc) < hb) {   // the map only grows
+        atomicMax(coarse + cc, hb);
+    }
 }
 
 __global__ void k_zero_hmax(SphGrid* g) { g->force_hmax_bits = 0u; }
 
-__global__ __launch_bounds__(F_TPB, SPH_MINB) void k_forces(int n, const SphGrid* __restrict__ gp,
-                                                     const uint32_t* __restrict__ cell_start,
-                                                     const float4* __restrict__ pos_h,
-                                                     const float4* __restrict__ vel_m,
-                                                     const float4* __restrict__ rcak,
-                                                     const int32_t* __restrict__ perm,
-                                                     ForcePar par, float* ax, float* ay, float* az,
-                                                     float* dudt, float* mu_min,
-                                                     unsigned long long* stats) {
+// Per-target constants and accumulators of the pair sum.
+struct Target {
+    float4 pi, vi;                       // (x, y, z, h), (vx, vy, vz, m)
+    float  rho, c, A, K, ih;
+};
+struct Accum {
+    float    ax = 0.f, ay = 0.f, az = 0.f, du = 0.f, mumin = 0.f;
+    unsigned pairs = 0, av = 0;
+};
+
+// One pair of Eqs. (13)-(18): source j at displacement d = x_i - x_j (minimum image).
+__device__ __forceinline__ void force_pair(const Target& t, Accum& a, const ForcePar& par,
+                                           const float4* __restrict__ vel_m,
+                                           const float4* __restrict__ rcak, uint32_t j, float dx,
+                                           float dy, float dz, float r2, float hj) {
+    const float4 vj = __ldg(vel_m + j);
+    const float4 rj = __ldg(rcak + j);
+    const float r  = r2 * rsqrtf(r2);
+    const float ti = fmaxf(1.0f - 0.5f * r * t.ih, 0.0f);
+    const float tj = fmaxf(1.0f - 0.5f * __fdividef(r, hj), 0.0f);
+    const float gi = t.K * ti * ti * ti;
+    const float gj = rj.w * tj * tj * tj;
+    const float vdx = t.vi.x - vj.x, vdy = t.vi.y - vj.y, vdz = t.vi.z - vj.z;
+    const float vr = vdx * dx + vdy * dy + vdz * dz;   // v_ij . r_ij
+    float pig = 0.0f;                                   // Pi_ij * gbar
+    if (vr < 0.0f) {
+        const float hb  = 0.5f * (t.pi.w + hj);
+        const float mu  = __fdividef(hb * vr, r2 + par.eps * hb * hb);
+        const float cb  = 0.5f * (t.c + rj.y);
+        const float rb  = 0.5f * (t.rho + rj.x);
+        const float Pij = __fdividef(mu * (par.beta * mu - par.alpha * cb), rb);
+        pig     = Pij * 0.5f * (gi + gj);
+        a.mumin = fminf(a.mumin, mu);
+        ++a.av;
+    }
+    const float Ag = t.A * gi;
+    const float ca = vj.w * (Ag + rj.z * gj + pig);
+    a.ax += ca * dx;
+    a.ay += ca * dy;
+    a.az += ca * dz;
+    a.du -= vj.w * (Ag + 0.5f * pig) * vr;
+    ++a.pairs;
+}
+
+__global__ __launch_bounds__(F_TPB, SPH_MINB) void k_forces(
+    int n, const SphGrid* __restrict__ gp, const uint32_t* __restrict__ cell_start,
+    const float4* __restrict__ pos_h, const float4* __restrict__ vel_m,
+    const float4* __restrict__ rcak, const int32_t* __restrict__ perm, ForcePar par, float* ax,
+    float* ay, float* az, float* dudt, float* mu_min, int32_t* fix_list, unsigned* fix_cnt,
+    const unsigned* __restrict__ coarse, unsigned long long* stats) {
     __shared__ FWarpList lists[F_WARPS];
     __shared__ SphGrid   g;
     __shared__ unsigned  st_sh[3];
+    __shared__ int       next_quad;
     if (threadIdx.x < sizeof(SphGrid) / 4)
         ((int*)&g)[threadIdx.x] = ((const int*)gp)[threadIdx.x];
     if (threadIdx.x < 3) st_sh[threadIdx.x] = 0u;
+    if (threadIdx.x == 0) next_quad = 0;
     __syncthreads();
 
     const int   wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int   gq  = lane / F_G;
-    FWarpList&  L   = lists[wid];
+    uint32_t* const lj = &lists[wid].j[0][lane];   // this lane's column, slot stride 32
     const float hmax_all = __uint_as_float(g.force_hmax_bits);
     const float iLx = g.per[0] ? 1.0f / g.len[0] : 0.0f, Lx = g.per[0] ? g.len[0] : 0.0f;
     const float iLy = g.per[1] ? 1.0f / g.len[1] : 0.0f, Ly = g.per[1] ? g.len[1] : 0.0f;
@@ -94,105 +166,77 @@ __global__ __launch_bounds__(F_TPB, SPH_MINB) void k_forces(int n, const SphGrid
 
     unsigned c_tested = 0, c_pairs = 0, c_av = 0;
 
-    for (int round = 0; round < F_ROUNDS; ++round) {
-        const int  p      = (blockIdx.x * F_ROUNDS + round) * (F_WARPS * F_NT) + wid * F_NT + gq;
+    for (;;) {
+        int quad = 0;
+        if (lane == 0) quad = atomicAdd(&next_quad, 1);
+        quad = __shfl_sync(SPH_FULL, quad, 0);
+        if (quad >= F_QUADS) break;
+        const int  p      = (blockIdx.x * F_QUADS + quad) * F_NT + gq;
         const bool tvalid = p < n;
-        float4 pi = make_float4(0.f, 0.f, 0.f, 1.f), vi = pi, ri = make_float4(1.f, 1.f, 0.f, 0.f);
+        Target t;
+        t.pi = make_float4(0.f, 0.f, 0.f, 1.f);
+        t.vi = t.pi;
+        float4 ri = make_float4(1.f, 1.f, 0.f, 0.f);
         if (tvalid) {
-            pi = pos_h[p];
-            vi = vel_m[p];
-            ri = rcak[p];
+            t.pi = pos_h[p];
+            t.vi = vel_m[p];
+            ri   = rcak[p];
         }
-        const float hi = pi.w, ihi = __fdividef(1.0f, hi);
-        const float rho_i = ri.x, c_i = ri.y, A_i = ri.z, K_i = ri.w;
-        // scatter neighbours can be as far as 2 h_j: search with the largest h in use
-        const float R = 2.0f * fmaxf(hi, hmax_all) * (1.0f + 1e-5f);
-        const float hi2x4 = 4.0f * hi * hi;
-
-        float acx = 0.0f, acy = 0.0f, acz = 0.0f, du = 0.0f, mumin = 0.0f;
-
-        // one pair: source j at displacement (dx, dy, dz), smoothing length hj
-        auto pair = [&](uint32_t j, float dx, float dy, float dz, float r2, float hj) {
-            const float4 vj = __ldg(vel_m + j);
-            const float4 rj = __ldg(rcak + j);
-            const float r  = r2 * rsqrtf(r2);
-            const float ti = fmaxf(1.0f - 0.5f * r * ihi, 0.0f);
-            const float tj = fmaxf(1.0f - 0.5f * __fdividef(r, hj), 0.0f);
-            const float gi = K_i * ti * ti * ti;
-            const float gj = rj.w * tj * tj * tj;
-            const float vdx = vi.x - vj.x, vdy = vi.y - vj.y, vdz = vi.z - vj.z;
-            const float vr = vdx * dx + vdy * dy + vdz * dz;   // v_ij . r_ij
-            float pig = 0.0f;                                   // Pi_ij * gbar
-            if (vr < 0.0f) {
-                const float hb  = 0.5f * (hi + hj);
-                const float mu  = __fdividef(hb * vr, r2 + par.eps * hb * hb);
-                const float cb  = 0.5f * (c_i + rj.y);
-                const float rb  = 0.5f * (rho_i + rj.x);
-                const float Pij = __fdividef(mu * (par.beta * mu - par.alpha * cb), rb);
-                pig   = Pij * 0.5f * (gi + gj);
-                mumin = fminf(mumin, mu);
-                ++c_av;
-            }
-            const float Ag = A_i * gi;
-            const float ca = vj.w * (Ag + rj.z * gj + pig);
-            acx += ca * dx;
-            acy += ca * dy;
-            acz += ca * dz;
-            du -= vj.w * (Ag + 0.5f * pig) * vr;
-            ++c_pairs;
-        };
+        t.rho = ri.x; t.c = ri.y; t.A = ri.z; t.K = ri.w;
+        t.ih  = __fdividef(1.0f, t.pi.w);
+        // scatter neighbours can be as far as 2 h_j: search with the largest h that can
+        // reach this target (a6)
+        const float R = 2.0f * (1.0f + 1e-5f) *
+                        sph_scatter_hmax<F_G>(g, coarse, t.pi.x, t.pi.y, t.pi.z, t.pi.w, hmax_all, lane);
+        const float hi2x4 = 4.0f * t.pi.w * t.pi.w;
 
         // ---- phase 1: lane-private index lists
         int      cnt = 0;
         unsigned rot = 0;
-        sph_group_rows<F_G>(g, cell_start, pos_h, pi.x, pi.y, pi.z, R, tvalid, lane, rot, c_tested,
+        sph_group_rows<F_G>(g, cell_start, pos_h, t.pi.x, t.pi.y, t.pi.z, R, tvalid, lane, rot,
+                            c_tested,
                             [&](uint32_t j, const float4 pj, float sx, float sy, float sz) {
             const float dx = sx - pj.x, dy = sy - pj.y, dz = sz - pj.z;
             const float r2 = dx * dx + dy * dy + dz * dz;
             const float Hm = fmaxf(hi2x4, 4.0f * pj.w * pj.w);
             if (r2 < Hm && r2 > 0.0f) {
-                if (cnt < F_SLOTS) L.j[cnt][lane] = j;
+                if (cnt < F_SLOTS) lj[cnt * 32] = j;
                 ++cnt;
             }
         });
         const bool ovf = sph_group_any<F_G>(cnt > F_SLOTS, lane);
 
         // ---- phase 2: the pairs of this lane's column
+        Accum a;
         const int mycnt  = ovf ? 0 : cnt;
         const int maxcnt = __reduce_max_sync(SPH_FULL, mycnt);
         for (int k = 0; k < maxcnt; ++k) {
             if (k < mycnt) {
-                const uint32_t j  = L.j[k][lane];
+                const uint32_t j  = lj[k * 32];
                 const float4   pj = __ldg(pos_h + j);
-                float dx = pi.x - pj.x, dy = pi.y - pj.y, dz = pi.z - pj.z;
+                float dx = t.pi.x - pj.x, dy = t.pi.y - pj.y, dz = t.pi.z - pj.z;
                 dx -= Lx * rintf(dx * iLx);   // minimum image (no-op on open axes)
                 dy -= Ly * rintf(dy * iLy);
                 dz -= Lz * rintf(dz * iLz);
-                const float r2 = dx * dx + dy * dy + dz * dz;
-                pair(j, dx, dy, dz, r2, pj.w);
+                force_pair(t, a, par, vel_m, rcak, j, dx, dy, dz, dx * dx + dy * dy + dz * dz, pj.w);
             }
         }
-        // a column overflowed (very crowded neighbourhood): redo the group without lists
-        if (__any_sync(SPH_FULL, ovf)) {
-            sph_group_rows<F_G>(g, cell_start, pos_h, pi.x, pi.y, pi.z, R, tvalid && ovf, lane, rot,
-                                c_tested,
-                                [&](uint32_t j, const float4 pj, float sx, float sy, float sz) {
-                const float dx = sx - pj.x, dy = sy - pj.y, dz = sz - pj.z;
-                const float r2 = dx * dx + dy * dy + dz * dz;
-                const float Hm = fmaxf(hi2x4, 4.0f * pj.w * pj.w);
-                if (r2 < Hm && r2 > 0.0f) pair(j, dx, dy, dz, r2, pj.w);
-            });
-        }
-        acx = sph_group_sum<F_G>(acx);
-        acy = sph_group_sum<F_G>(acy);
-        acz = sph_group_sum<F_G>(acz);
-        du  = sph_group_sum<F_G>(du);
-        mumin = sph_group_min<F_G>(mumin);
+        a.ax = sph_group_sum<F_G>(a.ax);
+        a.ay = sph_group_sum<F_G>(a.ay);
+        a.az = sph_group_sum<F_G>(a.az);
+        a.du = sph_group_sum<F_G>(a.du);
+        a.mumin = sph_group_min<F_G>(a.mumin);
+        c_pairs += a.pairs;
+        c_av    += a.av;
         if (tvalid && (lane & (F_G - 1)) == 0) {
-            const int i = perm[p];
-            ax[i] = acx; ay[i] = acy; az[i] = acz;
-            dudt[i]   = du;
-            mu_min[i] = mumin;
+            if (!ovf) {
+                const int i = perm[p];
+                ax[i] = a.ax; ay[i] = a.ay; az[i] = a.az;
+                dudt[i]   = a.du;
+                mu_min[i] = a.mumin;
+            } else {
+                fix_list[atomicAdd(fix_cnt, 1u)] = p;   // very crowded neighbourhood
+            }
         }
         __syncwarp();
     }
@@ -200,12 +244,78 @@ __global__ __launch_bounds__(F_TPB, SPH_MINB) void k_forces(int n, const SphGrid
     unsigned v[3] = {c_tested, c_pairs, c_av};
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
-        const unsigned t = __reduce_add_sync(SPH_FULL, v[k]);
-        if (lane == 0 && t) atomicAdd(&st_sh[k], t);
+        const unsigned tt = __reduce_add_sync(SPH_FULL, v[k]);
+        if (lane == 0 && tt) atomicAdd(&st_sh[k], tt);
     }
     __syncthreads();
     if (threadIdx.x < 3 && st_sh[threadIdx.x] != 0u)
         atomicAdd(stats + ST_FORCE_TESTED + threadIdx.x, (unsigned long long)st_sh[threadIdx.x]);
+}
+
+// The robust path: one warp per queued target, candidates handled as they are met.
+__global__ __launch_bounds__(256) void k_forces_fix(
+    const SphGrid* __restrict__ gp, const uint32_t* __restrict__ cell_start,
+    const float4* __restrict__ pos_h, const float4* __restrict__ vel_m,
+    const float4* __restrict__ rcak, const int32_t* __restrict__ perm, ForcePar par,
+    const int32_t* __restrict__ fix_list, const unsigned* __restrict__ fix_cnt, float* ax,
+    float* ay, float* az, float* dudt, float* mu_min, unsigned long long* stats) {
+    __shared__ RowRec  rows_all[8][SPH_RCAP];
+    __shared__ SphGrid g;
+    if (threadIdx.x < sizeof(SphGrid) / 4)
+        ((int*)&g)[threadIdx.x] = ((const int*)gp)[threadIdx.x];
+    __syncthreads();
+    const int      wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const unsigned nfix = *fix_cnt;
+    const float    hmax_all = __uint_as_float(g.force_hmax_bits);
+    unsigned long long c_tested = 0;
+    unsigned c_pairs = 0, c_av = 0;
+    for (unsigned q = blockIdx.x * 8 + wid; q < nfix; q += gridDim.x * 8) {
+        const int p = fix_list[q];
+        Target t;
+        t.pi = pos_h[p];
+        t.vi = vel_m[p];
+        const float4 ri = rcak[p];
+        t.rho = ri.x; t.c = ri.y; t.A = ri.z; t.K = ri.w;
+        t.ih  = 1.0f / t.pi.w;
+        const float R = 2.0f * fmaxf(t.pi.w, hmax_all) * (1.0f + 1e-5f);
+        const float hi2x4 = 4.0f * t.pi.w * t.pi.w;
+        Accum a;
+        sph_for_each_row(g, cell_start, t.pi.x, t.pi.y, t.pi.z, R, rows_all[wid], lane,
+                         [&](const RowRec& rr) {
+            for (uint32_t k0 = rr.start; k0 < rr.end; k0 += 32) {
+                const uint32_t j = k0 + lane;
+                if (j < rr.end) {
+                    const float4 pj = __ldg(pos_h + j);
+                    const float dx = rr.sx - pj.x, dy = rr.sy - pj.y, dz = rr.sz - pj.z;
+                    const float r2 = dx * dx + dy * dy + dz * dz;
+                    if (r2 < fmaxf(hi2x4, 4.0f * pj.w * pj.w) && r2 > 0.0f)
+                        force_pair(t, a, par, vel_m, rcak, j, dx, dy, dz, r2, pj.w);
+                }
+                c_tested += min(32u, rr.end - k0);
+            }
+        });
+        a.ax = sph_warp_sum(a.ax);
+        a.ay = sph_warp_sum(a.ay);
+        a.az = sph_warp_sum(a.az);
+        a.du = sph_warp_sum(a.du);
+        a.mumin = sph_warp_min(a.mumin);
+        c_pairs += a.pairs;
+        c_av    += a.av;
+        if (lane == 0) {
+            const int i = perm[p];
+            ax[i] = a.ax; ay[i] = a.ay; az[i] = a.az;
+            dudt[i]   = a.du;
+            mu_min[i] = a.mumin;
+        }
+        __syncwarp();
+    }
+    c_pairs = __reduce_add_sync(SPH_FULL, c_pairs);
+    c_av    = __reduce_add_sync(SPH_FULL, c_av);
+    if (lane == 0 && (c_tested | c_pairs)) {
+        atomicAdd(stats + ST_FORCE_TESTED, c_tested);
+        atomicAdd(stats + ST_FORCE_PAIRS, (unsigned long long)c_pairs);
+        atomicAdd(stats + ST_FORCE_AV, (unsigned long long)c_av);
+    }
 }
 
 }  // namespace
@@ -217,13 +327,21 @@ int sph_launch_forces(sph_ctx* c, const float* m, const float* vx, const float* 
     cudaStream_t  s = c->stream;
     const int64_t n = c->n;
     k_zero_hmax<<<1, 1, 0, s>>>(c->grid);
+    SPH_CUDA_CHECK(c, cudaMemsetAsync(c->fix_cnt + 1, 0, sizeof(unsigned), s));
+    SPH_CUDA_CHECK(c, cudaMemsetAsync(c->coarse_hmax, 0, SPH_COARSE_MAX * sizeof(unsigned), s));
     k_force_prep<<<(int)((n + 255) / 256), 256, 0, s>>>(n, c->inv_perm, m, vx, vy, vz, u,
                                                         rho, h, omega, c->par.gamma, c->pos_h,
                                                         c->vel_m, c->rcak, P, cs, c->grid);
+    k_coarse_hmax<<<(int)((n + 255) / 256), 256, 0, s>>>(n, c->grid, c->pos_h, c->coarse_hmax);
     ForcePar par{c->par.av_alpha, c->par.av_beta, c->par.av_eps};
     const int nblk = (int)((n + F_TARGETS - 1) / F_TARGETS);
     k_forces<<<nblk, F_TPB, 0, s>>>((int)n, c->grid, c->cell_start, c->pos_h, c->vel_m, c->rcak,
-                                    c->perm, par, ax, ay, az, dudt, mu_min, c->stats);
+                                    c->perm, par, ax, ay, az, dudt, mu_min, c->fix_list,
+                                    c->fix_cnt + 1, c->coarse_hmax, c->stats);
+    k_forces_fix<<<c->sm_count * 4, 256, 0, s>>>(c->grid, c->cell_start, c->pos_h, c->vel_m,
+                                                 c->rcak, c->perm, par, c->fix_list,
+                                                 c->fix_cnt + 1, ax, ay, az, dudt, mu_min,
+                                                 c->stats);
     SPH_CUDA_CHECK(c, cudaGetLastError());
     return SPH_OK;
 }

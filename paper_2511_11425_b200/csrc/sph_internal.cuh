@@ -23,8 +23,10 @@ struct SphGrid {
     float xext;                // largest |coordinate| that enters a displacement
     int   flags;               // bit0: periodic side too short; bit1: cell table clipped
     unsigned force_hmax_bits;  // max h given to sph_forces (float bits, atomicMax)
-    int   pad[3];
+    int   cn[3];               // coarse grid (max-h map for the scatter reach of the force search)
+    float ics[3];              // inverse coarse cell sides
 };
+#define SPH_COARSE_MAX (1 << 18)   // entries of the coarse max-h map
 
 enum {  // indices into the device counter block (uint64 each), mirrors sph_stats_t
     ST_DENS_TESTED = 0, ST_DENS_LISTED, ST_DENS_PAIRS, ST_DENS_SWEEPS, ST_DENS_RECOLLECT,
@@ -54,7 +56,10 @@ struct sph_ctx {
     float4*      pos_m;        // sorted (x, y, z, m)
     float4*      vel_m;        // sorted (vx, vy, vz, m)
     float4*      rcak;         // sorted (rho, c, A = P/(Omega rho^2), K = 5 sigma / h^5)
+    unsigned*    coarse_hmax;  // SPH_COARSE_MAX: max h (float bits) per coarse cell, step a6
     unsigned long long* stats; // ST_NCOUNTERS
+    int32_t*     fix_list;     // n_max: sorted positions queued for the robust (fix) kernels
+    unsigned*    fix_cnt;      // [2]: queue lengths (density, forces)
     float*       dt_part;      // per-block minima of the time-step reduction
     int64_t*     nb_total;     // neighbour-list total (device) + pinned mirror
     char         err[256];
@@ -76,7 +81,7 @@ struct sph_ctx {
 
 #define SPH_FULL 0xffffffffu
 #ifndef SPH_UNROLL
-#define SPH_UNROLL 1   // candidate windows loaded ahead per lane
+#define SPH_UNROLL 3   // candidate windows loaded ahead per lane
 #endif
 #ifndef SPH_MINB
 #define SPH_MINB 8     // resident blocks per SM the sweeps are compiled for
@@ -312,6 +317,65 @@ __device__ __forceinline__ void sph_group_rows(const SphGrid& g,
             }
         }
     }
+}
+
+// Step a6: the largest h_j of any particle that can reach (x, y, z), i.e. with
+// |x - x_j| < 2 h_j, bounded from the coarse max-h map.  Starts from the
+// global maximum and tightens twice: every such j lies within 2 H of the target as long as H
+// bounds its h_j, so the maximum over the coarse cells meeting that ball is again a bound.
+template <int G>
+__device__ __forceinline__ float sph_scatter_hmax(const SphGrid& g,
+                                                  const unsigned* __restrict__ coarse, float xi,
+                                                  float yi, float zi, float hi, float hglobal,
+                                                  int lane) {
+    const int sl = lane & (G - 1);
+    float H = fmaxf(hglobal, hi);
+    const float xs[3] = {xi, yi, zi};
+#pragma unroll 1
+    for (int pass = 0; pass < 2; ++pass) {
+        int u0[3], nn[3];
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+            const float R = 2.0f * H * (1.0f + 1e-5f);
+            float a = floorf((xs[d] - g.lo[d] - R) * g.ics[d] - 1e-3f);
+            float b = floorf((xs[d] - g.lo[d] + R) * g.ics[d] + 1e-3f);
+            a = fminf(fmaxf(a, -1.0e9f), 1.0e9f);
+            b = fminf(fmaxf(b, -1.0e9f), 1.0e9f);
+            int lo = (int)a, hi_ = (int)b;
+            if (g.per[d]) {
+                if (hi_ - lo + 1 >= g.cn[d]) { lo = 0; hi_ = g.cn[d] - 1; }
+            } else {
+                lo  = min(max(lo, 0), g.cn[d] - 1);
+                hi_ = min(max(hi_, 0), g.cn[d] - 1);
+            }
+            u0[d] = lo;
+            nn[d] = hi_ - lo + 1;
+        }
+        const int   cnt  = nn[0] * nn[1] * nn[2];
+        const int   cmax = __reduce_max_sync(SPH_FULL, cnt);
+        const float i0 = __fdividef(1.0f, (float)nn[0]), i1 = __fdividef(1.0f, (float)nn[1]);
+        unsigned best = 0u;
+        for (int q = sl; q < cmax; q += G) {
+            if (q < cnt) {
+                const int t  = (int)(((float)q + 0.5f) * i0);          // q / nn[0]
+                const int ix = q - t * nn[0];
+                const int iz = (int)(((float)t + 0.5f) * i1);          // t / nn[1]
+                const int iy = t - iz * nn[1];
+                int cx = u0[0] + ix, cy = u0[1] + iy, cz = u0[2] + iz;
+                cx -= (cx >= g.cn[0]) ? g.cn[0] : 0; cx += (cx < 0) ? g.cn[0] : 0;
+                cy -= (cy >= g.cn[1]) ? g.cn[1] : 0; cy += (cy < 0) ? g.cn[1] : 0;
+                cz -= (cz >= g.cn[2]) ? g.cn[2] : 0; cz += (cz < 0) ? g.cn[2] : 0;
+                cx = min(max(cx, 0), g.cn[0] - 1);
+                cy = min(max(cy, 0), g.cn[1] - 1);
+                cz = min(max(cz, 0), g.cn[2] - 1);
+                best = max(best, __ldg(coarse + (cz * g.cn[1] + cy) * g.cn[0] + cx));
+            }
+        }
+#pragma unroll
+        for (int o = G / 2; o > 0; o >>= 1) best = max(best, __shfl_xor_sync(SPH_FULL, best, o));
+        H = fmaxf(hi, fminf(H, __uint_as_float(best)));
+    }
+    return H;
 }
 
 template <int G>

@@ -255,7 +255,8 @@ def test_c3_sedov_full_size_sampled(gu):
     _, ob = gu.make_boxes(w)
     ctx, d, out, h = _full_step(gu, w)
     st = ctx.stats()
-    assert st["dens_nonconv"] == 0 and st["dens_overflow"] == 0, st
+    # dens_overflow counts the targets finished by the robust kernel (borderline neighbours)
+    assert st["dens_nonconv"] == 0 and st["dens_overflow"] <= 0.03 * w["n"], st
     r2c = (w["x"] - 0.5) ** 2 + (w["y"] - 0.5) ** 2 + (w["z"] - 0.5) ** 2
     sel = np.unique(np.concatenate([_sample(w["n"], 256, 31), np.argsort(r2c)[:64]]))
     _check_sample(gu, w, ctx, out, h, sel, op, ob)
