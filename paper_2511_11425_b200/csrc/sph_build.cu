@@ -250,6 +250,8 @@ int sph_launch_build(sph_ctx* c, int64_t n, const float* x, const float* y, cons
     cudaStream_t s  = c->stream;
     const int    nb = (int)((n + TPB - 1) / TPB);
     const int    gs = c->sm_count * 8;
+    // new positions: the neighbour lists kept from the last density sweep are void
+    SPH_CUDA_CHECK(c, cudaMemsetAsync(c->nb_rkeep, 0, (size_t)n * sizeof(float), s));
     k_init_red<<<1, 1, 0, s>>>(c->red);
     k_reduce_h<<<min(nb, gs), TPB, 0, s>>>(n, x, y, z, h, c->red);
     k_grid_setup<<<1, 1, 0, s>>>(c->grid, c->red, c->box, c->par.search_slack, c->par.cell_div_x,

@@ -25,13 +25,14 @@
 
 namespace {
 
-constexpr int   D_G      = 8;             // lanes per target
+constexpr int   D_G      = SPH_G;         // lanes per target
 constexpr int   D_NT     = 32 / D_G;      // targets per warp
 constexpr int   D_WARPS  = 4;
 constexpr int   D_TPB    = D_WARPS * 32;
 constexpr int   D_QUADS  = 16;            // target quads per block, handed out dynamically
 constexpr int   D_TARGETS = D_NT * D_QUADS;
-constexpr int   D_SLOTS  = 28;            // list entries per lane
+constexpr int   D_SLOTS  = SPH_SLOTS;     // list entries per lane
+constexpr float D_KEEP   = 1.05f;         // lists are kept for the force sweep out to 2h x this
 constexpr float D_ACCEPT = 3.0e-4f;
 
 struct DensPar {
@@ -96,8 +97,8 @@ __device__ __forceinline__ float density_hcap(const SphGrid& g) {
 __global__ __launch_bounds__(D_TPB, SPH_MINB) void k_density(
     int n, const SphGrid* __restrict__ gp, const uint32_t* __restrict__ cell_start,
     const float4* __restrict__ pos_m, const int32_t* __restrict__ perm, DensPar par, float* h_io,
-    float* rho, float* omega, int32_t* nn, int32_t* fix_list, unsigned* fix_cnt,
-    unsigned long long* stats) {
+    float* rho, float* omega, int32_t* nn, int32_t* fix_list, unsigned* fix_cnt, uint32_t* nb_j,
+    uint32_t* nb_mask, float* nb_rkeep, unsigned long long* stats) {
     __shared__ WarpList lists[D_WARPS];
     __shared__ SphGrid  g;
     __shared__ unsigned st_sh[5];
@@ -136,6 +137,8 @@ __global__ __launch_bounds__(D_TPB, SPH_MINB) void k_density(
         if (!(h > 0.0f) || !(h < 3.0e38f)) h = g.hmin;
         h = fminf(h, hcap);
         const float T = par.n_ngb * pi.w * (1.0f / 14.0f);
+        // this lane's column of the kept list: [target][slot][lane of the group]
+        uint32_t* const gj = nb_j + ((size_t)(tvalid ? p : 0) * D_SLOTS * D_G + (lane & (D_G - 1)));
         float    hlo = 0.0f, hhi = __int_as_float(0x7f800000);
         float    Rc = 0.0f;         // radius the list is complete for
         int      cnt = 0;           // entries in this lane's column
@@ -166,6 +169,7 @@ __global__ __launch_bounds__(D_TPB, SPH_MINB) void k_density(
                         if (cnt < D_SLOTS) {
                             lr[cnt * 32] = r2 * rsqrtf(fmaxf(r2, 1e-35f));
                             lm[cnt * 32] = pj.w;
+                            gj[cnt * D_G] = j;
                         }
                         ++cnt;
                     }
@@ -211,20 +215,25 @@ __global__ __launch_bounds__(D_TPB, SPH_MINB) void k_density(
         // ---- n_i = #{j : r_ij < 2h} from the list; an entry inside the FP32-uncertain band
         // around 2h sends the target to the exact recount of k_density_fix.
         const float H = 2.0f * h, tauH = (1e-6f + band_c / h) * H;
-        int  ni = 0;
-        bool edge = false;
+        const float Rk = fminf(Rc, H * D_KEEP);   // the kept list is complete inside Rk
+        int      ni = 0;
+        unsigned keep = 0u;
+        bool     edge = false;
         if (tvalid && !fix) {
             for (int k = 0; k < cnt; ++k) {
                 const float r = lr[k * 32];
                 ni += (r < H) ? 1 : 0;
                 edge |= fabsf(r - H) <= tauH;
+                keep |= (r < Rk) ? (1u << k) : 0u;
             }
+            nb_mask[(size_t)p * D_G + (lane & (D_G - 1))] = keep;
         }
         const bool recount = sph_group_any<D_G>(edge, lane) && !fix;   // h, rho, Omega stand
         ni = sph_group_sum_int<D_G>(ni);
         if (tvalid) c_listed += cnt;
         if (tvalid && leader) {
             h_io[i] = h;   // final, or the best iterate for the fix kernel to start from
+            nb_rkeep[p] = fix ? 0.0f : Rk;
             c_sweeps += sweeps;
             if (!fix) {
                 const float ih = 1.0f / h;
@@ -375,7 +384,8 @@ int sph_launch_density(sph_ctx* c, const float* m, float* h, float* rho, float* 
     DensPar par{c->par.n_ngb, c->par.h_tol, c->par.search_slack, c->par.h_max_iter};
     const int nblk = (int)((n + D_TARGETS - 1) / D_TARGETS);
     k_density<<<nblk, D_TPB, 0, s>>>((int)n, c->grid, c->cell_start, c->pos_m, c->perm, par, h, rho,
-                                     omega, nn, c->fix_list, c->fix_cnt, c->stats);
+                                     omega, nn, c->fix_list, c->fix_cnt, c->nb_j, c->nb_mask,
+                                     c->nb_rkeep, c->stats);
     k_density_fix<<<c->sm_count * 4, 256, 0, s>>>(c->grid, c->cell_start, c->pos_m, c->perm, par,
                                                   c->fix_list, c->fix_cnt, h, rho, omega, nn,
                                                   c->stats);

@@ -20,13 +20,16 @@
 
 namespace {
 
-constexpr int F_G      = 8;
+#ifndef SPH_FMINB
+#define SPH_FMINB SPH_MINB
+#endif
+constexpr int F_G      = SPH_G;
 constexpr int F_NT     = 32 / F_G;
 constexpr int F_WARPS  = 4;
 constexpr int F_TPB    = F_WARPS * 32;
 constexpr int F_QUADS  = 16;   // target quads per block, handed out dynamically
 constexpr int F_TARGETS = F_NT * F_QUADS;
-constexpr int F_SLOTS  = 26;   // list entries per lane
+constexpr int F_SLOTS  = SPH_SLOTS;   // list entries per lane
 
 struct ForcePar {
     float alpha, beta, eps;
@@ -108,11 +111,8 @@ struct Accum {
 
 // One pair of Eqs. (13)-(18): source j at displacement d = x_i - x_j (minimum image).
 __device__ __forceinline__ void force_pair(const Target& t, Accum& a, const ForcePar& par,
-                                           const float4* __restrict__ vel_m,
-                                           const float4* __restrict__ rcak, uint32_t j, float dx,
+                                           const float4 vj, const float4 rj, float dx,
                                            float dy, float dz, float r2, float hj) {
-    const float4 vj = __ldg(vel_m + j);
-    const float4 rj = __ldg(rcak + j);
     const float r  = r2 * rsqrtf(r2);
     const float ti = fmaxf(1.0f - 0.5f * r * t.ih, 0.0f);
     const float tj = fmaxf(1.0f - 0.5f * __fdividef(r, hj), 0.0f);
@@ -140,12 +140,14 @@ __device__ __forceinline__ void force_pair(const Target& t, Accum& a, const Forc
     ++a.pairs;
 }
 
-__global__ __launch_bounds__(F_TPB, SPH_MINB) void k_forces(
+__global__ __launch_bounds__(F_TPB, SPH_FMINB) void k_forces(
     int n, const SphGrid* __restrict__ gp, const uint32_t* __restrict__ cell_start,
     const float4* __restrict__ pos_h, const float4* __restrict__ vel_m,
     const float4* __restrict__ rcak, const int32_t* __restrict__ perm, ForcePar par, float* ax,
     float* ay, float* az, float* dudt, float* mu_min, int32_t* fix_list, unsigned* fix_cnt,
-    const unsigned* __restrict__ coarse, unsigned long long* stats) {
+    const unsigned* __restrict__ coarse, const uint32_t* __restrict__ nb_j,
+    const uint32_t* __restrict__ nb_mask, const float* __restrict__ nb_rkeep,
+    unsigned long long* stats) {
     __shared__ FWarpList lists[F_WARPS];
     __shared__ SphGrid   g;
     __shared__ unsigned  st_sh[3];
@@ -184,41 +186,84 @@ __global__ __launch_bounds__(F_TPB, SPH_MINB) void k_forces(
         }
         t.rho = ri.x; t.c = ri.y; t.A = ri.z; t.K = ri.w;
         t.ih  = __fdividef(1.0f, t.pi.w);
-        // scatter neighbours can be as far as 2 h_j: search with the largest h that can
-        // reach this target (a6)
+        // scatter neighbours can be as far as 2 h_j: the reach is set by the largest h that
+        // can get to this target (a6)
         const float R = 2.0f * (1.0f + 1e-5f) *
                         sph_scatter_hmax<F_G>(g, coarse, t.pi.x, t.pi.y, t.pi.z, t.pi.w, hmax_all, lane);
         const float hi2x4 = 4.0f * t.pi.w * t.pi.w;
 
-        // ---- phase 1: lane-private index lists
+        // ---- phase 1: lane-private index lists.  If the list kept by the density sweep is
+        // complete out to R (same positions) it is copied; else search.
+        const float rk      = tvalid ? nb_rkeep[p] : 0.0f;
+        const float tau     = 1e-6f + 2.5e-7f * g.xext * t.ih;
+        const bool  covered = tvalid && (R * (1.0f + 4.0f * tau) <= rk);
         int      cnt = 0;
         unsigned rot = 0;
-        sph_group_rows<F_G>(g, cell_start, pos_h, t.pi.x, t.pi.y, t.pi.z, R, tvalid, lane, rot,
-                            c_tested,
-                            [&](uint32_t j, const float4 pj, float sx, float sy, float sz) {
-            const float dx = sx - pj.x, dy = sy - pj.y, dz = sz - pj.z;
-            const float r2 = dx * dx + dy * dy + dz * dz;
-            const float Hm = fmaxf(hi2x4, 4.0f * pj.w * pj.w);
-            if (r2 < Hm && r2 > 0.0f) {
-                if (cnt < F_SLOTS) lj[cnt * 32] = j;
-                ++cnt;
+        {   // copied entries are dealt out evenly: entry f of the target goes to slot f / 8 of
+            // lane f % 8 of the group, so that phase 2 has equally long columns
+            const int       sl = lane & (F_G - 1), g0 = lane & ~(F_G - 1);
+            unsigned        mk = covered ? nb_mask[(size_t)p * F_G + sl] : 0u;
+            const uint32_t* gj = nb_j + ((size_t)(covered ? p : 0) * F_SLOTS * F_G + sl);
+            const int       mine = __popc(mk);
+            int f = mine;   // inclusive scan over the group's lanes
+#pragma unroll
+            for (int o = 1; o < F_G; o <<= 1) {
+                const int v = __shfl_up_sync(SPH_FULL, f, o, F_G);
+                if (sl >= o) f += v;
             }
-        });
+            const int total = __shfl_sync(SPH_FULL, f, F_G - 1, F_G);
+            f -= mine;
+            uint32_t* const lbase = &lists[wid].j[0][g0];
+            while (mk) {
+                const int k = __ffs(mk) - 1;
+                mk &= mk - 1u;
+                lbase[(f >> 3) * 32 + (f & (F_G - 1))] = gj[k * F_G];
+                ++f;
+            }
+            __syncwarp();
+            if (covered) cnt = (total - sl + F_G - 1) / F_G;   // entries sl, sl + 8, ...
+        }
+        if (__any_sync(SPH_FULL, tvalid && !covered)) {
+            sph_group_rows<F_G>(g, cell_start, pos_h, t.pi.x, t.pi.y, t.pi.z, R, tvalid && !covered,
+                                lane, rot, c_tested,
+                                [&](uint32_t j, const float4 pj, float sx, float sy, float sz) {
+                const float dx = sx - pj.x, dy = sy - pj.y, dz = sz - pj.z;
+                const float r2 = dx * dx + dy * dy + dz * dz;
+                const float Hm = fmaxf(hi2x4, 4.0f * pj.w * pj.w);
+                if (r2 < Hm && r2 > 0.0f) {
+                    if (cnt < F_SLOTS) lj[cnt * 32] = j;
+                    ++cnt;
+                }
+            });
+        }
         const bool ovf = sph_group_any<F_G>(cnt > F_SLOTS, lane);
 
         // ---- phase 2: the pairs of this lane's column
         Accum a;
         const int mycnt  = ovf ? 0 : cnt;
         const int maxcnt = __reduce_max_sync(SPH_FULL, mycnt);
+        // software-pipelined: the three records of entry k+1 are in flight while entry k is
+        // worked on (the loads are dependent L1/L2 gathers; nothing else hides their latency)
+        float4 pn = t.pi, vn = t.vi, rn = ri;
+        if (mycnt > 0) {
+            const uint32_t j = lj[0];
+            pn = __ldg(pos_h + j); vn = __ldg(vel_m + j); rn = __ldg(rcak + j);
+        }
         for (int k = 0; k < maxcnt; ++k) {
+            const float4 pj = pn, vj = vn, rj = rn;
+            if (k + 1 < mycnt) {
+                const uint32_t j = lj[(k + 1) * 32];
+                pn = __ldg(pos_h + j); vn = __ldg(vel_m + j); rn = __ldg(rcak + j);
+            }
             if (k < mycnt) {
-                const uint32_t j  = lj[k * 32];
-                const float4   pj = __ldg(pos_h + j);
                 float dx = t.pi.x - pj.x, dy = t.pi.y - pj.y, dz = t.pi.z - pj.z;
                 dx -= Lx * rintf(dx * iLx);   // minimum image (no-op on open axes)
                 dy -= Ly * rintf(dy * iLy);
                 dz -= Lz * rintf(dz * iLz);
-                force_pair(t, a, par, vel_m, rcak, j, dx, dy, dz, dx * dx + dy * dy + dz * dz, pj.w);
+                const float r2 = dx * dx + dy * dy + dz * dz;
+                // copied lists hold everything inside the kept radius: apply the pair test
+                if (r2 < fmaxf(hi2x4, 4.0f * pj.w * pj.w) && r2 > 0.0f)
+                    force_pair(t, a, par, vj, rj, dx, dy, dz, r2, pj.w);
             }
         }
         a.ax = sph_group_sum<F_G>(a.ax);
@@ -289,7 +334,7 @@ __global__ __launch_bounds__(256) void k_forces_fix(
                     const float dx = rr.sx - pj.x, dy = rr.sy - pj.y, dz = rr.sz - pj.z;
                     const float r2 = dx * dx + dy * dy + dz * dz;
                     if (r2 < fmaxf(hi2x4, 4.0f * pj.w * pj.w) && r2 > 0.0f)
-                        force_pair(t, a, par, vel_m, rcak, j, dx, dy, dz, r2, pj.w);
+                        force_pair(t, a, par, __ldg(vel_m + j), __ldg(rcak + j), dx, dy, dz, r2, pj.w);
                 }
                 c_tested += min(32u, rr.end - k0);
             }
@@ -337,7 +382,8 @@ int sph_launch_forces(sph_ctx* c, const float* m, const float* vx, const float* 
     const int nblk = (int)((n + F_TARGETS - 1) / F_TARGETS);
     k_forces<<<nblk, F_TPB, 0, s>>>((int)n, c->grid, c->cell_start, c->pos_h, c->vel_m, c->rcak,
                                     c->perm, par, ax, ay, az, dudt, mu_min, c->fix_list,
-                                    c->fix_cnt + 1, c->coarse_hmax, c->stats);
+                                    c->fix_cnt + 1, c->coarse_hmax, c->nb_j, c->nb_mask,
+                                    c->nb_rkeep, c->stats);
     k_forces_fix<<<c->sm_count * 4, 256, 0, s>>>(c->grid, c->cell_start, c->pos_h, c->vel_m,
                                                  c->rcak, c->perm, par, c->fix_list,
                                                  c->fix_cnt + 1, ax, ay, az, dudt, mu_min,

@@ -27,6 +27,8 @@ struct SphGrid {
     float ics[3];              // inverse coarse cell sides
 };
 #define SPH_COARSE_MAX (1 << 18)   // entries of the coarse max-h map
+#define SPH_G 8                    // lanes per target in the sweeps
+#define SPH_SLOTS 28               // list entries per lane (28 x 8 = 224 per target)
 
 enum {  // indices into the device counter block (uint64 each), mirrors sph_stats_t
     ST_DENS_TESTED = 0, ST_DENS_LISTED, ST_DENS_PAIRS, ST_DENS_SWEEPS, ST_DENS_RECOLLECT,
@@ -58,6 +60,10 @@ struct sph_ctx {
     float4*      rcak;         // sorted (rho, c, A = P/(Omega rho^2), K = 5 sigma / h^5)
     unsigned*    coarse_hmax;  // SPH_COARSE_MAX: max h (float bits) per coarse cell, step a6
     unsigned long long* stats; // ST_NCOUNTERS
+    uint32_t*    nb_j;         // n_max x SPH_SLOTS x SPH_G: the density sweep's neighbour indices,
+                               // [target][slot][lane]; reused by the force sweep
+    uint32_t*    nb_mask;      // n_max x SPH_G: slots of a lane's column with r < nb_rkeep
+    float*       nb_rkeep;     // n_max: radius inside which list + mask are complete (0: none)
     int32_t*     fix_list;     // n_max: sorted positions queued for the robust (fix) kernels
     unsigned*    fix_cnt;      // [2]: queue lengths (density, forces)
     float*       dt_part;      // per-block minima of the time-step reduction
@@ -240,18 +246,9 @@ __device__ __forceinline__ void sph_group_rows(const SphGrid& g,
     constexpr unsigned GM = (G == 32) ? 0xffffffffu : ((1u << G) - 1u);
     const int sl = lane & (G - 1);
     const int g0 = lane & ~(G - 1);
-    int x0, x1, y0, y1, z0, z1;
-    sph_axis_range(xi, R, g.lo[0], g.isx, g.nx, g.per[0], x0, x1);
+    int y0, y1, z0, z1;
     sph_axis_range(yi, R, g.lo[1], g.isy, g.ny, g.per[1], y0, y1);
     sph_axis_range(zi, R, g.lo[2], g.isz, g.nz, g.per[2], z0, z1);
-    int         kx0;
-    const int   c0   = sph_wrap(x0, g.nx, kx0);
-    const int   span = x1 - x0;
-    const int   a_c1 = min(c0 + span, g.nx - 1);
-    const bool  two  = (c0 + span > g.nx - 1);
-    const int   b_c1 = min(c0 + span - g.nx, g.nx - 1);
-    const float sxA  = xi - (float)kx0 * g.len[0];
-    const float sxB  = xi - (float)(kx0 + 1) * g.len[0];
     const int   nyr  = y1 - y0 + 1, nzr = z1 - z0 + 1;
     const int   nrow = active ? nyr * nzr : 0;
     const float inv_nyr = __fdividef(1.0f, (float)nyr);
@@ -264,29 +261,37 @@ __device__ __forceinline__ void sph_group_rows(const SphGrid& g,
         const int iz = (int)(((float)r + 0.5f) * inv_nyr), iy = r - iz * nyr;
         const int uy = y0 + iy, uz = z0 + iz;
         uint32_t  a0 = 0, a1 = 0, b0 = 0, b1 = 0;
-        float     sy = yi, sz = zi;
+        float     sy = yi, sz = zi, sxa = xi;
+        float     d2 = 0.0f;
         if (ok) {
             const float dy = sph_slab_dist(yi, uy, g.lo[1], g.sy, g.ny, g.per[1]);
             const float dz = sph_slab_dist(zi, uz, g.lo[2], g.sz, g.nz, g.per[2]);
-            ok = (dy * dy + dz * dz <= R2);
+            d2 = dy * dy + dz * dz;
+            ok = (d2 <= R2);
         }
         if (ok) {
-            int ky, kz;
+            int ky, kz, kx0;
             const int cy = sph_wrap(uy, g.ny, ky), cz = sph_wrap(uz, g.nz, kz);
             sy = yi - (float)ky * g.len[1];
             sz = zi - (float)kz * g.len[2];
+            // the row only matters over the chord of the search ball at its distance
+            int x0, x1;
+            sph_axis_range(xi, sqrtf(R2 - d2), g.lo[0], g.isx, g.nx, g.per[0], x0, x1);
+            const int c0   = sph_wrap(x0, g.nx, kx0);
+            const int span = x1 - x0;
+            sxa = xi - (float)kx0 * g.len[0];
             const uint32_t rq = (uint32_t)(cz * g.ny + cy) * (uint32_t)g.nx;
             a0 = __ldg(cell_start + rq + c0);
-            a1 = __ldg(cell_start + rq + a_c1 + 1);
-            if (two) {
+            a1 = __ldg(cell_start + rq + min(c0 + span, g.nx - 1) + 1);
+            if (c0 + span > g.nx - 1) {   // the row crosses the periodic face: second segment
                 b0 = __ldg(cell_start + rq);
-                b1 = __ldg(cell_start + rq + b_c1 + 1);
+                b1 = __ldg(cell_start + rq + min(c0 + span - g.nx, g.nx - 1) + 1);
             }
         }
         const int nseg = __any_sync(SPH_FULL, b1 > b0) ? 2 : 1;
         for (int seg = 0; seg < nseg; ++seg) {
             const uint32_t s0 = seg ? b0 : a0, s1 = seg ? b1 : a1;
-            const float    sxx = seg ? sxB : sxA;
+            const float    sxs = seg ? sxa - g.len[0] : sxa;
             unsigned gm = (__ballot_sync(SPH_FULL, s1 > s0) >> g0) & GM;
             const int nk = __reduce_max_sync(SPH_FULL, __popc(gm));
             for (int k = 0; k < nk; ++k) {
@@ -295,6 +300,7 @@ __device__ __forceinline__ void sph_group_rows(const SphGrid& g,
                 gm &= gm - 1u;
                 uint32_t       rs  = __shfl_sync(SPH_FULL, s0, src);
                 uint32_t       re  = __shfl_sync(SPH_FULL, s1, src);
+                const float    sxx = __shfl_sync(SPH_FULL, sxs, src);
                 const float    rsy = __shfl_sync(SPH_FULL, sy, src);
                 const float    rsz = __shfl_sync(SPH_FULL, sz, src);
                 if (!have) re = rs;
