@@ -66,7 +66,7 @@ extern "C" int sph_create(sph_ctx** out, const sph_params* params, const sph_box
     ok = ok && dalloc(&c->stats, (size_t)ST_NCOUNTERS) == cudaSuccess;
     ok = ok && dalloc(&c->coarse_hmax, (size_t)SPH_COARSE_MAX) == cudaSuccess;
     ok = ok && dalloc(&c->nb_j, (size_t)n_max * SPH_SLOTS * SPH_G) == cudaSuccess;
-    ok = ok && dalloc(&c->nb_mask, (size_t)n_max * SPH_G) == cudaSuccess;
+    ok = ok && dalloc(&c->nb_cnt, (size_t)n_max) == cudaSuccess;
     ok = ok && dalloc(&c->nb_rkeep, (size_t)n_max) == cudaSuccess;
     ok = ok && dalloc(&c->fix_list, (size_t)n_max) == cudaSuccess;
     ok = ok && dalloc(&c->fix_cnt, (size_t)2) == cudaSuccess;
@@ -94,7 +94,7 @@ extern "C" void sph_destroy(sph_ctx* c) {
     cudaFree(c->rcak);      cudaFree(c->stats);     cudaFree(c->dt_part);
     cudaFree(c->nb_total);  cudaFree(c->fix_list);  cudaFree(c->fix_cnt);
     cudaFree(c->coarse_hmax);
-    cudaFree(c->nb_j);      cudaFree(c->nb_mask);   cudaFree(c->nb_rkeep);
+    cudaFree(c->nb_j);      cudaFree(c->nb_cnt);   cudaFree(c->nb_rkeep);
     delete c;
 }
 

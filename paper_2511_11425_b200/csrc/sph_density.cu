@@ -2,10 +2,11 @@
 // length solve, PAPER.md:137-154 (Section 2.3.3), Eqs. (5)-(7).
 //
 // G = 8 lanes per target particle, four targets per warp.  The lanes of a group walk the
-// candidate rows of the cell grid (coalesced float4 loads), every lane keeps the candidates
-// it accepted in a private column of a shared-memory list (r, m) -- the paper's "we keep the
-// precomputed interaction list", built for a "slightly larger kernel" -- and
-// the root of Eq. (6) is then found on that list alone.  Targets the lean kernel cannot
+// candidate rows of the cell grid (coalesced float4 loads); the accepted candidates of a
+// target are numbered by a group ballot and dealt out to the 8 lanes' columns of a shared-
+// memory list (r, m) -- the paper's "we keep the precomputed interaction list", built for a
+// "slightly larger kernel" -- and the root of Eq. (6) is then found on that
+// list alone.  The indices j go to a global list that the force sweep reuses.  Targets the lean kernel cannot
 // finish (a list column overflows, an entry sits in the FP32-uncertain band around 2h, the
 // iteration does not converge) are queued for k_density_fix, which re-walks the rows in
 // every sweep with one warp per target and decides borderline neighbours in FP64.
@@ -98,7 +99,7 @@ __global__ __launch_bounds__(D_TPB, SPH_MINB) void k_density(
     int n, const SphGrid* __restrict__ gp, const uint32_t* __restrict__ cell_start,
     const float4* __restrict__ pos_m, const int32_t* __restrict__ perm, DensPar par, float* h_io,
     float* rho, float* omega, int32_t* nn, int32_t* fix_list, unsigned* fix_cnt, uint32_t* nb_j,
-    uint32_t* nb_mask, float* nb_rkeep, unsigned long long* stats) {
+    uint32_t* nb_cnt, float* nb_rkeep, unsigned long long* stats) {
     __shared__ WarpList lists[D_WARPS];
     __shared__ SphGrid  g;
     __shared__ unsigned st_sh[5];
@@ -112,8 +113,11 @@ __global__ __launch_bounds__(D_TPB, SPH_MINB) void k_density(
     const int   wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int   gq  = lane / D_G;
     const bool  leader = (lane & (D_G - 1)) == 0;
+    const int   sl = lane & (D_G - 1), g0 = lane & ~(D_G - 1);
     float* const lr = &lists[wid].r[0][lane];   // this lane's column, slot stride 32 floats
     float* const lm = &lists[wid].m[0][lane];
+    float* const gr = &lists[wid].r[0][g0];     // the group's columns: entry f -> [f / 8][f % 8]
+    float* const gm_ = &lists[wid].m[0][g0];
     const float hcap   = density_hcap(g);
     const float band_c = 2.5e-7f * g.xext;      // sph_band(h) = 1e-6 + band_c / h
 
@@ -137,12 +141,11 @@ __global__ __launch_bounds__(D_TPB, SPH_MINB) void k_density(
         if (!(h > 0.0f) || !(h < 3.0e38f)) h = g.hmin;
         h = fminf(h, hcap);
         const float T = par.n_ngb * pi.w * (1.0f / 14.0f);
-        // this lane's column of the kept list: [target][slot][lane of the group]
-        uint32_t* const gj = nb_j + ((size_t)(tvalid ? p : 0) * D_SLOTS * D_G + (lane & (D_G - 1)));
+        // the target's kept list: entry f at [target][f]
+        uint32_t* const gj = nb_j + (size_t)(tvalid ? p : 0) * (D_SLOTS * D_G);
         float    hlo = 0.0f, hhi = __int_as_float(0x7f800000);
         float    Rc = 0.0f;         // radius the list is complete for
-        int      cnt = 0;           // entries in this lane's column
-        unsigned rot = 0;
+        int      cnt = 0;           // entries in the target's list (uniform in the group)
         bool     first = true, done = !tvalid, fix = false;
         float    S = 0.0f, E = 0.0f;
         int      sweeps = 0;
@@ -160,28 +163,27 @@ __global__ __launch_bounds__(D_TPB, SPH_MINB) void k_density(
                     cnt   = 0;
                 }
                 const float Rc2 = Rc * Rc;
-                sph_group_rows<D_G>(g, cell_start, pos_m, pi.x, pi.y, pi.z, Rc, need, lane, rot,
-                                    c_tested,
-                                    [&](uint32_t j, const float4 pj, float sx, float sy, float sz) {
-                    const float dx = sx - pj.x, dy = sy - pj.y, dz = sz - pj.z;
-                    const float r2 = dx * dx + dy * dy + dz * dz;
-                    if (r2 < Rc2) {
-                        if (cnt < D_SLOTS) {
-                            lr[cnt * 32] = r2 * rsqrtf(fmaxf(r2, 1e-35f));
-                            lm[cnt * 32] = pj.w;
-                            gj[cnt * D_G] = j;
-                        }
-                        ++cnt;
+                sph_group_collect<D_G>(g, cell_start, pos_m, pi.x, pi.y, pi.z, Rc, need, lane,
+                                       c_tested, cnt,
+                                       [&](const float4, float r2) { return r2 < Rc2; },
+                                       [&](int f, uint32_t j, const float4 pj, float, float, float,
+                                           float r2) {
+                    if (f < D_SLOTS * D_G) {
+                        const int o = (f >> 3) * 32 + (f & (D_G - 1));
+                        gr[o]  = r2 * rsqrtf(fmaxf(r2, 1e-35f));
+                        gm_[o] = pj.w;
+                        gj[f]  = j;
                     }
                 });
-                if (sph_group_any<D_G>(need && cnt > D_SLOTS, lane) && need) {
-                    done = true;     // a column overflowed: leave the target to k_density_fix
+                __syncwarp();
+                if (need && cnt > D_SLOTS * D_G) {
+                    done = true;     // the list overflowed: leave the target to k_density_fix
                     fix  = true;
                 }
             }
             // ---- one sweep over the lists: S(h), E(h), F(h)
             float s = 0.0f, e = 0.0f, f2 = 0.0f;
-            const int mycnt  = done ? 0 : cnt;
+            const int mycnt  = done ? 0 : (cnt - sl + D_G - 1) >> 3;   // entries sl, sl + 8, ...
             const int maxcnt = __reduce_max_sync(SPH_FULL, mycnt);
             for (int k = 0; k < maxcnt; ++k) {
                 if (k < mycnt) {
@@ -216,24 +218,33 @@ __global__ __launch_bounds__(D_TPB, SPH_MINB) void k_density(
         // around 2h sends the target to the exact recount of k_density_fix.
         const float H = 2.0f * h, tauH = (1e-6f + band_c / h) * H;
         const float Rk = fminf(Rc, H * D_KEEP);   // the kept list is complete inside Rk
-        int      ni = 0;
-        unsigned keep = 0u;
-        bool     edge = false;
-        if (tvalid && !fix) {
-            for (int k = 0; k < cnt; ++k) {
-                const float r = lr[k * 32];
+        // The same pass compacts the global index list in place to the entries inside Rk.
+        int  ni = 0, kept = 0;
+        bool edge = false;
+        {
+            const int mycnt  = (tvalid && !fix) ? (cnt - sl + D_G - 1) >> 3 : 0;
+            const int maxcnt = __reduce_max_sync(SPH_FULL, mycnt);
+            for (int k = 0; k < maxcnt; ++k) {
+                const bool  valid = k < mycnt;
+                const float r = valid ? lr[k * 32] : 3.0e38f;
                 ni += (r < H) ? 1 : 0;
                 edge |= fabsf(r - H) <= tauH;
-                keep |= (r < Rk) ? (1u << k) : 0u;
+                const bool     keep = r < Rk;
+                const unsigned km = (__ballot_sync(SPH_FULL, keep) >> g0) & ((1u << D_G) - 1u);
+                uint32_t j = 0;
+                if (keep) j = gj[k * D_G + sl];
+                __syncwarp();   // all reads of this slot before any lane overwrites part of it
+                if (keep) gj[kept + __popc(km & ((1u << sl) - 1u))] = j;   // target <= source
+                kept += __popc(km);
             }
-            nb_mask[(size_t)p * D_G + (lane & (D_G - 1))] = keep;
         }
         const bool recount = sph_group_any<D_G>(edge, lane) && !fix;   // h, rho, Omega stand
         ni = sph_group_sum_int<D_G>(ni);
-        if (tvalid) c_listed += cnt;
+        if (tvalid && leader) c_listed += cnt;
         if (tvalid && leader) {
             h_io[i] = h;   // final, or the best iterate for the fix kernel to start from
             nb_rkeep[p] = fix ? 0.0f : Rk;
+            nb_cnt[p]   = kept;
             c_sweeps += sweeps;
             if (!fix) {
                 const float ih = 1.0f / h;
@@ -384,7 +395,7 @@ int sph_launch_density(sph_ctx* c, const float* m, float* h, float* rho, float* 
     DensPar par{c->par.n_ngb, c->par.h_tol, c->par.search_slack, c->par.h_max_iter};
     const int nblk = (int)((n + D_TARGETS - 1) / D_TARGETS);
     k_density<<<nblk, D_TPB, 0, s>>>((int)n, c->grid, c->cell_start, c->pos_m, c->perm, par, h, rho,
-                                     omega, nn, c->fix_list, c->fix_cnt, c->nb_j, c->nb_mask,
+                                     omega, nn, c->fix_list, c->fix_cnt, c->nb_j, c->nb_cnt,
                                      c->nb_rkeep, c->stats);
     k_density_fix<<<c->sm_count * 4, 256, 0, s>>>(c->grid, c->cell_start, c->pos_m, c->perm, par,
                                                   c->fix_list, c->fix_cnt, h, rho, omega, nn,

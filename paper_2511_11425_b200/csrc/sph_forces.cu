@@ -4,9 +4,10 @@
 //
 // G = 8 lanes per target, four targets per warp.  Phase 1: the lanes of a group distance-
 // test the candidates of the rows in reach (0 < r < 2 max(h_i,h_j), gather and scatter,
-// PAPER.md:191) and each lane notes the indices it accepted in a private column of a
-// shared-memory list.  Phase 2: every lane works through its own column -- the pair
-// arithmetic runs without divergence between accepted and rejected candidates.  A group
+// PAPER.md:191); the accepted ones are numbered by a group ballot into the target's index
+// list -- or, when the list the density sweep kept already covers the reach, that list is
+// used as it is.  Phase 2: lane l of the group works through entries l, l + 8, ... -- the
+// pair arithmetic runs without divergence between accepted and rejected candidates.  A group
 // whose column overflows is queued for k_forces_fix (one warp per target, no list).
 //
 // Pair arithmetic (d = x_i - x_j, r = |d|, q_a = r/h_a, g_a = K_a (1-q_a/2)_+^3 with
@@ -146,7 +147,7 @@ __global__ __launch_bounds__(F_TPB, SPH_FMINB) void k_forces(
     const float4* __restrict__ rcak, const int32_t* __restrict__ perm, ForcePar par, float* ax,
     float* ay, float* az, float* dudt, float* mu_min, int32_t* fix_list, unsigned* fix_cnt,
     const unsigned* __restrict__ coarse, const uint32_t* __restrict__ nb_j,
-    const uint32_t* __restrict__ nb_mask, const float* __restrict__ nb_rkeep,
+    const uint32_t* __restrict__ nb_cnt, const float* __restrict__ nb_rkeep,
     unsigned long long* stats) {
     __shared__ FWarpList lists[F_WARPS];
     __shared__ SphGrid   g;
@@ -192,67 +193,47 @@ __global__ __launch_bounds__(F_TPB, SPH_FMINB) void k_forces(
                         sph_scatter_hmax<F_G>(g, coarse, t.pi.x, t.pi.y, t.pi.z, t.pi.w, hmax_all, lane);
         const float hi2x4 = 4.0f * t.pi.w * t.pi.w;
 
-        // ---- phase 1: lane-private index lists.  If the list kept by the density sweep is
-        // complete out to R (same positions) it is copied; else search.
+        // ---- phase 1: the target's index list, entry f handled by lane f % 8 of the group.
+        // If the list kept by the density sweep is complete out to R (same positions,
+        // DESIGN.md section 7) it is read in place from global memory; else search.
+        const int   sl = lane & (F_G - 1), g0 = lane & ~(F_G - 1);
         const float rk      = tvalid ? nb_rkeep[p] : 0.0f;
         const float tau     = 1e-6f + 2.5e-7f * g.xext * t.ih;
         const bool  covered = tvalid && (R * (1.0f + 4.0f * tau) <= rk);
-        int      cnt = 0;
-        unsigned rot = 0;
-        {   // copied entries are dealt out evenly: entry f of the target goes to slot f / 8 of
-            // lane f % 8 of the group, so that phase 2 has equally long columns
-            const int       sl = lane & (F_G - 1), g0 = lane & ~(F_G - 1);
-            unsigned        mk = covered ? nb_mask[(size_t)p * F_G + sl] : 0u;
-            const uint32_t* gj = nb_j + ((size_t)(covered ? p : 0) * F_SLOTS * F_G + sl);
-            const int       mine = __popc(mk);
-            int f = mine;   // inclusive scan over the group's lanes
-#pragma unroll
-            for (int o = 1; o < F_G; o <<= 1) {
-                const int v = __shfl_up_sync(SPH_FULL, f, o, F_G);
-                if (sl >= o) f += v;
-            }
-            const int total = __shfl_sync(SPH_FULL, f, F_G - 1, F_G);
-            f -= mine;
-            uint32_t* const lbase = &lists[wid].j[0][g0];
-            while (mk) {
-                const int k = __ffs(mk) - 1;
-                mk &= mk - 1u;
-                lbase[(f >> 3) * 32 + (f & (F_G - 1))] = gj[k * F_G];
-                ++f;
-            }
+        int cnt = covered ? (int)nb_cnt[p] : 0;
+        const bool search = tvalid && !covered;
+        if (__any_sync(SPH_FULL, search)) {
+            uint32_t* const gl = &lists[wid].j[0][g0];
+            sph_group_collect<F_G>(g, cell_start, pos_h, t.pi.x, t.pi.y, t.pi.z, R, search, lane,
+                                   c_tested, cnt,
+                                   [&](const float4 pj, float r2) {
+                                       return r2 < fmaxf(hi2x4, 4.0f * pj.w * pj.w) && r2 > 0.0f;
+                                   },
+                                   [&](int f, uint32_t j, const float4, float, float, float, float) {
+                                       if (f < F_SLOTS * F_G) gl[(f >> 3) * 32 + (f & (F_G - 1))] = j;
+                                   });
             __syncwarp();
-            if (covered) cnt = (total - sl + F_G - 1) / F_G;   // entries sl, sl + 8, ...
         }
-        if (__any_sync(SPH_FULL, tvalid && !covered)) {
-            sph_group_rows<F_G>(g, cell_start, pos_h, t.pi.x, t.pi.y, t.pi.z, R, tvalid && !covered,
-                                lane, rot, c_tested,
-                                [&](uint32_t j, const float4 pj, float sx, float sy, float sz) {
-                const float dx = sx - pj.x, dy = sy - pj.y, dz = sz - pj.z;
-                const float r2 = dx * dx + dy * dy + dz * dz;
-                const float Hm = fmaxf(hi2x4, 4.0f * pj.w * pj.w);
-                if (r2 < Hm && r2 > 0.0f) {
-                    if (cnt < F_SLOTS) lj[cnt * 32] = j;
-                    ++cnt;
-                }
-            });
-        }
-        const bool ovf = sph_group_any<F_G>(cnt > F_SLOTS, lane);
+        const bool ovf = search && cnt > F_SLOTS * F_G;
 
-        // ---- phase 2: the pairs of this lane's column
+        // ---- phase 2: entries sl, sl + 8, ... of the list.  The 8 lanes of a group work on 8
+        // consecutive entries, i.e. mostly on neighbouring records of the sorted arrays, so the
+        // three 16-byte gathers per pair touch a few lines per group instead of one per lane.
         Accum a;
-        const int mycnt  = ovf ? 0 : cnt;
+        const uint32_t* const src = covered ? nb_j + ((size_t)p * (F_SLOTS * F_G) + sl) : lj;
+        const int stride = covered ? F_G : 32;
+        const int mycnt  = ovf ? 0 : (cnt - sl + F_G - 1) >> 3;
         const int maxcnt = __reduce_max_sync(SPH_FULL, mycnt);
-        // software-pipelined: the three records of entry k+1 are in flight while entry k is
-        // worked on (the loads are dependent L1/L2 gathers; nothing else hides their latency)
+        // software-pipelined: the records of entry k+1 are in flight while entry k is worked on
         float4 pn = t.pi, vn = t.vi, rn = ri;
         if (mycnt > 0) {
-            const uint32_t j = lj[0];
+            const uint32_t j = src[0];
             pn = __ldg(pos_h + j); vn = __ldg(vel_m + j); rn = __ldg(rcak + j);
         }
         for (int k = 0; k < maxcnt; ++k) {
             const float4 pj = pn, vj = vn, rj = rn;
             if (k + 1 < mycnt) {
-                const uint32_t j = lj[(k + 1) * 32];
+                const uint32_t j = src[(k + 1) * stride];
                 pn = __ldg(pos_h + j); vn = __ldg(vel_m + j); rn = __ldg(rcak + j);
             }
             if (k < mycnt) {
@@ -261,7 +242,7 @@ __global__ __launch_bounds__(F_TPB, SPH_FMINB) void k_forces(
                 dy -= Ly * rintf(dy * iLy);
                 dz -= Lz * rintf(dz * iLz);
                 const float r2 = dx * dx + dy * dy + dz * dz;
-                // copied lists hold everything inside the kept radius: apply the pair test
+                // kept lists hold everything inside the kept radius: apply the pair test
                 if (r2 < fmaxf(hi2x4, 4.0f * pj.w * pj.w) && r2 > 0.0f)
                     force_pair(t, a, par, vj, rj, dx, dy, dz, r2, pj.w);
             }
@@ -382,7 +363,7 @@ int sph_launch_forces(sph_ctx* c, const float* m, const float* vx, const float* 
     const int nblk = (int)((n + F_TARGETS - 1) / F_TARGETS);
     k_forces<<<nblk, F_TPB, 0, s>>>((int)n, c->grid, c->cell_start, c->pos_h, c->vel_m, c->rcak,
                                     c->perm, par, ax, ay, az, dudt, mu_min, c->fix_list,
-                                    c->fix_cnt + 1, c->coarse_hmax, c->nb_j, c->nb_mask,
+                                    c->fix_cnt + 1, c->coarse_hmax, c->nb_j, c->nb_cnt,
                                     c->nb_rkeep, c->stats);
     k_forces_fix<<<c->sm_count * 4, 256, 0, s>>>(c->grid, c->cell_start, c->pos_h, c->vel_m,
                                                  c->rcak, c->perm, par, c->fix_list,

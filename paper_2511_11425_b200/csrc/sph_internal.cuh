@@ -61,8 +61,8 @@ struct sph_ctx {
     unsigned*    coarse_hmax;  // SPH_COARSE_MAX: max h (float bits) per coarse cell, step a6
     unsigned long long* stats; // ST_NCOUNTERS
     uint32_t*    nb_j;         // n_max x SPH_SLOTS x SPH_G: the density sweep's neighbour indices,
-                               // [target][slot][lane]; reused by the force sweep
-    uint32_t*    nb_mask;      // n_max x SPH_G: slots of a lane's column with r < nb_rkeep
+                               // [target][entry]; reused by the force sweep
+    uint32_t*    nb_cnt;       // n_max: entries of the kept list (those with r < nb_rkeep)
     float*       nb_rkeep;     // n_max: radius inside which list + mask are complete (0: none)
     int32_t*     fix_list;     // n_max: sorted positions queued for the robust (fix) kernels
     unsigned*    fix_cnt;      // [2]: queue lengths (density, forces)
@@ -231,18 +231,22 @@ __device__ __forceinline__ int sph_wrap(int u, int n, int& k) {   // u = c + k n
     return min(max(c, 0), n - 1);   // memory-safe even for coordinates outside a periodic box
 }
 
-// Calls test(j, pj, sx, sy, sz) on ONE lane for every candidate source j of that lane's
-// target: pj = pos[j], and d = (sx - pj.x, sy - pj.y, sz - pj.z) is the displacement to the
-// right periodic image.  `active` (uniform in a group) switches a group off.  `rot`
-// (uniform in a group) rotates the lane a row starts on, so that candidates -- and with them
-// the lane-private lists built from them -- spread evenly over the G lanes.  `tested` is
-// advanced by the number of candidates on the group's first lane.
-template <int G, class Test>
-__device__ __forceinline__ void sph_group_rows(const SphGrid& g,
-                                               const uint32_t* __restrict__ cell_start,
-                                               const float4* __restrict__ pos, float xi, float yi,
-                                               float zi, float R, bool active, int lane,
-                                               unsigned& rot, unsigned& tested, Test&& test) {
+// Walks the candidate sources of every group's target and compacts the accepted ones.
+// For candidate j (pj = pos[j], d = displacement to the right periodic image, r2 = |d|^2)
+// `accept(pj, r2)` decides; the accepted candidates of a target are numbered 0, 1, 2, ... in
+// the order of the sorted arrays (group ballot), and `store(f, j, pj, dx, dy, dz, r2)` is
+// called on the lane that tested number f.  Keeping entry f in slot f / G of lane f % G
+// gives every lane of the group an equally long column AND makes the G lanes work on G
+// consecutive -- mostly memory-adjacent -- sources later.  `total` (uniform in a group) is
+// advanced by the number accepted, `tested` by the number of candidates (first lane only).
+// `active` (uniform in a group) switches a group off.
+template <int G, class Accept, class Store>
+__device__ __forceinline__ void sph_group_collect(const SphGrid& g,
+                                                  const uint32_t* __restrict__ cell_start,
+                                                  const float4* __restrict__ pos, float xi,
+                                                  float yi, float zi, float R, bool active,
+                                                  int lane, unsigned& tested, int& total,
+                                                  Accept&& accept, Store&& store) {
     constexpr unsigned GM = (G == 32) ? 0xffffffffu : ((1u << G) - 1u);
     const int sl = lane & (G - 1);
     const int g0 = lane & ~(G - 1);
@@ -304,20 +308,26 @@ __device__ __forceinline__ void sph_group_rows(const SphGrid& g,
                 const float    rsy = __shfl_sync(SPH_FULL, sy, src);
                 const float    rsz = __shfl_sync(SPH_FULL, sz, src);
                 if (!have) re = rs;
-                uint32_t c = rs + ((sl - rot) & (G - 1));
-                rot = (rot + (re - rs)) & (G - 1);
+                uint32_t c = rs + sl;
                 if (sl == 0) tested += re - rs;
                 do {   // SPH_UNROLL windows per trip: as many independent loads in flight
-                    bool   vv[SPH_UNROLL];
                     float4 pp[SPH_UNROLL];
 #pragma unroll
                     for (int u = 0; u < SPH_UNROLL; ++u) {
-                        vv[u] = c + u * G < re;
-                        if (vv[u]) pp[u] = __ldg(pos + c + u * G);
+                        pp[u] = make_float4(3.0e18f, 3.0e18f, 3.0e18f, 0.0f);
+                        if (c + u * G < re) pp[u] = __ldg(pos + c + u * G);
                     }
 #pragma unroll
-                    for (int u = 0; u < SPH_UNROLL; ++u)
-                        if (vv[u]) test(c + u * G, pp[u], sxx, rsy, rsz);
+                    for (int u = 0; u < SPH_UNROLL; ++u) {
+                        const float dx = sxx - pp[u].x, dy = rsy - pp[u].y, dz = rsz - pp[u].z;
+                        const float r2 = dx * dx + dy * dy + dz * dz;
+                        const bool  acc = (c + u * G < re) && accept(pp[u], r2);
+                        const unsigned gm = (__ballot_sync(SPH_FULL, acc) >> g0) & GM;
+                        if (acc)
+                            store(total + __popc(gm & ((1u << sl) - 1u)), c + u * G, pp[u], dx, dy,
+                                  dz, r2);
+                        total += __popc(gm);
+                    }
                     c += SPH_UNROLL * G;
                 } while (__any_sync(SPH_FULL, c < re));
             }
