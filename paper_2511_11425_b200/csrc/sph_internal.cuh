@@ -28,7 +28,7 @@ struct SphGrid {
 };
 #define SPH_COARSE_MAX (1 << 18)   // entries of the coarse max-h map
 #define SPH_G 8                    // lanes per target in the sweeps
-#define SPH_SLOTS 28               // list entries per lane (28 x 8 = 224 per target)
+#define SPH_SLOTS 24               // list entries per lane (24 x 8 = 192 per target)
 
 enum {  // indices into the device counter block (uint64 each), mirrors sph_stats_t
     ST_DENS_TESTED = 0, ST_DENS_LISTED, ST_DENS_PAIRS, ST_DENS_SWEEPS, ST_DENS_RECOLLECT,
