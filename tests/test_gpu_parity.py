@@ -288,3 +288,46 @@ def test_edge_cases_small_and_open_box(gu):
     off, idx = ctx.neighbors(h, 0)
     ooff, oidx = orc.neighbors(w["x"], w["y"], w["z"], h.cpu().numpy(), ob, 0)
     assert np.array_equal(off.cpu().numpy(), ooff)
+
+
+def test_c4_kelvin_helmholtz_full_size_sampled(gu):
+    """Config 4 (4 097 888 particles, 2:1 density slab with shear): a seeded sample plus the
+    particles nearest the two interfaces against the brute-force oracle."""
+    w = workloads.kelvin_helmholtz(h_start="warm")
+    _, op = gu.make_params(w)
+    _, ob = gu.make_boxes(w)
+    ctx, d, out, h = _full_step(gu, w)
+    st = ctx.stats()
+    assert st["dens_nonconv"] == 0 and st["grid_flags"] & 1 == 0, st
+    near = np.argsort(np.minimum(np.abs(w["y"] - 0.25), np.abs(w["y"] - 0.75)))[:4096]
+    sel = np.unique(np.concatenate([_sample(w["n"], 96, 41), near[_sample(len(near), 96, 42)]]))
+    _check_sample(gu, w, ctx, out, h, sel, op, ob)
+    assert st["force_av_pairs"] > 0          # the shear takes the viscosity branch
+
+
+def _impact_case(gu, n_target, n_impactor, k):
+    w = workloads.impact(n_target=n_target, n_impactor=n_impactor, h_start="warm")
+    _, op = gu.make_params(w)
+    _, ob = gu.make_boxes(w)
+    ctx, d, out, h = _full_step(gu, w)
+    st = ctx.stats()
+    assert st["dens_nonconv"] == 0, st
+    # free surfaces: half of the sample from the 2 % of particles with the largest h
+    big = np.argsort(w["h"])[-max(w["n"] // 50, k):]
+    sel = np.unique(np.concatenate([_sample(w["n"], k, 51), big[_sample(len(big), k, 52)]]))
+    _check_sample(gu, w, ctx, out, h, sel, op, ob)
+    hh = gu.np64(h)
+    assert hh.max() / hh.min() > 4.0         # the h contrast the configuration is there for
+    return st
+
+
+def test_c5_impact_reduced_size_free_surfaces(gu):
+    """Config 5's shape at 1/10 of its size (two n=1 polytropes in vacuum, ~1.3 M particles):
+    open box, one-sided neighbourhoods at the surfaces, h varying by an order of magnitude."""
+    _impact_case(gu, 1_200_000, 150_000, 64)
+
+
+def test_c5_impact_full_size_sampled(gu):
+    """Config 5 at BASELINE.json's full size: 12 M + 1.5 M lattice points before the surface
+    truncation (about 13.4 M particles), sampled like the reduced case (~25 s on a B200 box)."""
+    _impact_case(gu, 12_000_000, 1_500_000, 48)
