@@ -216,7 +216,16 @@ __global__ __launch_bounds__(D_TPB, SPH_MINB) void k_density(
 
         // ---- n_i = #{j : r_ij < 2h} from the list; an entry inside the FP32-uncertain band
         // around 2h sends the target to the exact recount of k_density_fix.
-        const float H = 2.0f * h, tauH = (1e-6f + band_c / h) * H;
+        // The FP32 distance is uncertain by tau(h) only for sources met through a periodic
+        // image (the shifted target coordinate is rounded); when the search ball stays inside
+        // the box the displacement x_i - x_j is exact to 2^-24 |d| and 2e-6 covers the rest.
+        bool wraps = false;
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+            const float xd = (d == 0 ? pi.x : d == 1 ? pi.y : pi.z) - g.lo[d];
+            wraps |= g.per[d] && (xd < Rc || xd + Rc > g.len[d]);
+        }
+        const float H = 2.0f * h, tauH = (wraps ? 1e-6f + band_c / h : 2e-6f) * H;
         const float Rk = fminf(Rc, H * D_KEEP);   // the kept list is complete inside Rk
         // The same pass compacts the global index list in place to the entries inside Rk.
         int  ni = 0, kept = 0;
