@@ -59,8 +59,8 @@ extern "C" int sph_create(sph_ctx** out, const sph_params* params, const sph_box
     ok = ok && dalloc(&c->perm, (size_t)n_max) == cudaSuccess;
     ok = ok && dalloc(&c->inv_perm, (size_t)n_max) == cudaSuccess;
     ok = ok && dalloc(&c->scan_part, (size_t)SPH_SCAN_BLOCKS + 1) == cudaSuccess;
-    ok = ok && dalloc(&c->pos_h, (size_t)n_max) == cudaSuccess;
-    ok = ok && dalloc(&c->pos_m, (size_t)n_max) == cudaSuccess;
+    ok = ok && dalloc(&c->pos_h, (size_t)n_max + SPH_POS_PAD) == cudaSuccess;
+    ok = ok && dalloc(&c->pos_m, (size_t)n_max + SPH_POS_PAD) == cudaSuccess;
     ok = ok && dalloc(&c->vel_m, (size_t)n_max) == cudaSuccess;
     ok = ok && dalloc(&c->rcak, (size_t)n_max) == cudaSuccess;
     ok = ok && dalloc(&c->stats, (size_t)ST_NCOUNTERS) == cudaSuccess;

@@ -4,6 +4,7 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <type_traits>
 #include "../../include/sph.h"
 
 // ---------------------------------------------------------------------------------------
@@ -27,6 +28,7 @@ struct SphGrid {
     float ics[3];              // inverse coarse cell sides
 };
 #define SPH_COARSE_MAX (1 << 18)   // entries of the coarse max-h map
+#define SPH_POS_PAD 64             // records of padding behind the sorted float4 arrays
 #define SPH_G 8                    // lanes per target in the sweeps
 #define SPH_SLOTS 24               // list entries per lane (24 x 8 = 192 per target)
 
@@ -310,15 +312,15 @@ __device__ __forceinline__ void sph_group_collect(const SphGrid& g,
                 if (!have) re = rs;
                 uint32_t c = rs + sl;
                 if (sl == 0) tested += re - rs;
-                do {   // SPH_UNROLL windows per trip: as many independent loads in flight
-                    float4 pp[SPH_UNROLL];
+                // NW windows of G candidates per trip, loaded unconditionally (the sorted arrays
+                // are padded by SPH_POS_PAD records, so reading past a row's end is harmless)
+                auto trip = [&](auto nw_tag) {
+                    constexpr int NW = decltype(nw_tag)::value;
+                    float4 pp[NW];
 #pragma unroll
-                    for (int u = 0; u < SPH_UNROLL; ++u) {
-                        pp[u] = make_float4(3.0e18f, 3.0e18f, 3.0e18f, 0.0f);
-                        if (c + u * G < re) pp[u] = __ldg(pos + c + u * G);
-                    }
+                    for (int u = 0; u < NW; ++u) pp[u] = __ldg(pos + c + u * G);
 #pragma unroll
-                    for (int u = 0; u < SPH_UNROLL; ++u) {
+                    for (int u = 0; u < NW; ++u) {
                         const float dx = sxx - pp[u].x, dy = rsy - pp[u].y, dz = rsz - pp[u].z;
                         const float r2 = dx * dx + dy * dy + dz * dz;
                         const bool  acc = (c + u * G < re) && accept(pp[u], r2);
@@ -328,8 +330,17 @@ __device__ __forceinline__ void sph_group_collect(const SphGrid& g,
                                   dz, r2);
                         total += __popc(gm);
                     }
-                    c += SPH_UNROLL * G;
-                } while (__any_sync(SPH_FULL, c < re));
+                    c += NW * G;
+                };
+                // the longest row among the four groups decides how many windows are issued
+                const int nwin = (__reduce_max_sync(SPH_FULL, re - rs) + (G - 1)) / G;
+                if (nwin == 1) {
+                    trip(std::integral_constant<int, 1>{});
+                } else if (nwin == 2) {
+                    trip(std::integral_constant<int, 2>{});
+                } else {
+                    for (int w = 0; w < nwin; w += SPH_UNROLL) trip(std::integral_constant<int, SPH_UNROLL>{});
+                }
             }
         }
     }
