@@ -6,10 +6,11 @@
 // target are numbered by a group ballot and dealt out to the 8 lanes' columns of a shared-
 // memory list (r, m) -- the paper's "we keep the precomputed interaction list", built for a
 // "slightly larger kernel" -- and the root of Eq. (6) is then found on that
-// list alone.  The indices j go to a global list that the force sweep reuses.  Targets the lean kernel cannot
-// finish (a list column overflows, an entry sits in the FP32-uncertain band around 2h, the
-// iteration does not converge) are queued for k_density_fix, which re-walks the rows in
-// every sweep with one warp per target and decides borderline neighbours in FP64.
+// list alone.  The indices j go to a global list that the force sweep reuses.
+// Targets the lean kernel cannot finish (a list longer than 192 entries, an entry in the
+// FP32-uncertain band around 2h, no convergence) are queued for k_density_fix, which
+// re-walks the rows in every sweep with one warp per target and decides borderline
+// neighbours in FP64.
 //
 // With w(q) = SIGMA wt(q), wt = (1-q/2)^4 (1+2q), t = 1-q/2, and per target
 //   S = sum_j m_j wt(q_j),  E = sum_j m_j 5 q^2 t^3,  F = sum_j m_j q^2 t^2 (10 t - 7.5 q):
