@@ -229,27 +229,53 @@ def run_gpu(a):
     h2d = sum(host[k].numel() * 4 for k in keys)
     d2h = sum(v.numel() * v.element_size() for v in outs_host.values()) + n * 4
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    # The copies of step k+1 (host -> device) and of step k-1 (device -> host) overlap the
+    # kernels of step k: two sets of device buffers, one copy stream per direction, events
+    # between them.  Every step still moves all of its inputs in and all of its results out.
+    main = torch.cuda.current_stream()
+    s_in, s_out = torch.cuda.Stream(), torch.cuda.Stream()
+    din = [d, {k: torch.empty_like(d[k]) for k in keys}]
+    dout = [out, sph.StepBuffers(n)]
+    dh = [h, torch.empty_like(h)]
+    ev_in = [torch.cuda.Event() for _ in range(2)]
+    ev_comp = [torch.cuda.Event() for _ in range(2)]
+    ev_out = [torch.cuda.Event() for _ in range(2)]
 
-    def e2e_step():
-        for k in keys:
-            d[k].copy_(host[k], non_blocking=True)
-        one_step()
-        for k, v in out.t.items():
-            outs_host[k].copy_(v, non_blocking=True)
-        h_host.copy_(h, non_blocking=True)
+    def e2e_step(k):
+        b = k & 1
+        with torch.cuda.stream(s_in):
+            s_in.wait_event(ev_comp[b])          # step k-2 no longer reads this input set
+            for key in keys:
+                din[b][key].copy_(host[key], non_blocking=True)
+            ev_in[b].record(s_in)
+        main.wait_event(ev_in[b])
+        main.wait_event(ev_out[b])               # step k-2's results have left this output set
+        dh[b].copy_(din[b]["h"])
+        sph.step(ctx, din[b], dout[b], dh[b])
+        ev_comp[b].record(main)
+        with torch.cuda.stream(s_out):
+            s_out.wait_event(ev_comp[b])
+            for key, v in dout[b].t.items():
+                outs_host[key].copy_(v, non_blocking=True)
+            h_host.copy_(dh[b], non_blocking=True)
+            ev_out[b].record(s_out)
 
-    e2e_step()
+    e2e_step(0)
+    e2e_step(1)
     barrier()
-    e0.record()
-    for _ in range(a.steps):
-        e2e_step()
-    e1.record()
+    e0.record(main)
+    s_in.wait_event(e0)
+    for k in range(a.steps):
+        e2e_step(k)
+    main.wait_stream(s_out)
+    main.wait_stream(s_in)
+    e1.record(main)
     barrier()
     e2e_ms = torch.tensor([e0.elapsed_time(e1)], device="cuda", dtype=torch.float64)
     if world > 1:
         dist.all_reduce(e2e_ms, op=dist.ReduceOp.MAX)
     clocks = sampler.stop() if sampler else None
-    assert abs(float(outs_host["dt_min"][0]) - float(out["dt_min"].item())) == 0.0
+    assert abs(float(outs_host["dt_min"][0]) - float(dout[(a.steps - 1) & 1]["dt_min"].item())) == 0.0
 
     if rank != 0:
         if world > 1:
@@ -297,7 +323,9 @@ def run_gpu(a):
                       step_frac=(f_dens + f_force) / (float(step_ms.mean()) * 1e-3) / 1e12 /
                                 NOMINAL_FP32_TFLOPS),
         e2e=dict(value=e2e_val, unit=UNIT, h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h,
-                 ms_per_step=float(e2e_ms.item()) / K),
+                 ms_per_step=float(e2e_ms.item()) / K,
+                 overlap="copies of steps k+1 / k-1 overlap the kernels of step k (two device "
+                         "buffer sets, one copy stream per direction)"),
         gpu_launches=KERNELS_PER_STEP * K, clocks=clocks)
     if world == 1 and not a.no_cpu_baseline:
         cb = oracle_sample(a.ref_nside, a.v_sigma)
