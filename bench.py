@@ -159,7 +159,7 @@ class ClockSampler:
 def run_gpu(a):
     import torch
     import torch.distributed as dist
-    from paper_2511_11425_b200 import sph, workloads
+    from paper_2511_11425_b200 import build as sph_build, sph, workloads
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -169,6 +169,10 @@ def run_gpu(a):
     torch.cuda.set_device(local)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if rank == 0:
+        sph_build.build()          # no-op when libsph_b200.so is up to date
+    if world > 1:
+        dist.barrier()
 
     def barrier():
         if world > 1:

@@ -6,7 +6,9 @@ import numpy as np
 import torch
 
 from oracle import sph_oracle as orc
-from paper_2511_11425_b200 import sph
+from paper_2511_11425_b200 import build as _build, sph
+
+_build.build()   # no-op when the library is up to date
 
 F_KEYS = ("x", "y", "z", "m", "vx", "vy", "vz", "u", "h")
 
