@@ -20,7 +20,7 @@
  *   - Call order: sph_build_cells -> sph_density_h -> sph_forces -> sph_timestep.
  *     sph_forces / sph_neighbors may be fed rho, h, Omega from elsewhere as long as
  *     sph_build_cells ran on the same positions (else SPH_ESTALE).
- *   - Kernel: Wendland C2 with support radius 2h (readings R2, R3)
+ *   - Kernels have support radius 2h (readings R2, R3), e.g. Wendland C2
  *       W(r,h) = h^-3 (21/(16 pi)) (1-q/2)^4 (1+2q),  q = r/h < 2.
  */
 #ifndef SPH_B200_H
@@ -50,7 +50,8 @@ typedef struct {
 } sph_box;
 
 typedef struct {
-    int32_t kernel;       /* 1 = Wendland C2 (the only one built)            */
+    int32_t kernel;       /* 0 cubic spline, 1 Wendland C2, 2 Wendland C4, 3 Wendland C6, all  */
+                          /* with support radius 2h                           */
     float   n_ngb;        /* kernel mass in units of m_i, Eq. (6) with R_kernel = 2h       */
     float   gamma;        /* ideal gas P = (gamma-1) rho u                  */
     float   av_alpha;     /* Eq. (15) alpha                                                */

@@ -6,7 +6,6 @@
 #include "sph_internal.cuh"
 
 static void fill_defaults(sph_params& p) {
-    if (p.kernel == 0) p.kernel = 1;
     if (!(p.n_ngb > 0.0f)) p.n_ngb = 64.0f;
     if (!(p.gamma > 1.0f)) p.gamma = 5.0f / 3.0f;
     if (!(p.av_eps > 0.0f)) p.av_eps = 0.01f;
@@ -27,8 +26,11 @@ static cudaError_t dalloc(T** p, size_t count) {
 extern "C" int sph_create(sph_ctx** out, const sph_params* params, const sph_box* box,
                           int64_t n_max, void* cuda_stream) {
     if (!out || !params || !box || n_max <= 0 || n_max > (int64_t)0x7fffff00) return SPH_EINVAL;
-    if (params->kernel != 0 && params->kernel != 1) return SPH_EINVAL;
-    if (params->n_ngb > 0.0f && params->n_ngb <= 14.0f) return SPH_EINVAL;  // root must exist
+    if (params->kernel < 0 || params->kernel > 3) return SPH_EINVAL;
+    {   // Eq. (6) has a root only if the target exceeds the self contribution (32 pi/3) W(0) h^3
+        static const float self[4] = {32.0f / 3.0f, 14.0f, 20.625f, 28.4375f};
+        if (params->n_ngb > 0.0f && params->n_ngb <= self[params->kernel]) return SPH_EINVAL;
+    }
     for (int d = 0; d < 3; ++d)
         if (!(box->len[d] > 0.0f)) return SPH_EINVAL;
     sph_ctx* c = new (std::nothrow) sph_ctx;

@@ -12,15 +12,16 @@
 // re-walks the rows in every sweep with one warp per target and decides borderline
 // neighbours in FP64.
 //
-// With w(q) = SIGMA wt(q), wt = (1-q/2)^4 (1+2q), t = 1-q/2, and per target
-//   S = sum_j m_j wt(q_j),  E = sum_j m_j 5 q^2 t^3,  F = sum_j m_j q^2 t^2 (10 t - 7.5 q):
-//   Eq. (6)  <=>  f(h) = S(h) - T = 0,  T = n_ngb m_i / 14         ((32 pi/3) SIGMA = 14)
+// With W = sigma h^-3 w(q) (SphKernel<KERN> in sph_internal.cuh) and per target
+//   S = sum_j m_j w(q_j),  E = -sum_j m_j q w'(q),  F = -sum_j m_j (q w' + q^2 w''):
+//   (Wendland C2: w = (1-q/2)^4 (1+2q), E-term 5 q^2 t^3, F-term q^2 t^2 (10 t - 7.5 q), t = 1-q/2)
+//   Eq. (6)  <=>  f(h) = S(h) - T = 0,  T = n_ngb m_i / ((32 pi/3) sigma)       (C2: 14)
 //   f' = dS/dh = E/h,   dE/dh = -F/h,   f'' = -(E + F)/h^2
 //   Halley step (the paper's Newton-Raphson with the second derivative added):
 //       dh = -2 f f' / (2 f'^2 - f f'') = -2 f E h / (2 E^2 + f (E + F))
 //   A step with |dh| <= 3e-4 h is accepted; S and E are carried to h + dh by their Taylor
 //   series (error O((dh/h)^3) and O((dh/h)^2)), so the accepted sweep is also the last one.
-//   Eq. (5)   rho = SIGMA S / h^3
+//   Eq. (5)   rho = sigma S / h^3
 //   Eq. (7)   Omega = 1 - D/(3S) with D = 3S - E  =>  Omega = E/(3S)
 #include <cstdio>
 #include "sph_internal.cuh"
@@ -96,6 +97,7 @@ __device__ __forceinline__ float density_hcap(const SphGrid& g) {
     return hcap;
 }
 
+template <int KERN>
 __global__ __launch_bounds__(D_TPB, SPH_MINB) void k_density(
     int n, const SphGrid* __restrict__ gp, const uint32_t* __restrict__ cell_start,
     const float4* __restrict__ pos_m, const int32_t* __restrict__ perm, DensPar par, float* h_io,
@@ -141,7 +143,7 @@ __global__ __launch_bounds__(D_TPB, SPH_MINB) void k_density(
         }
         if (!(h > 0.0f) || !(h < 3.0e38f)) h = g.hmin;
         h = fminf(h, hcap);
-        const float T = par.n_ngb * pi.w * (1.0f / 14.0f);
+        const float T = par.n_ngb * pi.w * (1.0f / SphKernel<KERN>::self);
         // the target's kept list: entry f at [target][f]
         uint32_t* const gj = nb_j + (size_t)(tvalid ? p : 0) * (D_SLOTS * D_G);
         float    hlo = 0.0f, hhi = __int_as_float(0x7f800000);
@@ -188,13 +190,12 @@ __global__ __launch_bounds__(D_TPB, SPH_MINB) void k_density(
             const int maxcnt = __reduce_max_sync(SPH_FULL, mycnt);
             for (int k = 0; k < maxcnt; ++k) {
                 if (k < mycnt) {
-                    const float q  = lr[k * 32] * ih;
                     const float mj = lm[k * 32];
-                    const float tt = fmaxf(1.0f - 0.5f * q, 0.0f);
-                    const float t2 = tt * tt, q2 = q * q;
-                    s  += mj * (t2 * t2 * (1.0f + 2.0f * q));
-                    e  += mj * (5.0f * q2 * t2 * tt);
-                    f2 += mj * (q2 * t2 * (10.0f * tt - 7.5f * q));
+                    float wq, eq, fq;
+                    SphKernel<KERN>::sums(lr[k * 32] * ih, wq, eq, fq);
+                    s  += mj * wq;
+                    e  += mj * eq;
+                    f2 += mj * fq;
                 }
             }
             s  = sph_group_sum<D_G>(s);
@@ -258,7 +259,7 @@ __global__ __launch_bounds__(D_TPB, SPH_MINB) void k_density(
             c_sweeps += sweeps;
             if (!fix) {
                 const float ih = 1.0f / h;
-                rho[i]   = SPH_SIGMA * S * ih * ih * ih;
+                rho[i]   = SphKernel<KERN>::sigma * S * ih * ih * ih;
                 omega[i] = E / (3.0f * S);
                 nn[i]    = ni;
             }
@@ -284,6 +285,7 @@ __global__ __launch_bounds__(D_TPB, SPH_MINB) void k_density(
 // The robust path: one warp per queued target, no list.  Every sweep re-walks the candidate
 // rows (32 lanes over each row), so neither crowding nor a growing h can break it, and the
 // final count decides neighbours inside the FP32-uncertain band in FP64.
+template <int KERN>
 __global__ __launch_bounds__(256) void k_density_fix(
     const SphGrid* __restrict__ gp, const uint32_t* __restrict__ cell_start,
     const float4* __restrict__ pos_m, const int32_t* __restrict__ perm, DensPar par,
@@ -307,7 +309,7 @@ __global__ __launch_bounds__(256) void k_density_fix(
         const int    p  = pq & 0x7fffffff;
         const float4 pi = pos_m[p];
         const int    i  = perm[p];
-        const float  T  = par.n_ngb * pi.w * (1.0f / 14.0f);
+        const float  T  = par.n_ngb * pi.w * (1.0f / SphKernel<KERN>::self);
         float h = fminf(h_io[i], hcap);
         float hlo = 0.0f, hhi = __int_as_float(0x7f800000);
         float S = 0.0f, E = 0.0f;
@@ -325,12 +327,11 @@ __global__ __launch_bounds__(256) void k_density_fix(
                         const float dx = rr.sx - pj.x, dy = rr.sy - pj.y, dz = rr.sz - pj.z;
                         const float r2 = dx * dx + dy * dy + dz * dz;
                         if (r2 < H2) {
-                            const float q  = sqrtf(r2) * ih;
-                            const float tt = fmaxf(1.0f - 0.5f * q, 0.0f);
-                            const float t2 = tt * tt, q2 = q * q;
-                            s  += pj.w * (t2 * t2 * (1.0f + 2.0f * q));
-                            e  += pj.w * (5.0f * q2 * t2 * tt);
-                            f2 += pj.w * (q2 * t2 * (10.0f * tt - 7.5f * q));
+                            float wq, eq, fq;
+                            SphKernel<KERN>::sums(sqrtf(r2) * ih, wq, eq, fq);
+                            s  += pj.w * wq;
+                            e  += pj.w * eq;
+                            f2 += pj.w * fq;
                         }
                     }
                     c_tested += min(32u, rr.end - k0);
@@ -373,7 +374,7 @@ __global__ __launch_bounds__(256) void k_density_fix(
             if (!count_only) {
                 const float ih = 1.0f / h;
                 h_io[i]  = h;
-                rho[i]   = SPH_SIGMA * S * ih * ih * ih;
+                rho[i]   = SphKernel<KERN>::sigma * S * ih * ih * ih;
                 omega[i] = E / (3.0f * S);
             }
         }
@@ -404,12 +405,21 @@ int sph_launch_density(sph_ctx* c, const float* m, float* h, float* rho, float* 
     SPH_CUDA_CHECK(c, cudaMemsetAsync(c->fix_cnt, 0, sizeof(unsigned), s));
     DensPar par{c->par.n_ngb, c->par.h_tol, c->par.search_slack, c->par.h_max_iter};
     const int nblk = (int)((n + D_TARGETS - 1) / D_TARGETS);
-    k_density<<<nblk, D_TPB, 0, s>>>((int)n, c->grid, c->cell_start, c->pos_m, c->perm, par, h, rho,
-                                     omega, nn, c->fix_list, c->fix_cnt, c->nb_j, c->nb_cnt,
-                                     c->nb_rkeep, c->stats);
-    k_density_fix<<<c->sm_count * 4, 256, 0, s>>>(c->grid, c->cell_start, c->pos_m, c->perm, par,
-                                                  c->fix_list, c->fix_cnt, h, rho, omega, nn,
-                                                  c->stats);
+    auto launch = [&](auto tag) {
+        constexpr int KERN = decltype(tag)::value;
+        k_density<KERN><<<nblk, D_TPB, 0, s>>>((int)n, c->grid, c->cell_start, c->pos_m, c->perm, par,
+                                               h, rho, omega, nn, c->fix_list, c->fix_cnt, c->nb_j,
+                                               c->nb_cnt, c->nb_rkeep, c->stats);
+        k_density_fix<KERN><<<c->sm_count * 4, 256, 0, s>>>(c->grid, c->cell_start, c->pos_m, c->perm,
+                                                            par, c->fix_list, c->fix_cnt, h, rho,
+                                                            omega, nn, c->stats);
+    };
+    switch (c->par.kernel) {
+    case 0: launch(std::integral_constant<int, 0>{}); break;
+    case 2: launch(std::integral_constant<int, 2>{}); break;
+    case 3: launch(std::integral_constant<int, 3>{}); break;
+    default: launch(std::integral_constant<int, 1>{}); break;
+    }
     SPH_CUDA_CHECK(c, cudaGetLastError());
     return SPH_OK;
 }

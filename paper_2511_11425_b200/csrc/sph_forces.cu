@@ -10,8 +10,8 @@
 // pair arithmetic runs without divergence between accepted and rejected candidates.  A group
 // whose column overflows is queued for k_forces_fix (one warp per target, no list).
 //
-// Pair arithmetic (d = x_i - x_j, r = |d|, q_a = r/h_a, g_a = K_a (1-q_a/2)_+^3 with
-// K_a = 5 SIGMA / h_a^5, so that dW/dr(r,h_a) = -g_a r):
+// Pair arithmetic (d = x_i - x_j, r = |d|, q_a = r/h_a, g_a = K_a g(q_a), g = -w'(q)/q, with
+// K_a = sigma / h_a^5, so that dW/dr(r,h_a) = -g_a r; Wendland C2: g = 5 (1-q/2)_+^3):
 //   Eq. 13+17:  a_i     = + sum_j m_j (A_i g_i + A_j g_j + Pi_ij gbar) d
 //   Eq. 14+18:  du_i/dt = - sum_j m_j (A_i g_i + Pi_ij gbar / 2) (v_ij . d)
 //   Eq. 15-16:  mu = hbar (v_ij.d)/(r^2 + eps hbar^2), Pi = mu (beta mu - alpha cbar)/rhobar
@@ -46,7 +46,7 @@ __global__ void k_force_prep(int64_t n, const int32_t* __restrict__ inv_perm,
                              const float* __restrict__ vx, const float* __restrict__ vy,
                              const float* __restrict__ vz, const float* __restrict__ u,
                              const float* __restrict__ rho, const float* __restrict__ h,
-                             const float* __restrict__ omega, float gamma, float4* pos_h,
+                             const float* __restrict__ omega, float gamma, float sigma, float4* pos_h,
                              float4* vel_m, float4* rcak, float* P, float* cs, SphGrid* g) {
     int64_t  i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     float    hi = 0.0f;
@@ -63,7 +63,7 @@ __global__ void k_force_prep(int64_t n, const int32_t* __restrict__ inv_perm,
         pos_h[p] = a;
         vel_m[p] = make_float4(vx[i], vy[i], vz[i], m[i]);
         const float h2 = hi * hi;
-        rcak[p] = make_float4(ri, ci, Pi / (om * ri * ri), 5.0f * SPH_SIGMA / (h2 * h2 * hi));
+        rcak[p] = make_float4(ri, ci, Pi / (om * ri * ri), sigma / (h2 * h2 * hi));
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) hi = fmaxf(hi, __shfl_xor_sync(SPH_FULL, hi, o));
@@ -111,14 +111,13 @@ struct Accum {
 };
 
 // One pair of Eqs. (13)-(18): source j at displacement d = x_i - x_j (minimum image).
+template <int KERN>
 __device__ __forceinline__ void force_pair(const Target& t, Accum& a, const ForcePar& par,
                                            const float4 vj, const float4 rj, float dx,
                                            float dy, float dz, float r2, float hj) {
     const float r  = r2 * rsqrtf(r2);
-    const float ti = fmaxf(1.0f - 0.5f * r * t.ih, 0.0f);
-    const float tj = fmaxf(1.0f - 0.5f * __fdividef(r, hj), 0.0f);
-    const float gi = t.K * ti * ti * ti;
-    const float gj = rj.w * tj * tj * tj;
+    const float gi = t.K * SphKernel<KERN>::g(r * t.ih);
+    const float gj = rj.w * SphKernel<KERN>::g(__fdividef(r, hj));
     const float vdx = t.vi.x - vj.x, vdy = t.vi.y - vj.y, vdz = t.vi.z - vj.z;
     const float vr = vdx * dx + vdy * dy + vdz * dz;   // v_ij . r_ij
     float pig = 0.0f;                                   // Pi_ij * gbar
@@ -141,6 +140,7 @@ __device__ __forceinline__ void force_pair(const Target& t, Accum& a, const Forc
     ++a.pairs;
 }
 
+template <int KERN>
 __global__ __launch_bounds__(F_TPB, SPH_FMINB) void k_forces(
     int n, const SphGrid* __restrict__ gp, const uint32_t* __restrict__ cell_start,
     const float4* __restrict__ pos_h, const float4* __restrict__ vel_m,
@@ -244,7 +244,7 @@ __global__ __launch_bounds__(F_TPB, SPH_FMINB) void k_forces(
                 const float r2 = dx * dx + dy * dy + dz * dz;
                 // kept lists hold everything inside the kept radius: apply the pair test
                 if (r2 < fmaxf(hi2x4, 4.0f * pj.w * pj.w) && r2 > 0.0f)
-                    force_pair(t, a, par, vj, rj, dx, dy, dz, r2, pj.w);
+                    force_pair<KERN>(t, a, par, vj, rj, dx, dy, dz, r2, pj.w);
             }
         }
         a.ax = sph_group_sum<F_G>(a.ax);
@@ -279,6 +279,7 @@ __global__ __launch_bounds__(F_TPB, SPH_FMINB) void k_forces(
 }
 
 // The robust path: one warp per queued target, candidates handled as they are met.
+template <int KERN>
 __global__ __launch_bounds__(256) void k_forces_fix(
     const SphGrid* __restrict__ gp, const uint32_t* __restrict__ cell_start,
     const float4* __restrict__ pos_h, const float4* __restrict__ vel_m,
@@ -315,7 +316,7 @@ __global__ __launch_bounds__(256) void k_forces_fix(
                     const float dx = rr.sx - pj.x, dy = rr.sy - pj.y, dz = rr.sz - pj.z;
                     const float r2 = dx * dx + dy * dy + dz * dz;
                     if (r2 < fmaxf(hi2x4, 4.0f * pj.w * pj.w) && r2 > 0.0f)
-                        force_pair(t, a, par, __ldg(vel_m + j), __ldg(rcak + j), dx, dy, dz, r2, pj.w);
+                        force_pair<KERN>(t, a, par, __ldg(vel_m + j), __ldg(rcak + j), dx, dy, dz, r2, pj.w);
                 }
                 c_tested += min(32u, rr.end - k0);
             }
@@ -352,23 +353,35 @@ int sph_launch_forces(sph_ctx* c, const float* m, const float* vx, const float* 
                       float* mu_min, float* P, float* cs) {
     cudaStream_t  s = c->stream;
     const int64_t n = c->n;
+    static const float sigmas[4] = {SphKernel<0>::sigma, SphKernel<1>::sigma, SphKernel<2>::sigma,
+                                    SphKernel<3>::sigma};
+    const float sigma = sigmas[(c->par.kernel >= 0 && c->par.kernel <= 3) ? c->par.kernel : 1];
     k_zero_hmax<<<1, 1, 0, s>>>(c->grid);
     SPH_CUDA_CHECK(c, cudaMemsetAsync(c->fix_cnt + 1, 0, sizeof(unsigned), s));
     SPH_CUDA_CHECK(c, cudaMemsetAsync(c->coarse_hmax, 0, SPH_COARSE_MAX * sizeof(unsigned), s));
     k_force_prep<<<(int)((n + 255) / 256), 256, 0, s>>>(n, c->inv_perm, m, vx, vy, vz, u,
-                                                        rho, h, omega, c->par.gamma, c->pos_h,
+                                                        rho, h, omega, c->par.gamma, sigma, c->pos_h,
                                                         c->vel_m, c->rcak, P, cs, c->grid);
     k_coarse_hmax<<<(int)((n + 255) / 256), 256, 0, s>>>(n, c->grid, c->pos_h, c->coarse_hmax);
     ForcePar par{c->par.av_alpha, c->par.av_beta, c->par.av_eps};
     const int nblk = (int)((n + F_TARGETS - 1) / F_TARGETS);
-    k_forces<<<nblk, F_TPB, 0, s>>>((int)n, c->grid, c->cell_start, c->pos_h, c->vel_m, c->rcak,
-                                    c->perm, par, ax, ay, az, dudt, mu_min, c->fix_list,
-                                    c->fix_cnt + 1, c->coarse_hmax, c->nb_j, c->nb_cnt,
-                                    c->nb_rkeep, c->stats);
-    k_forces_fix<<<c->sm_count * 4, 256, 0, s>>>(c->grid, c->cell_start, c->pos_h, c->vel_m,
-                                                 c->rcak, c->perm, par, c->fix_list,
-                                                 c->fix_cnt + 1, ax, ay, az, dudt, mu_min,
-                                                 c->stats);
+    auto launch = [&](auto tag) {
+        constexpr int KERN = decltype(tag)::value;
+        k_forces<KERN><<<nblk, F_TPB, 0, s>>>((int)n, c->grid, c->cell_start, c->pos_h, c->vel_m,
+                                              c->rcak, c->perm, par, ax, ay, az, dudt, mu_min,
+                                              c->fix_list, c->fix_cnt + 1, c->coarse_hmax, c->nb_j,
+                                              c->nb_cnt, c->nb_rkeep, c->stats);
+        k_forces_fix<KERN><<<c->sm_count * 4, 256, 0, s>>>(c->grid, c->cell_start, c->pos_h, c->vel_m,
+                                                           c->rcak, c->perm, par, c->fix_list,
+                                                           c->fix_cnt + 1, ax, ay, az, dudt, mu_min,
+                                                           c->stats);
+    };
+    switch (c->par.kernel) {
+    case 0: launch(std::integral_constant<int, 0>{}); break;
+    case 2: launch(std::integral_constant<int, 2>{}); break;
+    case 3: launch(std::integral_constant<int, 3>{}); break;
+    default: launch(std::integral_constant<int, 1>{}); break;
+    }
     SPH_CUDA_CHECK(c, cudaGetLastError());
     return SPH_OK;
 }

@@ -95,8 +95,67 @@ struct sph_ctx {
 #define SPH_MINB 8     // resident blocks per SM the sweeps are compiled for
 #endif
 
-// Wendland C2, support 2h: w(q) = SIGMA (1-q/2)^4 (1+2q); (32 pi/3) SIGMA = 14.
-#define SPH_SIGMA 0.41778172561566733f   /* 21/(16 pi) */
+// SPH kernels with support radius 2h (PAPER.md:105 offers the cubic spline and the Wendland
+// C2, C4, C6 functions; forms of Dehnen & Aly 2012 rescaled to 2h, reading R3):
+// W(r,h) = sigma h^-3 w(q), q = r/h, x = q/2, y = (1-x)_+.  Every kernel provides
+//   sums(q, w, e, f):  w(q),  e = -q w'(q),  f = -(q w'(q) + q^2 w''(q))
+//                      (S = sum m w, dS/dh = E/h, dE/dh = -F/h with E = sum m e, F = sum m f)
+//   g(q) = -w'(q)/q    (dW/dr = -sigma h^-5 g(q) r: no division by r in the force sweep)
+//   self = (32 pi/3) sigma w(0): the neighbour "count" of a particle alone in its kernel.
+template <int KERN> struct SphKernel;
+template <> struct SphKernel<0> {   // cubic spline (Monaghan 1992)
+    static constexpr float sigma = 0.31830988618379067f, self = 32.0f / 3.0f;
+    static __device__ __forceinline__ void sums(float q, float& w, float& e, float& f) {
+        const float u = fmaxf(2.0f - q, 0.0f), q2 = q * q;
+        const bool  in = q < 1.0f;
+        w = in ? 1.0f - q2 * (1.5f - 0.75f * q) : 0.25f * u * u * u;
+        e = in ? q2 * (3.0f - 2.25f * q) : 0.75f * q * u * u;
+        f = in ? q2 * (6.0f - 6.75f * q) : 0.75f * q * u * (u - 2.0f * q);
+    }
+    static __device__ __forceinline__ float g(float q) {
+        const float u = fmaxf(2.0f - q, 0.0f);
+        return q < 1.0f ? 3.0f - 2.25f * q : __fdividef(0.75f * u * u, q);
+    }
+};
+template <> struct SphKernel<1> {   // Wendland C2: w = y^4 (1 + 4x)
+    static constexpr float sigma = 0.41778172561566733f, self = 14.0f;
+    static __device__ __forceinline__ void sums(float q, float& w, float& e, float& f) {
+        const float t = fmaxf(1.0f - 0.5f * q, 0.0f), t2 = t * t, q2 = q * q;
+        w = t2 * t2 * (1.0f + 2.0f * q);
+        e = 5.0f * q2 * t2 * t;
+        f = q2 * t2 * (10.0f * t - 7.5f * q);
+    }
+    static __device__ __forceinline__ float g(float q) {
+        const float t = fmaxf(1.0f - 0.5f * q, 0.0f);
+        return 5.0f * t * t * t;
+    }
+};
+template <> struct SphKernel<2> {   // Wendland C4: w = y^6 (1 + 6x + 35/3 x^2)
+    static constexpr float sigma = 0.61548200648818910f, self = 20.625f;
+    static __device__ __forceinline__ void sums(float q, float& w, float& e, float& f) {
+        const float x = 0.5f * q, y = fmaxf(1.0f - x, 0.0f), y2 = y * y, y4 = y2 * y2, x2 = x * x;
+        w = y4 * y2 * (1.0f + x * (6.0f + (35.0f / 3.0f) * x));
+        e = (56.0f / 3.0f) * x2 * y4 * y * (1.0f + 5.0f * x);
+        f = (56.0f / 3.0f) * x2 * y4 * (2.0f + x * (8.0f - 40.0f * x));
+    }
+    static __device__ __forceinline__ float g(float q) {
+        const float x = 0.5f * q, y = fmaxf(1.0f - x, 0.0f), y2 = y * y;
+        return (14.0f / 3.0f) * y2 * y2 * y * (1.0f + 5.0f * x);
+    }
+};
+template <> struct SphKernel<3> {   // Wendland C6: w = y^8 (1 + 8x + 25x^2 + 32x^3)
+    static constexpr float sigma = 0.84861913015795750f, self = 28.4375f;
+    static __device__ __forceinline__ void sums(float q, float& w, float& e, float& f) {
+        const float x = 0.5f * q, y = fmaxf(1.0f - x, 0.0f), y2 = y * y, y6 = y2 * y2 * y2, x2 = x * x;
+        w = y6 * y2 * (1.0f + x * (8.0f + x * (25.0f + 32.0f * x)));
+        e = 22.0f * x2 * y6 * y * (1.0f + x * (7.0f + 16.0f * x));
+        f = 22.0f * x2 * y6 * (2.0f + x * (12.0f - x * (6.0f + 176.0f * x)));
+    }
+    static __device__ __forceinline__ float g(float q) {
+        const float x = 0.5f * q, y = fmaxf(1.0f - x, 0.0f), y2 = y * y;
+        return 5.5f * y2 * y2 * y2 * y * (1.0f + x * (7.0f + 16.0f * x));
+    }
+};
 
 __device__ __forceinline__ int sph_fdiv(int u, int n) {   // floor(u / n), n > 0
     return (u >= 0) ? (u / n) : -((-u + n - 1) / n);

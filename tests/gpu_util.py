@@ -20,7 +20,8 @@ def to_device(w):
 def make_params(w, **kw):
     gp = sph.Params(gamma=float(w["gamma"]), av_alpha=float(w["av_alpha"]),
                     av_beta=float(w["av_beta"]), **kw)
-    op = orc.Params(gamma=float(np.float32(w["gamma"])), av_alpha=float(np.float32(w["av_alpha"])),
+    op = orc.Params(kernel=gp.kernel, n_ngb=float(np.float32(gp.n_ngb)),
+                    gamma=float(np.float32(w["gamma"])), av_alpha=float(np.float32(w["av_alpha"])),
                     av_beta=float(np.float32(w["av_beta"])), av_eps=float(np.float32(0.01)),
                     eta_cfl=float(np.float32(0.3)), eta_acc=float(np.float32(0.2)))
     return gp, op

@@ -331,3 +331,24 @@ def test_c5_impact_full_size_sampled(gu):
     """Config 5 at BASELINE.json's full size: 12 M + 1.5 M lattice points before the surface
     truncation (about 13.4 M particles), sampled like the reduced case (~25 s on a B200 box)."""
     _impact_case(gu, 12_000_000, 1_500_000, 48)
+
+
+# ------------------------------------------------------------------------------------------
+# The other kernels the paper offers (PAPER.md:105): cubic spline, Wendland C4 and C6.
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("kernel,n_ngb", [(0, 32.0), (2, 64.0), (3, 64.0), (3, 200.0), (1, 100.0)])
+def test_c1_other_kernels_and_neighbour_numbers(gu, kernel, n_ngb):
+    """Config 1 with the cubic spline / 32, Wendland C4 and C6, and neighbour
+    numbers beyond the 192-entry lists (those targets run through the list-free kernels):
+    every particle against the brute-force oracle."""
+    w = workloads.uniform_cube(h_start="warm")
+    scale = (n_ngb / 64.0) ** (1.0 / 3.0) * {0: 0.96, 1: 1.0, 2: 1.0, 3: 1.0}[kernel]
+    w["h"] = (w["h"] * np.float32(scale)).astype(np.float32)
+    _, op = gu.make_params(w, kernel=kernel, n_ngb=n_ngb)
+    _, ob = gu.make_boxes(w)
+    ctx, d, out, h = _full_step(gu, w, kernel=kernel, n_ngb=n_ngb)
+    st = ctx.stats()
+    assert st["dens_nonconv"] == 0, st
+    _check_sample(gu, w, ctx, out, h, np.arange(w["n"]), op, ob)
+    if n_ngb >= 200.0:
+        assert st["dens_overflow"] > 0      # the robust path was exercised
