@@ -127,6 +127,23 @@ int  sph_forces(sph_ctx* ctx, const float* m, const float* vx, const float* vy, 
 int  sph_timestep(sph_ctx* ctx, const float* h, const float* c, const float* ax, const float* ay,
                   const float* az, const float* mu_min, float* dt_i, float* dt_min_device);
 
+/* Time integration with a global step, PAPER.md:227-261 (Section 2.3.6), Eqs. (19)-(25):
+ * kick-drift-kick with predicted v, u for the force pass.  Element-wise; arrays of length n
+ * in the caller's order.  The step is dt = dt_scale x *dt_device (dt_device: one float in
+ * device memory, e.g. the dt_min_device of sph_timestep), so no host round trip is needed.
+ *   sph_predict  Eqs. (19)-(20): q_pred = q + (dt/2) qdot        (q = v, u; qdot of the last step)
+ *   sph_kick     Eqs. (21)-(24): q += (dt/2) qdot, in place      (closing and opening kick)
+ *   sph_drift    Eq. (25):       x += dt v, wrapped into [lo, lo+len) on periodic axes        */
+int  sph_predict(sph_ctx* ctx, int64_t n, const float* dt_device, float dt_scale, const float* vx,
+                 const float* vy, const float* vz, const float* u, const float* ax, const float* ay,
+                 const float* az, const float* dudt, float* vx_pred, float* vy_pred,
+                 float* vz_pred, float* u_pred);
+int  sph_kick(sph_ctx* ctx, int64_t n, const float* dt_device, float dt_scale, float* vx, float* vy,
+              float* vz, float* u, const float* ax, const float* ay, const float* az,
+              const float* dudt);
+int  sph_drift(sph_ctx* ctx, int64_t n, const float* dt_device, float dt_scale, float* x, float* y,
+               float* z, const float* vx, const float* vy, const float* vz);
+
 /* Diagnostic: CSR neighbour lists at a prescribed h, caller indices; a list is a set, the
  * order inside it is unspecified.
  * mode 0: j with r_ij < 2 h_i (self included); mode 1: j != i with r_ij < 2 max(h_i,h_j).

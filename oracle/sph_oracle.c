@@ -646,3 +646,30 @@ int orc_num_threads(void)
     return 1;
 #endif
 }
+
+/* ------------------------------------------------------------------------- *
+ * Time integration with a global step, PAPER.md:227-261 (Section 2.3.6),
+ * Eqs. (19)-(25): kick-drift-kick with predicted v, u for the force pass.
+ *   Eqs. (19)-(20)  predict:  q_pred = q_{i-1/2} + (dt/2) qdot_{i-1}   (q = v, u)
+ *   Eqs. (21)-(24)  kick:     q     += (dt/2) qdot_i   (closing and opening kick)
+ *   Eq.  (25)       drift:    x_{i+1} = x_i + dt v_{i+1/2}, wrapped into the
+ *                   periodic box [lo, lo+len) (PAPER.md:297 periodic tests)
+ * Plain statements of the update formulas; one array at a time.
+ * ------------------------------------------------------------------------- */
+void orc_axpy(int64_t n, double a, const double *x, const double *y, double *out)
+{   /* out = y + a x : the form shared by Eqs. (19)-(24) with a = dt/2 */
+    for (int64_t i = 0; i < n; i++) out[i] = y[i] + a * x[i];
+}
+
+void orc_drift(int64_t n, double dt, const double *v, double lo, double len, int periodic,
+               double *x)
+{
+    for (int64_t i = 0; i < n; i++) {
+        double xn = x[i] + dt * v[i];                       /* Eq. (25) */
+        if (periodic) {
+            xn -= len * floor((xn - lo) / len);
+            if (xn >= lo + len) xn = lo;                    /* rounding at the upper face */
+        }
+        x[i] = xn;
+    }
+}

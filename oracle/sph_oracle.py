@@ -208,3 +208,19 @@ def timestep(h, c, ax, ay, az, mu_min, par: Params):
     lib().orc_timestep(C.c_int64(len(h)), _p(h), _p(c), _p(ax), _p(ay), _p(az), _p(mu),
                        C.byref(p), _p(dti), C.byref(dtm))
     return dti, dtm.value
+
+
+def axpy(a, x, y):
+    """y + a x in FP64: the kick / predict update of Eqs. (19)-(24) with a = dt/2."""
+    x, y = _d(x), _d(y)
+    out = np.empty_like(x)
+    lib().orc_axpy(C.c_int64(len(x)), C.c_double(a), _p(x), _p(y), _p(out))
+    return out
+
+
+def drift(x, v, dt, lo, length, periodic):
+    """Eq. (25) with the periodic wrap; returns the new coordinate array (FP64)."""
+    x, v = _d(x).copy(), _d(v)
+    lib().orc_drift(C.c_int64(len(x)), C.c_double(dt), _p(v), C.c_double(float(np.float32(lo))),
+                    C.c_double(float(np.float32(length))), C.c_int(int(periodic)), _p(x))
+    return x

@@ -1,0 +1,95 @@
+"""Global-time-step kick-drift-kick driver over the C-ABI calls (Section 2.3.6,
+Eqs. 19-25; the dynamic global step of PAPER.md:325).  Plumbing only: every update runs in the
+library's kernels, the step length never leaves the device.
+
+One step, in the paper's order:
+  1. density pass at time i                                   sph_build_cells, sph_density_h
+  2. predict v, u to time i with the derivatives of i-1       sph_predict          (Eqs. 19-20)
+  4. force pass with the predicted values, new global dt      sph_forces, sph_timestep
+     closing kick of the previous step (its dt)               sph_kick             (Eqs. 21-22)
+     opening kick of the new step (new dt)                    sph_kick             (Eqs. 23-24)
+  5. drift                                                    sph_drift            (Eq. 25)
+(step 3, the interface correction, is not built.)  Between steps v and u live at the half step.
+"""
+from __future__ import annotations
+
+import numpy as np
+import torch
+
+from . import sph
+
+_KEYS = ("x", "y", "z", "m", "vx", "vy", "vz", "u", "h")
+
+
+class Simulation:
+    def __init__(self, w: dict, **params):
+        n = int(w["n"])
+        self.n = n
+        self.d = {k: torch.from_numpy(np.ascontiguousarray(w[k], np.float32)).cuda() for k in _KEYS}
+        self.ctx = sph.Sph(sph.Params(gamma=float(w["gamma"]), av_alpha=float(w["av_alpha"]),
+                                      av_beta=float(w["av_beta"]), **params),
+                           sph.Box(w["box_lo"], w["box_len"], w["periodic"]), n)
+        self.out = sph.StepBuffers(n)
+        f = dict(dtype=torch.float32, device="cuda")
+        self.pred = {k: torch.empty(n, **f) for k in ("vx", "vy", "vz", "u")}
+        for k in ("ax", "ay", "az", "dudt"):
+            self.out[k].zero_()
+        self.dt_prev = torch.zeros(1, **f)     # no half kick is pending before the first step
+        self.dt_new = self.out["dt_min"]
+        self.t = torch.zeros(1, dtype=torch.float64, device="cuda")
+        self.steps = 0
+
+    def _derivatives(self):
+        """Steps 1, 2, 4a: density, prediction, forces and the new global dt."""
+        d, o, c = self.d, self.out, self.ctx
+        c.build_cells(d["x"], d["y"], d["z"], d["h"])
+        c.density_h(d["m"], d["h"], o["rho"], o["omega"], o["n_ngb"])
+        p = self.pred
+        c.predict(self.dt_prev, 1.0, d["vx"], d["vy"], d["vz"], d["u"], o["ax"], o["ay"], o["az"],
+                  o["dudt"], p["vx"], p["vy"], p["vz"], p["u"])
+        c.forces(d["m"], p["vx"], p["vy"], p["vz"], p["u"], o["rho"], d["h"], o["omega"], o["ax"],
+                 o["ay"], o["az"], o["dudt"], o["mu_min"], o["P"], o["c"])
+        c.timestep(d["h"], o["c"], o["ax"], o["ay"], o["az"], o["mu_min"], o["dt_i"], self.dt_new)
+        # closing kick of the step that ends here (Eqs. 21-22); a no-op before the first step
+        c.kick(self.dt_prev, 1.0, d["vx"], d["vy"], d["vz"], d["u"], o["ax"], o["ay"], o["az"],
+               o["dudt"])
+
+    def step(self, dt_cap: float | None = None):
+        """Advance by one global step dt = min_i dt_i (optionally capped)."""
+        d, o, c = self.d, self.out, self.ctx
+        self._derivatives()
+        if dt_cap is not None:
+            self.dt_new.clamp_(max=float(dt_cap))
+        c.kick(self.dt_new, 1.0, d["vx"], d["vy"], d["vz"], d["u"], o["ax"], o["ay"], o["az"],
+               o["dudt"])                                             # opening kick, Eqs. 23-24
+        c.drift(self.dt_new, 1.0, d["x"], d["y"], d["z"], d["vx"], d["vy"], d["vz"])   # Eq. 25
+        self.t += self.dt_new.double()
+        self.dt_prev.copy_(self.dt_new)
+        self.steps += 1
+
+    def synchronise(self):
+        """Bring v, u from the half step to the current time (density, forces, closing kick),
+        e.g. before measuring energies.  The next step() then starts without a pending kick."""
+        self._derivatives()
+        self.dt_prev.zero_()
+
+    def run_until(self, t_end: float, max_steps: int = 100000):
+        while self.steps < max_steps:
+            t = float(self.t.item())
+            if t >= t_end * (1.0 - 1e-12):
+                break
+            self.step(dt_cap=t_end - t)
+        self.synchronise()
+
+    def energies(self):
+        """Total kinetic and internal energy (FP64 sums on the device)."""
+        d = self.d
+        m = d["m"].double()
+        ek = 0.5 * (m * (d["vx"].double() ** 2 + d["vy"].double() ** 2 + d["vz"].double() ** 2)).sum()
+        eu = (m * d["u"].double()).sum()
+        return float(ek.item()), float(eu.item())
+
+    def momentum(self):
+        d = self.d
+        m = d["m"].double()
+        return [float((m * d[k].double()).sum().item()) for k in ("vx", "vy", "vz")]

@@ -19,7 +19,7 @@ SPH_OK, SPH_EINVAL, SPH_EBOX, SPH_ENOMEM, SPH_ECUDA, SPH_ESTALE, SPH_ENOSPC = 0,
 
 # every symbol include/sph.h declares (tests check the library exports exactly these)
 SYMBOLS = ["sph_create", "sph_destroy", "sph_build_cells", "sph_density_h", "sph_forces",
-           "sph_timestep", "sph_neighbors", "sph_stats", "sph_stats_reset", "sph_permutation",
+           "sph_timestep", "sph_predict", "sph_kick", "sph_drift", "sph_neighbors", "sph_stats", "sph_stats_reset", "sph_permutation",
            "sph_fp32_peak", "sph_strerror", "sph_last_error"]
 
 
@@ -102,6 +102,9 @@ def load():
     lib.sph_density_h.argtypes = [vp] + [fp] * 5
     lib.sph_forces.argtypes = [vp] + [fp] * 15
     lib.sph_timestep.argtypes = [vp] + [fp] * 8
+    lib.sph_predict.argtypes = [vp, i64, fp, C.c_float] + [fp] * 12
+    lib.sph_kick.argtypes = [vp, i64, fp, C.c_float] + [fp] * 8
+    lib.sph_drift.argtypes = [vp, i64, fp, C.c_float] + [fp] * 6
     lib.sph_neighbors.argtypes = [vp, fp, i32, fp, fp, i64, C.POINTER(i64)]
     lib.sph_stats.argtypes = [vp, C.POINTER(_Stats)]
     lib.sph_stats_reset.argtypes = [vp]
@@ -195,6 +198,22 @@ class Sph:
         n, f = self.n, torch.float32
         args = [_ptr(t, f, n) for t in (h, c, ax, ay, az, mu_min, dt_i)]
         self._check(self.lib.sph_timestep(self._ctx, *args, _ptr(dt_min, f, 1)))
+
+    # ---- time integration (Eqs. 19-25) ----------------------------------------------------
+    def predict(self, dt, scale, vx, vy, vz, u, ax, ay, az, dudt, vxp, vyp, vzp, up):
+        n, f = vx.numel(), torch.float32
+        args = [_ptr(t, f, n) for t in (vx, vy, vz, u, ax, ay, az, dudt, vxp, vyp, vzp, up)]
+        self._check(self.lib.sph_predict(self._ctx, n, _ptr(dt, f, 1), scale, *args))
+
+    def kick(self, dt, scale, vx, vy, vz, u, ax, ay, az, dudt):
+        n, f = vx.numel(), torch.float32
+        args = [_ptr(t, f, n) for t in (vx, vy, vz, u, ax, ay, az, dudt)]
+        self._check(self.lib.sph_kick(self._ctx, n, _ptr(dt, f, 1), scale, *args))
+
+    def drift(self, dt, scale, x, y, z, vx, vy, vz):
+        n, f = x.numel(), torch.float32
+        args = [_ptr(t, f, n) for t in (x, y, z, vx, vy, vz)]
+        self._check(self.lib.sph_drift(self._ctx, n, _ptr(dt, f, 1), scale, *args))
 
     # ---- diagnostics --------------------------------------------------------------------
     def neighbors(self, h, mode=0):

@@ -71,8 +71,10 @@ def uniform_cube(nside=16, jitter=0.05, seed=114251, h_start="cold", v_sigma=0.0
     return _finish(w, rng, 1.0, h_start)
 
 
-def sod_tube(ncross=38, seed=114252, h_start="warm"):
-    """C2: periodic 1 x 1/8 x 1/8 box; left half rho=1,P=1; right half rho=1/8,P=0.1; gamma=1.4."""
+def sod_tube(ncross=38, seed=114252, h_start="warm", jitter=0.0):
+    """C2: periodic 1 x 1/8 x 1/8 box; left half rho=1,P=1; right half rho=1/8,P=0.1; gamma=1.4.
+    jitter > 0 (in units of the local spacing) breaks the symmetry of the perfect lattice, which
+    otherwise cannot rearrange when the flow stretches it along x only (evolution tests)."""
     rng = np.random.default_rng(seed)
     dl = 0.125 / ncross
     dr = 2.0 * dl
@@ -81,6 +83,11 @@ def sod_tube(ncross=38, seed=114252, h_start="warm"):
     x = np.concatenate([xl, xr]); y = np.concatenate([yl, yr]); z = np.concatenate([zl, zr])
     m = dl ** 3
     left = np.arange(len(x)) < len(xl)
+    if jitter > 0:
+        sp = np.where(left, dl, dr)
+        x = (x + rng.uniform(-jitter, jitter, len(x)) * sp) % 1.0
+        y = (y + rng.uniform(-jitter, jitter, len(x)) * sp) % 0.125
+        z = (z + rng.uniform(-jitter, jitter, len(x)) * sp) % 0.125
     rho = np.where(left, 1.0, 0.125)
     P = np.where(left, 1.0, 0.1)
     gamma = 1.4

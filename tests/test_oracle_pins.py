@@ -476,3 +476,39 @@ def test_workload_shapes():
     assert k["n"] == 40 * 20 * 5 + 48 * 24 * 6
     i = W.impact(n_target=20000, n_impactor=2500)
     assert i["periodic"] == (0, 0, 0) and 15000 < i["n"] < 30000
+
+
+# ------------------------------------------------------------------------------------------
+# Time integration, Eqs. (19)-(25): the oracle's update formulas against closed forms.
+# ------------------------------------------------------------------------------------------
+def test_kick_drift_kick_is_exact_for_constant_acceleration():
+    """A kick-drift-kick step with constant a reproduces x0 + v0 t + a t^2/2 and v0 + a t
+    exactly (to round-off), whatever the sequence of step lengths."""
+    rng = np.random.default_rng(7)
+    n = 64
+    x0, v0, a = rng.uniform(-1, 1, n), rng.normal(0, 1, n), rng.normal(0, 2, n)
+    x, v, t = x0.copy(), v0.copy(), 0.0
+    for dt in (0.1, 0.03, 0.2, 0.07):
+        v = orc.axpy(0.5 * dt, a, v)                       # opening kick, Eq. (23)
+        x = orc.drift(x, v, dt, -100.0, 200.0, 0)          # drift, Eq. (25)
+        v = orc.axpy(0.5 * dt, a, v)                       # closing kick, Eq. (21)
+        t += dt
+    assert np.abs(x - (x0 + v0 * t + 0.5 * a * t * t)).max() < 1e-13
+    assert np.abs(v - (v0 + a * t)).max() < 1e-13
+
+
+def test_predict_is_half_a_step_of_the_rate():
+    q, qdot = np.array([1.0, -2.0, 0.5]), np.array([4.0, 0.25, -8.0])
+    assert np.array_equal(orc.axpy(0.5 * 0.125, qdot, q), q + 0.0625 * qdot)   # Eqs. (19)-(20)
+
+
+def test_drift_wraps_into_the_periodic_box():
+    x = np.array([0.95, 0.05, 0.5, 0.999999])
+    v = np.array([1.0, -1.0, 0.0, 1.0])
+    xn = orc.drift(x, v, 0.1, 0.0, 1.0, 1)
+    assert np.allclose(xn, [0.05, 0.95, 0.5, 0.099999], atol=1e-12)
+    assert (xn >= 0.0).all() and (xn < 1.0).all()
+    # open axis: no wrap
+    assert np.allclose(orc.drift(x, v, 0.1, 0.0, 1.0, 0), x + 0.1 * v)
+    # a shifted box
+    assert np.allclose(orc.drift(np.array([2.9]), np.array([1.0]), 0.2, 1.0, 2.0, 1), [1.1])
