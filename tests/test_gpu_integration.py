@@ -193,3 +193,33 @@ def test_sod_shock_tube_against_the_exact_solution(gu):
     prr = mean[(xc > 0.615) & (xc < 0.655)].mean()
     assert abs(pl / 0.42632 - 1) <= 0.02, pl
     assert abs(prr / 0.26557 - 1) <= 0.03, prr
+
+
+def test_sedov_taylor_blast_shock_radius_and_energy(gu):
+    """Config 3's shape at 64^3 evolved with the dynamic global step: the
+    shock sits at the Sedov-Taylor radius R = 1.152 (E t^2 / rho)^(1/5) (gamma = 5/3), the
+    compression behind it is strong (4 in the continuum limit, smeared over ~2h here) and the
+    total energy is conserved to the paper's 0.2 % class."""
+    from paper_2511_11425_b200.integrate import Simulation
+    w = workloads.sedov(nside=64, h_start="warm")
+    sim = Simulation(w)
+    sim.synchronise()
+    e0 = sum(sim.energies())
+    R = 0.3
+    sim.run_until((R / 1.152) ** 2.5)
+    e1 = sum(sim.energies())
+    assert abs(e1 / e0 - 1) <= 3e-3, e1 / e0 - 1
+    assert sim.ctx.stats()["dens_nonconv"] == 0
+    x, y, z = (gu.np64(sim.d[k]) - 0.5 for k in "xyz")
+    r = np.sqrt(x * x + y * y + z * z)
+    rho = gu.np64(sim.out["rho"])
+    edges = np.linspace(0.0, 0.5, 101)
+    idx = np.digitize(r, edges) - 1
+    ok = idx < 100
+    mean = np.bincount(idx[ok], rho[ok], 100) / np.maximum(np.bincount(idx[ok], None, 100), 1)
+    k = int(np.argmax(mean))
+    r_peak = 0.5 * (edges[k] + edges[k + 1])
+    assert abs(r_peak / R - 1) <= 0.04, r_peak           # shock position
+    assert mean[k] >= 2.3, mean[k]                       # compression behind the shock
+    assert abs(mean[edges[:-1] > 0.4].mean() / 1.0146 - 1) <= 2e-3   # undisturbed gas ahead
+    assert mean[:20].max() < 0.2                         # evacuated interior
