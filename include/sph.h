@@ -127,6 +127,20 @@ int  sph_forces(sph_ctx* ctx, const float* m, const float* vx, const float* vy, 
 int  sph_timestep(sph_ctx* ctx, const float* h, const float* c, const float* ax, const float* ay,
                   const float* az, const float* mu_min, float* dt_i, float* dt_min_device);
 
+/* Interface correction for the ideal gas, PAPER.md:158-182 (Section 2.3.4), Eqs. (8)-(12);
+ * call between sph_density_h and sph_forces and hand rho_corr to sph_forces.  Gather sums over
+ * r_ij < 2 h_i, self included.
+ *   imbalance  I_i = alpha |sum_j kappa_ij (r_j - r_i) m_j W_ij(h_i)| / (h_i sum_j m_j W_ij(h_i)),
+ *              kappa_ij = +1 for equal material ids, -1 otherwise (mat may be NULL: one material)
+ *   rho_corr   Eq. (12) with T = u / c_v: P~ / ((gamma-1) u~), where P~, u~ are P_i, u_i mixed
+ *              with their e^{-I_j^2} W_ij(h_i)-weighted kernel averages by e^{-I_i^2} (Eqs. 9-11)
+ *   P_corr     P~ (may be NULL)
+ * alpha: the "normalization parameter" of Eq. (8); the paper gives no value (1.5 in the
+ * method it cites).  Needs sph_build_cells for the same positions (else SPH_ESTALE).            */
+int  sph_interface_correction(sph_ctx* ctx, const float* m, const float* u, const float* rho,
+                              const float* h, const int32_t* mat, float alpha, float* imbalance,
+                              float* rho_corr, float* P_corr);
+
 /* Time integration with a global step, PAPER.md:227-261 (Section 2.3.6), Eqs. (19)-(25):
  * kick-drift-kick with predicted v, u for the force pass.  Element-wise; arrays of length n
  * in the caller's order.  The step is dt = dt_scale x *dt_device (dt_device: one float in

@@ -673,3 +673,71 @@ void orc_drift(int64_t n, double dt, const double *v, double lo, double len, int
         x[i] = xn;
     }
 }
+
+/* ------------------------------------------------------------------------- *
+ * Interface correction, PAPER.md:158-182 (Section 2.3.4), Eqs. (8)-(12), for
+ * the built-in ideal gas.  Brute force: every target against all particles.
+ *
+ *   Eq. (8)   I_i = alpha |sum_j kappa_ij (r_j - r_i) m_j W_ij(h_i)|
+ *                   / (h_i sum_j m_j W_ij(h_i)),
+ *             kappa_ij = +1 same material, -1 different material; the sums run
+ *             over the gather neighbours r_ij < 2 h_i, self included (reading
+ *             R25; the self term adds nothing to the numerator).  alpha is "a
+ *             normalization parameter" (no value in the paper, reading R24).
+ *   Eq. (9)   Tbar_i = sum_j T_j e^{-I_j^2} W_ij(h_i) / sum_j e^{-I_j^2} W_ij(h_i),
+ *             Pbar_i likewise (no m_j in the weights, as printed: reading R27)
+ *   Eq. (10)  P~_i = e^{-I_i^2} P_i + (1 - e^{-I_i^2}) Pbar_i
+ *   Eq. (11)  T~_i likewise
+ *   Eq. (12)  rho~_i = rho_EOS(T~_i, P~_i); ideal gas with T = u / c_v:
+ *             rho~ = P~ / ((gamma-1) u~), c_v cancels (reading R26), so the
+ *             "temperature" handled here is u itself.
+ * mat == NULL means one material.
+ * ------------------------------------------------------------------------- */
+int orc_imbalance_brute(int64_t n, const double *x, const double *y, const double *z,
+                        const double *m, const double *h, const int32_t *mat, const orc_box *box,
+                        const orc_params *p, double alpha, int64_t nt, const int64_t *targets,
+                        double *imb)
+{
+#pragma omp parallel for schedule(dynamic, 8)
+    for (int64_t t = 0; t < nt; t++) {
+        int64_t i = targets ? targets[t] : t;
+        double s[3] = {0.0, 0.0, 0.0}, den = 0.0, d[3];
+        for (int64_t j = 0; j < n; j++) {
+            double r2 = orc_r2(x, y, z, i, j, box, d);   /* d = x_i - x_j */
+            if (r2 >= 4.0 * h[i] * h[i]) continue;
+            double w = orc_w(p->kernel, sqrt(r2) / h[i]);      /* W up to the common h^-3 */
+            double kappa = (mat && mat[i] != mat[j]) ? -1.0 : 1.0;
+            for (int k = 0; k < 3; k++) s[k] += kappa * (-d[k]) * m[j] * w;   /* r_j - r_i */
+            den += m[j] * w;
+        }
+        imb[t] = alpha * sqrt(s[0] * s[0] + s[1] * s[1] + s[2] * s[2]) / (h[i] * den);
+    }
+    return 0;
+}
+
+int orc_interface_brute(int64_t n, const double *x, const double *y, const double *z,
+                        const double *h, const double *u, const double *rho, const double *imb,
+                        const orc_box *box, const orc_params *p, int64_t nt,
+                        const int64_t *targets, double *rho_corr, double *P_corr, double *u_corr)
+{
+#pragma omp parallel for schedule(dynamic, 8)
+    for (int64_t t = 0; t < nt; t++) {
+        int64_t i = targets ? targets[t] : t;
+        double nT = 0.0, nP = 0.0, den = 0.0, d[3];
+        for (int64_t j = 0; j < n; j++) {
+            double r2 = orc_r2(x, y, z, i, j, box, d);
+            if (r2 >= 4.0 * h[i] * h[i]) continue;
+            double w = orc_w(p->kernel, sqrt(r2) / h[i]) * exp(-imb[j] * imb[j]);
+            double Pj = (p->gamma - 1.0) * rho[j] * u[j];
+            nT += u[j] * w; nP += Pj * w; den += w;                       /* Eq. (9) */
+        }
+        double e = exp(-imb[i] * imb[i]);
+        double Pi = (p->gamma - 1.0) * rho[i] * u[i];
+        double Pt = e * Pi + (1.0 - e) * nP / den;                        /* Eq. (10) */
+        double Tt = e * u[i] + (1.0 - e) * nT / den;                      /* Eq. (11) */
+        rho_corr[t] = Pt / ((p->gamma - 1.0) * Tt);                       /* Eq. (12) */
+        if (P_corr) P_corr[t] = Pt;
+        if (u_corr) u_corr[t] = Tt;
+    }
+    return 0;
+}

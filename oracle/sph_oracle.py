@@ -224,3 +224,31 @@ def drift(x, v, dt, lo, length, periodic):
     lib().orc_drift(C.c_int64(len(x)), C.c_double(dt), _p(v), C.c_double(float(np.float32(lo))),
                     C.c_double(float(np.float32(length))), C.c_int(int(periodic)), _p(x))
     return x
+
+
+def imbalance(x, y, z, m, h, mat, box: Box, par: Params, alpha: float, targets=None):
+    """Kernel imbalance I_i of Eq. (8) (brute force).  mat: int material ids or None."""
+    x, y, z, m, h = map(_d, (x, y, z, m, h))
+    n = len(x)
+    b, p = box.c(), par.c()
+    nt, t = _targets(n, targets)
+    out = np.empty(nt)
+    mm = None if mat is None else np.ascontiguousarray(np.asarray(mat), dtype=np.int32)
+    lib().orc_imbalance_brute(C.c_int64(n), _p(x), _p(y), _p(z), _p(m), _p(h),
+                              _p(mm, C.c_int32) if mm is not None else None, C.byref(b),
+                              C.byref(p), C.c_double(alpha), C.c_int64(nt), _p(t, C.c_int64),
+                              _p(out))
+    return out
+
+
+def interface_correction(x, y, z, h, u, rho, imb, box: Box, par: Params, targets=None):
+    """Eqs. (9)-(12) for the ideal gas (brute force): corrected rho, P and u (= c_v T)."""
+    x, y, z, h, u, rho, imb = map(_d, (x, y, z, h, u, rho, imb))
+    n = len(x)
+    b, p = box.c(), par.c()
+    nt, t = _targets(n, targets)
+    rc = np.empty(nt); pc = np.empty(nt); uc = np.empty(nt)
+    lib().orc_interface_brute(C.c_int64(n), _p(x), _p(y), _p(z), _p(h), _p(u), _p(rho), _p(imb),
+                              C.byref(b), C.byref(p), C.c_int64(nt), _p(t, C.c_int64), _p(rc),
+                              _p(pc), _p(uc))
+    return rc, pc, uc

@@ -139,6 +139,17 @@ extern "C" int sph_forces(sph_ctx* c, const float* m, const float* vx, const flo
     return sph_launch_forces(c, m, vx, vy, vz, u, rho, h, omega, ax, ay, az, dudt, mu_min, P, cs);
 }
 
+extern "C" int sph_interface_correction(sph_ctx* c, const float* m, const float* u,
+                                        const float* rho, const float* h, const int32_t* mat,
+                                        float alpha, float* imbalance, float* rho_corr,
+                                        float* P_corr) {
+    if (!c) return SPH_EINVAL;
+    if (!m || !u || !rho || !h || !imbalance || !rho_corr || !(alpha >= 0.0f))
+        return fail(c, SPH_EINVAL, "sph_interface_correction: bad argument");
+    if (!c->built) return fail(c, SPH_ESTALE, "sph_interface_correction before sph_build_cells");
+    return sph_launch_interface(c, m, u, rho, h, mat, alpha, imbalance, rho_corr, P_corr);
+}
+
 extern "C" int sph_timestep(sph_ctx* c, const float* h, const float* cs, const float* ax,
                             const float* ay, const float* az, const float* mu_min, float* dt_i,
                             float* dt_min) {

@@ -116,6 +116,10 @@ template <> struct SphKernel<0> {   // cubic spline (Monaghan 1992)
         const float u = fmaxf(2.0f - q, 0.0f);
         return q < 1.0f ? 3.0f - 2.25f * q : __fdividef(0.75f * u * u, q);
     }
+    static __device__ __forceinline__ float w(float q) {
+        const float u = fmaxf(2.0f - q, 0.0f);
+        return q < 1.0f ? 1.0f - q * q * (1.5f - 0.75f * q) : 0.25f * u * u * u;
+    }
 };
 template <> struct SphKernel<1> {   // Wendland C2: w = y^4 (1 + 4x)
     static constexpr float sigma = 0.41778172561566733f, self = 14.0f;
@@ -128,6 +132,10 @@ template <> struct SphKernel<1> {   // Wendland C2: w = y^4 (1 + 4x)
     static __device__ __forceinline__ float g(float q) {
         const float t = fmaxf(1.0f - 0.5f * q, 0.0f);
         return 5.0f * t * t * t;
+    }
+    static __device__ __forceinline__ float w(float q) {
+        const float t = fmaxf(1.0f - 0.5f * q, 0.0f), t2 = t * t;
+        return t2 * t2 * (1.0f + 2.0f * q);
     }
 };
 template <> struct SphKernel<2> {   // Wendland C4: w = y^6 (1 + 6x + 35/3 x^2)
@@ -142,6 +150,10 @@ template <> struct SphKernel<2> {   // Wendland C4: w = y^6 (1 + 6x + 35/3 x^2)
         const float x = 0.5f * q, y = fmaxf(1.0f - x, 0.0f), y2 = y * y;
         return (14.0f / 3.0f) * y2 * y2 * y * (1.0f + 5.0f * x);
     }
+    static __device__ __forceinline__ float w(float q) {
+        const float x = 0.5f * q, y = fmaxf(1.0f - x, 0.0f), y2 = y * y;
+        return y2 * y2 * y2 * (1.0f + x * (6.0f + (35.0f / 3.0f) * x));
+    }
 };
 template <> struct SphKernel<3> {   // Wendland C6: w = y^8 (1 + 8x + 25x^2 + 32x^3)
     static constexpr float sigma = 0.84861913015795750f, self = 28.4375f;
@@ -154,6 +166,10 @@ template <> struct SphKernel<3> {   // Wendland C6: w = y^8 (1 + 8x + 25x^2 + 32
     static __device__ __forceinline__ float g(float q) {
         const float x = 0.5f * q, y = fmaxf(1.0f - x, 0.0f), y2 = y * y;
         return 5.5f * y2 * y2 * y2 * y * (1.0f + x * (7.0f + 16.0f * x));
+    }
+    static __device__ __forceinline__ float w(float q) {
+        const float x = 0.5f * q, y = fmaxf(1.0f - x, 0.0f), y2 = y * y, y4 = y2 * y2;
+        return y4 * y4 * (1.0f + x * (8.0f + x * (25.0f + 32.0f * x)));
     }
 };
 
@@ -537,3 +553,6 @@ int sph_launch_timestep(sph_ctx* c, const float* h, const float* cs, const float
 int sph_launch_neighbors(sph_ctx* c, const float* h, int32_t mode, int64_t* offsets,
                          int32_t* indices, int64_t capacity, int64_t* needed);
 int sph_launch_fp32_peak(cudaStream_t s, float seconds, double* tflops);
+int sph_launch_interface(sph_ctx* c, const float* m, const float* u, const float* rho, const float* h,
+                         const int32_t* mat, float alpha, float* imbalance, float* rho_corr,
+                         float* P_corr);

@@ -352,3 +352,63 @@ def test_c1_other_kernels_and_neighbour_numbers(gu, kernel, n_ngb):
     _check_sample(gu, w, ctx, out, h, np.arange(w["n"]), op, ob)
     if n_ngb >= 200.0:
         assert st["dens_overflow"] > 0      # the robust path was exercised
+
+
+# ------------------------------------------------------------------------------------------
+# Interface correction, Eqs. (8)-(12)
+# ------------------------------------------------------------------------------------------
+def _interface_case(gu, w, mat, with_lists, kernel=1):
+    from paper_2511_11425_b200 import sph
+    _, op = gu.make_params(w, kernel=kernel)
+    _, ob = gu.make_boxes(w)
+    n = int(w["n"])
+    d = gu.to_device(w)
+    ctx = gu.make_ctx(w, kernel=kernel)
+    out = sph.StepBuffers(n)
+    h = d["h"].clone()
+    ctx.build_cells(d["x"], d["y"], d["z"], h)
+    if with_lists:     # the density sweep leaves its neighbour lists for the later sweeps
+        ctx.density_h(d["m"], h, out["rho"], out["omega"], out["n_ngb"])
+        rho = out["rho"]
+    else:              # no lists: the groups walk the cell rows themselves
+        rho = torch.from_numpy(np.random.default_rng(9).uniform(0.5, 2.0, n).astype(np.float32)).cuda()
+    tmat = None if mat is None else torch.from_numpy(mat.astype(np.int32)).cuda()
+    imb, rc, pc = (torch.empty(n, device="cuda") for _ in range(3))
+    alpha = 1.5
+    ctx.interface_correction(d["m"], d["u"], rho, h, tmat, alpha, imb, rc, pc)
+    torch.cuda.synchronize()
+    hg, rg = h.cpu().numpy(), rho.cpu().numpy()
+    oI = orc.imbalance(w["x"], w["y"], w["z"], w["m"], hg, mat, ob, op, alpha)
+    gI = gu.np64(imb)
+    assert np.abs(gI - oI).max() <= 2e-5 * max(oI.max(), 1e-3), np.abs(gI - oI).max()
+    # pass 2 on the device's own I (stage-isolated), every particle
+    orc_rc, orc_pc, _ = orc.interface_correction(w["x"], w["y"], w["z"], hg, w["u"], rg,
+                                                 imb.cpu().numpy(), ob, op)
+    assert _rel(gu.np64(rc), orc_rc).max() <= TOL_H
+    assert _rel(gu.np64(pc), orc_pc).max() <= TOL_H
+    return oI, gu.np64(rc), rg
+
+
+def test_interface_correction_two_materials_periodic(gu):
+    """Config 1 split into two materials at x = 0.5 with a 4:1 jump in u: I peaks at the
+    material interface (kappa = -1 across it), the correction mixes P and T there."""
+    w = workloads.uniform_cube(h_start="warm")
+    w["u"] = np.where(w["x"] < 0.5, 4.0, 1.0).astype(np.float32)
+    mat = (w["x"] >= 0.5).astype(np.int32)
+    oI, rc, rho = _interface_case(gu, w, mat, with_lists=True)
+    near = np.minimum(np.abs(w["x"] - 0.5), np.minimum(w["x"], 1 - w["x"])) < 0.03
+    far = np.abs(np.abs(w["x"] - 0.5) - 0.25) < 0.05
+    assert oI[near].mean() > 10 * max(oI[far].mean(), 1e-3)
+    assert np.abs(rc[far] / rho[far] - 1).max() < np.abs(rc[near] / rho[near] - 1).max()
+
+
+def test_interface_correction_free_surface_without_lists(gu):
+    """Open box (vacuum around a jittered cube), one material, no neighbour lists, random rho:
+    the search path of the sweep; and once more with the Wendland C4 kernel and lists."""
+    rng = np.random.default_rng(61)
+    w = workloads.uniform_cube(nside=12, h_start="warm")
+    w["periodic"] = (0, 0, 0)
+    w["u"] = rng.uniform(0.5, 3.0, w["n"]).astype(np.float32)
+    oI, _, _ = _interface_case(gu, w, None, with_lists=False)
+    assert oI.max() > 0.3                       # the surface layers are strongly one-sided
+    _interface_case(gu, w, None, with_lists=True, kernel=2)

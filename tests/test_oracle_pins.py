@@ -512,3 +512,77 @@ def test_drift_wraps_into_the_periodic_box():
     assert np.allclose(orc.drift(x, v, 0.1, 0.0, 1.0, 0), x + 0.1 * v)
     # a shifted box
     assert np.allclose(orc.drift(np.array([2.9]), np.array([1.0]), 0.2, 1.0, 2.0, 1), [1.1])
+
+
+# ------------------------------------------------------------------------------------------
+# Interface correction, Eqs. (8)-(12): closed forms and invariants of the oracle.
+# ------------------------------------------------------------------------------------------
+def _three_in_a_row(d, h):
+    x = np.array([0.0, d, -d]); z = np.zeros(3)
+    return x, z, z, np.full(3, 1.0), np.full(3, h)
+
+
+def test_imbalance_closed_forms_and_material_sign():
+    """Middle particle with a neighbour on either side at distance d: same material -> the
+    two terms cancel, I = 0; the far side of another material -> kappa = -1 adds them,
+    I = alpha 2 (d/h) w(q) / (w(0) + 2 w(q)).  One neighbour only: alpha (d/h) w/(w(0)+w)."""
+    box = orc.Box((-10, -10, -10), (20, 20, 20), (0, 0, 0))
+    par = orc.Params()
+    d, h, alpha = 0.7, 0.5, 1.5
+    x, y, z, m, hh = _three_in_a_row(d, h)
+    w0, wq = orc.w(1, 0.0), orc.w(1, d / h)
+    same = orc.imbalance(x, y, z, m, hh, None, box, par, alpha, targets=[0])
+    assert abs(same[0]) < 1e-15
+    mixed = orc.imbalance(x, y, z, m, hh, [0, 0, 1], box, par, alpha, targets=[0])
+    assert abs(mixed[0] - alpha * 2 * (d / h) * wq / (w0 + 2 * wq)) < 1e-14
+    one = orc.imbalance(x[:2], y[:2], z[:2], m[:2], hh[:2], None, box, par, alpha, targets=[0])
+    assert abs(one[0] - alpha * (d / h) * wq / (w0 + wq)) < 1e-14
+    # unequal masses weight the terms (Eq. 8 carries m_j)
+    m2 = np.array([1.0, 3.0, 1.0])
+    het = orc.imbalance(x, y, z, m2, hh, None, box, par, alpha, targets=[0])
+    assert abs(het[0] - alpha * (d / h) * 2 * wq / (w0 + 4 * wq)) < 1e-14
+
+
+def test_imbalance_vanishes_on_a_lattice_and_grows_towards_a_free_surface():
+    n1 = 10
+    g = (np.arange(n1) + 0.5) / n1
+    X, Y, Z = np.meshgrid(g, g, g, indexing="ij")
+    x, y, z = X.ravel(), Y.ravel(), Z.ravel()
+    m = np.full(x.size, 1.0 / x.size); h = np.full(x.size, 1.2347 / n1)
+    par = orc.Params()
+    per = orc.Box((0, 0, 0), (1, 1, 1), (1, 1, 1))
+    assert orc.imbalance(x, y, z, m, h, None, per, par, 1.5).max() < 1e-13
+    opn = orc.Box((0, 0, 0), (1, 1, 1), (0, 0, 0))
+    I = orc.imbalance(x, y, z, m, h, None, opn, par, 1.5)
+    centre = (np.abs(x - 0.5) < 0.11) & (np.abs(y - 0.5) < 0.11) & (np.abs(z - 0.5) < 0.11)
+    face = (x < 0.1) & (np.abs(y - 0.5) < 0.11) & (np.abs(z - 0.5) < 0.11)
+    second = (np.abs(x - 0.15) < 0.01) & (np.abs(y - 0.5) < 0.11) & (np.abs(z - 0.5) < 0.11)
+    assert I[centre].max() < 1e-13 and I[face].min() > 0.25 and I[second].max() < I[face].min()
+
+
+def test_interface_correction_leaves_a_uniform_state_alone_and_mixes_across_a_jump():
+    rng = np.random.default_rng(5)
+    n = 600
+    x, y, z = rng.uniform(0, 1, (3, n))
+    h = np.full(n, 0.12); par = orc.Params(gamma=1.4)
+    box = orc.Box((0, 0, 0), (1, 1, 1), (1, 1, 1))
+    m = np.full(n, 1.0 / n)
+    I = orc.imbalance(x, y, z, m, h, None, box, par, 1.5)
+    rho = np.full(n, 0.8); u = np.full(n, 2.5)
+    rc, pc, uc = orc.interface_correction(x, y, z, h, u, rho, I, box, par)
+    # P_j, T_j equal everywhere: Eqs. (9)-(11) return them unchanged, Eq. (12) gives rho back
+    assert np.abs(rc / 0.8 - 1).max() < 1e-14 and np.abs(pc / (0.4 * 0.8 * 2.5) - 1).max() < 1e-14
+    # I = 0 switches the correction off whatever the neighbours hold (Eqs. 10-11)
+    u2 = rng.uniform(1, 3, n); rho2 = rng.uniform(0.5, 2, n)
+    rc0, _, _ = orc.interface_correction(x, y, z, h, u2, rho2, np.zeros(n), box, par)
+    assert np.abs(rc0 / rho2 - 1).max() < 1e-14
+    # large I: the particle takes the kernel average of its neighbours (which all have I = 0
+    # except itself, whose weight e^{-I^2} vanishes)
+    Ibig = np.zeros(n); Ibig[0] = 10.0
+    rcb, pcb, ucb = orc.interface_correction(x, y, z, h, u2, rho2, Ibig, box, par, targets=[0])
+    d = np.stack([x - x[0], y - y[0], z - z[0]]); d -= np.rint(d)
+    r = np.sqrt((d * d).sum(0)); wgt = np.array([orc.w(1, q) for q in r / h[0]]); wgt[0] = 0.0
+    Pn = 0.4 * rho2 * u2
+    assert abs(pcb[0] - (Pn * wgt).sum() / wgt.sum()) < 1e-13
+    assert abs(ucb[0] - (u2 * wgt).sum() / wgt.sum()) < 1e-13
+    assert abs(rcb[0] - pcb[0] / (0.4 * ucb[0])) < 1e-13
