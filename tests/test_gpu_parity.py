@@ -412,3 +412,57 @@ def test_interface_correction_free_surface_without_lists(gu):
     oI, _, _ = _interface_case(gu, w, None, with_lists=False)
     assert oI.max() > 0.3                       # the surface layers are strongly one-sided
     _interface_case(gu, w, None, with_lists=True, kernel=2)
+
+
+# ------------------------------------------------------------------------------------------
+# Error behaviour of the boundary (include/sph.h): codes, no exceptions from the library
+# ------------------------------------------------------------------------------------------
+def test_error_codes_on_the_device(gu):
+    import ctypes as C
+    from paper_2511_11425_b200 import sph
+    w = workloads.uniform_cube(nside=8, h_start="warm")
+    d = gu.to_device(w)
+    n = int(w["n"])
+    ctx = sph.Sph(sph.Params(), sph.Box(), n)
+    out = sph.StepBuffers(n)
+    lib, c = ctx.lib, ctx._ctx
+    P = lambda t: C.c_void_p(t.data_ptr())
+    # calls before sph_build_cells
+    assert lib.sph_density_h(c, P(d["m"]), P(d["h"]), P(out["rho"]), P(out["omega"]),
+                             P(out["n_ngb"])) == sph.SPH_ESTALE
+    assert b"sph_build_cells" in lib.sph_last_error(c)
+    assert lib.sph_permutation(c, P(out["n_ngb"])) == sph.SPH_ESTALE
+    # n out of range, null arrays
+    assert lib.sph_build_cells(c, n + 1, P(d["x"]), P(d["y"]), P(d["z"]), P(d["h"])) == sph.SPH_EINVAL
+    assert lib.sph_build_cells(c, 0, P(d["x"]), P(d["y"]), P(d["z"]), P(d["h"])) == sph.SPH_EINVAL
+    assert lib.sph_build_cells(c, n, None, P(d["y"]), P(d["z"]), P(d["h"])) == sph.SPH_EINVAL
+    # a failed build leaves the context unbuilt
+    assert lib.sph_density_h(c, P(d["m"]), P(d["h"]), P(out["rho"]), P(out["omega"]),
+                             P(out["n_ngb"])) == sph.SPH_ESTALE
+    ctx.build_cells(d["x"], d["y"], d["z"], d["h"])
+    # neighbour lists: too small a buffer reports the size needed
+    off = torch.empty(n + 1, dtype=torch.int64, device="cuda")
+    idx = torch.empty(10, dtype=torch.int32, device="cuda")
+    need = C.c_int64(0)
+    rc = lib.sph_neighbors(c, P(d["h"]), 0, P(off), P(idx), 10, C.byref(need))
+    assert rc == sph.SPH_ENOSPC and need.value > 10
+    assert lib.sph_neighbors(c, P(d["h"]), 2, P(off), P(idx), 10, C.byref(need)) == sph.SPH_EINVAL
+    # creation: bad box, bad kernel, neighbour number below the self contribution
+    bad = C.c_void_p()
+    pp, bb = sph.Params().c(), sph.Box(len=(1.0, 0.0, 1.0)).c()
+    assert lib.sph_create(C.byref(bad), C.byref(pp), C.byref(bb), 10, None) == sph.SPH_EINVAL
+    pp, bb = sph.Params(kernel=7).c(), sph.Box().c()
+    assert lib.sph_create(C.byref(bad), C.byref(pp), C.byref(bb), 10, None) == sph.SPH_EINVAL
+    pp = sph.Params(kernel=3, n_ngb=20.0).c()          # Wendland C6 alone already counts 28.4
+    assert lib.sph_create(C.byref(bad), C.byref(pp), C.byref(bb), 10, None) == sph.SPH_EINVAL
+    # the Python binding turns codes into exceptions and checks tensors itself
+    with pytest.raises(sph.SphError):
+        ctx.density_h(d["m"].double(), d["h"], out["rho"], out["omega"], out["n_ngb"])
+    with pytest.raises(sph.SphError):
+        ctx.density_h(d["m"][:-1], d["h"], out["rho"], out["omega"], out["n_ngb"])
+    # a periodic box too small for the kernel support is flagged
+    w2 = workloads.uniform_cube(nside=4, h_start="warm")
+    c2 = gu.make_ctx(w2)
+    d2 = gu.to_device(w2)
+    c2.build_cells(d2["x"], d2["y"], d2["z"], d2["h"])
+    assert c2.stats()["grid_flags"] & 1
