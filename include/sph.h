@@ -127,6 +127,13 @@ int  sph_forces(sph_ctx* ctx, const float* m, const float* vx, const float* vy, 
 int  sph_timestep(sph_ctx* ctx, const float* h, const float* c, const float* ax, const float* ay,
                   const float* az, const float* mu_min, float* dt_i, float* dt_min_device);
 
+/* Time-step rungs.  rung_i = the smallest r >= 0 with 2^-r dt0 <= dt_i
+ * (Eq. 27, capped at max_rung <= 62), then the limiter of Saitoh & Makino (2009): rung_i >=
+ * rung_j - 2 for every particle j of the force pair set of i, one pass over the Eq. (27)
+ * values.  Uses the neighbour data of the last sph_forces (same positions, same h), else
+ * SPH_ESTALE.  rung: n int32, caller order.                                                  */
+int  sph_rungs(sph_ctx* ctx, const float* dt_i, float dt0, int32_t max_rung, int32_t* rung);
+
 /* Interface correction for the ideal gas, PAPER.md:158-182 (Section 2.3.4), Eqs. (8)-(12);
  * call between sph_density_h and sph_forces and hand rho_corr to sph_forces.  Gather sums over
  * r_ij < 2 h_i, self included.

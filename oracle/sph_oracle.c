@@ -741,3 +741,43 @@ int orc_interface_brute(int64_t n, const double *x, const double *y, const doubl
     }
     return 0;
 }
+
+/* ------------------------------------------------------------------------- *
+ * Time-step rungs.
+ *   Eq. (27)  the desired rung r_i: min(dt_a, dt_CFL) >= 2^-r_i dt0; taken as
+ *             the SMALLEST such r_i >= 0 (the largest admissible step), capped
+ *             at max_rung.
+ *   Limiter   (Saitoh & Makino 2009): no particle may have a step
+ *             larger than four times that of any particle it interacts with:
+ *             r_i >= r_j - 2 for all neighbours j.  One pass over the rungs of
+ *             Eq. (27) (reading R28); "interacts with" = the force pair set
+ *             0 < r_ij < 2 max(h_i, h_j) (reading R14).
+ * ------------------------------------------------------------------------- */
+void orc_rungs(int64_t n, const double *dt_i, double dt0, int32_t max_rung, int32_t *rung)
+{
+    for (int64_t i = 0; i < n; i++) {
+        int32_t r = 0;
+        double t = dt0;
+        while (r < max_rung && t > dt_i[i]) { t *= 0.5; r++; }
+        rung[i] = r;
+    }
+}
+
+void orc_rung_limiter_brute(int64_t n, const double *x, const double *y, const double *z,
+                            const double *h, const orc_box *box, const int32_t *rung_in,
+                            int64_t nt, const int64_t *targets, int32_t *rung_out)
+{
+#pragma omp parallel for schedule(dynamic, 8)
+    for (int64_t t = 0; t < nt; t++) {
+        int64_t i = targets ? targets[t] : t;
+        int32_t r = rung_in[i];
+        double d[3];
+        for (int64_t j = 0; j < n; j++) {
+            if (j == i) continue;
+            double r2 = orc_r2(x, y, z, i, j, box, d);
+            double hh = h[j] > h[i] ? h[j] : h[i];
+            if (r2 > 0.0 && r2 < 4.0 * hh * hh && rung_in[j] - 2 > r) r = rung_in[j] - 2;
+        }
+        rung_out[t] = r;
+    }
+}

@@ -252,3 +252,26 @@ def interface_correction(x, y, z, h, u, rho, imb, box: Box, par: Params, targets
                               C.byref(b), C.byref(p), C.c_int64(nt), _p(t, C.c_int64), _p(rc),
                               _p(pc), _p(uc))
     return rc, pc, uc
+
+
+def rungs(dt_i, dt0, max_rung):
+    """Eq. (27): smallest r >= 0 with 2^-r dt0 <= dt_i, capped at max_rung."""
+    dt_i = _d(dt_i)
+    out = np.empty(len(dt_i), np.int32)
+    lib().orc_rungs(C.c_int64(len(dt_i)), _p(dt_i), C.c_double(float(np.float32(dt0))),
+                    C.c_int32(int(max_rung)), _p(out, C.c_int32))
+    return out
+
+
+def rung_limiter(x, y, z, h, rung, box: Box, targets=None):
+    """r_i >= r_j - 2 over the force pair set, one pass (brute force)."""
+    x, y, z, h = map(_d, (x, y, z, h))
+    n = len(x)
+    b = box.c()
+    nt, t = _targets(n, targets)
+    rin = np.ascontiguousarray(np.asarray(rung), dtype=np.int32)
+    out = np.empty(nt, np.int32)
+    lib().orc_rung_limiter_brute(C.c_int64(n), _p(x), _p(y), _p(z), _p(h), C.byref(b),
+                                 _p(rin, C.c_int32), C.c_int64(nt), _p(t, C.c_int64),
+                                 _p(out, C.c_int32))
+    return out

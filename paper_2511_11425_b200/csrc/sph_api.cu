@@ -111,6 +111,7 @@ extern "C" int sph_build_cells(sph_ctx* c, int64_t n, const float* x, const floa
     if (!x || !y || !z || !h) return fail(c, SPH_EINVAL, "sph_build_cells: null array");
     if (n <= 0 || n > c->n_max) return fail(c, SPH_EINVAL, "sph_build_cells: n out of range");
     c->built = false;
+    c->forces_ready = false;
     int rc = sph_launch_build(c, n, x, y, z, h);
     if (rc == SPH_OK) {
         c->n     = n;
@@ -136,7 +137,9 @@ extern "C" int sph_forces(sph_ctx* c, const float* m, const float* vx, const flo
         !mu_min || !P || !cs)
         return fail(c, SPH_EINVAL, "sph_forces: null array");
     if (!c->built) return fail(c, SPH_ESTALE, "sph_forces before sph_build_cells");
-    return sph_launch_forces(c, m, vx, vy, vz, u, rho, h, omega, ax, ay, az, dudt, mu_min, P, cs);
+    const int rc = sph_launch_forces(c, m, vx, vy, vz, u, rho, h, omega, ax, ay, az, dudt, mu_min, P, cs);
+    c->forces_ready = (rc == SPH_OK);
+    return rc;
 }
 
 extern "C" int sph_interface_correction(sph_ctx* c, const float* m, const float* u,
@@ -148,6 +151,15 @@ extern "C" int sph_interface_correction(sph_ctx* c, const float* m, const float*
         return fail(c, SPH_EINVAL, "sph_interface_correction: bad argument");
     if (!c->built) return fail(c, SPH_ESTALE, "sph_interface_correction before sph_build_cells");
     return sph_launch_interface(c, m, u, rho, h, mat, alpha, imbalance, rho_corr, P_corr);
+}
+
+extern "C" int sph_rungs(sph_ctx* c, const float* dt_i, float dt0, int32_t max_rung, int32_t* rung) {
+    if (!c) return SPH_EINVAL;
+    if (!dt_i || !rung || !(dt0 > 0.0f) || max_rung < 0 || max_rung > 62)
+        return fail(c, SPH_EINVAL, "sph_rungs: bad argument");
+    if (!c->built || !c->forces_ready)
+        return fail(c, SPH_ESTALE, "sph_rungs needs sph_forces on the current positions");
+    return sph_launch_rungs(c, dt_i, dt0, max_rung, rung);
 }
 
 extern "C" int sph_timestep(sph_ctx* c, const float* h, const float* cs, const float* ax,

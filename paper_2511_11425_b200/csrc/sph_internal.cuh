@@ -45,6 +45,7 @@ struct sph_ctx {
     int64_t      cap_cells;
     cudaStream_t stream;
     bool         built;
+    bool         forces_ready; // sph_forces ran since the last build: pos_h.w, coarse map valid
     int          sm_count;
     // device memory
     SphGrid*     grid;
@@ -553,6 +554,7 @@ int sph_launch_timestep(sph_ctx* c, const float* h, const float* cs, const float
 int sph_launch_neighbors(sph_ctx* c, const float* h, int32_t mode, int64_t* offsets,
                          int32_t* indices, int64_t capacity, int64_t* needed);
 int sph_launch_fp32_peak(cudaStream_t s, float seconds, double* tflops);
+int sph_launch_rungs(sph_ctx* c, const float* dt_i, float dt0, int32_t max_rung, int32_t* rung);
 int sph_launch_interface(sph_ctx* c, const float* m, const float* u, const float* rho, const float* h,
                          const int32_t* mat, float alpha, float* imbalance, float* rho_corr,
                          float* P_corr);

@@ -19,7 +19,7 @@ SPH_OK, SPH_EINVAL, SPH_EBOX, SPH_ENOMEM, SPH_ECUDA, SPH_ESTALE, SPH_ENOSPC = 0,
 
 # every symbol include/sph.h declares (tests check the library exports exactly these)
 SYMBOLS = ["sph_create", "sph_destroy", "sph_build_cells", "sph_density_h", "sph_forces",
-           "sph_timestep", "sph_interface_correction", "sph_predict", "sph_kick", "sph_drift", "sph_neighbors", "sph_stats", "sph_stats_reset", "sph_permutation",
+           "sph_timestep", "sph_rungs", "sph_interface_correction", "sph_predict", "sph_kick", "sph_drift", "sph_neighbors", "sph_stats", "sph_stats_reset", "sph_permutation",
            "sph_fp32_peak", "sph_strerror", "sph_last_error"]
 
 
@@ -102,6 +102,7 @@ def load():
     lib.sph_density_h.argtypes = [vp] + [fp] * 5
     lib.sph_forces.argtypes = [vp] + [fp] * 15
     lib.sph_timestep.argtypes = [vp] + [fp] * 8
+    lib.sph_rungs.argtypes = [vp, fp, C.c_float, i32, fp]
     lib.sph_interface_correction.argtypes = [vp] + [fp] * 5 + [C.c_float] + [fp] * 3
     lib.sph_predict.argtypes = [vp, i64, fp, C.c_float] + [fp] * 12
     lib.sph_kick.argtypes = [vp, i64, fp, C.c_float] + [fp] * 8
@@ -199,6 +200,12 @@ class Sph:
         n, f = self.n, torch.float32
         args = [_ptr(t, f, n) for t in (h, c, ax, ay, az, mu_min, dt_i)]
         self._check(self.lib.sph_timestep(self._ctx, *args, _ptr(dt_min, f, 1)))
+
+    # ---- rungs (Eq. 27 + Saitoh-Makino limiter) ------------------------------------------
+    def rungs(self, dt_i, dt0, max_rung, rung):
+        n = self.n
+        self._check(self.lib.sph_rungs(self._ctx, _ptr(dt_i, torch.float32, n), float(dt0),
+                                       int(max_rung), _ptr(rung, torch.int32, n)))
 
     # ---- interface correction (Eqs. 8-12) -------------------------------------------------
     def interface_correction(self, m, u, rho, h, mat, alpha, imbalance, rho_corr, P_corr=None):

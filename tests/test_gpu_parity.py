@@ -466,3 +466,34 @@ def test_error_codes_on_the_device(gu):
     d2 = gu.to_device(w2)
     c2.build_cells(d2["x"], d2["y"], d2["z"], d2["h"])
     assert c2.stats()["grid_flags"] & 1
+
+
+# ------------------------------------------------------------------------------------------
+# Rungs: Eq. (27) and the Saitoh-Makino limiter, integers: bit-exact
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("which", ["uniform_cube", "sod_tube"])
+def test_rungs_and_limiter_bit_exact(gu, which):
+    from paper_2511_11425_b200 import sph
+    w = workloads.uniform_cube(h_start="warm") if which == "uniform_cube" else \
+        workloads.sod_tube(ncross=20, h_start="warm")
+    _, op = gu.make_params(w)
+    _, ob = gu.make_boxes(w)
+    ctx, d, out, h = _full_step(gu, w)
+    n = int(w["n"])
+    # the real dt_i of the step, and a synthetic field with isolated fast particles
+    rng = np.random.default_rng(71)
+    synth = (0.01 * 2.0 ** (-rng.integers(0, 9, n) * (rng.random(n) < 0.02))).astype(np.float32)
+    rung = torch.empty(n, dtype=torch.int32, device="cuda")
+    hg = h.cpu().numpy()
+    for dt_i, dt0 in ((out["dt_i"].cpu().numpy(), 4.0 * float(out["dt_min"].item())), (synth, 0.01)):
+        ctx.rungs(torch.from_numpy(dt_i).cuda(), dt0, 12, rung)
+        r0 = orc.rungs(dt_i, dt0, 12)
+        want = orc.rung_limiter(w["x"], w["y"], w["z"], hg, r0, ob)
+        got = rung.cpu().numpy()
+        assert np.array_equal(got, want), int((got != want).sum())
+        assert (want >= r0).all()
+    assert (want > r0).any()            # the limiter did raise neighbours of the fast particles
+    # needs the neighbour data of sph_forces
+    ctx.build_cells(d["x"], d["y"], d["z"], h)
+    with pytest.raises(sph.SphError):
+        ctx.rungs(out["dt_i"], 0.01, 12, rung)

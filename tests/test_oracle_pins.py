@@ -586,3 +586,32 @@ def test_interface_correction_leaves_a_uniform_state_alone_and_mixes_across_a_ju
     assert abs(pcb[0] - (Pn * wgt).sum() / wgt.sum()) < 1e-13
     assert abs(ucb[0] - (u2 * wgt).sum() / wgt.sum()) < 1e-13
     assert abs(rcb[0] - pcb[0] / (0.4 * ucb[0])) < 1e-13
+
+
+# ------------------------------------------------------------------------------------------
+# Rungs, Eq. (27), and the Saitoh-Makino limiter
+# ------------------------------------------------------------------------------------------
+def test_rungs_are_the_largest_admissible_power_of_two_steps():
+    dt0 = 1.0
+    dt = np.array([2.0, 1.0, 0.999, 0.5, 0.4999, 0.26, 0.25, 1e-9])
+    r = orc.rungs(dt, dt0, 20)
+    assert list(r) == [0, 0, 1, 1, 2, 2, 2, 20]          # last one capped
+    ok = dt0 * 0.5 ** r <= dt                             # Eq. (27) holds ...
+    assert ok[:-1].all()
+    assert ((r[:-1] == 0) | (dt0 * 0.5 ** (r[:-1] - 1) > dt[:-1])).all()   # ... and r is minimal
+
+
+def test_rung_limiter_on_a_line_of_particles():
+    n = 21
+    x = np.arange(n) * 1.0; z = np.zeros(n)
+    h = np.full(n, 0.6)                                   # support 1.2: nearest neighbours only
+    box = orc.Box((-5, -5, -5), (40, 10, 10), (0, 0, 0))
+    r0 = np.zeros(n, np.int32); r0[10] = 5
+    r1 = orc.rung_limiter(x, z, z, h, r0, box)
+    want = r0.copy(); want[9] = want[11] = 3
+    assert np.array_equal(r1, want)                       # one pass: no further propagation
+    h2 = h.copy(); h2[10] = 1.6                           # scatter: its 3.2-ball reaches 3 each side
+    r2 = orc.rung_limiter(x, z, z, h2, r0, box)
+    want2 = r0.copy(); want2[7:10] = 3; want2[11:14] = 3
+    assert np.array_equal(r2, want2)
+    assert np.array_equal(orc.rung_limiter(x, z, z, h, np.full(n, 4, np.int32), box), np.full(n, 4))
