@@ -59,8 +59,10 @@ typedef struct {
     float   av_eps;       /* Eq. (16) epsilon (0.01, Monaghan 1992)                        */
     float   eta_cfl;      /* Eq. (26) Courant parameter eta_C                              */
     float   eta_acc;      /* eta_a = 0.2                                    */
-    float   h_tol;        /* Newton stop |dh|/h (<= 0: default 1e-6)                       */
-    int32_t h_max_iter;   /* Newton sweep cap per particle (<= 0: default 40)              */
+    float   h_tol;        /* relative width at which a bisection bracket of h counts as     */
+                          /* converged (<= 0: default 1e-6); regular steps stop earlier:    */
+                          /* a Halley step below 3e-4 h is final      */
+    int32_t h_max_iter;   /* sweep cap per particle (<= 0: default 40)                      */
     float   search_slack; /* density search radius = 2 h_guess x this (<= 1: default 1.1);  */
                           /* PAPER.md:152 "slightly larger kernel"; results do not depend   */
                           /* on it                                                         */
@@ -71,9 +73,9 @@ typedef struct {
 /* 64-bit counters accumulated on the device since the last sph_stats_reset.             */
 typedef struct {
     int64_t dens_tested;      /* candidate pairs distance-tested by sph_density_h          */
-    int64_t dens_listed;      /* pairs kept in the per-target lists (within the slack ball) */
+    int64_t dens_listed;      /* pairs put on the per-target lists (within the slack ball)  */
     int64_t dens_pairs;       /* sum_i n_i at the final h (self included)                  */
-    int64_t dens_sweeps;      /* Newton sweeps summed over particles                       */
+    int64_t dens_sweeps;      /* sweeps over the neighbour lists, summed over particles    */
     int64_t dens_recollect;   /* targets whose search ball had to be rebuilt larger        */
     int64_t dens_overflow;    /* targets finished by the robust list-free kernel (a list   */
                               /* column overflowed, or an entry sat in the FP64 band)      */
@@ -104,8 +106,8 @@ int  sph_build_cells(sph_ctx* ctx, int64_t n, const float* x, const float* y, co
                      const float* h);
 
 /* Steps a4-a6: Eqs. (5)-(7).  For every particle finds h_i with
- * (32 pi/3) sum_j m_j w(r_ij/h_i) = n_ngb m_i (gather, self included) by safeguarded
- * Newton-Raphson on a per-target neighbour list, then writes
+ * (32 pi/3) sum_j m_j w(r_ij/h_i) = n_ngb m_i (gather, self included) by a safeguarded
+ * Newton-type (Halley) iteration on a per-target neighbour list, then writes
  *   h_inout (in: guess, out: solution), rho = sum_j m_j W_ij(h_i), omega (Eq. 7),
  *   n_ngb_out = #{j : r_ij < 2 h_i} (borderline pairs decided in FP64).                  */
 int  sph_density_h(sph_ctx* ctx, const float* m, float* h_inout, float* rho, float* omega,
