@@ -38,6 +38,11 @@ FLOP_DENS, FLOP_FORCE, FLOP_FORCE_AV = 27.0, 50.0, 70.0
 # dram__bytes_read.sum + dram__bytes_write.sum per launch on sedov_128^3, from the ncu --set full
 # capture summarised in profiles/r1e_density_forces.md (k_density / k_forces)
 NCU_DRAM_BYTES = {"density_h": 214.7e6 + 779.4e6, "forces": 942.4e6 + 43.4e6}
+# executed FP32 lane-operations per cycle (fadd + fmul + 2 ffma, predicated-on threads) over the
+# 148 x 128 x 2 the chip can retire, same capture: what the kernel executes, rejected candidates,
+# culling and Taylor/Halley bookkeeping included -- printed beside the useful (reject-free) fraction
+NCU_EXECUTED_FP32_FRAC = {"density_h": (692.2 + 1073.7 + 2 * 804.7) / (148 * 128 * 2),
+                          "forces": (690.3 + 1829.4 + 2 * 1327.6) / (148 * 128 * 2)}
 
 
 def parse():
@@ -323,6 +328,9 @@ def run_gpu(a):
                       traffic_source="profiles/r1e_density_forces.md (ncu --set full, bytes per launch)",
                       peak_source="derived: 148 SM x 128 FP32 lanes x 2 x 1.965 GHz",
                       measured_fma_peak=fma_peak, frac_of_measured_fma=ach / fma_peak,
+                      useful_frac=ach / NOMINAL_FP32_TFLOPS,
+                      executed_fp32_frac=(NCU_EXECUTED_FP32_FRAC.get(names[dom])
+                                          if a.nside == 128 else None),
                       algorithmic_flops_per_launch=dom_flops,
                       step_frac=(f_dens + f_force) / (float(step_ms.mean()) * 1e-3) / 1e12 /
                                 NOMINAL_FP32_TFLOPS),

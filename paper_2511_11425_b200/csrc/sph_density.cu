@@ -43,10 +43,15 @@ struct DensPar {
     int   max_iter;
 };
 
+// A target's list: entry f at float f of its group's segment; the segments of the four groups
+// of a warp start 8 banks apart (D_GSTRIDE = 192 + 8), so lane l of every group reading entry
+// 8k + l hits 32 different banks.
+constexpr int D_GSTRIDE = D_SLOTS * D_G + 8;
 struct WarpList {
-    float r[D_SLOTS][32];
-    float m[D_SLOTS][32];
+    float r[D_NT * D_GSTRIDE];
+    float m[D_NT * D_GSTRIDE];
 };
+constexpr int D_MOFF = D_NT * D_GSTRIDE * 4;   // byte offset of m behind r
 
 __global__ void k_pack_pos_m(int64_t n, const float4* __restrict__ pos_h,
                              const int32_t* __restrict__ perm, const float* __restrict__ m,
@@ -111,20 +116,23 @@ __global__ __launch_bounds__(D_TPB, SPH_MINB) void k_density(
         ((int*)&g)[threadIdx.x] = ((const int*)gp)[threadIdx.x];
     if (threadIdx.x < 5) st_sh[threadIdx.x] = 0u;
     if (threadIdx.x == 0) next_quad = 0;
+    // stale list entries are read (with weight 0) by lanes past their count: keep them finite
+    for (int k = threadIdx.x; k < (int)(sizeof(lists) / 4); k += D_TPB) ((float*)lists)[k] = 0.0f;
     __syncthreads();
 
-    const int   wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int   wid = threadIdx.x >> 5;
+    int         lane = threadIdx.x & 31;
+    asm volatile("" : "+r"(lane));              // one register instead of SR_TID re-reads
     const int   gq  = lane / D_G;
     const bool  leader = (lane & (D_G - 1)) == 0;
     const int   sl = lane & (D_G - 1), g0 = lane & ~(D_G - 1);
-    float* const lr = &lists[wid].r[0][lane];   // this lane's column, slot stride 32 floats
-    float* const lm = &lists[wid].m[0][lane];
-    float* const gr = &lists[wid].r[0][g0];     // the group's columns: entry f -> [f / 8][f % 8]
-    float* const gm_ = &lists[wid].m[0][g0];
+    // shared addresses (bytes) of the group's segment and of this lane's first entry in it
+    const uint32_t gb = sph_smem_addr(&lists[wid].r[gq * D_GSTRIDE]);
+    const uint32_t lb = gb + 4u * sl;
     const float hcap   = density_hcap(g);
     const float band_c = 2.5e-7f * g.xext;      // sph_band(h) = 1e-6 + band_c / h
 
-    unsigned c_tested = 0, c_listed = 0, c_pairs = 0, c_sweeps = 0, c_recollect = 0;
+    unsigned c_tested = 0;   // the other counters go to st_sh once per target
 
     for (;;) {
         int quad = 0;
@@ -145,7 +153,8 @@ __global__ __launch_bounds__(D_TPB, SPH_MINB) void k_density(
         h = fminf(h, hcap);
         const float T = par.n_ngb * pi.w * (1.0f / SphKernel<KERN>::self);
         // the target's kept list: entry f at [target][f]
-        uint32_t* const gj = nb_j + (size_t)(tvalid ? p : 0) * (D_SLOTS * D_G);
+        uint32_t* gj = nb_j + (size_t)(tvalid ? p : 0) * (D_SLOTS * D_G);
+        asm volatile("" : "+l"(gj));   // a register pair: entry addresses are one IMAD.WIDE
         float    hlo = 0.0f, hhi = __int_as_float(0x7f800000);
         float    Rc = 0.0f;         // radius the list is complete for
         int      cnt = 0;           // entries in the target's list (uniform in the group)
@@ -161,7 +170,7 @@ __global__ __launch_bounds__(D_TPB, SPH_MINB) void k_density(
             if (__any_sync(SPH_FULL, need)) {
                 if (need) {
                     Rc = 2.0f * h * (first ? par.slack : fmaxf(par.slack, 1.25f));
-                    if (!first && leader) ++c_recollect;
+                    if (!first && leader) atomicAdd(&st_sh[4], 1u);
                     first = false;
                     cnt   = 0;
                 }
@@ -172,10 +181,10 @@ __global__ __launch_bounds__(D_TPB, SPH_MINB) void k_density(
                                        [&](int f, uint32_t j, const float4 pj, float, float, float,
                                            float r2) {
                     if (f < D_SLOTS * D_G) {
-                        const int o = (f >> 3) * 32 + (f & (D_G - 1));
-                        gr[o]  = r2 * rsqrtf(fmaxf(r2, 1e-35f));
-                        gm_[o] = pj.w;
-                        gj[f]  = j;
+                        const uint32_t a = gb + 4u * f;
+                        sph_sts<0>(a, r2 * rsqrtf(fmaxf(r2, 1e-35f)));
+                        sph_sts<D_MOFF>(a, pj.w);
+                        sph_stg(gj + f, j);
                     }
                 });
                 __syncwarp();
@@ -188,15 +197,14 @@ __global__ __launch_bounds__(D_TPB, SPH_MINB) void k_density(
             float s = 0.0f, e = 0.0f, f2 = 0.0f;
             const int mycnt  = done ? 0 : (cnt - sl + D_G - 1) >> 3;   // entries sl, sl + 8, ...
             const int maxcnt = __reduce_max_sync(SPH_FULL, mycnt);
-            for (int k = 0; k < maxcnt; ++k) {
-                if (k < mycnt) {
-                    const float mj = lm[k * 32];
-                    float wq, eq, fq;
-                    SphKernel<KERN>::sums(lr[k * 32] * ih, wq, eq, fq);
-                    s  += mj * wq;
-                    e  += mj * eq;
-                    f2 += mj * fq;
-                }
+            uint32_t la = lb;
+            for (int k = 0; k < maxcnt; ++k, la += 4u * D_G) {
+                const float mj = (k < mycnt) ? sph_lds<D_MOFF>(la) : 0.0f;
+                float wq, eq, fq;
+                SphKernel<KERN>::sums(sph_lds<0>(la) * ih, wq, eq, fq);
+                s  += mj * wq;
+                e  += mj * eq;
+                f2 += mj * fq;
             }
             s  = sph_group_sum<D_G>(s);
             e  = sph_group_sum<D_G>(e);
@@ -235,28 +243,29 @@ __global__ __launch_bounds__(D_TPB, SPH_MINB) void k_density(
         {
             const int mycnt  = (tvalid && !fix) ? (cnt - sl + D_G - 1) >> 3 : 0;
             const int maxcnt = __reduce_max_sync(SPH_FULL, mycnt);
-            for (int k = 0; k < maxcnt; ++k) {
+            uint32_t la = lb;
+            for (int k = 0; k < maxcnt; ++k, la += 4u * D_G) {
                 const bool  valid = k < mycnt;
-                const float r = valid ? lr[k * 32] : 3.0e38f;
+                const float r = valid ? sph_lds<0>(la) : 3.0e38f;
                 ni += (r < H) ? 1 : 0;
                 edge |= fabsf(r - H) <= tauH;
                 const bool     keep = r < Rk;
                 const unsigned km = (__ballot_sync(SPH_FULL, keep) >> g0) & ((1u << D_G) - 1u);
                 uint32_t j = 0;
-                if (keep) j = gj[k * D_G + sl];
+                if (keep) j = sph_ldg_rw(gj + k * D_G + sl);
                 __syncwarp();   // all reads of this slot before any lane overwrites part of it
-                if (keep) gj[kept + __popc(km & ((1u << sl) - 1u))] = j;   // target <= source
+                if (keep) sph_stg(gj + kept + __popc(km & ((1u << sl) - 1u)), j);   // target <= source
                 kept += __popc(km);
             }
         }
         const bool recount = sph_group_any<D_G>(edge, lane) && !fix;   // h, rho, Omega stand
         ni = sph_group_sum_int<D_G>(ni);
-        if (tvalid && leader) c_listed += cnt;
         if (tvalid && leader) {
+            atomicAdd(&st_sh[1], (unsigned)cnt);
+            atomicAdd(&st_sh[3], (unsigned)sweeps);
             h_io[i] = h;   // final, or the best iterate for the fix kernel to start from
             nb_rkeep[p] = fix ? 0.0f : Rk;
             nb_cnt[p]   = kept;
-            c_sweeps += sweeps;
             if (!fix) {
                 const float ih = 1.0f / h;
                 rho[i]   = SphKernel<KERN>::sigma * S * ih * ih * ih;
@@ -265,17 +274,15 @@ __global__ __launch_bounds__(D_TPB, SPH_MINB) void k_density(
             }
             if (fix)          fix_list[atomicAdd(fix_cnt, 1u)] = p;
             else if (recount) fix_list[atomicAdd(fix_cnt, 1u)] = p | (int32_t)0x80000000;
-            else              c_pairs += ni;
+            else              atomicAdd(&st_sh[2], (unsigned)ni);
         }
         __syncwarp();
     }
 
     // ---- counters: lanes -> warp -> block -> one atomic per block and counter
-    unsigned v[5] = {c_tested, c_listed, c_pairs, c_sweeps, c_recollect};
-#pragma unroll
-    for (int k = 0; k < 5; ++k) {
-        const unsigned t = __reduce_add_sync(SPH_FULL, v[k]);
-        if (lane == 0 && t) atomicAdd(&st_sh[k], t);
+    {
+        const unsigned t = __reduce_add_sync(SPH_FULL, c_tested);
+        if (lane == 0 && t) atomicAdd(&st_sh[0], t);
     }
     __syncthreads();
     if (threadIdx.x < 5 && st_sh[threadIdx.x] != 0u)

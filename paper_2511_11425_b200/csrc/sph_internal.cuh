@@ -174,6 +174,33 @@ template <> struct SphKernel<3> {   // Wendland C6: w = y^8 (1 + 8x + 25x^2 + 32
     }
 };
 
+// Shared-memory accesses through a 32-bit shared-window address that lives in a register
+// (base + immediate): the hot list stores/loads cost one address add each instead of the
+// re-derivation from SR_TID / the CTA's shared base that the compiler otherwise emits.
+__device__ __forceinline__ uint32_t sph_smem_addr(const void* p) {
+    uint32_t a = (uint32_t)__cvta_generic_to_shared(p);
+    asm volatile("" : "+r"(a));
+    return a;
+}
+template <int OFF> __device__ __forceinline__ void sph_sts(uint32_t a, float v) {
+    asm volatile("st.shared.f32 [%0+%2], %1;" ::"r"(a), "f"(v), "n"(OFF));
+}
+// global accesses through a pointer that was pinned to a register pair (the pin hides the
+// address space from the compiler, which would otherwise emit generic accesses)
+__device__ __forceinline__ void sph_stg(uint32_t* p, uint32_t v) {
+    asm volatile("st.global.u32 [%0], %1;" ::"l"(p), "r"(v));
+}
+__device__ __forceinline__ uint32_t sph_ldg_rw(const uint32_t* p) {
+    uint32_t v;
+    asm volatile("ld.global.u32 %0, [%1];" : "=r"(v) : "l"(p));
+    return v;
+}
+template <int OFF> __device__ __forceinline__ float sph_lds(uint32_t a) {
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1+%2];" : "=f"(v) : "r"(a), "n"(OFF));
+    return v;
+}
+
 __device__ __forceinline__ int sph_fdiv(int u, int n) {   // floor(u / n), n > 0
     return (u >= 0) ? (u / n) : -((-u + n - 1) / n);
 }
@@ -326,8 +353,11 @@ __device__ __forceinline__ void sph_group_collect(const SphGrid& g,
                                                   int lane, unsigned& tested, int& total,
                                                   Accept&& accept, Store&& store) {
     constexpr unsigned GM = (G == 32) ? 0xffffffffu : ((1u << G) - 1u);
-    const int sl = lane & (G - 1);
-    const int g0 = lane & ~(G - 1);
+    int      sl = lane & (G - 1);
+    int      g0 = lane & ~(G - 1);
+    unsigned lt = (1u << sl) - 1u;   // the lanes of the group below this one
+    // kept in registers: without this the compiler re-derives them from SR_TID in every trip
+    asm volatile("" : "+r"(sl), "+r"(g0), "+r"(lt));
     int y0, y1, z0, z1;
     sph_axis_range(yi, R, g.lo[1], g.isy, g.ny, g.per[1], y0, y1);
     sph_axis_range(zi, R, g.lo[2], g.isz, g.nz, g.per[2], z0, z1);
@@ -402,8 +432,7 @@ __device__ __forceinline__ void sph_group_collect(const SphGrid& g,
                         const bool  acc = (c + u * G < re) && accept(pp[u], r2);
                         const unsigned gm = (__ballot_sync(SPH_FULL, acc) >> g0) & GM;
                         if (acc)
-                            store(total + __popc(gm & ((1u << sl) - 1u)), c + u * G, pp[u], dx, dy,
-                                  dz, r2);
+                            store(total + __popc(gm & lt), c + u * G, pp[u], dx, dy, dz, r2);
                         total += __popc(gm);
                     }
                     c += NW * G;
