@@ -166,6 +166,7 @@ __global__ __launch_bounds__(F_TPB, SPH_FMINB) void k_forces(
     const float iLx = g.per[0] ? 1.0f / g.len[0] : 0.0f, Lx = g.per[0] ? g.len[0] : 0.0f;
     const float iLy = g.per[1] ? 1.0f / g.len[1] : 0.0f, Ly = g.per[1] ? g.len[1] : 0.0f;
     const float iLz = g.per[2] ? 1.0f / g.len[2] : 0.0f, Lz = g.per[2] ? g.len[2] : 0.0f;
+    const bool  anyper = (g.per[0] | g.per[1] | g.per[2]) != 0;
 
     unsigned c_tested = 0, c_pairs = 0, c_av = 0;
 
@@ -238,9 +239,11 @@ __global__ __launch_bounds__(F_TPB, SPH_FMINB) void k_forces(
             }
             if (k < mycnt) {
                 float dx = t.pi.x - pj.x, dy = t.pi.y - pj.y, dz = t.pi.z - pj.z;
-                dx -= Lx * rintf(dx * iLx);   // minimum image (no-op on open axes)
-                dy -= Ly * rintf(dy * iLy);
-                dz -= Lz * rintf(dz * iLz);
+                if (anyper) {   // minimum image
+                    dx -= Lx * rintf(dx * iLx);
+                    dy -= Ly * rintf(dy * iLy);
+                    dz -= Lz * rintf(dz * iLz);
+                }
                 const float r2 = dx * dx + dy * dy + dz * dz;
                 // kept lists hold everything inside the kept radius: apply the pair test
                 if (r2 < fmaxf(hi2x4, 4.0f * pj.w * pj.w) && r2 > 0.0f)
