@@ -136,6 +136,28 @@ int  sph_timestep(sph_ctx* ctx, const float* h, const float* c, const float* ax,
  * SPH_ESTALE.  rung: n int32, caller order.                                                  */
 int  sph_rungs(sph_ctx* ctx, const float* dt_i, float dt0, int32_t max_rung, int32_t* rung);
 
+/* The active set of a rung, PAPER.md:229, 274 ("only the particles on the active rungs are
+ * updated").  active: n bytes in device memory, caller order, non-zero = active; NULL = all
+ * particles again.  Until the next sph_build_cells (which clears the set: it is held as a
+ * list of positions in the index) sph_density_h and sph_forces take their TARGETS from the
+ * set only -- the entries of their output arrays that belong to inactive particles are not
+ * touched -- while the sources remain all particles, whose input arrays (m, h, rho, ...)
+ * must therefore be valid for every particle.  The results for an active particle are the
+ * ones of the full sweep.  sph_timestep, sph_rungs and the other calls ignore the set.
+ * SPH_ESTALE before sph_build_cells.                                                       */
+int  sph_set_active(sph_ctx* ctx, const uint8_t* active);
+
+/* The FastGas marking pass: "mark all particles that would end up on
+ * interaction lists of active particles".  mark_i = 1 if src_i != 0 or if some particle j
+ * with src_j != 0 interacts with i (the force pair set 0 < r_ij < 2 max(h_i, h_j), with the
+ * h given to sph_build_cells or, once sph_forces has run on this index, the h given to it);
+ * else 0.  Borderline pairs are decided in FP64, so the marks are exact.  A second call with
+ * src = the first marks gives the paper's second marking pass.  src, mark: n bytes, device
+ * memory, caller order; they may not alias.  Only the particles of src walk their
+ * neighbourhood (the pair set is symmetric), so the cost follows the size of the set.
+ * SPH_ESTALE before sph_build_cells.                                                       */
+int  sph_mark_neighbors(sph_ctx* ctx, const uint8_t* src, uint8_t* mark);
+
 /* Interface correction for the ideal gas, PAPER.md:158-182 (Section 2.3.4), Eqs. (8)-(12);
  * call between sph_density_h and sph_forces and hand rho_corr to sph_forces.  Gather sums over
  * r_ij < 2 h_i, self included.

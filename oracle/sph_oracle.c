@@ -781,3 +781,24 @@ void orc_rung_limiter_brute(int64_t n, const double *x, const double *y, const d
         rung_out[t] = r;
     }
 }
+
+/* The FastGas marking pass: "we mark all particles that would end up on
+ * interaction lists of active particles".  mark_i = 1 if src_i, or if a particle j with
+ * src_j interacts with i: 0 < r_ij < 2 max(h_i, h_j) (the pair set of PAPER.md:191;
+ * DESIGN.md reading R29).  Brute force over all pairs. */
+void orc_mark_brute(int64_t n, const double *x, const double *y, const double *z,
+                    const double *h, const orc_box *box, const uint8_t *src, uint8_t *mark)
+{
+#pragma omp parallel for schedule(dynamic, 8)
+    for (int64_t i = 0; i < n; i++) {
+        uint8_t mk = src[i] ? 1 : 0;
+        double d[3];
+        for (int64_t j = 0; j < n && !mk; j++) {
+            if (j == i || !src[j]) continue;
+            double r2 = orc_r2(x, y, z, i, j, box, d);
+            double hh = h[j] > h[i] ? h[j] : h[i];
+            if (r2 > 0.0 && r2 < 4.0 * hh * hh) mk = 1;
+        }
+        mark[i] = mk;
+    }
+}

@@ -275,3 +275,16 @@ def rung_limiter(x, y, z, h, rung, box: Box, targets=None):
                                  _p(rin, C.c_int32), C.c_int64(nt), _p(t, C.c_int64),
                                  _p(out, C.c_int32))
     return out
+
+
+def mark_neighbors(x, y, z, h, src, box: Box):
+    """FastGas marking pass: src itself plus everything on the interaction
+    lists (force pair set) of the particles of src; brute force."""
+    x, y, z, h = map(_d, (x, y, z, h))
+    n = len(x)
+    b = box.c()
+    sin = np.ascontiguousarray(np.asarray(src) != 0, dtype=np.uint8)
+    out = np.empty(n, np.uint8)
+    lib().orc_mark_brute(C.c_int64(n), _p(x), _p(y), _p(z), _p(h), C.byref(b),
+                         _p(sin, C.c_uint8), _p(out, C.c_uint8))
+    return out

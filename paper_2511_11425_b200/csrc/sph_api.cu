@@ -72,6 +72,8 @@ extern "C" int sph_create(sph_ctx** out, const sph_params* params, const sph_box
     ok = ok && dalloc(&c->nb_rkeep, (size_t)n_max) == cudaSuccess;
     ok = ok && dalloc(&c->fix_list, (size_t)n_max) == cudaSuccess;
     ok = ok && dalloc(&c->fix_cnt, (size_t)2) == cudaSuccess;
+    ok = ok && dalloc(&c->act_list, (size_t)n_max) == cudaSuccess;
+    ok = ok && dalloc(&c->act_cnt, (size_t)2) == cudaSuccess;
     ok = ok && dalloc(&c->dt_part, (size_t)1024) == cudaSuccess;
     ok = ok && dalloc(&c->nb_total, (size_t)2) == cudaSuccess;
     if (ok) ok = cudaMemsetAsync(c->stats, 0, ST_NCOUNTERS * sizeof(unsigned long long),
@@ -96,6 +98,7 @@ extern "C" void sph_destroy(sph_ctx* c) {
     cudaFree(c->rcak);      cudaFree(c->stats);     cudaFree(c->dt_part);
     cudaFree(c->nb_total);  cudaFree(c->fix_list);  cudaFree(c->fix_cnt);
     cudaFree(c->coarse_hmax);
+    cudaFree(c->act_list);  cudaFree(c->act_cnt);
     cudaFree(c->nb_j);      cudaFree(c->nb_cnt);   cudaFree(c->nb_rkeep);
     delete c;
 }
@@ -112,6 +115,7 @@ extern "C" int sph_build_cells(sph_ctx* c, int64_t n, const float* x, const floa
     if (n <= 0 || n > c->n_max) return fail(c, SPH_EINVAL, "sph_build_cells: n out of range");
     c->built = false;
     c->forces_ready = false;
+    c->act_on = false;   // the active set is a list of sorted positions of the old index
     int rc = sph_launch_build(c, n, x, y, z, h);
     if (rc == SPH_OK) {
         c->n     = n;
@@ -151,6 +155,26 @@ extern "C" int sph_interface_correction(sph_ctx* c, const float* m, const float*
         return fail(c, SPH_EINVAL, "sph_interface_correction: bad argument");
     if (!c->built) return fail(c, SPH_ESTALE, "sph_interface_correction before sph_build_cells");
     return sph_launch_interface(c, m, u, rho, h, mat, alpha, imbalance, rho_corr, P_corr);
+}
+
+// sweeps over the active set of a rung, and the FastGas marking pass
+extern "C" int sph_set_active(sph_ctx* c, const uint8_t* active) {
+    if (!c) return SPH_EINVAL;
+    if (!c->built) return fail(c, SPH_ESTALE, "sph_set_active before sph_build_cells");
+    if (!active) {
+        c->act_on = false;
+        return SPH_OK;
+    }
+    const int rc = sph_launch_set_active(c, active);
+    c->act_on = (rc == SPH_OK);
+    return rc;
+}
+
+extern "C" int sph_mark_neighbors(sph_ctx* c, const uint8_t* src, uint8_t* mark) {
+    if (!c) return SPH_EINVAL;
+    if (!src || !mark) return fail(c, SPH_EINVAL, "sph_mark_neighbors: null array");
+    if (!c->built) return fail(c, SPH_ESTALE, "sph_mark_neighbors before sph_build_cells");
+    return sph_launch_mark(c, src, mark);
 }
 
 extern "C" int sph_rungs(sph_ctx* c, const float* dt_i, float dt0, int32_t max_rung, int32_t* rung) {

@@ -107,7 +107,11 @@ __global__ __launch_bounds__(D_TPB, SPH_MINB) void k_density(
     int n, const SphGrid* __restrict__ gp, const uint32_t* __restrict__ cell_start,
     const float4* __restrict__ pos_m, const int32_t* __restrict__ perm, DensPar par, float* h_io,
     float* rho, float* omega, int32_t* nn, int32_t* fix_list, unsigned* fix_cnt, uint32_t* nb_j,
-    uint32_t* nb_cnt, float* nb_rkeep, unsigned long long* stats) {
+    uint32_t* nb_cnt, float* nb_rkeep, const uint32_t* __restrict__ act_list,
+    const unsigned* __restrict__ act_cnt, unsigned long long* stats) {
+    // targets: all n sorted positions, or the act_cnt entries of act_list (the active set)
+    const int nt = act_list ? (int)*act_cnt : n;
+    if (blockIdx.x * D_TARGETS >= nt) return;
     __shared__ WarpList lists[D_WARPS];
     __shared__ SphGrid  g;
     __shared__ unsigned st_sh[5];
@@ -139,8 +143,9 @@ __global__ __launch_bounds__(D_TPB, SPH_MINB) void k_density(
         if (lane == 0) quad = atomicAdd(&next_quad, 1);
         quad = __shfl_sync(SPH_FULL, quad, 0);
         if (quad >= D_QUADS) break;
-        const int  p      = (blockIdx.x * D_QUADS + quad) * D_NT + gq;
-        const bool tvalid = p < n;
+        const int  idx    = (blockIdx.x * D_QUADS + quad) * D_NT + gq;
+        const bool tvalid = idx < nt;
+        const int  p      = (act_list && tvalid) ? (int)act_list[idx] : idx;
         float4 pi = make_float4(0.f, 0.f, 0.f, 1.f);
         int    i  = 0;
         float  h  = g.hmin;
@@ -416,7 +421,9 @@ int sph_launch_density(sph_ctx* c, const float* m, float* h, float* rho, float* 
         constexpr int KERN = decltype(tag)::value;
         k_density<KERN><<<nblk, D_TPB, 0, s>>>((int)n, c->grid, c->cell_start, c->pos_m, c->perm, par,
                                                h, rho, omega, nn, c->fix_list, c->fix_cnt, c->nb_j,
-                                               c->nb_cnt, c->nb_rkeep, c->stats);
+                                               c->nb_cnt, c->nb_rkeep,
+                                               c->act_on ? c->act_list : nullptr, c->act_cnt,
+                                               c->stats);
         k_density_fix<KERN><<<c->sm_count * 4, 256, 0, s>>>(c->grid, c->cell_start, c->pos_m, c->perm,
                                                             par, c->fix_list, c->fix_cnt, h, rho,
                                                             omega, nn, c->stats);

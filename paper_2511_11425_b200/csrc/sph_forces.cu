@@ -148,7 +148,11 @@ __global__ __launch_bounds__(F_TPB, SPH_FMINB) void k_forces(
     float* ay, float* az, float* dudt, float* mu_min, int32_t* fix_list, unsigned* fix_cnt,
     const unsigned* __restrict__ coarse, const uint32_t* __restrict__ nb_j,
     const uint32_t* __restrict__ nb_cnt, const float* __restrict__ nb_rkeep,
+    const uint32_t* __restrict__ act_list, const unsigned* __restrict__ act_cnt,
     unsigned long long* stats) {
+    // targets: all n sorted positions, or the act_cnt entries of act_list (the active set)
+    const int nt = act_list ? (int)*act_cnt : n;
+    if (blockIdx.x * F_TARGETS >= nt) return;
     __shared__ FWarpList lists[F_WARPS];
     __shared__ SphGrid   g;
     __shared__ unsigned  st_sh[3];
@@ -175,8 +179,9 @@ __global__ __launch_bounds__(F_TPB, SPH_FMINB) void k_forces(
         if (lane == 0) quad = atomicAdd(&next_quad, 1);
         quad = __shfl_sync(SPH_FULL, quad, 0);
         if (quad >= F_QUADS) break;
-        const int  p      = (blockIdx.x * F_QUADS + quad) * F_NT + gq;
-        const bool tvalid = p < n;
+        const int  idx    = (blockIdx.x * F_QUADS + quad) * F_NT + gq;
+        const bool tvalid = idx < nt;
+        const int  p      = (act_list && tvalid) ? (int)act_list[idx] : idx;
         Target t;
         t.pi = make_float4(0.f, 0.f, 0.f, 1.f);
         t.vi = t.pi;
@@ -350,6 +355,16 @@ __global__ __launch_bounds__(256) void k_forces_fix(
 
 }  // namespace
 
+// a6 alone: the coarse max-h map of the h held in pos_h.w (used by the marking pass)
+int sph_launch_coarse_map(sph_ctx* c) {
+    cudaStream_t  s = c->stream;
+    const int64_t n = c->n;
+    SPH_CUDA_CHECK(c, cudaMemsetAsync(c->coarse_hmax, 0, SPH_COARSE_MAX * sizeof(unsigned), s));
+    k_coarse_hmax<<<(int)((n + 255) / 256), 256, 0, s>>>(n, c->grid, c->pos_h, c->coarse_hmax);
+    SPH_CUDA_CHECK(c, cudaGetLastError());
+    return SPH_OK;
+}
+
 int sph_launch_forces(sph_ctx* c, const float* m, const float* vx, const float* vy,
                       const float* vz, const float* u, const float* rho, const float* h,
                       const float* omega, float* ax, float* ay, float* az, float* dudt,
@@ -373,7 +388,9 @@ int sph_launch_forces(sph_ctx* c, const float* m, const float* vx, const float* 
         k_forces<KERN><<<nblk, F_TPB, 0, s>>>((int)n, c->grid, c->cell_start, c->pos_h, c->vel_m,
                                               c->rcak, c->perm, par, ax, ay, az, dudt, mu_min,
                                               c->fix_list, c->fix_cnt + 1, c->coarse_hmax, c->nb_j,
-                                              c->nb_cnt, c->nb_rkeep, c->stats);
+                                              c->nb_cnt, c->nb_rkeep,
+                                              c->act_on ? c->act_list : nullptr, c->act_cnt,
+                                              c->stats);
         k_forces_fix<KERN><<<c->sm_count * 4, 256, 0, s>>>(c->grid, c->cell_start, c->pos_h, c->vel_m,
                                                            c->rcak, c->perm, par, c->fix_list,
                                                            c->fix_cnt + 1, ax, ay, az, dudt, mu_min,

@@ -69,6 +69,9 @@ struct sph_ctx {
     float*       nb_rkeep;     // n_max: radius inside which list + mask are complete (0: none)
     int32_t*     fix_list;     // n_max: sorted positions queued for the robust (fix) kernels
     unsigned*    fix_cnt;      // [2]: queue lengths (density, forces)
+    uint32_t*    act_list;     // n_max: sorted positions of the active set, ascending
+    unsigned*    act_cnt;      // [2]: its length; [1]: length of the marking pass's source list
+    bool         act_on;       // sph_set_active gave a mask since the last build
     float*       dt_part;      // per-block minima of the time-step reduction
     int64_t*     nb_total;     // neighbour-list total (device) + pinned mirror
     char         err[256];
@@ -584,6 +587,10 @@ int sph_launch_neighbors(sph_ctx* c, const float* h, int32_t mode, int64_t* offs
                          int32_t* indices, int64_t capacity, int64_t* needed);
 int sph_launch_fp32_peak(cudaStream_t s, float seconds, double* tflops);
 int sph_launch_rungs(sph_ctx* c, const float* dt_i, float dt0, int32_t max_rung, int32_t* rung);
+int sph_launch_coarse_map(sph_ctx* c);
+int sph_launch_mark(sph_ctx* c, const uint8_t* src, uint8_t* mark);
+int sph_launch_set_active(sph_ctx* c, const uint8_t* active);
+int sph_launch_compact(sph_ctx* c, const uint8_t* mask, uint32_t* list, unsigned* cnt);
 int sph_launch_interface(sph_ctx* c, const float* m, const float* u, const float* rho, const float* h,
                          const int32_t* mat, float alpha, float* imbalance, float* rho_corr,
                          float* P_corr);

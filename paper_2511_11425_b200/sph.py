@@ -19,7 +19,8 @@ SPH_OK, SPH_EINVAL, SPH_EBOX, SPH_ENOMEM, SPH_ECUDA, SPH_ESTALE, SPH_ENOSPC = 0,
 
 # every symbol include/sph.h declares (tests check the library exports exactly these)
 SYMBOLS = ["sph_create", "sph_destroy", "sph_build_cells", "sph_density_h", "sph_forces",
-           "sph_timestep", "sph_rungs", "sph_interface_correction", "sph_predict", "sph_kick", "sph_drift", "sph_neighbors", "sph_stats", "sph_stats_reset", "sph_permutation",
+           "sph_timestep", "sph_rungs", "sph_set_active", "sph_mark_neighbors",
+           "sph_interface_correction", "sph_predict", "sph_kick", "sph_drift", "sph_neighbors", "sph_stats", "sph_stats_reset", "sph_permutation",
            "sph_fp32_peak", "sph_strerror", "sph_last_error"]
 
 
@@ -206,6 +207,17 @@ class Sph:
         n = self.n
         self._check(self.lib.sph_rungs(self._ctx, _ptr(dt_i, torch.float32, n), float(dt0),
                                        int(max_rung), _ptr(rung, torch.int32, n)))
+
+    # ---- active set of a rung and the FastGas marking pass --------------
+    def set_active(self, active):
+        """active: uint8 tensor of n flags (caller order), or None for all particles."""
+        ptr = _ptr(active, torch.uint8, self.n) if active is not None else None
+        self._check(self.lib.sph_set_active(self._ctx, ptr))
+
+    def mark_neighbors(self, src, mark):
+        n = self.n
+        self._check(self.lib.sph_mark_neighbors(self._ctx, _ptr(src, torch.uint8, n),
+                                                _ptr(mark, torch.uint8, n)))
 
     # ---- interface correction (Eqs. 8-12) -------------------------------------------------
     def interface_correction(self, m, u, rho, h, mat, alpha, imbalance, rho_corr, P_corr=None):

@@ -497,3 +497,133 @@ def test_rungs_and_limiter_bit_exact(gu, which):
     ctx.build_cells(d["x"], d["y"], d["z"], h)
     with pytest.raises(sph.SphError):
         ctx.rungs(out["dt_i"], 0.01, 12, rung)
+
+
+# ------------------------------------------------------------------------------------------
+# Active-set sweeps and the FastGas marking pass
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("which", ["uniform_cube", "sod_tube"])
+def test_marking_pass_bit_exact(gu, which):
+    w = workloads.uniform_cube(h_start="warm") if which == "uniform_cube" else \
+        workloads.sod_tube(ncross=20, h_start="warm")
+    _, ob = gu.make_boxes(w)
+    n = int(w["n"])
+    d = gu.to_device(w)
+    ctx = gu.make_ctx(w)
+    rng = np.random.default_rng(5)
+    src = (rng.random(n) < 0.01).astype(np.uint8)
+    src_d = torch.from_numpy(src).cuda()
+    mark = torch.full((n,), 7, dtype=torch.uint8, device="cuda")
+    # (a) straight after the build: the h given to sph_build_cells decides
+    ctx.build_cells(d["x"], d["y"], d["z"], d["h"])
+    ctx.mark_neighbors(src_d, mark)
+    want = orc.mark_neighbors(w["x"], w["y"], w["z"], w["h"], src, ob)
+    got = mark.cpu().numpy()
+    assert np.array_equal(got, want), int((got != want).sum())
+    assert (want >= src).all() and want.sum() > 10 * src.sum()
+    # second marking pass: the neighbours of the marked
+    mark2 = torch.empty_like(mark)
+    ctx.mark_neighbors(mark, mark2)
+    want2 = orc.mark_neighbors(w["x"], w["y"], w["z"], w["h"], want, ob)
+    assert np.array_equal(mark2.cpu().numpy(), want2)
+    assert want2.sum() > want.sum()
+    # (b) after a full step on the same index: the solved h decides (kept lists in use)
+    from paper_2511_11425_b200 import sph
+    out = sph.StepBuffers(n)
+    h = d["h"].clone()
+    sph.step(ctx, d, out, h)
+    ctx.mark_neighbors(src_d, mark)
+    want = orc.mark_neighbors(w["x"], w["y"], w["z"], h.cpu().numpy(), src, ob)
+    assert np.array_equal(mark.cpu().numpy(), want)
+    # degenerate sets
+    ctx.mark_neighbors(torch.zeros(n, dtype=torch.uint8, device="cuda"), mark)
+    assert int(mark.sum().item()) == 0
+    ctx.mark_neighbors(torch.ones(n, dtype=torch.uint8, device="cuda"), mark)
+    assert int(mark.sum().item()) == n
+
+
+def test_active_set_sweeps_match_the_full_sweeps(gu, c1):
+    """Targets from the active set only; results identical to the full sweep's, the rest of
+    the output arrays untouched."""
+    w, d = c1["w"], c1["d"]
+    n = int(w["n"])
+    ctx = gu.make_ctx(w)
+    hf, rhof, omf, nnf = gu.run_density(ctx, d)
+    of = gu.run_forces(ctx, d, rhof, hf, omf)
+    rng = np.random.default_rng(9)
+    for frac in (0.1, 0.0, 1.0):
+        act = rng.random(n) < frac
+        act_d = torch.from_numpy(act.astype(np.uint8)).cuda()
+        a = torch.from_numpy(act).cuda()
+        ctx.build_cells(d["x"], d["y"], d["z"], d["h"])
+        ctx.set_active(act_d)
+        h = d["h"].clone()
+        rho = torch.full((n,), -1.0, device="cuda")
+        om = torch.full((n,), -2.0, device="cuda")
+        nn = torch.full((n,), -3, dtype=torch.int32, device="cuda")
+        ctx.density_h(d["m"], h, rho, om, nn)
+        assert torch.equal(h[a], hf[a]) and torch.equal(rho[a], rhof[a])
+        assert torch.equal(om[a], omf[a]) and torch.equal(nn[a], nnf[a])
+        assert torch.equal(h[~a], d["h"][~a])
+        assert (rho[~a] == -1.0).all() and (om[~a] == -2.0).all() and (nn[~a] == -3).all()
+        # forces on the active set: sources need valid rho, h, Omega everywhere
+        o = {k: torch.full((n,), 9.0, device="cuda") for k in ("ax", "ay", "az", "dudt", "mu_min")}
+        P = torch.empty(n, device="cuda")
+        cs = torch.empty(n, device="cuda")
+        ctx.forces(d["m"], d["vx"], d["vy"], d["vz"], d["u"], rhof, hf, omf, o["ax"], o["ay"],
+                   o["az"], o["dudt"], o["mu_min"], P, cs)
+        for k in o:
+            assert torch.equal(o[k][a], of[k][a]), k
+            assert (o[k][~a] == 9.0).all(), k
+        assert torch.equal(P, of["P"]) and torch.equal(cs, of["c"])   # EOS: every particle
+        # against the oracle as well
+        if frac == 0.1:
+            sel = np.flatnonzero(act)
+            assert _rel(gu.np64(rho)[sel], c1["rho"][sel]).max() <= TOL_H
+            assert np.array_equal(nn.cpu().numpy()[sel], orc.density_at_h(
+                w["x"], w["y"], w["z"], w["m"], h.cpu().numpy(), c1["ob"], c1["op"], targets=sel)[2])
+    # back to all particles, and the set does not survive a rebuild
+    ctx.set_active(None)
+    h2, rho2, _, _ = gu.run_density(ctx, d)
+    assert torch.equal(rho2, rhof)
+    ctx.set_active(torch.zeros(n, dtype=torch.uint8, device="cuda"))
+    h3, rho3, _, _ = gu.run_density(ctx, d)     # run_density rebuilds the index first
+    assert torch.equal(rho3, rhof)
+
+
+def test_fastgas_flow_on_a_small_active_set(gu, c1):
+    """mark the interaction partners of the active particles, update the density
+    of the marked only, then the forces of the active only -- equal to the full step there."""
+    w, d = c1["w"], c1["d"]
+    n = int(w["n"])
+    ctx = gu.make_ctx(w)
+    hf, rhof, omf, _ = gu.run_density(ctx, d)
+    of = gu.run_forces(ctx, d, rhof, hf, omf)
+    r = np.sqrt((w["x"] - 0.5) ** 2 + (w["y"] - 0.5) ** 2 + (w["z"] - 0.5) ** 2)
+    act = r < 0.12
+    act_d = torch.from_numpy(act.astype(np.uint8)).cuda()
+    mark = torch.empty(n, dtype=torch.uint8, device="cuda")
+    ctx.build_cells(d["x"], d["y"], d["z"], hf)            # last step's h
+    ctx.mark_neighbors(act_d, mark)
+    mk = mark.bool()
+    assert act.sum() < int(mk.sum().item()) < n // 2
+    ctx.set_active(mark)
+    nan = float("nan")
+    h = hf.clone()
+    rho = torch.full((n,), nan, device="cuda")
+    om = torch.full((n,), nan, device="cuda")
+    nn = torch.zeros(n, dtype=torch.int32, device="cuda")
+    ctx.density_h(d["m"], h, rho, om, nn)
+    assert torch.isnan(rho[~mk]).all() and not torch.isnan(rho[mk]).any()
+    assert _rel(gu.np64(rho[mk]), gu.np64(rhof[mk])).max() <= TOL_H
+    ctx.set_active(act_d)
+    o = gu.run_forces(ctx, d, rho, h, om)
+    a = torch.from_numpy(act).cuda()
+    sel = np.flatnonzero(act)
+    ref = orc.forces(w["x"], w["y"], w["z"], w["m"], w["vx"], w["vy"], w["vz"], w["u"],
+                     rhof.cpu().numpy(), hf.cpu().numpy(), omf.cpu().numpy(), c1["ob"], c1["op"],
+                     targets=sel)
+    ea, eu = gu.force_errors(o, ref, sel)
+    assert ea.max() <= TOL_F and eu.max() <= TOL_F, (ea.max(), eu.max())
+    for k in ("ax", "ay", "az", "dudt"):
+        assert not torch.isnan(o[k][a]).any()

@@ -615,3 +615,55 @@ def test_rung_limiter_on_a_line_of_particles():
     want2 = r0.copy(); want2[7:10] = 3; want2[11:14] = 3
     assert np.array_equal(r2, want2)
     assert np.array_equal(orc.rung_limiter(x, z, z, h, np.full(n, 4, np.int32), box), np.full(n, 4))
+
+
+# ------------------------------------------------------------------------------------------
+# The FastGas marking pass
+# ------------------------------------------------------------------------------------------
+def test_marking_pass_on_a_line_of_particles():
+    n = 21
+    x = np.arange(n) * 1.0; z = np.zeros(n)
+    h = np.full(n, 0.6)                                   # support 1.2: nearest neighbours only
+    box = orc.Box((-5, -5, -5), (40, 10, 10), (0, 0, 0))
+    src = np.zeros(n, np.uint8); src[10] = 1
+    want = src.copy(); want[9] = want[11] = 1
+    m1 = orc.mark_neighbors(x, z, z, h, src, box)
+    assert np.array_equal(m1, want)
+    m2 = orc.mark_neighbors(x, z, z, h, m1, box)          # the second marking pass
+    want2 = want.copy(); want2[8] = want2[12] = 1
+    assert np.array_equal(m2, want2)
+    # gather side: a wide source reaches three particles on each side ...
+    h2 = h.copy(); h2[10] = 1.6
+    w3 = src.copy(); w3[7:14] = 1
+    assert np.array_equal(orc.mark_neighbors(x, z, z, h2, src, box), w3)
+    # ... scatter side: a wide particle three places away is on the narrow source's list
+    h3 = h.copy(); h3[13] = 1.6
+    w4 = want.copy(); w4[13] = 1
+    assert np.array_equal(orc.mark_neighbors(x, z, z, h3, src, box), w4)
+    # through a periodic face only if the axis is periodic: x = 0 and x = 20 in a box of 21
+    e = np.zeros(n, np.uint8); e[0] = 1
+    per = orc.Box((-0.5, -5, -5), (21, 10, 10), (1, 0, 0))
+    opn = orc.Box((-0.5, -5, -5), (21, 10, 10), (0, 0, 0))
+    assert orc.mark_neighbors(x, z, z, h, e, per)[20] == 1
+    assert orc.mark_neighbors(x, z, z, h, e, opn)[20] == 0
+    # nothing and everything
+    assert orc.mark_neighbors(x, z, z, h, np.zeros(n), box).sum() == 0
+    assert orc.mark_neighbors(x, z, z, h, np.ones(n), box).sum() == n
+
+
+def test_marking_pass_is_the_union_of_the_pair_lists():
+    """On the jittered cube: marks == source set + the (separately pinned) force pair lists of
+    its members, and the marks grow with the source set."""
+    w = W.uniform_cube(h_start="warm")
+    box = orc.Box(w["box_lo"], w["box_len"], w["periodic"])
+    n = int(w["n"])
+    rng = np.random.default_rng(3)
+    src = (rng.random(n) < 0.02).astype(np.uint8)
+    got = orc.mark_neighbors(w["x"], w["y"], w["z"], w["h"], src, box)
+    off, idx = orc.neighbors(w["x"], w["y"], w["z"], w["h"], box, mode=1)
+    want = src.copy()
+    for i in np.flatnonzero(src):
+        want[idx[off[i]:off[i + 1]]] = 1
+    assert np.array_equal(got, want)
+    more = src.copy(); more[rng.integers(0, n, 30)] = 1
+    assert (orc.mark_neighbors(w["x"], w["y"], w["z"], w["h"], more, box) >= got).all()
