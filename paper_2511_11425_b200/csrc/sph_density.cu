@@ -242,25 +242,37 @@ __global__ __launch_bounds__(D_TPB, SPH_MINB) void k_density(
         }
         const float H = 2.0f * h, tauH = (wraps ? 1e-6f + band_c / h : 2e-6f) * H;
         const float Rk = fminf(Rc, H * D_KEEP);   // the kept list is complete inside Rk
-        // The same pass compacts the global index list in place to the entries inside Rk.
+        // A second pass compacts the global index list in place to the entries inside Rk --
+        // skipped when no list of the warp has an entry outside (then they are compact as
+        // they stand; always so on a lattice, where whole shells of neighbours enter together).
         int  ni = 0, kept = 0;
         bool edge = false;
         {
             const int mycnt  = (tvalid && !fix) ? (cnt - sl + D_G - 1) >> 3 : 0;
             const int maxcnt = __reduce_max_sync(SPH_FULL, mycnt);
             uint32_t la = lb;
+            int nk = 0;
             for (int k = 0; k < maxcnt; ++k, la += 4u * D_G) {
-                const bool  valid = k < mycnt;
-                const float r = valid ? sph_lds<0>(la) : 3.0e38f;
+                const float r = (k < mycnt) ? sph_lds<0>(la) : 3.0e38f;
                 ni += (r < H) ? 1 : 0;
+                nk += (r < Rk) ? 1 : 0;
                 edge |= fabsf(r - H) <= tauH;
-                const bool     keep = r < Rk;
-                const unsigned km = (__ballot_sync(SPH_FULL, keep) >> g0) & ((1u << D_G) - 1u);
-                uint32_t j = 0;
-                if (keep) j = sph_ldg_rw(gj + k * D_G + sl);
-                __syncwarp();   // all reads of this slot before any lane overwrites part of it
-                if (keep) sph_stg(gj + kept + __popc(km & ((1u << sl) - 1u)), j);   // target <= source
-                kept += __popc(km);
+            }
+            kept = sph_group_sum_int<D_G>(nk);
+            const bool full = !tvalid || fix || kept == cnt;
+            if (!__all_sync(SPH_FULL, full)) {
+                kept = 0;
+                la   = lb;
+                for (int k = 0; k < maxcnt; ++k, la += 4u * D_G) {
+                    const float    r = (k < mycnt) ? sph_lds<0>(la) : 3.0e38f;
+                    const bool     keep = r < Rk;
+                    const unsigned km = (__ballot_sync(SPH_FULL, keep) >> g0) & ((1u << D_G) - 1u);
+                    uint32_t j = 0;
+                    if (keep) j = sph_ldg_rw(gj + k * D_G + sl);
+                    __syncwarp();   // all reads of this slot before any lane overwrites part of it
+                    if (keep) sph_stg(gj + kept + __popc(km & ((1u << sl) - 1u)), j);   // target <= source
+                    kept += __popc(km);
+                }
             }
         }
         const bool recount = sph_group_any<D_G>(edge, lane) && !fix;   // h, rho, Omega stand
