@@ -65,8 +65,8 @@ struct sph_ctx {
     unsigned long long* stats; // ST_NCOUNTERS
     uint32_t*    nb_j;         // n_max x SPH_SLOTS x SPH_G: the density sweep's neighbour indices,
                                // [target][entry]; reused by the force sweep
-    uint32_t*    nb_cnt;       // n_max: entries of the kept list (those with r < nb_rkeep)
-    float*       nb_rkeep;     // n_max: radius inside which list + mask are complete (0: none)
+    uint32_t*    nb_cnt;       // n_max: entries of the kept list
+    float*       nb_rkeep;     // n_max: radius inside which the kept list is complete (0: none)
     int32_t*     fix_list;     // n_max: sorted positions queued for the robust (fix) kernels
     unsigned*    fix_cnt;      // [2]: queue lengths (density, forces)
     uint32_t*    act_list;     // n_max: sorted positions of the active set, ascending
@@ -188,15 +188,10 @@ __device__ __forceinline__ uint32_t sph_smem_addr(const void* p) {
 template <int OFF> __device__ __forceinline__ void sph_sts(uint32_t a, float v) {
     asm volatile("st.shared.f32 [%0+%2], %1;" ::"r"(a), "f"(v), "n"(OFF));
 }
-// global accesses through a pointer that was pinned to a register pair (the pin hides the
-// address space from the compiler, which would otherwise emit generic accesses)
+// global store through a pointer that was pinned to a register pair (the pin hides the
+// address space from the compiler, which would otherwise emit a generic store)
 __device__ __forceinline__ void sph_stg(uint32_t* p, uint32_t v) {
     asm volatile("st.global.u32 [%0], %1;" ::"l"(p), "r"(v));
-}
-__device__ __forceinline__ uint32_t sph_ldg_rw(const uint32_t* p) {
-    uint32_t v;
-    asm volatile("ld.global.u32 %0, [%1];" : "=r"(v) : "l"(p));
-    return v;
 }
 template <int OFF> __device__ __forceinline__ float sph_lds(uint32_t a) {
     float v;
