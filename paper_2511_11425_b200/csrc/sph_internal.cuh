@@ -341,7 +341,7 @@ __device__ __forceinline__ int sph_wrap(int u, int n, int& k) {   // u = c + k n
 // called on the lane that tested number f.  Keeping entry f in slot f / G of lane f % G
 // gives every lane of the group an equally long column AND makes the G lanes work on G
 // consecutive -- mostly memory-adjacent -- sources later.  `total` (uniform in a group) is
-// advanced by the number accepted, `tested` by the number of candidates (first lane only).
+// advanced by the number accepted, `tested` by the number of candidates (summed over the lanes).
 // `active` (uniform in a group) switches a group off.
 template <int G, class Accept, class Store>
 __device__ __forceinline__ void sph_group_collect(const SphGrid& g,
@@ -404,6 +404,7 @@ __device__ __forceinline__ void sph_group_collect(const SphGrid& g,
             const float    sxs = seg ? sxa - g.len[0] : sxa;
             unsigned gm = (__ballot_sync(SPH_FULL, s1 > s0) >> g0) & GM;
             const int nk = __reduce_max_sync(SPH_FULL, __popc(gm));
+            if (s1 > s0) tested += s1 - s0;   // every candidate of this lane's row gets tested
             for (int k = 0; k < nk; ++k) {
                 const bool have = gm != 0u;
                 const int  src  = g0 + (have ? (__ffs(gm) - 1) : 0);
@@ -415,7 +416,6 @@ __device__ __forceinline__ void sph_group_collect(const SphGrid& g,
                 const float    rsz = __shfl_sync(SPH_FULL, sz, src);
                 if (!have) re = rs;
                 uint32_t c = rs + sl;
-                if (sl == 0) tested += re - rs;
                 // NW windows of G candidates per trip, loaded unconditionally (the sorted arrays
                 // are padded by SPH_POS_PAD records, so reading past a row's end is harmless)
                 auto trip = [&](auto nw_tag) {
