@@ -230,30 +230,37 @@ __global__ __launch_bounds__(F_TPB, SPH_FMINB) void k_forces(
         const int stride = covered ? F_G : 32;
         const int mycnt  = ovf ? 0 : (cnt - sl + F_G - 1) >> 3;
         const int maxcnt = __reduce_max_sync(SPH_FULL, mycnt);
-        // software-pipelined: the records of entry k+1 are in flight while entry k is worked on
-        float4 pn = t.pi, vn = t.vi, rn = ri;
-        if (mycnt > 0) {
-            const uint32_t j = src[0];
-            pn = __ldg(pos_h + j); vn = __ldg(vel_m + j); rn = __ldg(rcak + j);
-        }
-        for (int k = 0; k < maxcnt; ++k) {
-            const float4 pj = pn, vj = vn, rj = rn;
-            if (k + 1 < mycnt) {
-                const uint32_t j = src[(k + 1) * stride];
-                pn = __ldg(pos_h + j); vn = __ldg(vel_m + j); rn = __ldg(rcak + j);
+        // software-pipelined: the records of entry k+1 are in flight while entry k is worked on.
+        // Two record sets used in turn, two entries per trip (no register copies); the loads are
+        // unconditional -- past its last entry a lane re-reads that entry (an L1 hit) and a lane
+        // without entries reads the target's own record -- so the loop body has no branch
+        // around them.
+        const uint32_t jself = (uint32_t)(tvalid ? p : 0);
+        const int      klast = mycnt - 1;
+        auto fetch = [&](int k, float4& pj, float4& vj, float4& rj) {
+            uint32_t j = jself;
+            if (klast >= 0) j = src[min(k, klast) * stride];
+            pj = __ldg(pos_h + j); vj = __ldg(vel_m + j); rj = __ldg(rcak + j);
+        };
+        auto work = [&](int k, const float4& pj, const float4& vj, const float4& rj) {
+            float dx = t.pi.x - pj.x, dy = t.pi.y - pj.y, dz = t.pi.z - pj.z;
+            if (anyper) {   // minimum image
+                dx -= Lx * rintf(dx * iLx);
+                dy -= Ly * rintf(dy * iLy);
+                dz -= Lz * rintf(dz * iLz);
             }
-            if (k < mycnt) {
-                float dx = t.pi.x - pj.x, dy = t.pi.y - pj.y, dz = t.pi.z - pj.z;
-                if (anyper) {   // minimum image
-                    dx -= Lx * rintf(dx * iLx);
-                    dy -= Ly * rintf(dy * iLy);
-                    dz -= Lz * rintf(dz * iLz);
-                }
-                const float r2 = dx * dx + dy * dy + dz * dz;
-                // kept lists hold everything inside the kept radius: apply the pair test
-                if (r2 < fmaxf(hi2x4, 4.0f * pj.w * pj.w) && r2 > 0.0f)
-                    force_pair<KERN>(t, a, par, vj, rj, dx, dy, dz, r2, pj.w);
-            }
+            const float r2 = dx * dx + dy * dy + dz * dz;
+            // kept lists hold everything inside the kept radius: apply the pair test
+            if (k < mycnt && r2 < fmaxf(hi2x4, 4.0f * pj.w * pj.w) && r2 > 0.0f)
+                force_pair<KERN>(t, a, par, vj, rj, dx, dy, dz, r2, pj.w);
+        };
+        float4 pA, vA, rA, pB, vB, rB;
+        fetch(0, pA, vA, rA);
+        for (int k = 0; k < maxcnt; k += 2) {
+            fetch(k + 1, pB, vB, rB);
+            work(k, pA, vA, rA);
+            fetch(k + 2, pA, vA, rA);
+            work(k + 1, pB, vB, rB);
         }
         a.ax = sph_group_sum<F_G>(a.ax);
         a.ay = sph_group_sum<F_G>(a.ay);
