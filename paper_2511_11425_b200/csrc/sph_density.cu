@@ -186,7 +186,7 @@ __global__ __launch_bounds__(D_TPB, SPH_MINB) void k_density(
                                            float r2) {
                     if (f < D_SLOTS * D_G) {
                         const uint32_t a = gb + 4u * f;
-                        sph_sts<0>(a, r2 * rsqrtf(fmaxf(r2, 1e-35f)));
+                        sph_sts<0>(a, sph_sqrt(r2));
                         sph_sts<D_MOFF>(a, pj.w);
                         sph_stg(gj + f, j);
                     }

@@ -115,7 +115,7 @@ template <int KERN>
 __device__ __forceinline__ void force_pair(const Target& t, Accum& a, const ForcePar& par,
                                            const float4 vj, const float4 rj, float dx,
                                            float dy, float dz, float r2, float hj) {
-    const float r  = r2 * rsqrtf(r2);
+    const float r  = sph_sqrt(r2);
     const float gi = t.K * SphKernel<KERN>::g(r * t.ih);
     const float gj = rj.w * SphKernel<KERN>::g(__fdividef(r, hj));
     const float vdx = t.vi.x - vj.x, vdy = t.vi.y - vj.y, vdz = t.vi.z - vj.z;

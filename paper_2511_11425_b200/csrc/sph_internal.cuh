@@ -185,6 +185,12 @@ __device__ __forceinline__ uint32_t sph_smem_addr(const void* p) {
     asm volatile("" : "+r"(a));
     return a;
 }
+// sqrt.approx: one MUFU.SQRT, relative error 2^-23, sqrt(0) = 0
+__device__ __forceinline__ float sph_sqrt(float x) {
+    float y;
+    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
 template <int OFF> __device__ __forceinline__ void sph_sts(uint32_t a, float v) {
     asm volatile("st.shared.f32 [%0+%2], %1;" ::"r"(a), "f"(v), "n"(OFF));
 }
