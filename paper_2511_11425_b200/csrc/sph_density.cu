@@ -205,13 +205,13 @@ __global__ __launch_bounds__(D_TPB, SPH_MINB) void k_density(
             for (int k = 0; k < maxcnt; ++k, la += 4u * D_G) {
                 const float mj = (k < mycnt) ? sph_lds<D_MOFF>(la) : 0.0f;
                 float wq, eq, fq;
-                SphKernel<KERN>::sums(sph_lds<0>(la) * ih, wq, eq, fq);
+                SphKernel<KERN>::sums_s(sph_lds<0>(la) * ih, wq, eq, fq);
                 s  += mj * wq;
                 e  += mj * eq;
                 f2 += mj * fq;
             }
             s  = sph_group_sum<D_G>(s);
-            e  = sph_group_sum<D_G>(e);
+            e  = SphKernel<KERN>::escale * sph_group_sum<D_G>(e);
             f2 = sph_group_sum<D_G>(f2);
             if (done) continue;
             ++sweeps;
