@@ -116,8 +116,8 @@ __device__ __forceinline__ void force_pair(const Target& t, Accum& a, const Forc
                                            const float4 vj, const float4 rj, float dx,
                                            float dy, float dz, float r2, float hj) {
     const float r  = sph_sqrt(r2);
-    const float gi = t.K * SphKernel<KERN>::g(r * t.ih);
-    const float gj = rj.w * SphKernel<KERN>::g(__fdividef(r, hj));
+    const float gi = t.K * SphKernel<KERN>::g_s(r * t.ih);   // K carries gscale
+    const float gj = rj.w * SphKernel<KERN>::g_s(__fdividef(r, hj));
     const float vdx = t.vi.x - vj.x, vdy = t.vi.y - vj.y, vdz = t.vi.z - vj.z;
     const float vr = vdx * dx + vdy * dy + vdz * dz;   // v_ij . r_ij
     float pig = 0.0f;                                   // Pi_ij * gbar
@@ -378,8 +378,11 @@ int sph_launch_forces(sph_ctx* c, const float* m, const float* vx, const float* 
                       float* mu_min, float* P, float* cs) {
     cudaStream_t  s = c->stream;
     const int64_t n = c->n;
-    static const float sigmas[4] = {SphKernel<0>::sigma, SphKernel<1>::sigma, SphKernel<2>::sigma,
-                                    SphKernel<3>::sigma};
+    // K = gscale sigma / h^5: dW/dr = -K g_s(q) r
+    static const float sigmas[4] = {SphKernel<0>::sigma * SphKernel<0>::gscale,
+                                    SphKernel<1>::sigma * SphKernel<1>::gscale,
+                                    SphKernel<2>::sigma * SphKernel<2>::gscale,
+                                    SphKernel<3>::sigma * SphKernel<3>::gscale};
     const float sigma = sigmas[(c->par.kernel >= 0 && c->par.kernel <= 3) ? c->par.kernel : 1];
     k_zero_hmax<<<1, 1, 0, s>>>(c->grid);
     SPH_CUDA_CHECK(c, cudaMemsetAsync(c->fix_cnt + 1, 0, sizeof(unsigned), s));

@@ -60,7 +60,7 @@ struct sph_ctx {
     float4*      pos_h;        // sorted (x, y, z, h)
     float4*      pos_m;        // sorted (x, y, z, m)
     float4*      vel_m;        // sorted (vx, vy, vz, m)
-    float4*      rcak;         // sorted (rho, c, A = P/(Omega rho^2), K = 5 sigma / h^5)
+    float4*      rcak;         // sorted (rho, c, A = P/(Omega rho^2), K = gscale sigma / h^5)
     unsigned*    coarse_hmax;  // SPH_COARSE_MAX: max h (float bits) per coarse cell, step a6
     unsigned long long* stats; // ST_NCOUNTERS
     uint32_t*    nb_j;         // n_max x SPH_SLOTS x SPH_G: the density sweep's neighbour indices,
@@ -109,8 +109,11 @@ struct sph_ctx {
 template <int KERN> struct SphKernel;
 // sums_s / escale: the same sums with a constant factor of e left out of the loop,
 // E = escale * sum m e_s (only Wendland C2 has a cheaper form; the others pass through)
+// g_s / gscale: g(q) = gscale * g_s(q); the force sweep folds gscale into K = gscale sigma / h^5.
 template <class K> struct SphKernelPlain {
     static constexpr float escale = 1.0f;
+    static constexpr float gscale = 1.0f;
+    static __device__ __forceinline__ float g_s(float q) { return K::g(q); }
     static __device__ __forceinline__ void sums_s(float q, float& w, float& e, float& f) {
         K::sums(q, w, e, f);
     }
@@ -143,6 +146,11 @@ template <> struct SphKernel<1> {   // Wendland C2: w = y^4 (1 + 4x)
     }
     // 15 instead of 18 FP instructions per entry: a = q^2 t^2 shared, e_s = a t (factor 5
     // outside), and 10 t - 7.5 q = 10 - 12.5 q wherever t > 0 (a = 0 elsewhere)
+    static constexpr float gscale = 5.0f;
+    static __device__ __forceinline__ float g_s(float q) {
+        const float t = fmaxf(1.0f - 0.5f * q, 0.0f);
+        return t * t * t;
+    }
     static constexpr float escale = 5.0f;
     static __device__ __forceinline__ void sums_s(float q, float& w, float& e, float& f) {
         const float t = fmaxf(1.0f - 0.5f * q, 0.0f), t2 = t * t, a = (q * q) * t2;
