@@ -51,7 +51,7 @@ def parse():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--nside", type=int, default=int(os.environ.get("BENCH_NSIDE", "128")))
-    ap.add_argument("--ref-nside", type=int, default=64,
+    ap.add_argument("--ref-nside", type=int, default=96,
                     help="lattice side of the bounded sample the CPU oracle is timed on")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--slack", type=float, default=0.0, help="sph_params.search_slack (0: default)")
