@@ -44,6 +44,11 @@ NCU_DRAM_BYTES = {"density_h": 158.3e6 + 775.0e6, "forces": 941.5e6 + 43.4e6}
 NCU_EXECUTED_FP32_FRAC = {"density_h": (906.9 + 1490.3 + 2 * 1102.2) / (148 * 128 * 2),
                           "forces": (798.3 + 2018.8 + 2 * 1523.5) / (148 * 128 * 2)}
 
+def workloads_names():
+    from paper_2511_11425_b200 import workloads
+    return workloads.CONFIGS.keys()
+
+
 def parse():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -54,6 +59,9 @@ def parse():
     ap.add_argument("--ref-nside", type=int, default=96,
                     help="lattice side of the bounded sample the CPU oracle is timed on")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--workload", default="sedov", choices=sorted(workloads_names()),
+                    help="sedov (BASELINE.json's metric configuration, the default) or another of "
+                         "the five configurations at its full size, for the per-configuration table")
     ap.add_argument("--slack", type=float, default=0.0, help="sph_params.search_slack (0: default)")
     ap.add_argument("--cell-div-x", type=float, default=0.0, help="sph_params.cell_div_x (0: default)")
     ap.add_argument("--cell-div-yz", type=float, default=0.0, help="sph_params.cell_div_yz (0: default)")
@@ -184,7 +192,12 @@ def run_gpu(a):
         torch.cuda.synchronize()
 
     # ---- synthetic input (seeded; every rank its own replica of the same workload) --------
-    w = workloads.sedov(nside=a.nside, v_sigma=a.v_sigma, h_start="warm")
+    if a.workload == "sedov":
+        w = workloads.sedov(nside=a.nside, v_sigma=a.v_sigma, h_start="warm")
+        wname = f"sedov_{a.nside}^3" + ("_v" if a.v_sigma > 0 else "")
+    else:
+        w = workloads.make(a.workload, h_start="warm")
+        wname = a.workload
     n = int(w["n"])
     keys = ("x", "y", "z", "m", "vx", "vy", "vz", "u", "h")
     host = {k: torch.from_numpy(w[k]).pin_memory() for k in keys}
@@ -309,7 +322,7 @@ def run_gpu(a):
         metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=K, warmup=max(a.warmup, 3),
         ms_per_step=float(step_ms.mean()), higher_is_better=True, scaling="weak",
         vs_baseline=None, dtype="f32", data="synthetic",
-        config=dict(workload=f"sedov_{a.nside}^3" + ("_v" if a.v_sigma > 0 else ""),
+        config=dict(workload=wname,
                     n_particles=n, kernel="wendland_c2", n_ngb=64, h_start="warm +-2%",
                     l2_flush="256 MiB device write between timed steps, outside the events; "
                              "working set ~320 MB > L2",
@@ -323,13 +336,13 @@ def run_gpu(a):
         newton_sweeps_per_particle=sweeps, grid_dims=st["grid_dims"],
         roofline=dict(bound="alu", kernel=names[dom], achieved=ach, peak=NOMINAL_FP32_TFLOPS,
                       unit="TFLOP/s", frac=ach / NOMINAL_FP32_TFLOPS,
-                      traffic=(NCU_DRAM_BYTES.get(names[dom]) if a.nside == 128 else None),
+                      traffic=(NCU_DRAM_BYTES.get(names[dom]) if wname == "sedov_128^3" else None),
                       traffic_source="profiles/r1f_density_forces.md (ncu --set full, bytes per launch)",
                       peak_source="derived: 148 SM x 128 FP32 lanes x 2 x 1.965 GHz",
                       measured_fma_peak=fma_peak, frac_of_measured_fma=ach / fma_peak,
                       useful_frac=ach / NOMINAL_FP32_TFLOPS,
                       executed_fp32_frac=(NCU_EXECUTED_FP32_FRAC.get(names[dom])
-                                          if a.nside == 128 else None),
+                                          if wname == "sedov_128^3" else None),
                       algorithmic_flops_per_launch=dom_flops,
                       step_frac=(f_dens + f_force) / (float(step_ms.mean()) * 1e-3) / 1e12 /
                                 NOMINAL_FP32_TFLOPS),
