@@ -31,7 +31,7 @@ if ROOT not in sys.path:
 METRIC = "particle-neighbour interactions/sec per density+force step"
 UNIT = "interactions/s"
 NOMINAL_FP32_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12   # SMs x FP32 lanes x 2 (FMA) x max clock
-KERNELS_PER_STEP = 11 + 3 + 5 + 2   # build_cells, density_h, forces, timestep kernel launches
+KERNELS_PER_STEP = 11 + 3 + 6 + 2   # build_cells, density_h, forces, timestep kernel launches
 # algorithmic FLOPs: per accepted density pair and Newton
 # sweep 27; per force pair 50 (AV branch not taken) or 70 (taken)
 FLOP_DENS, FLOP_FORCE, FLOP_FORCE_AV = 27.0, 50.0, 70.0

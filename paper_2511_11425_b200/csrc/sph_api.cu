@@ -66,7 +66,7 @@ extern "C" int sph_create(sph_ctx** out, const sph_params* params, const sph_box
     ok = ok && dalloc(&c->vel_m, (size_t)n_max) == cudaSuccess;
     ok = ok && dalloc(&c->rcak, (size_t)n_max) == cudaSuccess;
     ok = ok && dalloc(&c->stats, (size_t)ST_NCOUNTERS) == cudaSuccess;
-    ok = ok && dalloc(&c->coarse_hmax, (size_t)SPH_COARSE_MAX) == cudaSuccess;
+    ok = ok && dalloc(&c->coarse_hmax, (size_t)2 * SPH_COARSE_MAX) == cudaSuccess;
     ok = ok && dalloc(&c->nb_j, (size_t)n_max * SPH_SLOTS * SPH_G) == cudaSuccess;
     ok = ok && dalloc(&c->nb_cnt, (size_t)n_max) == cudaSuccess;
     ok = ok && dalloc(&c->nb_rkeep, (size_t)n_max) == cudaSuccess;

@@ -107,6 +107,7 @@ __global__ void k_grid_setup(SphGrid* g, const unsigned* red, sph_box box, float
         cs *= (float)fmax(cbrt(prod / (double)SPH_COARSE_MAX) * 1.02, 1.05);
     }
     for (int d = 0; d < 3; ++d) g->ics[d] = (float)g->cn[d] / box.len[d];
+    for (int d = 0; d < 3; ++d) g->sn[d] = (g->cn[d] + 7) >> 3;
 }
 
 __global__ void k_zero_cells(const SphGrid* __restrict__ g, uint32_t* cnt) {

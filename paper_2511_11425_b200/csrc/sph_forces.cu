@@ -98,6 +98,24 @@ __global__ void k_coarse_hmax(int64_t n, const SphGrid* __restrict__ g,
     }
 }
 
+// second level of the map: one warp per block of 8 x 8 x 8 coarse cells, written behind the
+// first level (the float bits of positive h order like the floats)
+__global__ void k_coarse_blocks(const SphGrid* __restrict__ g, unsigned* coarse) {
+    const int lane = threadIdx.x & 31, nwarp = (int)((gridDim.x * blockDim.x) >> 5);
+    const int nb = g->sn[0] * g->sn[1] * g->sn[2];
+    for (int w = (int)((blockIdx.x * blockDim.x + threadIdx.x) >> 5); w < nb; w += nwarp) {
+        const int bx = w % g->sn[0], t = w / g->sn[0], by = t % g->sn[1], bz = t / g->sn[1];
+        unsigned  mx = 0u;
+        for (int q = lane; q < 512; q += 32) {
+            const int cx = bx * 8 + (q & 7), cy = by * 8 + ((q >> 3) & 7), cz = bz * 8 + (q >> 6);
+            if (cx < g->cn[0] && cy < g->cn[1] && cz < g->cn[2])
+                mx = max(mx, coarse[(cz * g->cn[1] + cy) * g->cn[0] + cx]);
+        }
+        mx = __reduce_max_sync(SPH_FULL, mx);
+        if (lane == 0) coarse[SPH_COARSE_MAX + w] = mx;
+    }
+}
+
 __global__ void k_zero_hmax(SphGrid* g) { g->force_hmax_bits = 0u; }
 
 // Per-target constants and accumulators of the pair sum.
@@ -368,6 +386,7 @@ int sph_launch_coarse_map(sph_ctx* c) {
     const int64_t n = c->n;
     SPH_CUDA_CHECK(c, cudaMemsetAsync(c->coarse_hmax, 0, SPH_COARSE_MAX * sizeof(unsigned), s));
     k_coarse_hmax<<<(int)((n + 255) / 256), 256, 0, s>>>(n, c->grid, c->pos_h, c->coarse_hmax);
+    k_coarse_blocks<<<c->sm_count, 256, 0, s>>>(c->grid, c->coarse_hmax);
     SPH_CUDA_CHECK(c, cudaGetLastError());
     return SPH_OK;
 }
@@ -391,6 +410,7 @@ int sph_launch_forces(sph_ctx* c, const float* m, const float* vx, const float* 
                                                         rho, h, omega, c->par.gamma, sigma, c->pos_h,
                                                         c->vel_m, c->rcak, P, cs, c->grid);
     k_coarse_hmax<<<(int)((n + 255) / 256), 256, 0, s>>>(n, c->grid, c->pos_h, c->coarse_hmax);
+    k_coarse_blocks<<<c->sm_count, 256, 0, s>>>(c->grid, c->coarse_hmax);
     ForcePar par{c->par.av_alpha, c->par.av_beta, c->par.av_eps};
     const int nblk = (int)((n + F_TARGETS - 1) / F_TARGETS);
     auto launch = [&](auto tag) {

@@ -26,8 +26,10 @@ struct SphGrid {
     unsigned force_hmax_bits;  // max h given to sph_forces (float bits, atomicMax)
     int   cn[3];               // coarse grid (max-h map for the scatter reach of the force search)
     float ics[3];              // inverse coarse cell sides
+    int   sn[3];               // second level of the map: blocks of 8 x 8 x 8 coarse cells
 };
-#define SPH_COARSE_MAX (1 << 18)   // entries of the coarse max-h map
+#define SPH_COARSE_MAX (1 << 18)   // entries of the coarse max-h map (the second level, of
+                                   // at most as many, follows it in the same allocation)
 #define SPH_POS_PAD 64             // records of padding behind the sorted float4 arrays
 #define SPH_G 8                    // lanes per target in the sweeps
 #define SPH_SLOTS 24               // list entries per lane (24 x 8 = 192 per target)
@@ -482,8 +484,14 @@ __device__ __forceinline__ void sph_group_collect(const SphGrid& g,
 
 // Step a6: the largest h_j of any particle that can reach (x, y, z), i.e. with
 // |x - x_j| < 2 h_j, bounded from the coarse max-h map.  Starts from the
-// global maximum and tightens twice: every such j lies within 2 H of the target as long as H
-// bounds its h_j, so the maximum over the coarse cells meeting that ball is again a bound.
+// global maximum and tightens two or three times: every such j lies within 2 H of the target as long
+// as H bounds its h_j, so the maximum over the coarse cells meeting that ball is again a bound.
+// The map has two levels (coarse cells, and blocks of 8^3 of them behind SPH_COARSE_MAX): a
+// pass whose ball meets more than SPH_HMAP_CELLS coarse cells reads the blocks instead, so a
+// target with a very large h -- or the first pass, from the global maximum, under a deep h
+// contrast -- costs tens of loads, not tens of thousands.  (A ball that crosses a periodic
+// face always reads the first level.)
+#define SPH_HMAP_CELLS 64
 template <int G>
 __device__ __forceinline__ float sph_scatter_hmax(const SphGrid& g,
                                                   const unsigned* __restrict__ coarse, float xi,
@@ -492,9 +500,11 @@ __device__ __forceinline__ float sph_scatter_hmax(const SphGrid& g,
     const int sl = lane & (G - 1);
     float H = fmaxf(hglobal, hi);
     const float xs[3] = {xi, yi, zi};
+    int npass = 2;        // one more if the first one had to read the blocks (warp-uniform)
 #pragma unroll 1
-    for (int pass = 0; pass < 2; ++pass) {
-        int u0[3], nn[3];
+    for (int pass = 0; pass < npass; ++pass) {
+        int  u0[3], nn[3];
+        bool inside = true;   // the ball stays clear of the periodic faces
 #pragma unroll
         for (int d = 0; d < 3; ++d) {
             const float R = 2.0f * H * (1.0f + 1e-5f);
@@ -504,6 +514,7 @@ __device__ __forceinline__ float sph_scatter_hmax(const SphGrid& g,
             b = fminf(fmaxf(b, -1.0e9f), 1.0e9f);
             int lo = (int)a, hi_ = (int)b;
             if (g.per[d]) {
+                inside = inside && lo >= 0 && hi_ <= g.cn[d] - 1;
                 if (hi_ - lo + 1 >= g.cn[d]) { lo = 0; hi_ = g.cn[d] - 1; }
             } else {
                 lo  = min(max(lo, 0), g.cn[d] - 1);
@@ -512,25 +523,45 @@ __device__ __forceinline__ float sph_scatter_hmax(const SphGrid& g,
             u0[d] = lo;
             nn[d] = hi_ - lo + 1;
         }
-        const int   cnt  = nn[0] * nn[1] * nn[2];
-        const int   cmax = __reduce_max_sync(SPH_FULL, cnt);
-        const float i0 = __fdividef(1.0f, (float)nn[0]), i1 = __fdividef(1.0f, (float)nn[1]);
+        // second level: the blocks that hold the cells [u0, u0 + nn)
+        const bool blocks = inside && nn[0] * nn[1] * nn[2] > SPH_HMAP_CELLS;
+        const bool anyblk = __any_sync(SPH_FULL, blocks);
+        if (pass == 0 && anyblk) npass = 3;
         unsigned best = 0u;
-        for (int q = sl; q < cmax; q += G) {
-            if (q < cnt) {
-                const int t  = (int)(((float)q + 0.5f) * i0);          // q / nn[0]
-                const int ix = q - t * nn[0];
-                const int iz = (int)(((float)t + 0.5f) * i1);          // t / nn[1]
-                const int iy = t - iz * nn[1];
-                int cx = u0[0] + ix, cy = u0[1] + iy, cz = u0[2] + iz;
-                cx -= (cx >= g.cn[0]) ? g.cn[0] : 0; cx += (cx < 0) ? g.cn[0] : 0;
-                cy -= (cy >= g.cn[1]) ? g.cn[1] : 0; cy += (cy < 0) ? g.cn[1] : 0;
-                cz -= (cz >= g.cn[2]) ? g.cn[2] : 0; cz += (cz < 0) ? g.cn[2] : 0;
-                cx = min(max(cx, 0), g.cn[0] - 1);
-                cy = min(max(cy, 0), g.cn[1] - 1);
-                cz = min(max(cz, 0), g.cn[2] - 1);
-                best = max(best, __ldg(coarse + (cz * g.cn[1] + cy) * g.cn[0] + cx));
+        auto sweep = [&](const unsigned* __restrict__ map, int dx, int dy, int dz) {
+            const int   cnt  = nn[0] * nn[1] * nn[2];
+            const int   cmax = __reduce_max_sync(SPH_FULL, cnt);
+            const float i0 = __fdividef(1.0f, (float)nn[0]), i1 = __fdividef(1.0f, (float)nn[1]);
+            for (int q = sl; q < cmax; q += G) {
+                if (q < cnt) {
+                    const int t  = (int)(((float)q + 0.5f) * i0);          // q / nn[0]
+                    const int ix = q - t * nn[0];
+                    const int iz = (int)(((float)t + 0.5f) * i1);          // t / nn[1]
+                    const int iy = t - iz * nn[1];
+                    int cx = u0[0] + ix, cy = u0[1] + iy, cz = u0[2] + iz;
+                    cx -= (cx >= dx) ? dx : 0; cx += (cx < 0) ? dx : 0;    // periodic images
+                    cy -= (cy >= dy) ? dy : 0; cy += (cy < 0) ? dy : 0;    // (first level only)
+                    cz -= (cz >= dz) ? dz : 0; cz += (cz < 0) ? dz : 0;
+                    cx = min(max(cx, 0), dx - 1);
+                    cy = min(max(cy, 0), dy - 1);
+                    cz = min(max(cz, 0), dz - 1);
+                    best = max(best, __ldg(map + (cz * dy + cy) * dx + cx));
+                }
             }
+        };
+        if (!anyblk) {   // the common case: every ball of the warp meets a few coarse cells
+            sweep(coarse, g.cn[0], g.cn[1], g.cn[2]);
+        } else {
+            if (blocks) {
+#pragma unroll
+                for (int d = 0; d < 3; ++d) {
+                    const int b0 = u0[d] >> 3, b1 = (u0[d] + nn[d] - 1) >> 3;
+                    u0[d] = b0;
+                    nn[d] = b1 - b0 + 1;
+                }
+            }
+            sweep(blocks ? coarse + SPH_COARSE_MAX : coarse, blocks ? g.sn[0] : g.cn[0],
+                  blocks ? g.sn[1] : g.cn[1], blocks ? g.sn[2] : g.cn[2]);
         }
 #pragma unroll
         for (int o = G / 2; o > 0; o >>= 1) best = max(best, __shfl_xor_sync(SPH_FULL, best, o));
