@@ -329,7 +329,7 @@ __global__ __launch_bounds__(256) void k_density_fix(
                     const uint32_t j = k0 + lane;
                     if (j < rr.end) {
                         const float4 pj = __ldg(pos_m + j);
-                        const float dx = rr.sx - pj.x, dy = rr.sy - pj.y, dz = rr.sz - pj.z;
+                        const float dx = (rr.sx - pj.x) + rr.lx, dy = (rr.sy - pj.y) + rr.ly, dz = (rr.sz - pj.z) + rr.lz;
                         const float r2 = dx * dx + dy * dy + dz * dz;
                         if (r2 < H2) {
                             float wq, eq, fq;
@@ -362,7 +362,7 @@ __global__ __launch_bounds__(256) void k_density_fix(
                 const uint32_t j = k0 + lane;
                 if (j < rr.end) {
                     const float4 pj = __ldg(pos_m + j);
-                    const float dx = rr.sx - pj.x, dy = rr.sy - pj.y, dz = rr.sz - pj.z;
+                    const float dx = (rr.sx - pj.x) + rr.lx, dy = (rr.sy - pj.y) + rr.ly, dz = (rr.sz - pj.z) + rr.lz;
                     const float r2 = dx * dx + dy * dy + dz * dz;
                     bool in = r2 < H2;
                     if (fabsf(r2 - H2) <= 2.0f * tau * H2) {

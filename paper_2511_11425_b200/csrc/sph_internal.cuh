@@ -263,11 +263,29 @@ __device__ __forceinline__ void sph_axis_range(float x, float R, float lo, float
     }
 }
 
+// The target coordinate seen from periodic image k: s + l = x - k L exactly (FP64 on the FP32
+// inputs), s the nearest float.  d = (s - x_j) + l then has the relative error of one FP32
+// subtraction, as for a pair that does not wrap.
+__device__ __forceinline__ void sph_image_shift(float x, int k, float L, float& s, float& l) {
+    if (abs(k) <= 1) {   // k L is a float: the sum and its rounding error in six additions
+        const float b = -(float)k * L;
+        s = x + b;
+        const float bb = s - x;
+        l = (x - (s - bb)) + (b - bb);
+    } else {             // grids of fewer than 8 cells along an axis
+        const double t = (double)x - (double)k * (double)L;
+        s = (float)t;
+        l = (float)(t - (double)s);
+    }
+}
+
 // One contiguous run of candidate sources: sorted positions [start, end), and the target's
-// coordinates shifted by the periodic image of the run, so that d = s - x_j.
+// coordinates shifted by the periodic image of the run, so that d = s - x_j (+ l: what the
+// rounding of the shift dropped, for the callers that want the displacement to 2^-24 |d|).
 struct RowRec {
     uint32_t start, end;
     float    sx, sy, sz;
+    float    lx, ly, lz;
 };
 #define SPH_RCAP 64   // two x segments for each of 32 rows built per batch
 
@@ -303,8 +321,9 @@ __device__ __forceinline__ void sph_for_each_row(const SphGrid& g,
     const int   a_c1 = min(c0 + span, g.nx - 1);
     const bool  two  = (c0 + span > g.nx - 1);
     const int   b_c1 = c0 + span - g.nx;
-    const float sxA  = xi - (float)kx0 * g.len[0];
-    const float sxB  = xi - (float)(kx0 + 1) * g.len[0];
+    float sxA = xi, sxB = xi, lxA = 0.0f, lxB = 0.0f;
+    if (kx0) sph_image_shift(xi, kx0, g.len[0], sxA, lxA);
+    if (kx0 + 1) sph_image_shift(xi, kx0 + 1, g.len[0], sxB, lxB);
     const int   nyr  = y1 - y0 + 1, nzr = z1 - z0 + 1, nrow = nyr * nzr;
     const float R2   = R * R * (1.0f + 1e-5f);
     const unsigned lt = (1u << lane) - 1u;
@@ -315,7 +334,7 @@ __device__ __forceinline__ void sph_for_each_row(const SphGrid& g,
         const int iz = r / nyr, iy = r - iz * nyr;
         const int uy = y0 + iy, uz = z0 + iz;
         uint32_t  a0 = 0, a1 = 0, b0 = 0, b1 = 0;
-        float     sy = yi, sz = zi;
+        float     sy = yi, sz = zi, ly = 0.0f, lz = 0.0f;
         if (ok) {
             float dy = sph_slab_dist(yi, uy, g.lo[1], g.sy, g.ny, g.per[1]);
             float dz = sph_slab_dist(zi, uz, g.lo[2], g.sz, g.nz, g.per[2]);
@@ -324,8 +343,8 @@ __device__ __forceinline__ void sph_for_each_row(const SphGrid& g,
         if (ok) {
             const int ky = sph_fdiv(uy, g.ny), cy = uy - ky * g.ny;
             const int kz = sph_fdiv(uz, g.nz), cz = uz - kz * g.nz;
-            sy = yi - (float)ky * g.len[1];
-            sz = zi - (float)kz * g.len[2];
+            if (ky) sph_image_shift(yi, ky, g.len[1], sy, ly);
+            if (kz) sph_image_shift(zi, kz, g.len[2], sz, lz);
             const uint32_t rb = (uint32_t)(cz * g.ny + cy) * (uint32_t)g.nx;
             a0 = __ldg(cell_start + rb + c0);
             a1 = __ldg(cell_start + rb + a_c1 + 1);
@@ -338,11 +357,11 @@ __device__ __forceinline__ void sph_for_each_row(const SphGrid& g,
         const unsigned ma = __ballot_sync(SPH_FULL, va), mb = __ballot_sync(SPH_FULL, vb);
         const int      na = __popc(ma);
         if (va) {
-            RowRec rr{a0, a1, sxA, sy, sz};
+            RowRec rr{a0, a1, sxA, sy, sz, lxA, ly, lz};
             rows[__popc(ma & lt)] = rr;
         }
         if (vb) {
-            RowRec rr{b0, b1, sxB, sy, sz};
+            RowRec rr{b0, b1, sxB, sy, sz, lxB, ly, lz};
             rows[na + __popc(mb & lt)] = rr;
         }
         __syncwarp();
@@ -365,6 +384,11 @@ __device__ __forceinline__ int sph_wrap(int u, int n, int& k) {   // u = c + k n
     else        k = sph_fdiv(u, n);
     int c = u - k * n;
     return min(max(c, 0), n - 1);   // memory-safe even for coordinates outside a periodic box
+}
+
+// The image k that a rounded shift s = fl(x - k L) belongs to (0 on a non-periodic axis).
+__device__ __forceinline__ int sph_image_of(float x, float s, float L, int per) {
+    return per ? __float2int_rn(__fdividef(x - s, L)) : 0;
 }
 
 // Walks the candidate sources of every group's target and compacts the accepted ones.
@@ -405,6 +429,7 @@ __device__ __forceinline__ void sph_group_collect(const SphGrid& g,
         const int uy = y0 + iy, uz = z0 + iz;
         uint32_t  a0 = 0, a1 = 0, b0 = 0, b1 = 0;
         float     sy = yi, sz = zi, sxa = xi;
+        bool      shifted = false;
         float     d2 = 0.0f;
         if (ok) {
             const float dy = sph_slab_dist(yi, uy, g.lo[1], g.sy, g.ny, g.per[1]);
@@ -430,55 +455,81 @@ __device__ __forceinline__ void sph_group_collect(const SphGrid& g,
                 b0 = __ldg(cell_start + rq);
                 b1 = __ldg(cell_start + rq + min(c0 + span - g.nx, g.nx - 1) + 1);
             }
+            shifted = (ky | kz | kx0) != 0 || b1 > b0;
         }
-        const int nseg = __any_sync(SPH_FULL, b1 > b0) ? 2 : 1;
-        for (int seg = 0; seg < nseg; ++seg) {
-            const uint32_t s0 = seg ? b0 : a0, s1 = seg ? b1 : a1;
-            const float    sxs = seg ? sxa - g.len[0] : sxa;
-            unsigned gm = (__ballot_sync(SPH_FULL, s1 > s0) >> g0) & GM;
-            const int nk = __reduce_max_sync(SPH_FULL, __popc(gm));
-            if (s1 > s0) tested += s1 - s0;   // every candidate of this lane's row gets tested
-            for (int k = 0; k < nk; ++k) {
-                const bool have = gm != 0u;
-                const int  src  = g0 + (have ? (__ffs(gm) - 1) : 0);
-                gm &= gm - 1u;
-                uint32_t       rs  = __shfl_sync(SPH_FULL, s0, src);
-                uint32_t       re  = __shfl_sync(SPH_FULL, s1, src);
-                const float    sxx = __shfl_sync(SPH_FULL, sxs, src);
-                const float    rsy = __shfl_sync(SPH_FULL, sy, src);
-                const float    rsz = __shfl_sync(SPH_FULL, sz, src);
-                if (!have) re = rs;
-                uint32_t c = rs + sl;
-                // NW windows of G candidates per trip, loaded unconditionally (the sorted arrays
-                // are padded by SPH_POS_PAD records, so reading past a row's end is harmless)
-                auto trip = [&](auto nw_tag) {
-                    constexpr int NW = decltype(nw_tag)::value;
-                    float4 pp[NW];
-#pragma unroll
-                    for (int u = 0; u < NW; ++u) pp[u] = __ldg(pos + c + u * G);
-#pragma unroll
-                    for (int u = 0; u < NW; ++u) {
-                        const float dx = sxx - pp[u].x, dy = rsy - pp[u].y, dz = rsz - pp[u].z;
-                        const float r2 = dx * dx + dy * dy + dz * dz;
-                        const bool  acc = (c + u * G < re) && accept(pp[u], r2);
-                        const unsigned gm = (__ballot_sync(SPH_FULL, acc) >> g0) & GM;
-                        if (acc)
-                            store(total + __popc(gm & lt), c + u * G, pp[u], dx, dy, dz, r2);
-                        total += __popc(gm);
+        // Warp-uniform: some row of this batch is met through a periodic image.  The rounded
+        // shift x_i - k L is off by up to 2^-24 |x|, which relative to a displacement of a few
+        // h is far more than one FP32 subtraction's 2^-24 |d|.  Such a batch takes the second
+        // copy of the candidate loop, which carries what the rounding dropped (three more
+        // additions per candidate); batches inside the box run the plain loop unchanged.
+        const bool wrapany = __any_sync(SPH_FULL, shifted);
+        const int  nseg = __any_sync(SPH_FULL, b1 > b0) ? 2 : 1;
+        auto segments = [&](auto wrap_tag) {
+            constexpr bool WRAP = decltype(wrap_tag)::value;
+            float ly = 0.0f, lz = 0.0f;
+            if (WRAP) {   // exact shifts of this lane's row, redone from the image it was given
+                sph_image_shift(yi, sph_image_of(yi, sy, g.len[1], g.per[1]), g.len[1], sy, ly);
+                sph_image_shift(zi, sph_image_of(zi, sz, g.len[2], g.per[2]), g.len[2], sz, lz);
+            }
+            for (int seg = 0; seg < nseg; ++seg) {
+                const uint32_t s0 = seg ? b0 : a0, s1 = seg ? b1 : a1;
+                float          sxs = seg ? sxa - g.len[0] : sxa, lxs = 0.0f;
+                if (WRAP)
+                    sph_image_shift(xi, sph_image_of(xi, sxa, g.len[0], g.per[0]) + seg, g.len[0], sxs, lxs);
+                unsigned gm = (__ballot_sync(SPH_FULL, s1 > s0) >> g0) & GM;
+                const int nk = __reduce_max_sync(SPH_FULL, __popc(gm));
+                if (s1 > s0) tested += s1 - s0;   // every candidate of this lane's row gets tested
+                for (int k = 0; k < nk; ++k) {
+                    const bool have = gm != 0u;
+                    const int  src  = g0 + (have ? (__ffs(gm) - 1) : 0);
+                    gm &= gm - 1u;
+                    uint32_t       rs  = __shfl_sync(SPH_FULL, s0, src);
+                    uint32_t       re  = __shfl_sync(SPH_FULL, s1, src);
+                    const float    sxx = __shfl_sync(SPH_FULL, sxs, src);
+                    const float    rsy = __shfl_sync(SPH_FULL, sy, src);
+                    const float    rsz = __shfl_sync(SPH_FULL, sz, src);
+                    float          rlx = 0.0f, rly = 0.0f, rlz = 0.0f;
+                    if (WRAP) {
+                        rlx = __shfl_sync(SPH_FULL, lxs, src);
+                        rly = __shfl_sync(SPH_FULL, ly, src);
+                        rlz = __shfl_sync(SPH_FULL, lz, src);
                     }
-                    c += NW * G;
-                };
-                // the longest row among the four groups decides how many windows are issued
-                const int nwin = (__reduce_max_sync(SPH_FULL, re - rs) + (G - 1)) / G;
-                if (nwin == 1) {
-                    trip(std::integral_constant<int, 1>{});
-                } else if (nwin == 2) {
-                    trip(std::integral_constant<int, 2>{});
-                } else {
-                    for (int w = 0; w < nwin; w += SPH_UNROLL) trip(std::integral_constant<int, SPH_UNROLL>{});
+                    if (!have) re = rs;
+                    uint32_t c = rs + sl;
+                    // NW windows of G candidates per trip, loaded unconditionally (the sorted arrays
+                    // are padded by SPH_POS_PAD records, so reading past a row's end is harmless)
+                    auto trip = [&](auto nw_tag) {
+                        constexpr int NW = decltype(nw_tag)::value;
+                        float4 pp[NW];
+#pragma unroll
+                        for (int u = 0; u < NW; ++u) pp[u] = __ldg(pos + c + u * G);
+#pragma unroll
+                        for (int u = 0; u < NW; ++u) {
+                            float dx = sxx - pp[u].x, dy = rsy - pp[u].y, dz = rsz - pp[u].z;
+                            if (WRAP) { dx += rlx; dy += rly; dz += rlz; }
+                            const float r2 = dx * dx + dy * dy + dz * dz;
+                            const bool  acc = (c + u * G < re) && accept(pp[u], r2);
+                            const unsigned gm = (__ballot_sync(SPH_FULL, acc) >> g0) & GM;
+                            if (acc)
+                                store(total + __popc(gm & lt), c + u * G, pp[u], dx, dy, dz, r2);
+                            total += __popc(gm);
+                        }
+                        c += NW * G;
+                    };
+                    // the longest row among the four groups decides how many windows are issued
+                    const int nwin = (__reduce_max_sync(SPH_FULL, re - rs) + (G - 1)) / G;
+                    if (nwin == 1) {
+                        trip(std::integral_constant<int, 1>{});
+                    } else if (nwin == 2) {
+                        trip(std::integral_constant<int, 2>{});
+                    } else {
+                        for (int w = 0; w < nwin; w += SPH_UNROLL) trip(std::integral_constant<int, SPH_UNROLL>{});
+                    }
                 }
             }
-        }
+        };
+        if (wrapany) segments(std::true_type{});
+        else         segments(std::false_type{});
     }
 }
 
