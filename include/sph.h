@@ -109,7 +109,11 @@ int  sph_build_cells(sph_ctx* ctx, int64_t n, const float* x, const float* y, co
  * (32 pi/3) sum_j m_j w(r_ij/h_i) = n_ngb m_i (gather, self included) by a safeguarded
  * Newton-type (Halley) iteration on a per-target neighbour list, then writes
  *   h_inout (in: guess, out: solution), rho = sum_j m_j W_ij(h_i), omega (Eq. 7),
- *   n_ngb_out = #{j : r_ij < 2 h_i} (borderline pairs decided in FP64).                  */
+ *   n_ngb_out = #{j : r_ij < 2 h_i} (borderline pairs decided in FP64).
+ * Along a periodic axis of side L, h_i is capped at L/5: the search ball 2 h x 1.25 then
+ * stays below L/2, where the minimum image is unique (PAPER.md:297 asks for the same).  A
+ * particle whose root lies above the cap, or that runs out of h_max_iter sweeps, keeps its
+ * last iterate and is counted in sph_stats_t.dens_nonconv (no host synchronisation here). */
 int  sph_density_h(sph_ctx* ctx, const float* m, float* h_inout, float* rho, float* omega,
                    int32_t* n_ngb_out);
 

@@ -27,8 +27,9 @@
  * Parity pins: kernel normalisation and derivatives, root residual and
  * monotonicity, infinite-lattice density, momentum / energy / angular-momentum
  * conservation, Galilean / translation / permutation invariance, two-particle
- * and homologous-flow closed forms, static-gas dt -- see
- * tests/test_oracle_pins.py.  No function here is "parity unpinned".
+ * and homologous-flow closed forms, static-gas dt, the entropy-conserving
+ * variant (viscous heating alone conserves energy; P / rho^gamma invariant) --
+ * see tests/test_oracle_pins.py.  No function here is "parity unpinned".
  *
  * All arithmetic is double precision.  Inputs arrive as double arrays holding
  * the exact values of the caller's FP32 inputs.
@@ -55,6 +56,8 @@ typedef struct {
     double gamma;       /* ideal gas                         */
     double av_alpha, av_beta, av_eps; /* Eqs. 15-16; eps reading R8         */
     double eta_cfl, eta_acc;          /* Eq. 26 / PAPER.md:263              */
+    int32_t entropy;    /* 1: Eq. (14) is discarded, du/dt is the
+                           viscous heating of Eq. (18) alone; reading R22     */
 } orc_params;
 
 /* ------------------------------------------------------------------------- *
@@ -358,7 +361,8 @@ static int orc_pair_force(const orc_params *p, const double d[3], double r2, dou
     double C = Ai * Fi + Aj * Fj + Pi * Fbar;                      /* Eqs. (13)+(17) */
     for (int k = 0; k < 3; k++) out->a[k] = -mj * C * d[k] / r;
     double vrhat = vr / r;
-    double E = (Ai * Fi + 0.5 * Pi * Fbar) * vrhat;                /* Eqs. (14)+(18) */
+    double E = 0.5 * Pi * Fbar * vrhat;                            /* Eq. (18) */
+    if (!p->entropy) E += Ai * Fi * vrhat;                         /* Eq. (14) */
     out->dudt = mj * E;
     out->mu = mu;
     out->absC = mj * fabs(C);
@@ -659,6 +663,18 @@ int orc_num_threads(void)
 void orc_axpy(int64_t n, double a, const double *x, const double *y, double *out)
 {   /* out = y + a x : the form shared by Eqs. (19)-(24) with a = dt/2 */
     for (int64_t i = 0; i < n; i++) out[i] = y[i] + a * x[i];
+}
+
+/* Entropy-conserving update of the ideal gas: "uses the old
+ * density and internal energy to calculate the isentropic evolution to the new
+ * density, by having the EOS solve u_new = u(rho_new, s(rho_old, u_old))".  For
+ * P = (gamma-1) rho u an isentrope is P / rho^gamma = const
+ * (the entropic function of Springel & Hernquist 2002, cited there), hence
+ *   u_new = u_old (rho_new / rho_old)^(gamma-1).           (reading R22) */
+void orc_isentropic_u(int64_t n, double gamma, const double *rho_old, const double *rho_new,
+                      const double *u_old, double *u_new)
+{
+    for (int64_t i = 0; i < n; i++) u_new[i] = u_old[i] * pow(rho_new[i] / rho_old[i], gamma - 1.0);
 }
 
 void orc_drift(int64_t n, double dt, const double *v, double lo, double len, int periodic,

@@ -37,7 +37,7 @@ class _Box(C.Structure):
 class _Params(C.Structure):
     _fields_ = [("kernel", C.c_int32), ("n_ngb", C.c_double), ("gamma", C.c_double),
                 ("av_alpha", C.c_double), ("av_beta", C.c_double), ("av_eps", C.c_double),
-                ("eta_cfl", C.c_double), ("eta_acc", C.c_double)]
+                ("eta_cfl", C.c_double), ("eta_acc", C.c_double), ("entropy", C.c_int32)]
 
 
 @dataclass
@@ -50,10 +50,11 @@ class Params:
     av_eps: float = 0.01
     eta_cfl: float = 0.3
     eta_acc: float = 0.2
+    entropy: int = 0         # 1: du/dt = Eq. (18) only (reading R22)
 
     def c(self) -> _Params:
         return _Params(self.kernel, self.n_ngb, self.gamma, self.av_alpha, self.av_beta,
-                       self.av_eps, self.eta_cfl, self.eta_acc)
+                       self.av_eps, self.eta_cfl, self.eta_acc, int(self.entropy))
 
 
 @dataclass
@@ -215,6 +216,14 @@ def axpy(a, x, y):
     x, y = _d(x), _d(y)
     out = np.empty_like(x)
     lib().orc_axpy(C.c_int64(len(x)), C.c_double(a), _p(x), _p(y), _p(out))
+    return out
+
+
+def isentropic_u(rho_old, rho_new, u, gamma):
+    """u (rho_new/rho_old)^(gamma-1): the isentropic update of PAPER.md:197 (reading R22)."""
+    ro, rn, u = _d(rho_old), _d(rho_new), _d(u)
+    out = np.empty_like(u)
+    lib().orc_isentropic_u(C.c_int64(len(u)), C.c_double(gamma), _p(ro), _p(rn), _p(u), _p(out))
     return out
 
 

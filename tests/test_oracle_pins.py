@@ -667,3 +667,58 @@ def test_marking_pass_is_the_union_of_the_pair_lists():
     assert np.array_equal(got, want)
     more = src.copy(); more[rng.integers(0, n, 30)] = 1
     assert (orc.mark_neighbors(w["x"], w["y"], w["z"], w["h"], more, box) >= got).all()
+
+
+# ------------------------------------------- entropy-conserving variant (R22)
+def test_entropy_variant_keeps_the_viscous_heating_only(c1_forces):
+    """PAPER.md:197 discards Eq. (14); Eq. (18) stays "active independent if the
+    entropy conservation scheme is active or not".  Pinned through the (pinned) full form:
+    (i) a, mu_min do not change; (ii) without viscosity du/dt vanishes identically;
+    (iii) du/dt = [Eq. 14 + Eq. 18] - [Eq. 14], the latter being the full form without
+    viscosity; (iv) heating is never negative (Pi > 0 only for approaching pairs, where
+    v_ij.r_ij and dW/dr are both negative)."""
+    w, u, args, full = c1_forces
+    ent = orc.forces(*args, _box(w), _par(w, entropy=1))
+    for k in ("ax", "ay", "az", "mu_min", "Sa"):
+        assert np.array_equal(ent[k], full[k])
+    noav_full = orc.forces(*args, _box(w), _par(w, av_alpha=0.0, av_beta=0.0))
+    noav_ent = orc.forces(*args, _box(w), _par(w, av_alpha=0.0, av_beta=0.0, entropy=1))
+    assert np.all(noav_ent["dudt"] == 0.0) and np.all(noav_ent["Su"] == 0.0)
+    assert np.abs(noav_full["dudt"]).max() > 0
+    assert np.allclose(ent["dudt"], full["dudt"] - noav_full["dudt"], rtol=0, atol=1e-12 * full["Su"].max())
+    assert ent["dudt"].min() >= 0.0 and ent["dudt"].max() > 0.0
+
+
+def test_viscous_heating_alone_conserves_energy(c1_forces):
+    """With P = 0 (u = 0) only Eqs. (17)-(18) act: sum_i m_i (v_i.a_i + du_i/dt) = 0 to
+    round-off, in the entropy variant as in the full one (which coincide there).  Fails if the
+    1/2 of Eq. (18) or the averaged kernel goes missing in the variant."""
+    w, u, args, _ = c1_forces
+    args = list(args)
+    args[7] = np.zeros_like(u)
+    par = _par(w, entropy=1)
+    f = orc.forces(*args, _box(w), par)
+    g = orc.forces(*args, _box(w), _par(w))
+    assert np.array_equal(f["dudt"], g["dudt"]) and np.array_equal(f["ax"], g["ax"])
+    m = w["m"].astype(np.float64)
+    v = [w[k].astype(np.float64) for k in ("vx", "vy", "vz")]
+    e = (m * (v[0] * f["ax"] + v[1] * f["ay"] + v[2] * f["az"] + f["dudt"])).sum()
+    scale = (m * (f["Su"] + np.abs(v[0]) * f["Sa"])).sum()
+    assert scale > 0 and abs(e) < 1e-12 * scale
+
+
+def test_isentropic_update_keeps_the_entropic_function():
+    """PAPER.md:197 with the ideal gas of PAPER.md:111: P / rho^gamma is unchanged, updates
+    compose (rho0 -> rho1 -> rho2 equals rho0 -> rho2), and gamma = 5/3 with an eightfold
+    compression multiplies u by exactly 4."""
+    rng = np.random.default_rng(3)
+    n, gamma = 1000, 1.4
+    r0, r1, r2 = (rng.uniform(0.1, 10.0, n) for _ in range(3))
+    u0 = rng.uniform(0.1, 5.0, n)
+    u1 = orc.isentropic_u(r0, r1, u0, gamma)
+    P0, _ = orc.eos(r0, u0, gamma)
+    P1, _ = orc.eos(r1, u1, gamma)
+    assert np.allclose(P1 / r1 ** gamma, P0 / r0 ** gamma, rtol=1e-13)
+    assert np.allclose(orc.isentropic_u(r1, r2, u1, gamma), orc.isentropic_u(r0, r2, u0, gamma), rtol=1e-13)
+    assert np.array_equal(orc.isentropic_u(r0, r0, u0, gamma), u0)
+    assert np.allclose(orc.isentropic_u(np.ones(3), np.full(3, 8.0), np.full(3, 0.75), 5.0 / 3.0), 3.0, rtol=1e-15)
