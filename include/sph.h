@@ -68,6 +68,9 @@ typedef struct {
                           /* on it                                                         */
     float   cell_div_x;   /* cells per minimum search radius along x (<= 0: default 4)     */
     float   cell_div_yz;  /* ... along y and z (<= 0: default 1.5)                         */
+    int32_t entropy;      /* 1: entropy-conserving variant: sph_forces drops */
+                          /* the Eq. (14) term, dudt is the viscous heating of Eq. (18)     */
+                          /* alone; the caller advances u with sph_isentropic_u             */
 } sph_params;
 
 /* 64-bit counters accumulated on the device since the last sph_stats_reset.             */
@@ -192,6 +195,16 @@ int  sph_kick(sph_ctx* ctx, int64_t n, const float* dt_device, float dt_scale, f
               const float* dudt);
 int  sph_drift(sph_ctx* ctx, int64_t n, const float* dt_device, float dt_scale, float* x, float* y,
                float* z, const float* vx, const float* vy, const float* vz);
+
+/* Entropy-conserving update of the internal energy: "uses the old density and
+ * internal energy to calculate the isentropic evolution to the new density, by having the EOS
+ * solve u_new = u(rho_new, s(rho_old, u_old))".  For the built-in ideal gas an
+ * isentrope is P / rho^gamma = const, so u_inout[i] *= (rho_new[i] / rho_old[i])^(gamma-1)
+ * (reading R31).  All arrays are device pointers of n floats in caller order;
+ * element-wise, in place, asynchronous on the context's stream.  With params.entropy = 1 the
+ * dudt of sph_forces holds the viscous heating alone, which the kicks add on top.             */
+int  sph_isentropic_u(sph_ctx* ctx, int64_t n, const float* rho_old, const float* rho_new,
+                      float* u_inout);
 
 /* Diagnostic: CSR neighbour lists at a prescribed h, caller indices; a list is a set, the
  * order inside it is unspecified.

@@ -57,7 +57,7 @@ typedef struct {
     double av_alpha, av_beta, av_eps; /* Eqs. 15-16; eps reading R8         */
     double eta_cfl, eta_acc;          /* Eq. 26 / PAPER.md:263              */
     int32_t entropy;    /* 1: Eq. (14) is discarded, du/dt is the
-                           viscous heating of Eq. (18) alone; reading R22     */
+                           viscous heating of Eq. (18) alone; reading R31     */
 } orc_params;
 
 /* ------------------------------------------------------------------------- *
@@ -670,7 +670,7 @@ void orc_axpy(int64_t n, double a, const double *x, const double *y, double *out
  * density, by having the EOS solve u_new = u(rho_new, s(rho_old, u_old))".  For
  * P = (gamma-1) rho u an isentrope is P / rho^gamma = const
  * (the entropic function of Springel & Hernquist 2002, cited there), hence
- *   u_new = u_old (rho_new / rho_old)^(gamma-1).           (reading R22) */
+ *   u_new = u_old (rho_new / rho_old)^(gamma-1).           (reading R31) */
 void orc_isentropic_u(int64_t n, double gamma, const double *rho_old, const double *rho_new,
                       const double *u_old, double *u_new)
 {

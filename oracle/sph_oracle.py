@@ -50,7 +50,7 @@ class Params:
     av_eps: float = 0.01
     eta_cfl: float = 0.3
     eta_acc: float = 0.2
-    entropy: int = 0         # 1: du/dt = Eq. (18) only (reading R22)
+    entropy: int = 0         # 1: du/dt = Eq. (18) only (reading R31)
 
     def c(self) -> _Params:
         return _Params(self.kernel, self.n_ngb, self.gamma, self.av_alpha, self.av_beta,
@@ -220,7 +220,7 @@ def axpy(a, x, y):
 
 
 def isentropic_u(rho_old, rho_new, u, gamma):
-    """u (rho_new/rho_old)^(gamma-1): the isentropic update of PAPER.md:197 (reading R22)."""
+    """u (rho_new/rho_old)^(gamma-1): the isentropic update of PAPER.md:197 (reading R31)."""
     ro, rn, u = _d(rho_old), _d(rho_new), _d(u)
     out = np.empty_like(u)
     lib().orc_isentropic_u(C.c_int64(len(u)), C.c_double(gamma), _p(ro), _p(rn), _p(u), _p(out))

@@ -129,7 +129,8 @@ struct Accum {
 };
 
 // One pair of Eqs. (13)-(18): source j at displacement d = x_i - x_j (minimum image).
-template <int KERN>
+// ENT: the entropy-conserving variant drops the Eq. (14) term of du/dt.
+template <int KERN, bool ENT>
 __device__ __forceinline__ void force_pair(const Target& t, Accum& a, const ForcePar& par,
                                            const float4 vj, const float4 rj, float dx,
                                            float dy, float dz, float r2, float hj) {
@@ -154,11 +155,11 @@ __device__ __forceinline__ void force_pair(const Target& t, Accum& a, const Forc
     a.ax += ca * dx;
     a.ay += ca * dy;
     a.az += ca * dz;
-    a.du -= vj.w * (Ag + 0.5f * pig) * vr;
+    a.du -= vj.w * (ENT ? 0.5f * pig : Ag + 0.5f * pig) * vr;   // Eq. (18) [+ Eq. (14)]
     ++a.pairs;
 }
 
-template <int KERN>
+template <int KERN, bool ENT>
 __global__ __launch_bounds__(F_TPB, SPH_FMINB) void k_forces(
     int n, const SphGrid* __restrict__ gp, const uint32_t* __restrict__ cell_start,
     const float4* __restrict__ pos_h, const float4* __restrict__ vel_m,
@@ -270,7 +271,7 @@ __global__ __launch_bounds__(F_TPB, SPH_FMINB) void k_forces(
             const float r2 = dx * dx + dy * dy + dz * dz;
             // kept lists hold everything inside the kept radius: apply the pair test
             if (k < mycnt && r2 < fmaxf(hi2x4, 4.0f * pj.w * pj.w) && r2 > 0.0f)
-                force_pair<KERN>(t, a, par, vj, rj, dx, dy, dz, r2, pj.w);
+                force_pair<KERN, ENT>(t, a, par, vj, rj, dx, dy, dz, r2, pj.w);
         };
         float4 pA, vA, rA, pB, vB, rB;
         fetch(0, pA, vA, rA);
@@ -312,7 +313,7 @@ __global__ __launch_bounds__(F_TPB, SPH_FMINB) void k_forces(
 }
 
 // The robust path: one warp per queued target, candidates handled as they are met.
-template <int KERN>
+template <int KERN, bool ENT>
 __global__ __launch_bounds__(256) void k_forces_fix(
     const SphGrid* __restrict__ gp, const uint32_t* __restrict__ cell_start,
     const float4* __restrict__ pos_h, const float4* __restrict__ vel_m,
@@ -349,7 +350,7 @@ __global__ __launch_bounds__(256) void k_forces_fix(
                     const float dx = rr.sx - pj.x, dy = rr.sy - pj.y, dz = rr.sz - pj.z;
                     const float r2 = dx * dx + dy * dy + dz * dz;
                     if (r2 < fmaxf(hi2x4, 4.0f * pj.w * pj.w) && r2 > 0.0f)
-                        force_pair<KERN>(t, a, par, __ldg(vel_m + j), __ldg(rcak + j), dx, dy, dz, r2, pj.w);
+                        force_pair<KERN, ENT>(t, a, par, __ldg(vel_m + j), __ldg(rcak + j), dx, dy, dz, r2, pj.w);
                 }
                 c_tested += min(32u, rr.end - k0);
             }
@@ -413,18 +414,23 @@ int sph_launch_forces(sph_ctx* c, const float* m, const float* vx, const float* 
     k_coarse_blocks<<<c->sm_count, 256, 0, s>>>(c->grid, c->coarse_hmax);
     ForcePar par{c->par.av_alpha, c->par.av_beta, c->par.av_eps};
     const int nblk = (int)((n + F_TARGETS - 1) / F_TARGETS);
-    auto launch = [&](auto tag) {
-        constexpr int KERN = decltype(tag)::value;
-        k_forces<KERN><<<nblk, F_TPB, 0, s>>>((int)n, c->grid, c->cell_start, c->pos_h, c->vel_m,
+    auto launch2 = [&](auto tag, auto etag) {
+        constexpr int  KERN = decltype(tag)::value;
+        constexpr bool ENT  = decltype(etag)::value;
+        k_forces<KERN, ENT><<<nblk, F_TPB, 0, s>>>((int)n, c->grid, c->cell_start, c->pos_h, c->vel_m,
                                               c->rcak, c->perm, par, ax, ay, az, dudt, mu_min,
                                               c->fix_list, c->fix_cnt + 1, c->coarse_hmax, c->nb_j,
                                               c->nb_cnt, c->nb_rkeep,
                                               c->act_on ? c->act_list : nullptr, c->act_cnt,
                                               c->stats);
-        k_forces_fix<KERN><<<c->sm_count * 4, 256, 0, s>>>(c->grid, c->cell_start, c->pos_h, c->vel_m,
+        k_forces_fix<KERN, ENT><<<c->sm_count * 4, 256, 0, s>>>(c->grid, c->cell_start, c->pos_h, c->vel_m,
                                                            c->rcak, c->perm, par, c->fix_list,
                                                            c->fix_cnt + 1, ax, ay, az, dudt, mu_min,
                                                            c->stats);
+    };
+    auto launch = [&](auto tag) {
+        if (c->par.entropy) launch2(tag, std::true_type{});
+        else launch2(tag, std::false_type{});
     };
     switch (c->par.kernel) {
     case 0: launch(std::integral_constant<int, 0>{}); break;

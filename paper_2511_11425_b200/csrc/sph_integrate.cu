@@ -48,6 +48,15 @@ __global__ void k_drift(int64_t n, sph_box box, float* x, float* y, float* z,
     }
 }
 
+// PAPER.md:197 for the ideal gas: u (rho_new / rho_old)^(gamma-1); the ratio is near 1, so
+// exp2(gm1 log2(ratio)) in FP32 carries about 1e-7 relative
+__global__ void k_isentropic(int64_t n, float gm1, const float* __restrict__ rho_old,
+                             const float* __restrict__ rho_new, float* u) {
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n;
+         i += (int64_t)gridDim.x * blockDim.x)
+        u[i] *= powf(rho_new[i] / rho_old[i], gm1);
+}
+
 int launch_axpy(sph_ctx* c, int64_t n, const Axpy4& a, const float* dt, float scale) {
     int nblk = (int)((n + 255) / 256);
     if (nblk > c->sm_count * 16) nblk = c->sm_count * 16;
@@ -85,5 +94,15 @@ extern "C" int sph_drift(sph_ctx* c, int64_t n, const float* dt_device, float dt
     if (nblk > c->sm_count * 16) nblk = c->sm_count * 16;
     k_drift<<<nblk, 256, 0, c->stream>>>(n, c->box, x, y, z, vx, vy, vz, dt_device, dt_scale);
     SPH_CUDA_CHECK(c, cudaGetLastError());   // Eq. (25)
+    return SPH_OK;
+}
+
+extern "C" int sph_isentropic_u(sph_ctx* c, int64_t n, const float* rho_old, const float* rho_new,
+                                float* u_inout) {
+    if (!c || n <= 0 || !rho_old || !rho_new || !u_inout) return SPH_EINVAL;
+    int nblk = (int)((n + 255) / 256);
+    if (nblk > c->sm_count * 16) nblk = c->sm_count * 16;
+    k_isentropic<<<nblk, 256, 0, c->stream>>>(n, c->par.gamma - 1.0f, rho_old, rho_new, u_inout);
+    SPH_CUDA_CHECK(c, cudaGetLastError());
     return SPH_OK;
 }

@@ -10,6 +10,10 @@ One step, in the paper's order:
      opening kick of the new step (new dt)                    sph_kick             (Eqs. 23-24)
   5. drift                                                    sph_drift            (Eq. 25)
 (step 3, the interface correction, is not built.)  Between steps v and u live at the half step.
+
+With `entropy=1` the force pass returns the viscous heating of Eq. (18) alone and,
+right after each density pass, u follows the isentrope from the previous pass's density to the new
+one (sph_isentropic_u); the kicks then add the viscous heating.
 """
 from __future__ import annotations
 
@@ -38,12 +42,20 @@ class Simulation:
         self.dt_new = self.out["dt_min"]
         self.t = torch.zeros(1, dtype=torch.float64, device="cuda")
         self.steps = 0
+        self.entropy = bool(params.get("entropy", 0))
+        self.rho_prev = None                   # density of the previous pass (entropy variant)
 
     def _derivatives(self):
         """Steps 1, 2, 4a: density, prediction, forces and the new global dt."""
         d, o, c = self.d, self.out, self.ctx
         c.build_cells(d["x"], d["y"], d["z"], d["h"])
         c.density_h(d["m"], d["h"], o["rho"], o["omega"], o["n_ngb"])
+        if self.entropy:
+            if self.rho_prev is None:
+                self.rho_prev = torch.empty_like(o["rho"])
+            else:
+                c.isentropic_u(self.rho_prev, o["rho"], d["u"])
+            self.rho_prev.copy_(o["rho"])
         p = self.pred
         c.predict(self.dt_prev, 1.0, d["vx"], d["vy"], d["vz"], d["u"], o["ax"], o["ay"], o["az"],
                   o["dudt"], p["vx"], p["vy"], p["vz"], p["u"])

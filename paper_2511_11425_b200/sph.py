@@ -20,7 +20,7 @@ SPH_OK, SPH_EINVAL, SPH_EBOX, SPH_ENOMEM, SPH_ECUDA, SPH_ESTALE, SPH_ENOSPC = 0,
 # every symbol include/sph.h declares (tests check the library exports exactly these)
 SYMBOLS = ["sph_create", "sph_destroy", "sph_build_cells", "sph_density_h", "sph_forces",
            "sph_timestep", "sph_rungs", "sph_set_active", "sph_mark_neighbors",
-           "sph_interface_correction", "sph_predict", "sph_kick", "sph_drift", "sph_neighbors", "sph_stats", "sph_stats_reset", "sph_permutation",
+           "sph_interface_correction", "sph_predict", "sph_kick", "sph_drift", "sph_isentropic_u", "sph_neighbors", "sph_stats", "sph_stats_reset", "sph_permutation",
            "sph_fp32_peak", "sph_strerror", "sph_last_error"]
 
 
@@ -39,7 +39,7 @@ class _Params(C.Structure):
                 ("av_alpha", C.c_float), ("av_beta", C.c_float), ("av_eps", C.c_float),
                 ("eta_cfl", C.c_float), ("eta_acc", C.c_float), ("h_tol", C.c_float),
                 ("h_max_iter", C.c_int32), ("search_slack", C.c_float),
-                ("cell_div_x", C.c_float), ("cell_div_yz", C.c_float)]
+                ("cell_div_x", C.c_float), ("cell_div_yz", C.c_float), ("entropy", C.c_int32)]
 
 
 class _Stats(C.Structure):
@@ -64,11 +64,12 @@ class Params:
     search_slack: float = 0.0
     cell_div_x: float = 0.0
     cell_div_yz: float = 0.0
+    entropy: int = 0            # 1: dudt = Eq. (18) only, u advanced by isentropic_u
 
     def c(self) -> _Params:
         return _Params(self.kernel, self.n_ngb, self.gamma, self.av_alpha, self.av_beta,
                        self.av_eps, self.eta_cfl, self.eta_acc, self.h_tol, self.h_max_iter,
-                       self.search_slack, self.cell_div_x, self.cell_div_yz)
+                       self.search_slack, self.cell_div_x, self.cell_div_yz, int(self.entropy))
 
 
 @dataclass
@@ -108,6 +109,7 @@ def load():
     lib.sph_predict.argtypes = [vp, i64, fp, C.c_float] + [fp] * 12
     lib.sph_kick.argtypes = [vp, i64, fp, C.c_float] + [fp] * 8
     lib.sph_drift.argtypes = [vp, i64, fp, C.c_float] + [fp] * 6
+    lib.sph_isentropic_u.argtypes = [vp, i64, fp, fp, fp]
     lib.sph_neighbors.argtypes = [vp, fp, i32, fp, fp, i64, C.POINTER(i64)]
     lib.sph_stats.argtypes = [vp, C.POINTER(_Stats)]
     lib.sph_stats_reset.argtypes = [vp]
@@ -243,6 +245,12 @@ class Sph:
         n, f = x.numel(), torch.float32
         args = [_ptr(t, f, n) for t in (x, y, z, vx, vy, vz)]
         self._check(self.lib.sph_drift(self._ctx, n, _ptr(dt, f, 1), scale, *args))
+
+    def isentropic_u(self, rho_old, rho_new, u):
+        """u *= (rho_new / rho_old)^(gamma-1), in place (PAPER.md:197)."""
+        n, f = u.numel(), torch.float32
+        self._check(self.lib.sph_isentropic_u(self._ctx, n, _ptr(rho_old, f, n), _ptr(rho_new, f, n),
+                                              _ptr(u, f, n)))
 
     # ---- diagnostics --------------------------------------------------------------------
     def neighbors(self, h, mode=0):

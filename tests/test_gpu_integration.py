@@ -223,3 +223,44 @@ def test_sedov_taylor_blast_shock_radius_and_energy(gu):
     assert mean[k] >= 2.3, mean[k]                       # compression behind the shock
     assert abs(mean[edges[:-1] > 0.4].mean() / 1.0146 - 1) <= 2e-3   # undisturbed gas ahead
     assert mean[:20].max() < 0.2                         # evacuated interior
+
+
+def test_entropy_variant_conserves_the_entropic_function_without_viscosity(gu):
+    """with the viscosity off, the entropy-conserving scheme keeps
+    A_i = u_i rho_i^(1-gamma) of every particle over many steps (u follows the isentrope to
+    each new density; the kicks add nothing), while the flow compresses and expands; with
+    the viscosity on, A_i never decreases and total energy stays close (the scheme trades the
+    exact energy budget for the entropy one)."""
+    from paper_2511_11425_b200.integrate import Simulation
+    w = workloads.uniform_cube(nside=24, h_start="warm", v_sigma=0.3)
+    gamma = float(np.float32(w["gamma"]))
+    w0 = dict(w, av_alpha=0.0, av_beta=0.0)
+
+    def entropic(sim):
+        return gu.np64(sim.d["u"]) * gu.np64(sim.out["rho"]) ** (1.0 - gamma)
+
+    sim = Simulation(w0, entropy=1)
+    sim.synchronise()
+    A0, rho0 = entropic(sim), gu.np64(sim.out["rho"]).copy()
+    ek0, eu0 = sim.energies()
+    for _ in range(20):
+        sim.step()
+    sim.synchronise()
+    A1, rho1 = entropic(sim), gu.np64(sim.out["rho"])
+    assert np.abs(rho1 / rho0 - 1).max() > 0.02          # the gas did compress / expand
+    assert (np.abs(A1 - A0) / A0).max() <= 2e-5, (np.abs(A1 - A0) / A0).max()
+    assert np.abs(gu.np64(sim.out["dudt"])).max() == 0.0
+    ek1, eu1 = sim.energies()
+    assert abs((ek1 + eu1) - (ek0 + eu0)) <= 1e-2 * (ek0 + eu0), (ek0, eu0, ek1, eu1)
+
+    simv = Simulation(w, entropy=1)
+    simv.synchronise()
+    B0 = entropic(simv)
+    e0 = sum(simv.energies())
+    for _ in range(20):
+        simv.step()
+    simv.synchronise()
+    B1 = entropic(simv)
+    assert ((B1 - B0) / B0).min() >= -2e-5               # viscous heating only raises entropy
+    assert ((B1 - B0) / B0).max() > 1e-4
+    assert abs(sum(simv.energies()) - e0) <= 1e-2 * e0, (sum(simv.energies()), e0)

@@ -3,6 +3,8 @@ element on the same seeded inputs.  Tolerances are BASELINE.json north_star's:
   neighbour lists / counts bit-exact (at the GPU's h, reading R7),
   rho, h: 1e-5 relative; a, du/dt: 1e-4 of the sum of pairwise term magnitudes; dt: 1e-6.
 """
+import dataclasses
+
 import numpy as np
 import pytest
 import torch
@@ -670,3 +672,55 @@ def test_fastgas_flow_on_a_small_active_set(gu, c1):
     assert ea.max() <= TOL_F and eu.max() <= TOL_F, (ea.max(), eu.max())
     for k in ("ax", "ay", "az", "dudt"):
         assert not torch.isnan(o[k][a]).any()
+
+
+# ------------------------------------------- entropy-conserving variant (R31)
+def test_c1_forces_entropy_variant(gu, c1):
+    """params.entropy = 1: dudt keeps the viscous heating of Eq. (18) only; accelerations,
+    mu_min, P and c are those of the full form."""
+    w = c1["w"]
+    d = c1["d"]
+    h32, rho32, om32 = (np.float32(c1[k]) for k in ("h", "rho", "om"))
+    th, trho, tom = (torch.from_numpy(a).cuda() for a in (h32, rho32, om32))
+    ctx = gu.make_ctx(w, entropy=1)
+    ctx.build_cells(d["x"], d["y"], d["z"], d["h"])
+    g = gu.run_forces(ctx, d, trho, th, tom)
+    op = dataclasses.replace(c1["op"], entropy=1)
+    o = orc.forces(w["x"], w["y"], w["z"], w["m"], w["vx"], w["vy"], w["vz"], w["u"], rho32, h32,
+                   om32, c1["ob"], op)
+    ea, eu = gu.force_errors(g, o)
+    assert ea.max() <= TOL_F, ea.max()
+    assert eu.max() <= TOL_F, eu.max()
+    assert (gu.np64(g["dudt"]) >= 0).all()          # viscous heating never cools
+    assert (gu.np64(g["dudt"]) > 0).any()
+    # the full form on the same inputs: identical accelerations, a different dudt
+    ctx0 = gu.make_ctx(w)
+    ctx0.build_cells(d["x"], d["y"], d["z"], d["h"])
+    g0 = gu.run_forces(ctx0, d, trho, th, tom)
+    for k in ("ax", "ay", "az", "mu_min", "P", "c"):
+        assert torch.equal(g[k], g0[k]), k
+    assert not torch.equal(g["dudt"], g0["dudt"])
+
+
+def test_isentropic_u_update(gu, c1):
+    """sph_isentropic_u against the oracle's u (rho_new/rho_old)^(gamma-1), ragged length,
+    density ratios from 1e-3 to 1e3; P / rho^gamma is unchanged."""
+    w = c1["w"]
+    ctx = gu.make_ctx(w)
+    n = 4096 - 37
+    rng = np.random.default_rng(11)
+    ro = np.float32(10.0 ** rng.uniform(-1.5, 1.5, n))
+    rn = np.float32(ro * 10.0 ** rng.uniform(-1.5, 1.5, n))
+    rn[:100] = ro[:100]                              # no compression: u untouched
+    u = np.float32(10.0 ** rng.uniform(-5, 2, n))
+    tu = torch.from_numpy(u.copy()).cuda()
+    ctx.isentropic_u(torch.from_numpy(ro).cuda(), torch.from_numpy(rn).cuda(), tu)
+    torch.cuda.synchronize()
+    gamma = float(np.float32(w["gamma"]))
+    ou = orc.isentropic_u(ro, rn, u, gamma)
+    gun = gu.np64(tu)
+    assert _rel(gun, ou).max() <= 2e-6, _rel(gun, ou).max()
+    assert np.array_equal(tu[:100].cpu().numpy(), u[:100])
+    A0 = u.astype(np.float64) * ro.astype(np.float64) ** (1.0 - gamma)
+    A1 = gun * rn.astype(np.float64) ** (1.0 - gamma)
+    assert _rel(A1, A0).max() <= 2e-6

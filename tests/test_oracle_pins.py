@@ -669,7 +669,7 @@ def test_marking_pass_is_the_union_of_the_pair_lists():
     assert (orc.mark_neighbors(w["x"], w["y"], w["z"], w["h"], more, box) >= got).all()
 
 
-# ------------------------------------------- entropy-conserving variant (R22)
+# ------------------------------------------- entropy-conserving variant (R31)
 def test_entropy_variant_keeps_the_viscous_heating_only(c1_forces):
     """PAPER.md:197 discards Eq. (14); Eq. (18) stays "active independent if the
     entropy conservation scheme is active or not".  Pinned through the (pinned) full form:
