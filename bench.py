@@ -36,13 +36,13 @@ KERNELS_PER_STEP = 11 + 3 + 6 + 2   # build_cells, density_h, forces, timestep k
 # sweep 27; per force pair 50 (AV branch not taken) or 70 (taken)
 FLOP_DENS, FLOP_FORCE, FLOP_FORCE_AV = 27.0, 50.0, 70.0
 # dram__bytes_read.sum + dram__bytes_write.sum per launch on sedov_128^3, from the ncu --set full
-# capture summarised in profiles/r1g_density_forces.md (k_density / k_forces)
-NCU_DRAM_BYTES = {"density_h": 159.0e6 + 780.1e6, "forces": 942.7e6 + 45.1e6}
+# capture summarised in profiles/r1h_density_forces.md (k_density / k_forces)
+NCU_DRAM_BYTES = {"density_h": 158.0e6 + 783.7e6, "forces": 941.9e6 + 43.6e6}
 # executed FP32 lane-operations per cycle (fadd + fmul + 2 ffma, predicated-on threads) over the
 # 148 x 128 x 2 the chip can retire, same capture: what the kernel executes, rejected candidates,
 # culling and Taylor/Halley bookkeeping included -- printed beside the useful (reject-free) fraction
-NCU_EXECUTED_FP32_FRAC = {"density_h": (933.4 + 1213.5 + 2 * 1134.3) / (148 * 128 * 2),
-                          "forces": (786.0 + 1747.8 + 2 * 1500.1) / (148 * 128 * 2)}
+NCU_EXECUTED_FP32_FRAC = {"density_h": (1013.1 + 1190.0 + 2 * 1101.9) / (148 * 128 * 2),
+                          "forces": (783.6 + 1742.4 + 2 * 1495.4) / (148 * 128 * 2)}
 
 def workloads_names():
     from paper_2511_11425_b200 import workloads
@@ -337,7 +337,7 @@ def run_gpu(a):
         roofline=dict(bound="alu", kernel=names[dom], achieved=ach, peak=NOMINAL_FP32_TFLOPS,
                       unit="TFLOP/s", frac=ach / NOMINAL_FP32_TFLOPS,
                       traffic=(NCU_DRAM_BYTES.get(names[dom]) if wname == "sedov_128^3" else None),
-                      traffic_source="profiles/r1g_density_forces.md (ncu --set full, bytes per launch)",
+                      traffic_source="profiles/r1h_density_forces.md (ncu --set full, bytes per launch)",
                       peak_source="derived: 148 SM x 128 FP32 lanes x 2 x 1.965 GHz",
                       measured_fma_peak=fma_peak, frac_of_measured_fma=ach / fma_peak,
                       useful_frac=ach / NOMINAL_FP32_TFLOPS,
