@@ -28,7 +28,9 @@
  * monotonicity, infinite-lattice density, momentum / energy / angular-momentum
  * conservation, Galilean / translation / permutation invariance, two-particle
  * and homologous-flow closed forms, static-gas dt, the entropy-conserving
- * variant (viscous heating alone conserves energy; P / rho^gamma invariant) --
+ * variant (viscous heating alone conserves energy; P / rho^gamma invariant),
+ * the block-step bookkeeping (ruler sequence, exact leap-frog under constant
+ * acceleration for any rung history) --
  * see tests/test_oracle_pins.py.  No function here is "parity unpinned".
  *
  * All arithmetic is double precision.  Inputs arrive as double arrays holding
@@ -687,6 +689,60 @@ void orc_drift(int64_t n, double dt, const double *v, double lo, double len, int
             if (xn >= lo + len) xn = lo;                    /* rounding at the upper face */
         }
         x[i] = xn;
+    }
+}
+
+/* ------------------------------------------------------------------------- *
+ * Block time steps, PAPER.md:229 ("each particle is integrated with a time
+ * step size that is a power-of-two fraction of the global timestep"), the
+ * substep of PAPER.md:231-261 per particle, rung changes of PAPER.md:270.
+ * Reading R32: time is counted in substeps of delta = dt0 / 2^R,
+ * R the deepest rung; a step of rung r spans L(r) = 2^(R-r) substeps.  Per
+ * particle: rung, tnext (the substep at which its running step ends, i.e. at
+ * which it is active next) and hk (the half-step length of its last opening
+ * kick; 0 before the first one), so that its v, u are those of the time
+ * tnext delta - hk.
+ * ------------------------------------------------------------------------- */
+
+/* the lowest rung whose steps begin at substep s ("moving to a lower rung is only
+ * possible on substeps that correspond to the rung it wants to move to") */
+int32_t orc_block_floor_rung(int64_t s, int32_t R)
+{
+    for (int32_t r = 0; r < R; r++)
+        if (s % ((int64_t)1 << (R - r)) == 0) return r;
+    return R;
+}
+
+/* Eqs. (19)-(20) for every particle, active or not (the sources of the force pass need
+ * predicted values too): from the time of its v, u to the time s delta of the substep */
+void orc_block_predict(int64_t n, int64_t s, double delta, const int32_t *tnext, const double *hk,
+                       const double *base, const double *rate, double *out)
+{
+    for (int64_t i = 0; i < n; i++) {
+        double tau = (double)(s - (int64_t)tnext[i]) * delta + hk[i];
+        out[i] = base[i] + tau * rate[i];
+    }
+}
+
+/* Step 4 of PAPER.md:245-259 for the particles whose step ends at substep s: closing kick
+ * over the old half step (Eqs. 21-22), rung change (up at once, down only as far as the
+ * substep allows, capped at R), opening kick over the new half step (Eqs. 23-24).
+ * q, rate: nq arrays of n values each, one after the other.                              */
+void orc_block_kick(int64_t n, int64_t s, int32_t R, double delta, const int32_t *rung_des,
+                    int32_t *rung, int32_t *tnext, double *hk, int32_t nq, double *q,
+                    const double *rate)
+{
+    int32_t fl = orc_block_floor_rung(s, R);
+    for (int64_t i = 0; i < n; i++) {
+        if ((int64_t)tnext[i] != s) continue;
+        for (int32_t k = 0; k < nq; k++) q[k * n + i] += hk[i] * rate[k * n + i];
+        int32_t r = rung_des[i] > fl ? rung_des[i] : fl;
+        if (r > R) r = R;
+        int64_t L = (int64_t)1 << (R - r);
+        hk[i] = 0.5 * (double)L * delta;
+        for (int32_t k = 0; k < nq; k++) q[k * n + i] += hk[i] * rate[k * n + i];
+        tnext[i] = (int32_t)(s + L);
+        rung[i] = r;
     }
 }
 

@@ -235,6 +235,39 @@ def drift(x, v, dt, lo, length, periodic):
     return x
 
 
+def block_floor_rung(s: int, R: int) -> int:
+    """Lowest rung whose steps begin at substep s (reading R32)."""
+    f = lib().orc_block_floor_rung
+    f.restype = C.c_int32
+    return int(f(C.c_int64(int(s)), C.c_int32(int(R))))
+
+
+def block_predict(s, delta, tnext, hk, base, rate):
+    """Eqs. (19)-(20) per particle at substep s: base + ((s - tnext) delta + hk) rate."""
+    tn = np.ascontiguousarray(tnext, np.int32)
+    hk, base, rate = _d(hk), _d(base), _d(rate)
+    out = np.empty_like(base)
+    lib().orc_block_predict(C.c_int64(len(base)), C.c_int64(int(s)), C.c_double(delta),
+                            _p(tn, C.c_int32), _p(hk), _p(base), _p(rate), _p(out))
+    return out
+
+
+def block_kick(s, R, delta, rung_des, rung, tnext, hk, q, rate):
+    """Closing kick, rung change, opening kick of the particles with tnext == s
+    (PAPER.md:245-259, 270).  q, rate: lists of arrays.  Returns (rung, tnext, hk, q)."""
+    rd = np.ascontiguousarray(rung_des, np.int32)
+    rg = np.ascontiguousarray(rung, np.int32).copy()
+    tn = np.ascontiguousarray(tnext, np.int32).copy()
+    hk = _d(hk).copy()
+    n, nq = len(rg), len(q)
+    qq = np.ascontiguousarray(np.stack([_d(a) for a in q]).reshape(-1))
+    rr = np.ascontiguousarray(np.stack([_d(a) for a in rate]).reshape(-1))
+    lib().orc_block_kick(C.c_int64(n), C.c_int64(int(s)), C.c_int32(int(R)), C.c_double(delta),
+                         _p(rd, C.c_int32), _p(rg, C.c_int32), _p(tn, C.c_int32), _p(hk),
+                         C.c_int32(nq), _p(qq), _p(rr))
+    return rg, tn, hk, [qq[k * n:(k + 1) * n].copy() for k in range(nq)]
+
+
 def imbalance(x, y, z, m, h, mat, box: Box, par: Params, alpha: float, targets=None):
     """Kernel imbalance I_i of Eq. (8) (brute force).  mat: int material ids or None."""
     x, y, z, m, h = map(_d, (x, y, z, m, h))

@@ -722,3 +722,74 @@ def test_isentropic_update_keeps_the_entropic_function():
     assert np.allclose(orc.isentropic_u(r1, r2, u1, gamma), orc.isentropic_u(r0, r2, u0, gamma), rtol=1e-13)
     assert np.array_equal(orc.isentropic_u(r0, r0, u0, gamma), u0)
     assert np.allclose(orc.isentropic_u(np.ones(3), np.full(3, 8.0), np.full(3, 0.75), 5.0 / 3.0), 3.0, rtol=1e-15)
+
+
+# ------------------------------------------- block time steps (reading R32)
+def test_block_floor_rung_is_the_ruler_sequence():
+    """With R = 3 a step of rung r spans 2^(3-r) substeps; the lowest rung whose steps begin
+    at substep s = 0..8 is 0 3 2 3 1 3 2 3 0 (written out by hand: 8 | s -> 0, 4 | s -> 1,
+    2 | s -> 2, odd -> 3).  R = 0: always 0."""
+    assert [orc.block_floor_rung(s, 3) for s in range(9)] == [0, 3, 2, 3, 1, 3, 2, 3, 0]
+    assert [orc.block_floor_rung(s, 0) for s in range(4)] == [0, 0, 0, 0]
+    assert orc.block_floor_rung(48, 5) == 1 and orc.block_floor_rung(40, 5) == 2
+
+
+def test_block_predict_hand_values():
+    """Eq. (19): an active particle (s = tnext) is predicted over its half step hk; an
+    inactive one over the part of it that has passed; before the first kick over nothing."""
+    tn = np.array([8, 8, 0, 16], np.int32)
+    hk = np.array([0.5, 0.5, 0.0, 1.0])
+    base = np.array([1.0, 1.0, 1.0, 1.0])
+    rate = np.array([2.0, 2.0, 2.0, -1.0])
+    #  s = 8, delta = 0.125: tau = 0.5 | 0.5 | 1.0 (8 substeps after a state at time 0) | 0
+    assert np.array_equal(orc.block_predict(8, 0.125, tn, hk, base, rate), [2.0, 2.0, 3.0, 1.0])
+    #  s = 5: tau = -3/8 + 1/2 = 1/8 | same | 5/8 | -11/8 + 1 = -3/8
+    assert np.array_equal(orc.block_predict(5, 0.125, tn, hk, base, rate), [1.25, 1.25, 2.25, 1.375])
+    assert np.array_equal(orc.block_predict(0, 0.125, tn[2:3], hk[2:3], base[2:3], rate[2:3]), [1.0])
+
+
+def test_block_steps_are_exact_under_constant_acceleration_for_any_rung_history():
+    """Closed form: with da/dt = 0 the kick-drift-kick leap-frog gives v = v0 + a t and
+    x = x0 + v0 t + a t^2 / 2 exactly, whatever the step sizes.  Particles change rungs at
+    random (seeded) while a stays fixed: (i) the predicted velocity of EVERY particle, active
+    or not, is v0 + a s delta at every substep; (ii) positions drifted with the half-step
+    velocities are on the parabola whenever a particle's own step ends; (iii) a particle's steps start at multiples of their own
+    length and never last longer than the rung asked for; (iv) with every
+    rung equal the scheme is the global-step one: hk = dt/2 for all.  A wrong half-step
+    length, a missed closing kick or a rung lowered too early fails (i) or (iii)."""
+    rng = np.random.default_rng(5)
+    n, R, dt0 = 64, 4, 0.5
+    delta = dt0 / 2 ** R
+    a = rng.normal(0, 1, n)
+    v0 = rng.normal(0, 1, n)
+    x0 = rng.normal(0, 1, n)
+    v, x = v0.copy(), x0.copy()
+    rung = np.zeros(n, np.int32)
+    tnext = np.zeros(n, np.int32)
+    hk = np.zeros(n)
+    seen_rungs = set()
+    for s in range(3 * 2 ** R):
+        t = s * delta
+        vp = orc.block_predict(s, delta, tnext, hk, v, a)
+        assert np.abs(vp - (v0 + a * t)).max() <= 1e-13
+        des = rng.integers(0, R + 3, n).astype(np.int32)          # some above the cap R
+        act = tnext == s
+        assert np.abs(x - (x0 + v0 * t + 0.5 * a * t * t))[act].max() <= 1e-12
+        assert act.any() and (s % 2 ** R != 0 or act.all())
+        old = rung.copy()
+        rung, tnext, hk, (v,) = orc.block_kick(s, R, delta, des, rung, tnext, hk, [v], [a])
+        L = 2 ** (R - rung)
+        assert np.array_equal(rung[~act], old[~act])
+        assert (rung[act] >= np.minimum(des[act], R)).all()       # never a longer step than asked
+        assert (rung[act] <= R).all()
+        assert (s % L[act] == 0).all()                            # steps start aligned
+        assert np.array_equal(tnext[act], s + L[act])
+        assert np.array_equal(hk[act], 0.5 * L[act] * delta)
+        seen_rungs |= set(rung.tolist())
+        x = x + delta * v                                         # Eq. (25), every particle
+    assert seen_rungs == set(range(R + 1))
+    # (iv) all on one rung: the global step
+    rung, tnext, hk, (v1,) = orc.block_kick(0, 2, 0.25, np.full(5, 1, np.int32), np.zeros(5, np.int32),
+                                            np.zeros(5, np.int32), np.zeros(5), [np.ones(5)], [np.full(5, 2.0)])
+    assert np.array_equal(hk, np.full(5, 0.25)) and np.array_equal(tnext, np.full(5, 2))
+    assert np.array_equal(v1, np.full(5, 1.5))                    # 1 + 0 * 2 + 0.25 * 2
