@@ -206,6 +206,39 @@ int  sph_drift(sph_ctx* ctx, int64_t n, const float* dt_device, float dt_scale, 
 int  sph_isentropic_u(sph_ctx* ctx, int64_t n, const float* rho_old, const float* rho_new,
                       float* u_inout);
 
+/* Block time steps, PAPER.md:229 ("each particle is integrated with a time step size that is a
+ * power-of-two fraction of the global timestep"), the substep of PAPER.md:231-261 per particle,
+ * rung changes of PAPER.md:270; bookkeeping of DESIGN.md reading R32.  Time is counted in
+ * substeps of delta = dt0 / 2^max_rung; a step of rung r spans 2^(max_rung - r) substeps.  Per
+ * particle (device arrays of n, caller order, owned by the caller): rung (int32), tnext (int32:
+ * the substep at which its running step ends; all 0 at the start) and hk (float: half-step
+ * length of its last opening kick; all 0 at the start).  Element-wise, asynchronous.
+ *   sph_block_predict  Eqs. (19)-(20) for EVERY particle (sources need predicted values too):
+ *                      q_pred = q + ((substep - tnext_i) delta + hk_i) dq/dt; for a particle
+ *                      whose step ends now this is the paper's dt_i / 2.
+ *   sph_block_active   active_i = (tnext_i == substep), the mask sph_set_active takes.
+ *   sph_block_kick     for those particles only: closing kick over hk_i (Eqs. 21-22), new rung
+ *                      min(max_rung, max(rung_desired_i, f)) with f the lowest rung whose steps
+ *                      begin at this substep ("moving to a lower rung is only possible on
+ *                      substeps that correspond to the rung it wants to move to"), opening kick
+ *                      over the new hk_i = 2^(max_rung - rung_i) delta / 2 (Eqs. 23-24), tnext_i
+ *                      += the new step.  rung_desired: the output of sph_rungs.  open = 0:
+ *                      the closing kick alone (v, u of the current time, e.g. for an
+ *                      output); hk_i becomes 0, tnext_i and rung_i stay: the starting state.
+ * max_rung <= 24; substep >= 0 (it may run past 2^max_rung: only substep mod 2^max_rung counts
+ * for f).  SPH_EINVAL on a NULL pointer or a bad scalar.                                      */
+int  sph_block_predict(sph_ctx* ctx, int64_t n, int32_t substep, float delta, const int32_t* tnext,
+                       const float* hk, const float* vx, const float* vy, const float* vz,
+                       const float* u, const float* ax, const float* ay, const float* az,
+                       const float* dudt, float* vx_pred, float* vy_pred, float* vz_pred,
+                       float* u_pred);
+int  sph_block_active(sph_ctx* ctx, int64_t n, int32_t substep, const int32_t* tnext,
+                      uint8_t* active);
+int  sph_block_kick(sph_ctx* ctx, int64_t n, int32_t substep, int32_t max_rung, float delta,
+                    const int32_t* rung_desired, int32_t* rung, int32_t* tnext, float* hk, float* vx,
+                    float* vy, float* vz, float* u, const float* ax, const float* ay,
+                    const float* az, const float* dudt, int32_t open);
+
 /* Diagnostic: CSR neighbour lists at a prescribed h, caller indices; a list is a set, the
  * order inside it is unspecified.
  * mode 0: j with r_ij < 2 h_i (self included); mode 1: j != i with r_ij < 2 max(h_i,h_j).

@@ -727,15 +727,18 @@ void orc_block_predict(int64_t n, int64_t s, double delta, const int32_t *tnext,
 /* Step 4 of PAPER.md:245-259 for the particles whose step ends at substep s: closing kick
  * over the old half step (Eqs. 21-22), rung change (up at once, down only as far as the
  * substep allows, capped at R), opening kick over the new half step (Eqs. 23-24).
- * q, rate: nq arrays of n values each, one after the other.                              */
+ * q, rate: nq arrays of n values each, one after the other.  open = 0: the closing kick
+ * alone (to bring v, u to the current time, e.g. for an output); hk becomes 0 and tnext
+ * stays s, the state in which a run starts.                                              */
 void orc_block_kick(int64_t n, int64_t s, int32_t R, double delta, const int32_t *rung_des,
                     int32_t *rung, int32_t *tnext, double *hk, int32_t nq, double *q,
-                    const double *rate)
+                    const double *rate, int32_t open)
 {
     int32_t fl = orc_block_floor_rung(s, R);
     for (int64_t i = 0; i < n; i++) {
         if ((int64_t)tnext[i] != s) continue;
         for (int32_t k = 0; k < nq; k++) q[k * n + i] += hk[i] * rate[k * n + i];
+        if (!open) { hk[i] = 0.0; continue; }   /* v, u now at the time s delta, as at the start */
         int32_t r = rung_des[i] > fl ? rung_des[i] : fl;
         if (r > R) r = R;
         int64_t L = (int64_t)1 << (R - r);

@@ -252,9 +252,10 @@ def block_predict(s, delta, tnext, hk, base, rate):
     return out
 
 
-def block_kick(s, R, delta, rung_des, rung, tnext, hk, q, rate):
+def block_kick(s, R, delta, rung_des, rung, tnext, hk, q, rate, open=1):
     """Closing kick, rung change, opening kick of the particles with tnext == s
-    (PAPER.md:245-259, 270).  q, rate: lists of arrays.  Returns (rung, tnext, hk, q)."""
+    (PAPER.md:245-259, 270); open=0: the closing kick alone.  q, rate: lists of arrays.
+    Returns (rung, tnext, hk, q)."""
     rd = np.ascontiguousarray(rung_des, np.int32)
     rg = np.ascontiguousarray(rung, np.int32).copy()
     tn = np.ascontiguousarray(tnext, np.int32).copy()
@@ -264,7 +265,7 @@ def block_kick(s, R, delta, rung_des, rung, tnext, hk, q, rate):
     rr = np.ascontiguousarray(np.stack([_d(a) for a in rate]).reshape(-1))
     lib().orc_block_kick(C.c_int64(n), C.c_int64(int(s)), C.c_int32(int(R)), C.c_double(delta),
                          _p(rd, C.c_int32), _p(rg, C.c_int32), _p(tn, C.c_int32), _p(hk),
-                         C.c_int32(nq), _p(qq), _p(rr))
+                         C.c_int32(nq), _p(qq), _p(rr), C.c_int32(int(open)))
     return rg, tn, hk, [qq[k * n:(k + 1) * n].copy() for k in range(nq)]
 
 

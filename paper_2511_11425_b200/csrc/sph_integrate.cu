@@ -57,6 +57,52 @@ __global__ void k_isentropic(int64_t n, float gm1, const float* __restrict__ rho
         u[i] *= powf(rho_new[i] / rho_old[i], gm1);
 }
 
+// ---- block time steps (reading R32) ----------------
+// Eqs. (19)-(20) for every particle: tau_i = (s - tnext_i) delta + hk_i
+__global__ void k_block_predict(int64_t n, Axpy4 a, int32_t s, float delta,
+                                const int32_t* __restrict__ tnext, const float* __restrict__ hk) {
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n;
+         i += (int64_t)gridDim.x * blockDim.x) {
+        const float tau = fmaf((float)(s - tnext[i]), delta, hk[i]);
+#pragma unroll
+        for (int k = 0; k < 4; ++k) a.out[k][i] = fmaf(tau, a.rate[k][i], a.base[k][i]);
+    }
+}
+
+__global__ void k_block_active(int64_t n, int32_t s, const int32_t* __restrict__ tnext,
+                               uint8_t* active) {
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n;
+         i += (int64_t)gridDim.x * blockDim.x)
+        active[i] = tnext[i] == s;
+}
+
+// closing kick (Eqs. 21-22), rung change, opening kick (Eqs. 23-24) of the particles whose
+// step ends at substep s
+__global__ void k_block_kick(int64_t n, Axpy4 a, int32_t s, int32_t R, int32_t floor_rung,
+                             float delta, const int32_t* __restrict__ rung_des, int32_t* rung,
+                             int32_t* tnext, float* hk, int32_t open) {
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n;
+         i += (int64_t)gridDim.x * blockDim.x) {
+        if (tnext[i] != s) continue;
+        const float   h0 = hk[i];
+        if (!open) {   // closing kick alone: v, u at the time of the substep, nothing pending
+#pragma unroll
+            for (int k = 0; k < 4; ++k) a.out[k][i] = fmaf(h0, a.rate[k][i], a.base[k][i]);
+            hk[i] = 0.0f;
+            continue;
+        }
+        const int32_t r  = min(R, max(rung_des[i], floor_rung));
+        const int32_t L  = 1 << (R - r);
+        const float   h1 = 0.5f * (float)L * delta;
+#pragma unroll
+        for (int k = 0; k < 4; ++k)
+            a.out[k][i] = fmaf(h1, a.rate[k][i], fmaf(h0, a.rate[k][i], a.base[k][i]));
+        hk[i]    = h1;
+        tnext[i] = s + L;
+        rung[i]  = r;
+    }
+}
+
 int launch_axpy(sph_ctx* c, int64_t n, const Axpy4& a, const float* dt, float scale) {
     int nblk = (int)((n + 255) / 256);
     if (nblk > c->sm_count * 16) nblk = c->sm_count * 16;
@@ -103,6 +149,52 @@ extern "C" int sph_isentropic_u(sph_ctx* c, int64_t n, const float* rho_old, con
     int nblk = (int)((n + 255) / 256);
     if (nblk > c->sm_count * 16) nblk = c->sm_count * 16;
     k_isentropic<<<nblk, 256, 0, c->stream>>>(n, c->par.gamma - 1.0f, rho_old, rho_new, u_inout);
+    SPH_CUDA_CHECK(c, cudaGetLastError());
+    return SPH_OK;
+}
+
+namespace {
+int block_grid(const sph_ctx* c, int64_t n) {
+    int nblk = (int)((n + 255) / 256);
+    return nblk > c->sm_count * 16 ? c->sm_count * 16 : nblk;
+}
+}  // namespace
+
+extern "C" int sph_block_predict(sph_ctx* c, int64_t n, int32_t substep, float delta,
+                                 const int32_t* tnext, const float* hk, const float* vx,
+                                 const float* vy, const float* vz, const float* u, const float* ax,
+                                 const float* ay, const float* az, const float* dudt, float* vx_pred,
+                                 float* vy_pred, float* vz_pred, float* u_pred) {
+    if (!c || n <= 0 || substep < 0 || !(delta > 0.0f) || !tnext || !hk || !vx || !vy || !vz || !u ||
+        !ax || !ay || !az || !dudt || !vx_pred || !vy_pred || !vz_pred || !u_pred)
+        return SPH_EINVAL;
+    Axpy4 a{{vx, vy, vz, u}, {ax, ay, az, dudt}, {vx_pred, vy_pred, vz_pred, u_pred}, 4};
+    k_block_predict<<<block_grid(c, n), 256, 0, c->stream>>>(n, a, substep, delta, tnext, hk);
+    SPH_CUDA_CHECK(c, cudaGetLastError());
+    return SPH_OK;
+}
+
+extern "C" int sph_block_active(sph_ctx* c, int64_t n, int32_t substep, const int32_t* tnext,
+                                uint8_t* active) {
+    if (!c || n <= 0 || substep < 0 || !tnext || !active) return SPH_EINVAL;
+    k_block_active<<<block_grid(c, n), 256, 0, c->stream>>>(n, substep, tnext, active);
+    SPH_CUDA_CHECK(c, cudaGetLastError());
+    return SPH_OK;
+}
+
+extern "C" int sph_block_kick(sph_ctx* c, int64_t n, int32_t substep, int32_t max_rung, float delta,
+                              const int32_t* rung_desired, int32_t* rung, int32_t* tnext, float* hk,
+                              float* vx, float* vy, float* vz, float* u, const float* ax,
+                              const float* ay, const float* az, const float* dudt, int32_t open) {
+    if (!c || n <= 0 || substep < 0 || max_rung < 0 || max_rung > 24 || !(delta > 0.0f) ||
+        !rung_desired || !rung || !tnext || !hk || !vx || !vy || !vz || !u || !ax || !ay || !az || !dudt)
+        return SPH_EINVAL;
+    // the lowest rung whose steps begin at this substep
+    int32_t fl = 0;
+    while (fl < max_rung && (substep & ((1 << (max_rung - fl)) - 1)) != 0) ++fl;
+    Axpy4 a{{vx, vy, vz, u}, {ax, ay, az, dudt}, {vx, vy, vz, u}, 4};
+    k_block_kick<<<block_grid(c, n), 256, 0, c->stream>>>(n, a, substep, max_rung, fl, delta,
+                                                          rung_desired, rung, tnext, hk, open);
     SPH_CUDA_CHECK(c, cudaGetLastError());
     return SPH_OK;
 }

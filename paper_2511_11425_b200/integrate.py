@@ -105,3 +105,88 @@ class Simulation:
         d = self.d
         m = d["m"].double()
         return [float((m * d[k].double()).sum().item()) for k in ("vx", "vy", "vz")]
+
+
+class BlockSimulation(Simulation):
+    """Block-time-step driver (reading R32): every particle
+    advances with dt0 / 2^rung, rung <= max_rung; time runs in substeps of delta = dt0 / 2^max_rung.
+
+    One substep s, in the paper's order (Figure 2):
+      1. density pass for all particles (with `fastgas`, on the substeps that do not start a
+         step of rung 0: marking pass, then the density of the marked particles only,
+         PAPER.md:276)                                      sph_build_cells, sph_density_h
+      2. prediction of v, u of every particle to the time of the substep   sph_block_predict
+      4. forces of the particles whose step ends now        sph_block_active, sph_set_active,
+                                                            sph_forces
+         their new desired rungs (Eq. 27 + limiter)         sph_timestep, sph_rungs
+         closing kick, rung change, opening kick            sph_block_kick
+      5. drift of all particles by delta                    sph_drift
+    Plumbing only; nothing is read back to the host inside a substep."""
+
+    def __init__(self, w: dict, dt0: float, max_rung: int, fastgas: bool = False, **params):
+        super().__init__(w, **params)
+        if self.entropy:
+            raise NotImplementedError("the entropy variant is wired into the global-step driver only")
+        if not 0 <= int(max_rung) <= 24:
+            raise ValueError("max_rung must be in 0..24")
+        n = self.n
+        self.dt0, self.max_rung = float(np.float32(dt0)), int(max_rung)
+        self.delta = float(np.float32(self.dt0 / 2 ** self.max_rung))
+        self.delta_dev = torch.full((1,), self.delta, dtype=torch.float32, device="cuda")
+        i32 = dict(dtype=torch.int32, device="cuda")
+        self.rung = torch.zeros(n, **i32)
+        self.rung_des = torch.zeros(n, **i32)
+        self.tnext = torch.zeros(n, **i32)
+        self.hk = torch.zeros(n, dtype=torch.float32, device="cuda")
+        self.active = torch.empty(n, dtype=torch.uint8, device="cuda")
+        self.mark = torch.empty(n, dtype=torch.uint8, device="cuda")
+        self.fastgas = bool(fastgas)
+        self.s = 0                              # substep counter (host integer, plumbing)
+        self.have_density = False
+
+    def _substep_derivatives(self):
+        d, o, c, s = self.d, self.out, self.ctx, self.s
+        c.block_active(s, self.tnext, self.active)
+        c.build_cells(d["x"], d["y"], d["z"], d["h"])
+        full = s % (1 << self.max_rung) == 0
+        if self.fastgas and self.have_density and not full:
+            c.mark_neighbors(self.active, self.mark)          # index holds the last pass's h
+            c.set_active(self.mark)
+        c.density_h(d["m"], d["h"], o["rho"], o["omega"], o["n_ngb"])
+        self.have_density = True
+        p = self.pred
+        c.block_predict(s, self.delta, self.tnext, self.hk, d["vx"], d["vy"], d["vz"], d["u"],
+                        o["ax"], o["ay"], o["az"], o["dudt"], p["vx"], p["vy"], p["vz"], p["u"])
+        c.set_active(self.active)
+        c.forces(d["m"], p["vx"], p["vy"], p["vz"], p["u"], o["rho"], d["h"], o["omega"], o["ax"],
+                 o["ay"], o["az"], o["dudt"], o["mu_min"], o["P"], o["c"])
+        c.timestep(d["h"], o["c"], o["ax"], o["ay"], o["az"], o["mu_min"], o["dt_i"], self.dt_new)
+        c.rungs(o["dt_i"], self.dt0, self.max_rung, self.rung_des)
+
+    def step(self, dt_cap=None):
+        """One substep of length delta."""
+        d, o, c = self.d, self.out, self.ctx
+        self._substep_derivatives()
+        c.block_kick(self.s, self.max_rung, self.delta, self.rung_des, self.rung, self.tnext,
+                     self.hk, d["vx"], d["vy"], d["vz"], d["u"], o["ax"], o["ay"], o["az"],
+                     o["dudt"])
+        c.drift(self.delta_dev, 1.0, d["x"], d["y"], d["z"], d["vx"], d["vy"], d["vz"])
+        self.s += 1
+        self.t += self.delta
+        self.steps += 1
+
+    def big_step(self):
+        """All substeps of one dt0; ends where every particle's step ends."""
+        for _ in range(1 << self.max_rung):
+            self.step()
+
+    def synchronise(self):
+        """At the end of a big step (every particle active): density, forces and the closing
+        kicks; v, u are then those of the current time and no kick is pending."""
+        if self.s % (1 << self.max_rung) != 0:
+            raise ValueError("synchronise() needs the end of a big step")
+        d, o, c = self.d, self.out, self.ctx
+        self._substep_derivatives()
+        c.block_kick(self.s, self.max_rung, self.delta, self.rung_des, self.rung, self.tnext,
+                     self.hk, d["vx"], d["vy"], d["vz"], d["u"], o["ax"], o["ay"], o["az"],
+                     o["dudt"], open=0)

@@ -20,7 +20,7 @@ SPH_OK, SPH_EINVAL, SPH_EBOX, SPH_ENOMEM, SPH_ECUDA, SPH_ESTALE, SPH_ENOSPC = 0,
 # every symbol include/sph.h declares (tests check the library exports exactly these)
 SYMBOLS = ["sph_create", "sph_destroy", "sph_build_cells", "sph_density_h", "sph_forces",
            "sph_timestep", "sph_rungs", "sph_set_active", "sph_mark_neighbors",
-           "sph_interface_correction", "sph_predict", "sph_kick", "sph_drift", "sph_isentropic_u", "sph_neighbors", "sph_stats", "sph_stats_reset", "sph_permutation",
+           "sph_interface_correction", "sph_predict", "sph_kick", "sph_drift", "sph_isentropic_u", "sph_block_predict", "sph_block_active", "sph_block_kick", "sph_neighbors", "sph_stats", "sph_stats_reset", "sph_permutation",
            "sph_fp32_peak", "sph_strerror", "sph_last_error"]
 
 
@@ -110,6 +110,9 @@ def load():
     lib.sph_kick.argtypes = [vp, i64, fp, C.c_float] + [fp] * 8
     lib.sph_drift.argtypes = [vp, i64, fp, C.c_float] + [fp] * 6
     lib.sph_isentropic_u.argtypes = [vp, i64, fp, fp, fp]
+    lib.sph_block_predict.argtypes = [vp, i64, i32, C.c_float] + [fp] * 14
+    lib.sph_block_active.argtypes = [vp, i64, i32, fp, fp]
+    lib.sph_block_kick.argtypes = [vp, i64, i32, i32, C.c_float] + [fp] * 12 + [i32]
     lib.sph_neighbors.argtypes = [vp, fp, i32, fp, fp, i64, C.POINTER(i64)]
     lib.sph_stats.argtypes = [vp, C.POINTER(_Stats)]
     lib.sph_stats_reset.argtypes = [vp]
@@ -251,6 +254,26 @@ class Sph:
         n, f = u.numel(), torch.float32
         self._check(self.lib.sph_isentropic_u(self._ctx, n, _ptr(rho_old, f, n), _ptr(rho_new, f, n),
                                               _ptr(u, f, n)))
+
+    # ---- block time steps (reading R32) ----------------------
+    def block_predict(self, s, delta, tnext, hk, vx, vy, vz, u, ax, ay, az, dudt, vxp, vyp, vzp, up):
+        n, f = vx.numel(), torch.float32
+        args = [_ptr(t, f, n) for t in (hk, vx, vy, vz, u, ax, ay, az, dudt, vxp, vyp, vzp, up)]
+        self._check(self.lib.sph_block_predict(self._ctx, n, int(s), float(delta),
+                                               _ptr(tnext, torch.int32, n), *args))
+
+    def block_active(self, s, tnext, active):
+        n = tnext.numel()
+        self._check(self.lib.sph_block_active(self._ctx, n, int(s), _ptr(tnext, torch.int32, n),
+                                              _ptr(active, torch.uint8, n)))
+
+    def block_kick(self, s, max_rung, delta, rung_des, rung, tnext, hk, vx, vy, vz, u, ax, ay, az,
+                   dudt, open=1):
+        n, f, i = vx.numel(), torch.float32, torch.int32
+        args = [_ptr(t, f, n) for t in (hk, vx, vy, vz, u, ax, ay, az, dudt)]
+        self._check(self.lib.sph_block_kick(self._ctx, n, int(s), int(max_rung), float(delta),
+                                            _ptr(rung_des, i, n), _ptr(rung, i, n),
+                                            _ptr(tnext, i, n), *args, int(open)))
 
     # ---- diagnostics --------------------------------------------------------------------
     def neighbors(self, h, mode=0):

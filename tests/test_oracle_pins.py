@@ -788,6 +788,12 @@ def test_block_steps_are_exact_under_constant_acceleration_for_any_rung_history(
         seen_rungs |= set(rung.tolist())
         x = x + delta * v                                         # Eq. (25), every particle
     assert seen_rungs == set(range(R + 1))
+    # closing kicks alone at the end of a big step: v itself is v0 + a t, nothing pending
+    s = 3 * 2 ** R
+    assert (tnext == s).all()
+    r2, t2, hk2, (vs,) = orc.block_kick(s, R, delta, rung, rung, tnext, hk, [v], [a], open=0)
+    assert np.abs(vs - (v0 + a * s * delta)).max() <= 1e-13
+    assert np.array_equal(r2, rung) and np.array_equal(t2, tnext) and not hk2.any()
     # (iv) all on one rung: the global step
     rung, tnext, hk, (v1,) = orc.block_kick(0, 2, 0.25, np.full(5, 1, np.int32), np.zeros(5, np.int32),
                                             np.zeros(5, np.int32), np.zeros(5), [np.ones(5)], [np.full(5, 2.0)])
