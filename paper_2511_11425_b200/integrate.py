@@ -123,7 +123,10 @@ class BlockSimulation(Simulation):
       5. drift of all particles by delta                    sph_drift
     Plumbing only; nothing is read back to the host inside a substep."""
 
-    def __init__(self, w: dict, dt0: float, max_rung: int, fastgas: bool = False, **params):
+    def __init__(self, w: dict, dt0: float, max_rung: int, fastgas: float = 0.0, **params):
+        """fastgas: 0 / False = off; a fraction in (0, 1] = use the marking pass on a substep when
+        the share of particles on its active rungs (rung histogram read once per big step, a
+        performance heuristic only: the results do not depend on it) is below it; True = 1."""
         super().__init__(w, **params)
         if self.entropy:
             raise NotImplementedError("the entropy variant is wired into the global-step driver only")
@@ -140,7 +143,8 @@ class BlockSimulation(Simulation):
         self.hk = torch.zeros(n, dtype=torch.float32, device="cuda")
         self.active = torch.empty(n, dtype=torch.uint8, device="cuda")
         self.mark = torch.empty(n, dtype=torch.uint8, device="cuda")
-        self.fastgas = bool(fastgas)
+        self.fastgas = float(fastgas)
+        self.rung_share = None                  # share of particles on rungs >= r, per r
         self.s = 0                              # substep counter (host integer, plumbing)
         self.have_density = False
 
@@ -148,8 +152,20 @@ class BlockSimulation(Simulation):
         d, o, c, s = self.d, self.out, self.ctx, self.s
         c.block_active(s, self.tnext, self.active)
         c.build_cells(d["x"], d["y"], d["z"], d["h"])
-        full = s % (1 << self.max_rung) == 0
-        if self.fastgas and self.have_density and not full:
+        sub = s % (1 << self.max_rung)
+        full = sub == 0
+        use_fastgas = False
+        if self.fastgas > 0.0 and self.have_density:
+            if full:
+                if self.fastgas < 1.0:    # one host read per big step
+                    pop = torch.bincount(self.rung, minlength=self.max_rung + 1).double().cpu().numpy()
+                    self.rung_share = np.cumsum(pop[::-1])[::-1] / max(pop.sum(), 1.0)
+            elif self.fastgas >= 1.0:
+                use_fastgas = True
+            elif self.rung_share is not None:
+                fl = self.max_rung - ((sub & -sub).bit_length() - 1)   # floor rung of the substep
+                use_fastgas = bool(self.rung_share[fl] < self.fastgas)
+        if use_fastgas:
             c.mark_neighbors(self.active, self.mark)          # index holds the last pass's h
             c.set_active(self.mark)
         c.density_h(d["m"], d["h"], o["rho"], o["omega"], o["n_ngb"])
