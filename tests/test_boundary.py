@@ -54,6 +54,10 @@ def test_error_strings_and_null_checks_without_a_device(lib):
     assert lib.sph_density_h(None, None, None, None, None, None) == -1
     assert lib.sph_create(None, None, None, 10, None) == -1
     assert lib.sph_fp32_peak(None, C.c_float(1.0), None) == -1
+    assert lib.sph_isentropic_u(None, 10, None, None, None) == -1
+    assert lib.sph_block_predict(None, 10, 0, C.c_float(0.1), *([None] * 14)) == -1
+    assert lib.sph_block_active(None, 10, 0, None, None) == -1
+    assert lib.sph_block_kick(None, 10, 0, 3, C.c_float(0.1), *([None] * 12), 1) == -1
 
 
 def test_binding_refuses_to_run_without_cuda():
