@@ -128,8 +128,6 @@ class BlockSimulation(Simulation):
         the share of particles on its active rungs (rung histogram read once per big step, a
         performance heuristic only: the results do not depend on it) is below it; True = 1."""
         super().__init__(w, **params)
-        if self.entropy:
-            raise NotImplementedError("the entropy variant is wired into the global-step driver only")
         if not 0 <= int(max_rung) <= 24:
             raise ValueError("max_rung must be in 0..24")
         n = self.n
@@ -170,6 +168,14 @@ class BlockSimulation(Simulation):
             c.set_active(self.mark)
         c.density_h(d["m"], d["h"], o["rho"], o["omega"], o["n_ngb"])
         self.have_density = True
+        if self.entropy:
+            # PAPER.md:197; entries the pass did not update (FastGas) hold the same density in
+            # both arrays, so their u stays as it is
+            if self.rho_prev is None:
+                self.rho_prev = torch.empty_like(o["rho"])
+            else:
+                c.isentropic_u(self.rho_prev, o["rho"], d["u"])
+            self.rho_prev.copy_(o["rho"])
         p = self.pred
         c.block_predict(s, self.delta, self.tnext, self.hk, d["vx"], d["vy"], d["vz"], d["u"],
                         o["ax"], o["ay"], o["az"], o["dudt"], p["vx"], p["vy"], p["vz"], p["u"])

@@ -364,3 +364,26 @@ def test_block_steps_on_the_sod_tube(gu, fastgas):
     exact, _, _ = _sod_exact(xc, t)
     l1 = np.abs(mean - exact).mean() / exact.mean()
     assert l1 <= 0.03, l1
+
+
+@pytest.mark.parametrize("fastgas", [0.0, 1.0])
+def test_block_steps_with_the_entropy_variant_keep_the_entropic_function(gu, fastgas):
+    """Block time steps + PAPER.md:197 without viscosity: u rho^(1-gamma) of every particle is
+    kept over two big steps of 8 substeps, on whatever rung it moves and whether its density
+    is refreshed on every substep or (FastGas) only when a neighbour is active."""
+    from paper_2511_11425_b200.integrate import BlockSimulation
+    w = dict(workloads.uniform_cube(nside=24, h_start="warm", v_sigma=0.3), av_alpha=0.0, av_beta=0.0)
+    gamma = float(np.float32(w["gamma"]))
+    sim = BlockSimulation(w, dt0=0.03, max_rung=3, fastgas=fastgas, entropy=1)
+    sim.synchronise()
+    A0 = gu.np64(sim.d["u"]) * gu.np64(sim.out["rho"]) ** (1.0 - gamma)
+    rho0 = gu.np64(sim.out["rho"]).copy()
+    for _ in range(2):
+        sim.big_step()
+    pop = np.bincount(sim.rung.cpu().numpy(), minlength=4)
+    sim.synchronise()
+    rho1 = gu.np64(sim.out["rho"])
+    A1 = gu.np64(sim.d["u"]) * rho1 ** (1.0 - gamma)
+    assert (pop > 0).sum() >= 2, pop
+    assert np.abs(rho1 / rho0 - 1).max() > 0.02
+    assert (np.abs(A1 - A0) / A0).max() <= 2e-5, (np.abs(A1 - A0) / A0).max()
