@@ -387,3 +387,59 @@ def test_block_steps_with_the_entropy_variant_keep_the_entropic_function(gu, fas
     assert (pop > 0).sum() >= 2, pop
     assert np.abs(rho1 / rho0 - 1).max() > 0.02
     assert (np.abs(A1 - A0) / A0).max() <= 2e-5, (np.abs(A1 - A0) / A0).max()
+
+
+def test_block_substeps_against_the_oracle_driven_evolution(gu):
+    """One big step of four substeps on mixed rungs (config 1 with fast random velocities), the
+    same sequence driven through the FP64 oracle: density of all, prediction of all, forces of
+    the particles whose step ends (brute force over those targets), Eq. (26), Eq. (27) +
+    limiter, closing kick / rung change / opening kick, drift.  Rungs and step ends must agree
+    exactly, the state within the tolerances of the global-step test."""
+    from paper_2511_11425_b200.integrate import BlockSimulation
+    w = workloads.uniform_cube(h_start="warm", v_sigma=0.3)
+    _, op = gu.make_params(w)
+    _, ob = gu.make_boxes(w)
+    R, dt0 = 2, float(np.float32(0.016))     # dt_i from 0.0058 to 0.0114: rungs 1 and 2
+    sim = BlockSimulation(w, dt0=dt0, max_rung=R)
+    delta = sim.delta
+    n = int(w["n"])
+    s = {k: w[k].astype(np.float64) for k in ("x", "y", "z", "m", "vx", "vy", "vz", "u", "h")}
+    a = {k: np.zeros(n) for k in ("ax", "ay", "az", "dudt")}
+    mu_min = np.zeros(n)
+    rung, tnext, hk = np.zeros(n, np.int32), np.zeros(n, np.int32), np.zeros(n)
+    kv, ka = ("vx", "vy", "vz", "u"), ("ax", "ay", "az", "dudt")
+    seen, partial = set(), 0
+    for sub in range(6):                              # one big step and two more substeps
+        sim.step()
+        act = np.flatnonzero(tnext == sub)
+        partial += 0 < len(act) < n
+        h, rho, om, _ = orc.density(s["x"], s["y"], s["z"], s["m"], s["h"], ob, op, cells=True)
+        vp = [orc.block_predict(sub, delta, tnext, hk, s[q], a[r]) for q, r in zip(kv, ka)]
+        o = orc.forces(s["x"], s["y"], s["z"], s["m"], vp[0], vp[1], vp[2], vp[3], rho, h, om, ob,
+                       op, targets=act)
+        for k in ka:
+            a[k][act] = o[k]
+        mu_min[act] = o["mu_min"]
+        _, c = orc.eos(rho, vp[3], op.gamma)
+        dt_i, _ = orc.timestep(h, c, a["ax"], a["ay"], a["az"], mu_min, op)
+        des = orc.rung_limiter(s["x"], s["y"], s["z"], h, orc.rungs(dt_i, dt0, R), ob)
+        rung, tnext, hk, q = orc.block_kick(sub, R, delta, des, rung, tnext, hk,
+                                            [s[k] for k in kv], [a[k] for k in ka])
+        for k, v in zip(kv, q):
+            s[k] = v
+        for d, (k, v) in enumerate(zip("xyz", ("vx", "vy", "vz"))):
+            s[k] = orc.drift(s[k], s[v], delta, ob.lo[d], ob.len[d], ob.periodic[d])
+        s["h"] = h
+        seen |= set(rung.tolist())
+        assert np.array_equal(sim.rung.cpu().numpy(), rung), (sub, int((sim.rung.cpu().numpy() != rung).sum()))
+        assert np.array_equal(sim.tnext.cpu().numpy(), tnext), sub
+    assert len(seen) >= 2, seen                       # more than one rung in use
+    assert partial >= 2                               # substeps with a partial active set
+    for d, k in enumerate("xyz"):
+        assert np.abs(_wrapdiff(gu.np64(sim.d[k]), s[k], 1.0, 1)).max() <= 5e-7
+    vscale = max(np.abs(s[k]).max() for k in ("vx", "vy", "vz"))
+    for k in ("vx", "vy", "vz"):
+        assert np.abs(gu.np64(sim.d[k]) - s[k]).max() <= 2e-5 * vscale
+    assert np.abs(gu.np64(sim.d["u"]) / s["u"] - 1).max() <= 2e-5
+    assert np.abs(gu.np64(sim.d["h"]) / s["h"] - 1).max() <= 1e-5
+    assert np.abs(gu.np64(sim.hk) - hk).max() <= 1e-7 * hk.max()
