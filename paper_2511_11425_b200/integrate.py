@@ -186,7 +186,7 @@ class BlockSimulation(Simulation):
         c.rungs(o["dt_i"], self.dt0, self.max_rung, self.rung_des)
 
     def step(self, dt_cap=None):
-        """One substep of length delta."""
+        """One substep of length delta (dt_cap is ignored: the substep length is fixed)."""
         d, o, c = self.d, self.out, self.ctx
         self._substep_derivatives()
         c.block_kick(self.s, self.max_rung, self.delta, self.rung_des, self.rung, self.tnext,
@@ -201,6 +201,15 @@ class BlockSimulation(Simulation):
         """All substeps of one dt0; ends where every particle's step ends."""
         for _ in range(1 << self.max_rung):
             self.step()
+
+    def run_until(self, t_end: float, max_steps: int = 100000):
+        """Whole big steps until t >= t_end (the end time is a multiple of dt0), then the
+        closing kicks."""
+        if self.s % (1 << self.max_rung) != 0:
+            raise ValueError("run_until() starts at the end of a big step")
+        while self.steps < max_steps and self.s * self.delta < t_end * (1.0 - 1e-12):
+            self.big_step()
+        self.synchronise()
 
     def synchronise(self):
         """At the end of a big step (every particle active): density, forces and the closing

@@ -344,10 +344,11 @@ def test_block_steps_on_the_sod_tube(gu, fastgas):
     sim = BlockSimulation(w, dt0=3.2e-3, max_rung=3, fastgas=fastgas)
     sim.synchronise()
     e0 = sum(sim.energies())
-    for _ in range(32):
+    for _ in range(31):
         sim.big_step()
     pop = np.bincount(sim.rung.cpu().numpy(), minlength=4)
-    sim.synchronise()
+    sim.run_until(0.1)                       # one more big step (to 32 dt0), then synchronise
+    assert sim.s == 32 * 8
     t = float(sim.t.item())
     assert abs(t - 0.1024) <= 1e-6
     e1 = sum(sim.energies())
