@@ -107,6 +107,13 @@ class Simulation:
         return [float((m * d[k].double()).sum().item()) for k in ("vx", "vy", "vz")]
 
 
+def floor_rung(substep: int, max_rung: int) -> int:
+    """Lowest rung whose steps begin at this substep: max_rung minus the number of
+    trailing zero bits of substep mod 2^max_rung; 0 at the start of a big step."""
+    sub = substep % (1 << max_rung)
+    return 0 if sub == 0 else max_rung - ((sub & -sub).bit_length() - 1)
+
+
 class BlockSimulation(Simulation):
     """Block-time-step driver (reading R32): every particle
     advances with dt0 / 2^rung, rung <= max_rung; time runs in substeps of delta = dt0 / 2^max_rung.
@@ -161,7 +168,7 @@ class BlockSimulation(Simulation):
             elif self.fastgas >= 1.0:
                 use_fastgas = True
             elif self.rung_share is not None:
-                fl = self.max_rung - ((sub & -sub).bit_length() - 1)   # floor rung of the substep
+                fl = floor_rung(s, self.max_rung)
                 use_fastgas = bool(self.rung_share[fl] < self.fastgas)
         if use_fastgas:
             c.mark_neighbors(self.active, self.mark)          # index holds the last pass's h

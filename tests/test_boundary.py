@@ -121,3 +121,13 @@ dist.destroy_process_group()
     r = subprocess.run(cmd, capture_output=True, text=True, timeout=300, cwd=ROOT)
     assert r.returncode == 0, r.stderr[-2000:]
     assert "VALUE 13.33" in r.stdout
+
+
+def test_driver_floor_rung_matches_the_oracle():
+    """Host logic of the block-step driver (which rungs a substep serves, for the FastGas
+    threshold) against the oracle's loop, all substeps of three big steps, R = 0..6."""
+    from oracle import sph_oracle as orc
+    from paper_2511_11425_b200.integrate import floor_rung
+    for R in range(7):
+        for s in range(3 * 2 ** R + 1):
+            assert floor_rung(s, R) == orc.block_floor_rung(s % 2 ** R, R) == orc.block_floor_rung(s, R)

@@ -367,7 +367,7 @@ def test_block_steps_on_the_sod_tube(gu, fastgas):
     assert l1 <= 0.03, l1
 
 
-@pytest.mark.parametrize("fastgas", [0.0, 1.0])
+@pytest.mark.parametrize("fastgas", [0.0, 0.5, 1.0])
 def test_block_steps_with_the_entropy_variant_keep_the_entropic_function(gu, fastgas):
     """Block time steps + PAPER.md:197 without viscosity: u rho^(1-gamma) of every particle is
     kept over two big steps of 8 substeps, on whatever rung it moves and whether its density
