@@ -9,7 +9,9 @@ One step, in the paper's order:
      closing kick of the previous step (its dt)               sph_kick             (Eqs. 21-22)
      opening kick of the new step (new dt)                    sph_kick             (Eqs. 23-24)
   5. drift                                                    sph_drift            (Eq. 25)
-(step 3, the interface correction, is not built.)  Between steps v and u live at the half step.
+Step 3, the interface correction (Eqs. 8-12), runs between 2 and 4 when `interface_alpha` is given
+(material ids from w["mat"], one material without it): sph_interface_correction on the predicted
+u, and the corrected density goes into the force pass.  Between steps v and u live at the half step.
 
 With `entropy=1` the force pass returns the viscous heating of Eq. (18) alone and,
 right after each density pass, u follows the isentrope from the previous pass's density to the new
@@ -26,8 +28,9 @@ _KEYS = ("x", "y", "z", "m", "vx", "vy", "vz", "u", "h")
 
 
 class Simulation:
-    def __init__(self, w: dict, **params):
+    def __init__(self, w: dict, interface_alpha: float | None = None, **params):
         n = int(w["n"])
+        self.interface_alpha = interface_alpha
         self.n = n
         self.d = {k: torch.from_numpy(np.ascontiguousarray(w[k], np.float32)).cuda() for k in _KEYS}
         self.ctx = sph.Sph(sph.Params(gamma=float(w["gamma"]), av_alpha=float(w["av_alpha"]),
@@ -42,6 +45,11 @@ class Simulation:
         self.dt_new = self.out["dt_min"]
         self.t = torch.zeros(1, dtype=torch.float64, device="cuda")
         self.steps = 0
+        if interface_alpha is not None:
+            self.mat = (torch.from_numpy(np.ascontiguousarray(w["mat"], np.int32)).cuda()
+                        if "mat" in w else None)
+            self.imbalance = torch.empty(n, **f)
+            self.rho_corr = torch.empty(n, **f)
         self.entropy = bool(params.get("entropy", 0))
         self.rho_prev = None                   # density of the previous pass (entropy variant)
 
@@ -59,7 +67,12 @@ class Simulation:
         p = self.pred
         c.predict(self.dt_prev, 1.0, d["vx"], d["vy"], d["vz"], d["u"], o["ax"], o["ay"], o["az"],
                   o["dudt"], p["vx"], p["vy"], p["vz"], p["u"])
-        c.forces(d["m"], p["vx"], p["vy"], p["vz"], p["u"], o["rho"], d["h"], o["omega"], o["ax"],
+        rho = o["rho"]
+        if self.interface_alpha is not None:      # step 3
+            c.interface_correction(d["m"], p["u"], o["rho"], d["h"], self.mat, self.interface_alpha,
+                                   self.imbalance, self.rho_corr)
+            rho = self.rho_corr
+        c.forces(d["m"], p["vx"], p["vy"], p["vz"], p["u"], rho, d["h"], o["omega"], o["ax"],
                  o["ay"], o["az"], o["dudt"], o["mu_min"], o["P"], o["c"])
         c.timestep(d["h"], o["c"], o["ax"], o["ay"], o["az"], o["mu_min"], o["dt_i"], self.dt_new)
         # closing kick of the step that ends here (Eqs. 21-22); a no-op before the first step
@@ -134,6 +147,8 @@ class BlockSimulation(Simulation):
         """fastgas: 0 / False = off; a fraction in (0, 1] = use the marking pass on a substep when
         the share of particles on its active rungs (rung histogram read once per big step, a
         performance heuristic only: the results do not depend on it) is below it; True = 1."""
+        if params.get("interface_alpha") is not None:
+            raise NotImplementedError("the interface correction is wired into the global-step driver only")
         super().__init__(w, **params)
         if not 0 <= int(max_rung) <= 24:
             raise ValueError("max_rung must be in 0..24")

@@ -444,3 +444,39 @@ def test_block_substeps_against_the_oracle_driven_evolution(gu):
     assert np.abs(gu.np64(sim.d["u"]) / s["u"] - 1).max() <= 2e-5
     assert np.abs(gu.np64(sim.d["h"]) / s["h"] - 1).max() <= 1e-5
     assert np.abs(gu.np64(sim.hk) - hk).max() <= 1e-7 * hk.max()
+
+
+def test_driver_with_the_interface_correction_pass(gu):
+    """Step 3 of PAPER.md:241 in the global-step driver, two materials split at x = 0.5 (and at
+    the periodic face).  One step = one force pass: the imbalance is non-zero within 2h of the
+    boundary and at the level of the lattice noise elsewhere, so the corrected density and
+    the velocities differ from the uncorrected run's near the boundary and hardly beyond 4h of
+    it.  With one uniform state the correction only smooths the lattice noise (below 5 % at the
+    boundary); with a 4:1 jump of u across it (P and T jump alike, so rho(P~, T~) moves little)
+    it acts somewhat more strongly, in the same place."""
+    from paper_2511_11425_b200.integrate import Simulation
+    w = workloads.uniform_cube(nside=32, h_start="warm", v_sigma=0.01)
+    w["mat"] = (w["x"] >= 0.5).astype(np.int32)
+    dist = np.minimum(np.abs(w["x"] - 0.5), np.minimum(w["x"], 1 - w["x"]))
+    far, near = dist > 0.2, dist < 0.03            # h = 0.04 here: 4h = 0.16
+
+    def run(ww, alpha):
+        sim = Simulation(ww, interface_alpha=alpha)
+        sim.step(dt_cap=2e-3)
+        return sim
+
+    def check(a, b):
+        ratio = gu.np64(b.rho_corr) / gu.np64(b.out["rho"]) - 1
+        imb = gu.np64(b.imbalance)
+        dv = np.abs(gu.np64(a.d["vx"]) - gu.np64(b.d["vx"]))
+        assert imb[near].mean() > 0.1 and imb[near].mean() > 5 * imb[far].max()
+        assert np.abs(ratio[far]).max() <= 1e-4          # e^(-I^2) of the lattice noise
+        assert dv[near].max() > 50 * dv[far].max(), (dv[near].max(), dv[far].max())
+        return np.abs(ratio[near]).max(), dv[near].max()
+
+    r1, dv1 = check(run(w, None), run(w, 1.5))
+    assert r1 <= 0.05
+    w2 = dict(w)
+    w2["u"] = np.where(w["x"] < 0.5, 4.0, 1.0).astype(np.float32)
+    r2, dv2 = check(run(w2, None), run(w2, 1.5))
+    assert r2 > r1 and dv2 > dv1, (r1, r2, dv1, dv2)
