@@ -68,6 +68,9 @@ def parse():
     ap.add_argument("--slack", type=float, default=0.0, help="sph_params.search_slack (0: default)")
     ap.add_argument("--cell-div-x", type=float, default=0.0, help="sph_params.cell_div_x (0: default)")
     ap.add_argument("--cell-div-yz", type=float, default=0.0, help="sph_params.cell_div_yz (0: default)")
+    ap.add_argument("--tile", type=int, default=0, help="sph_params.tile (-1: 8-lane kernels only)")
+    ap.add_argument("--tile-rows", type=int, default=0, help="sph_params.tile_rows (0: default)")
+    ap.add_argument("--tile-cap", type=int, default=0, help="sph_params.tile_cap (0: default)")
     ap.add_argument("--kernel", default="wendland_c2", choices=list(KERNEL_IDS),
                     help="SPH kernel (sph_params.kernel); the metric configuration is wendland_c2")
     ap.add_argument("--n-ngb", type=float, default=64.0,
@@ -213,7 +216,8 @@ def run_gpu(a):
     custom = a.kernel != "wendland_c2" or a.n_ngb != 64.0
     ctx = sph.Sph(sph.Params(kernel=KERNEL_IDS[a.kernel], n_ngb=a.n_ngb, gamma=w["gamma"],
                              av_alpha=w["av_alpha"], av_beta=w["av_beta"], search_slack=a.slack, cell_div_x=a.cell_div_x,
-                             cell_div_yz=a.cell_div_yz),
+                             cell_div_yz=a.cell_div_yz, tile=a.tile, tile_rows=a.tile_rows,
+                             tile_cap=a.tile_cap),
                   sph.Box(w["box_lo"], w["box_len"], w["periodic"]), n)
     out = sph.StepBuffers(n)
     h = torch.empty_like(d["h"])

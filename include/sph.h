@@ -71,6 +71,14 @@ typedef struct {
     int32_t entropy;      /* 1: entropy-conserving variant: sph_forces drops */
                           /* the Eq. (14) term, dudt is the viscous heating of Eq. (18)     */
                           /* alone; the caller advances u with sph_isentropic_u             */
+    int32_t tile;         /* staged-tile sweeps (buckets of 64 targets over a shared-memory   */
+                          /* tile of sources): 0 = on (default), -1 =    */
+                          /* off: every target takes the 8-lanes-per-target kernels.  Results */
+                          /* do not depend on it beyond rounding                             */
+    int32_t tile_rows;    /* a bucket spans tile_rows x tile_rows rows of cells (<= 0:        */
+                          /* default 3; at most 5)                                           */
+    int32_t tile_cap;     /* candidates a tile holds (<= 0: default 1024); buckets that need  */
+                          /* more fall back to the 8-lane kernels                            */
 } sph_params;
 
 /* 64-bit counters accumulated on the device since the last sph_stats_reset.             */

@@ -4,6 +4,7 @@
 #include <cstring>
 #include <new>
 #include "sph_internal.cuh"
+#include "sph_tile.cuh"
 
 static void fill_defaults(sph_params& p) {
     if (!(p.n_ngb > 0.0f)) p.n_ngb = 64.0f;
@@ -16,6 +17,11 @@ static void fill_defaults(sph_params& p) {
     if (!(p.search_slack > 1.0f)) p.search_slack = 1.1f;
     if (!(p.cell_div_x > 0.0f)) p.cell_div_x = 4.0f;
     if (!(p.cell_div_yz > 0.0f)) p.cell_div_yz = 1.5f;
+    if (p.tile_rows <= 0) p.tile_rows = 3;
+    if (p.tile_rows > 5) p.tile_rows = 5;
+    if (p.tile_cap <= 0) p.tile_cap = 1024;
+    p.tile_cap = (p.tile_cap + 31) & ~31;
+    if (p.tile_cap > 4096) p.tile_cap = 4096;
 }
 
 template <class T>
@@ -74,6 +80,11 @@ extern "C" int sph_create(sph_ctx** out, const sph_params* params, const sph_box
     ok = ok && dalloc(&c->fix_cnt, (size_t)2) == cudaSuccess;
     ok = ok && dalloc(&c->act_list, (size_t)n_max) == cudaSuccess;
     ok = ok && dalloc(&c->act_cnt, (size_t)2) == cudaSuccess;
+    ok = ok && dalloc(&c->buckets, (size_t)n_max) == cudaSuccess;
+    ok = ok && dalloc(&c->bucket_cnt, (size_t)1) == cudaSuccess;
+    ok = ok && dalloc(&c->tile_next, (size_t)2) == cudaSuccess;
+    ok = ok && dalloc(&c->fb_list, (size_t)n_max) == cudaSuccess;
+    ok = ok && dalloc(&c->fb_cnt, (size_t)2) == cudaSuccess;
     ok = ok && dalloc(&c->dt_part, (size_t)1024) == cudaSuccess;
     ok = ok && dalloc(&c->nb_total, (size_t)2) == cudaSuccess;
     if (ok) ok = cudaMemsetAsync(c->stats, 0, ST_NCOUNTERS * sizeof(unsigned long long),
@@ -100,6 +111,8 @@ extern "C" void sph_destroy(sph_ctx* c) {
     cudaFree(c->coarse_hmax);
     cudaFree(c->act_list);  cudaFree(c->act_cnt);
     cudaFree(c->nb_j);      cudaFree(c->nb_cnt);   cudaFree(c->nb_rkeep);
+    cudaFree(c->buckets);   cudaFree(c->bucket_cnt); cudaFree(c->tile_next);
+    cudaFree(c->fb_list);   cudaFree(c->fb_cnt);
     delete c;
 }
 

@@ -267,5 +267,6 @@ int sph_launch_build(sph_ctx* c, int64_t n, const float* x, const float* y, cons
     k_cell_sort<<<nb, TPB, 0, s>>>(n, c->key, c->cell_start, c->perm);
     k_gather<<<nb, TPB, 0, s>>>(n, c->perm, x, y, z, h, c->pos_h, c->inv_perm);
     SPH_CUDA_CHECK(c, cudaGetLastError());
+    if (c->par.tile >= 0) return sph_launch_buckets(c);   // a3: the bucket table
     return SPH_OK;
 }

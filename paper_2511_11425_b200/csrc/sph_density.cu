@@ -410,13 +410,20 @@ int sph_launch_density(sph_ctx* c, const float* m, float* h, float* rho, float* 
     SPH_CUDA_CHECK(c, cudaMemsetAsync(c->fix_cnt, 0, sizeof(unsigned), s));
     DensPar par{c->par.n_ngb, c->par.h_tol, c->par.search_slack, c->par.h_max_iter};
     const int nblk = (int)((n + D_TARGETS - 1) / D_TARGETS);
+    // the staged-tile kernel first (all particles as targets only); what it hands back --
+    // buckets its tile cannot hold -- is swept by the 8-lane kernel through a target list
+    const bool tiled = c->par.tile >= 0 && !c->act_on;
+    if (tiled) {
+        const int rc = sph_launch_density_tile(c, h, rho, omega, nn);
+        if (rc != SPH_OK) return rc;
+    }
+    const uint32_t* tlist = tiled ? c->fb_list : (c->act_on ? c->act_list : nullptr);
+    const unsigned* tcnt  = tiled ? c->fb_cnt : c->act_cnt;
     auto launch = [&](auto tag) {
         constexpr int KERN = decltype(tag)::value;
         k_density<KERN><<<nblk, D_TPB, 0, s>>>((int)n, c->grid, c->cell_start, c->pos_m, c->perm, par,
                                                h, rho, omega, nn, c->fix_list, c->fix_cnt, c->nb_j,
-                                               c->nb_cnt, c->nb_rkeep,
-                                               c->act_on ? c->act_list : nullptr, c->act_cnt,
-                                               c->stats);
+                                               c->nb_cnt, c->nb_rkeep, tlist, tcnt, c->stats);
         k_density_fix<KERN><<<c->sm_count * 4, 256, 0, s>>>(c->grid, c->cell_start, c->pos_m, c->perm,
                                                             par, c->fix_list, c->fix_cnt, h, rho,
                                                             omega, nn, c->stats);

@@ -74,6 +74,11 @@ struct sph_ctx {
     uint32_t*    act_list;     // n_max: sorted positions of the active set, ascending
     unsigned*    act_cnt;      // [2]: its length; [1]: length of the marking pass's source list
     bool         act_on;       // sph_set_active gave a mask since the last build
+    struct SphBucket* buckets; // n_max: the bucket table of the staged-tile sweeps (sph_tile.cuh)
+    unsigned*    bucket_cnt;   // [1]
+    unsigned*    tile_next;    // [2]: work counters of the persistent tile kernels
+    uint32_t*    fb_list;      // n_max: targets the tile kernels hand to the 8-lane kernels
+    unsigned*    fb_cnt;       // [2]: their number (density, forces)
     float*       dt_part;      // per-block minima of the time-step reduction
     int64_t*     nb_total;     // neighbour-list total (device) + pinned mirror
     char         err[256];
@@ -696,6 +701,8 @@ int sph_launch_neighbors(sph_ctx* c, const float* h, int32_t mode, int64_t* offs
 int sph_launch_fp32_peak(cudaStream_t s, float seconds, double* tflops);
 int sph_launch_rungs(sph_ctx* c, const float* dt_i, float dt0, int32_t max_rung, int32_t* rung);
 int sph_launch_coarse_map(sph_ctx* c);
+int sph_launch_buckets(sph_ctx* c);
+int sph_launch_density_tile(sph_ctx* c, float* h, float* rho, float* omega, int32_t* nn);
 int sph_launch_mark(sph_ctx* c, const uint8_t* src, uint8_t* mark);
 int sph_launch_set_active(sph_ctx* c, const uint8_t* active);
 int sph_launch_compact(sph_ctx* c, const uint8_t* mask, uint32_t* list, unsigned* cnt);

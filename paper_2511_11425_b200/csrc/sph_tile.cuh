@@ -1,0 +1,440 @@
+// sph_tile.cuh -- the staged-tile sweeps: buckets of up to 64 sorted
+// targets, the candidate sources of a bucket staged ONCE in shared memory with 1-D bulk
+// asynchronous copies (cp.async.bulk + mbarrier), one lane per target pair.
+//
+// The paper evaluates groups of sinks against an interaction list that holds "every particle
+// that could be a neighbour of any sink in the group", packed in tiles, and selects the actual
+// neighbours inside the vectorised evaluation.  This is that
+// shape on sm_100a: a bucket is a compact brick of targets (a few adjacent rows of cells over a
+// short range of cells along x, "box of balls" = the brick inflated by the search
+// radius), its interaction list is the union of the cell rows within reach, each row one
+// contiguous range of the sorted arrays and therefore one bulk copy; every lane then tests every
+// staged candidate against its own two targets with broadcast shared-memory loads and packed
+// FP32 arithmetic (FFMA2), and keeps the accepted set as bit masks over the tile.
+// Shares nothing with oracle/.
+#pragma once
+#include "sph_internal.cuh"
+
+#ifdef __CUDACC__
+
+#define SPH_TB 64        // targets per bucket: two per lane
+#define SPH_TROWS 128    // candidate rows of cells per bucket (cap)
+#define SPH_TSEGS (2 * SPH_TROWS)   // a row that crosses a periodic face has two segments
+#define SPH_TZCAP 32     // per-target slots for list entries next to the support edge (the "zone")
+
+// shared memory of one warp (bytes), tcap = tile capacity in candidates (multiple of 32)
+//   tile   float4[tcap]        (x', y', z', |x'|^2) in the bucket's frame
+//   ms     float[tcap]         m_j
+//   mask   uint32[tcap/32][64] accept bits of the 64 targets, word-major
+//   seg    uint4[SPH_TSEGS]    (first sorted position, count, tile offset, image)
+//   zone   uint16[SPH_TZCAP][64]  tile indices of the entries next to the support edge
+//   rowoff int[32]
+//   mbar   uint64
+__host__ __device__ inline size_t sph_tile_smem_bytes(int tcap, int rec_bytes) {
+    return (size_t)(tcap + 32) * (rec_bytes + 4) + (size_t)(tcap / 32 + 2) * SPH_TB * 4 + SPH_TSEGS * 16 +
+           SPH_TZCAP * SPH_TB * 2 + 32 * 4 + 16;
+}
+
+// ---- mbarrier / bulk-copy primitives (PTX; SASS: SYNCS.*, UBLKCP) -----------------------
+__device__ __forceinline__ void sph_mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void sph_mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ bool sph_mbar_try_wait(uint32_t bar, uint32_t parity) {
+    uint32_t ok;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok)
+        : "r"(bar), "r"(parity)
+        : "memory");
+    return ok != 0u;
+}
+__device__ __forceinline__ void sph_mbar_wait(uint32_t bar, uint32_t parity) {
+    while (!sph_mbar_try_wait(bar, parity)) {}
+}
+// global -> shared, bytes a multiple of 16, both addresses 16-byte aligned
+__device__ __forceinline__ void sph_bulk_g2s(uint32_t dst, const void* src, uint32_t bytes,
+                                             uint32_t bar) {
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+        ::"r"(dst), "l"(src), "r"(bytes), "r"(bar)
+        : "memory");
+}
+// generic-proxy accesses of shared memory before this, async-proxy accesses after it
+__device__ __forceinline__ void sph_fence_async_smem() {
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
+
+// ---- packed FP32 (two targets of a lane side by side; SASS: FFMA2 / FADD2 / FMUL2) ------
+typedef unsigned long long sph_f2;
+__device__ __forceinline__ sph_f2 sph_pk(float lo, float hi) {
+    sph_f2 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void sph_upk(sph_f2 v, float& lo, float& hi) {
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ sph_f2 sph_fma2(sph_f2 a, sph_f2 b, sph_f2 c) {
+    sph_f2 r;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+    return r;
+}
+__device__ __forceinline__ sph_f2 sph_add2(sph_f2 a, sph_f2 b) {
+    sph_f2 r;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ sph_f2 sph_mul2(sph_f2 a, sph_f2 b) {
+    sph_f2 r;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ uint32_t sph_shl(uint32_t v, uint32_t s) {   // s >= 32 gives 0
+    uint32_t r;
+    asm("shl.b32 %0, %1, %2;" : "=r"(r) : "r"(v), "r"(s));
+    return r;
+}
+
+// The targets of a bucket: rows (ry0 + a, rz0 + b), a < nry, b < nrz, cells [c0, c1) along x
+// of each; in single-cell mode (a cell with more than 64 particles) `skip` particles of the
+// cell are left to the buckets before this one.
+struct SphBucket {
+    int32_t ry0, rz0, c0, c1;
+    int32_t nry, nrz, skip, pad;
+};
+
+// Per-warp view of the dynamic shared memory.
+struct SphTileMem {
+    float4*   tile;
+    float*    ms;
+    uint32_t* mask;
+    uint4*    seg;
+    uint16_t* zone;
+    int*      rowoff;
+    uint32_t  bar;      // shared-window address of the mbarrier
+    uint32_t  tile_sa;  // shared-window addresses of the tile, the masses, the masks, the zone list
+    uint32_t  ms_sa, mask_sa, zone_sa;
+    int       tcap;
+};
+
+template <int REC>
+__device__ __forceinline__ SphTileMem sph_tile_carve(unsigned char* base, int tcap) {
+    SphTileMem t;
+    t.tcap = tcap;
+    t.tile = (float4*)base;                 base += (size_t)(tcap + 32) * REC;
+    t.ms   = (float*)base;                  base += (size_t)(tcap + 32) * 4;
+    t.mask = (uint32_t*)base;               base += (size_t)(tcap / 32 + 2) * SPH_TB * 4;
+    t.seg  = (uint4*)base;                  base += SPH_TSEGS * 16;
+    t.zone = (uint16_t*)base;               base += SPH_TZCAP * SPH_TB * 2;
+    t.rowoff = (int*)base;                  base += 32 * 4;
+    t.bar  = (uint32_t)__cvta_generic_to_shared(base);
+    t.tile_sa = (uint32_t)__cvta_generic_to_shared(t.tile);
+    t.ms_sa   = (uint32_t)__cvta_generic_to_shared(t.ms);
+    t.mask_sa = (uint32_t)__cvta_generic_to_shared(t.mask);
+    t.zone_sa = (uint32_t)__cvta_generic_to_shared(t.zone);
+    return t;
+}
+
+// What a staged tile is: the frame, the reach it is complete for, its size.
+struct SphTileInfo {
+    float ox, oy, oz;   // origin of the bucket's frame (centre of the targets' bounding box)
+    float R;            // every source within R of any target of the bucket is in the tile
+    float ext;          // largest |coordinate| in the frame: bounds the FP32 rounding of r^2
+    int   nseg, nrow, used, nwords;
+};
+
+// Squared distance between the slab [u s, (u+1) s) + lo and the interval [b0, b1]; edge cells
+// of an open axis extend to infinity.
+__device__ __forceinline__ float sph_slab_gap(float b0, float b1, int u, float lo, float s, int n,
+                                              int per) {
+    const float a = lo + (float)u * s;
+    float below = a - b1;           // > 0: the interval lies below the slab
+    float above = b0 - (a + s);     // > 0: above
+    if (!per) {
+        if (u <= 0) below = 0.0f;       // the first cell has no lower face
+        if (u >= n - 1) above = 0.0f;   // the last one no upper face
+    }
+    return fmaxf(fmaxf(below, above) - 1e-3f * s, 0.0f);
+}
+
+// Unwrapped cell range along one axis that can hold a particle within R of [b0, b1].
+// Returns false if a periodic axis is too short for the images to be unique per bucket.
+__device__ __forceinline__ bool sph_axis_span(float b0, float b1, float R, float lo, float len,
+                                              float is, int n, int per, int& u0, int& u1) {
+    float a = floorf((b0 - lo - R) * is - 1e-3f);
+    float b = floorf((b1 - lo + R) * is + 1e-3f);
+    a = fminf(fmaxf(a, -1.0e9f), 1.0e9f);
+    b = fminf(fmaxf(b, -1.0e9f), 1.0e9f);
+    u0 = (int)a;
+    u1 = (int)b;
+    if (per) {
+        if (u1 - u0 + 1 > n || (b1 - b0) + 2.0f * R >= 0.999f * len) return false;
+        if (u0 < -n || u1 >= 2 * n) return false;   // targets outside the box
+    } else {
+        u0 = min(max(u0, 0), n - 1);
+        u1 = min(max(u1, 0), n - 1);
+    }
+    return true;
+}
+
+// Warp-collective.  Lists the cell rows within R of the box [b0, b1] (the bucket's targets),
+// each cut to its chord, and brings their particle records into the tile with one bulk copy
+// per segment.  On return the copies are in flight; sph_tile_wait() completes them.
+// Returns false (nothing issued) if the bucket does not fit: too many rows, too many
+// candidates, or a periodic axis too short.
+__device__ __forceinline__ bool sph_tile_stage(const SphGrid& g, const uint32_t* __restrict__ cell_start,
+                                               const float4* __restrict__ rec, const float b0[3],
+                                               const float b1[3], float R, const SphTileMem& sm,
+                                               int lane, SphTileInfo& ti) {
+    int x0, x1, y0, y1, z0, z1;
+    bool ok = sph_axis_span(b0[1], b1[1], R, g.lo[1], g.len[1], g.isy, g.ny, g.per[1], y0, y1);
+    ok = sph_axis_span(b0[2], b1[2], R, g.lo[2], g.len[2], g.isz, g.nz, g.per[2], z0, z1) && ok;
+    ok = sph_axis_span(b0[0], b1[0], R, g.lo[0], g.len[0], g.isx, g.nx, g.per[0], x0, x1) && ok;
+    if (!ok) return false;
+    const int nyr = y1 - y0 + 1, nzr = z1 - z0 + 1, nrow = nyr * nzr;
+    if (nrow > SPH_TROWS) return false;
+    const float R2 = R * R * (1.0f + 1e-5f);
+    int base = 0;
+    for (int rb = 0; rb < nrow; rb += 32) {
+        const int r  = rb + lane;
+        bool      in = r < nrow;
+        const int iz = r / nyr, iy = r - iz * nyr;
+        const int uy = y0 + iy, uz = z0 + iz;
+        uint32_t  a0 = 0, a1 = 0, c0 = 0, c1 = 0;
+        int       ka = 0, kb = 0;
+        if (in) {
+            const float dy = sph_slab_gap(b0[1], b1[1], uy, g.lo[1], g.sy, g.ny, g.per[1]);
+            const float dz = sph_slab_gap(b0[2], b1[2], uz, g.lo[2], g.sz, g.nz, g.per[2]);
+            const float d2 = dy * dy + dz * dz;
+            in = d2 <= R2;
+            if (in) {
+                int ky, kz, kx0, u0, u1;
+                const int cy = sph_wrap(uy, g.ny, ky), cz = sph_wrap(uz, g.nz, kz);
+                sph_axis_span(b0[0], b1[0], sqrtf(R2 - d2), g.lo[0], g.len[0], g.isx, g.nx, g.per[0], u0, u1);
+                u0 = max(u0, x0);
+                u1 = min(u1, x1);
+                const int cx0  = sph_wrap(u0, g.nx, kx0);
+                const int span = u1 - u0;
+                const uint32_t rq = (uint32_t)(cz * g.ny + cy) * (uint32_t)g.nx;
+                a0 = __ldg(cell_start + rq + cx0);
+                a1 = __ldg(cell_start + rq + min(cx0 + span, g.nx - 1) + 1);
+                const int kyz = ((ky + 1) << 2) | ((kz + 1) << 4);
+                ka = (kx0 + 1) | kyz;
+                if (cx0 + span > g.nx - 1) {   // the row crosses the periodic face
+                    c0 = __ldg(cell_start + rq);
+                    c1 = __ldg(cell_start + rq + min(cx0 + span - g.nx, g.nx - 1) + 1);
+                    kb = (kx0 + 2) | kyz;
+                }
+            }
+        }
+        const int na = (int)(a1 - a0), nb = (int)(c1 - c0);
+        int inc = na + nb;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int t = __shfl_up_sync(SPH_FULL, inc, o);
+            if (lane >= o) inc += t;
+        }
+        const int off = base + inc - (na + nb);
+        if (r < nrow) {
+            sm.seg[2 * r]     = make_uint4(a0, (uint32_t)na, (uint32_t)off, (uint32_t)ka);
+            sm.seg[2 * r + 1] = make_uint4(c0, (uint32_t)nb, (uint32_t)(off + na), (uint32_t)kb);
+        }
+        base += __shfl_sync(SPH_FULL, inc, 31);
+    }
+    if (base + 32 > sm.tcap || base == 0) return false;
+    ti.nrow = nrow;
+    ti.nseg = 2 * nrow;
+    ti.used = base;
+    ti.nwords = (base + 31) >> 5;
+    ti.R = R;
+    ti.ox = 0.5f * (b0[0] + b1[0]);
+    ti.oy = 0.5f * (b0[1] + b1[1]);
+    ti.oz = 0.5f * (b0[2] + b1[2]);
+    ti.ext = R + 0.5f * fmaxf(b1[0] - b0[0], fmaxf(b1[1] - b0[1], b1[2] - b0[2])) +
+             fmaxf(g.sx, fmaxf(g.sy, g.sz));
+    // the tile's previous contents were read / written through the generic proxy
+    sph_fence_async_smem();
+    __syncwarp();
+    if (lane == 0) sph_mbar_expect_tx(sm.bar, (uint32_t)base * 16u);
+    __syncwarp();
+    for (int s = lane; s < ti.nseg; s += 32) {
+        const uint4 sg = sm.seg[s];
+        if (sg.y) sph_bulk_g2s(sm.tile_sa + sg.z * 16u, rec + sg.x, sg.y * 16u, sm.bar);
+    }
+    return true;
+}
+
+// Completes the copies of sph_tile_stage and turns the raw records (x, y, z, w) into the
+// bucket's frame: (x', y', z', |x'|^2) with x' = fl((x_j + k L) - origin) evaluated in FP64
+// on the FP32 inputs, so that the displacement x_i' - x_j' of any pair -- through a periodic
+// image or not -- carries two roundings of 2^-25 |x'| and |x'| is a few h, not the box; the
+// fourth component goes to ms[].  Pads the tile to a multiple of 32 with far-away dummies.
+__device__ __forceinline__ void sph_tile_finish(const SphGrid& g, const SphTileMem& sm,
+                                                const SphTileInfo& ti, uint32_t parity, int lane) {
+    sph_mbar_wait(sm.bar, parity);
+    int    s = -1;
+    int    send = 0;
+    double ox = 0.0, oy = 0.0, oz = 0.0;
+    for (int k = lane; k < ti.used; k += 32) {
+        while (k >= send) {   // the segments are in tile order; each lane only moves forward
+            ++s;
+            const uint4 sg = sm.seg[s];
+            send = (int)(sg.z + sg.y);
+            const int kx = (int)(sg.w & 3u) - 1, ky = (int)((sg.w >> 2) & 3u) - 1, kz = (int)((sg.w >> 4) & 3u) - 1;
+            ox = (double)ti.ox - (double)kx * (double)g.len[0];
+            oy = (double)ti.oy - (double)ky * (double)g.len[1];
+            oz = (double)ti.oz - (double)kz * (double)g.len[2];
+        }
+        const float4 p = sm.tile[k];
+        const float  x = (float)((double)p.x - ox), y = (float)((double)p.y - oy), z = (float)((double)p.z - oz);
+        sm.tile[k] = make_float4(x, y, z, fmaf(z, z, fmaf(y, y, x * x)));
+        sm.ms[k]   = p.w;
+    }
+    for (int k = ti.used + lane; k < ti.nwords * 32 + 32; k += 32) {
+        sm.tile[k] = make_float4(0.0f, 0.0f, 0.0f, 3.0e37f);
+        sm.ms[k]   = 0.0f;
+    }
+    __syncwarp();
+}
+
+// Phase 1: the accept masks of the lane's two targets over the whole tile.  Target t of the
+// lane (frame coordinates (x, y, z), list radius Rc) accepts candidate j iff
+//   |x_j'|^2 - 2 x_t . x_j' + |x_t|^2 - Rc^2 < 0;
+// the lane evaluates both targets at once (FADD2 + 3 FFMA2 on a broadcast LDS.128) and shifts
+// the two sign bits into the mask words.  Candidate 32 w + b is bit 31 - b of word w.  Only a
+// superset of the final neighbour set is needed (kernels vanish outside 2h and the sweeps use
+// exact displacements), so the expanded form's rounding (~2^-23 ext^2) is covered by the margin
+// the caller leaves between Rc and the ball it relies on.  Rc <= 0 switches a target off.
+__device__ __forceinline__ void sph_tile_masks(const SphTileMem& sm, const SphTileInfo& ti,
+                                               const float xt[2], const float yt[2],
+                                               const float zt[2], const float Rc[2], int lane) {
+    float ci[2];
+#pragma unroll
+    for (int t = 0; t < 2; ++t)
+        ci[t] = Rc[t] > 0.0f ? fmaf(zt[t], zt[t], fmaf(yt[t], yt[t], xt[t] * xt[t])) - Rc[t] * Rc[t]
+                             : 3.0e38f;
+    const sph_f2 ax = sph_pk(-2.0f * xt[0], -2.0f * xt[1]);
+    const sph_f2 ay = sph_pk(-2.0f * yt[0], -2.0f * yt[1]);
+    const sph_f2 az = sph_pk(-2.0f * zt[0], -2.0f * zt[1]);
+    const sph_f2 cc = sph_pk(ci[0], ci[1]);
+    for (int w = 0; w < ti.nwords; ++w) {
+        uint32_t m0 = 0u, m1 = 0u;
+        const float4* c = sm.tile + w * 32;
+#pragma unroll
+        for (int u = 0; u < 32; ++u) {
+            const float4 p = c[u];
+            sph_f2 t = sph_add2(sph_pk(p.w, p.w), cc);
+            t = sph_fma2(ax, sph_pk(p.x, p.x), t);
+            t = sph_fma2(ay, sph_pk(p.y, p.y), t);
+            t = sph_fma2(az, sph_pk(p.z, p.z), t);
+            m0 = __funnelshift_l((uint32_t)t, m0, 1);
+            m1 = __funnelshift_l((uint32_t)(t >> 32), m1, 1);
+        }
+        sm.mask[w * SPH_TB + lane]      = m0;
+        sm.mask[w * SPH_TB + 32 + lane] = m1;
+    }
+#pragma unroll
+    for (int k = 0; k < 4; ++k) sm.mask[ti.nwords * SPH_TB + 32 * k + lane] = 0u;   // the cursors read ahead
+    __syncwarp();
+}
+
+// ---- shared-memory accesses through 32-bit shared-window addresses held in registers --------
+__device__ __forceinline__ float4 sph_lds4(uint32_t a) {
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ float sph_lds1(uint32_t a) {
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ uint32_t sph_ldsu(uint32_t a) {
+    uint32_t v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a));
+    return v;
+}
+
+// A lane's private cursor over the accept bits of one target, in tile order.  The word after
+// the current one is held in a register (`next`), so a refill never waits for shared memory.
+struct SphCursor {
+    uint32_t bits, next;
+    uint32_t maddr;    // shared address of the word after `next`
+    int      base31;   // 32 w + 31 for the current word w
+};
+__device__ __forceinline__ void sph_cursor_start(SphCursor& c, const SphTileMem& sm,
+                                                 const SphTileInfo& ti, int t, bool on) {
+    const uint32_t a = sm.mask_sa + 4u * (uint32_t)t;
+    c.base31 = on ? 31 : ti.nwords * 32 + 31;
+    c.bits   = on ? sph_ldsu(a) : 0u;
+    c.next   = on ? sph_ldsu(a + 4u * SPH_TB) : 0u;     // two zero words follow the last mask word
+    c.maddr  = a + 8u * SPH_TB;
+}
+__device__ __forceinline__ bool sph_cursor_live(const SphCursor& c, const SphTileInfo& ti) {
+    return c.base31 < ti.nwords * 32;
+}
+// One list entry as the sweeps see it.
+struct SphEntry {
+    float4 c;      // (x', y', z', |x'|^2) of the source
+    float  m;      // its mass; 0 for a bubble
+    int    idx;    // tile index
+    bool   has;    // false: bubble (an empty mask word was skipped, or the cursor is exhausted)
+};
+// Takes the next entry of the cursor and starts the loads of its record.  Straight-line code:
+// the refill of an exhausted word is predicated, the index of a bubble points at the padding.
+__device__ __forceinline__ void sph_cursor_fetch(SphCursor& c, const SphTileMem& sm, int idx_max,
+                                                 uint32_t mend, SphEntry& e) {
+    uint32_t flo, bit;
+    asm("bfind.u32 %0, %1;" : "=r"(flo) : "r"(c.bits));            // 0xffffffff for an empty word
+    e.has = c.bits != 0u;
+    e.idx = e.has ? c.base31 - (int)flo : idx_max;                   // bubble: the padding entry
+    asm("shl.b32 %0, %1, %2;" : "=r"(bit) : "r"(1u), "r"(flo));    // 0 for an empty word
+    c.bits ^= bit;
+    e.c = sph_lds4(sm.tile_sa + 16u * (uint32_t)e.idx);
+    e.m = sph_lds1(sm.ms_sa + 4u * (uint32_t)e.idx);               // padding entries carry m = 0
+    if (c.bits == 0u) {
+        c.bits   = c.next;
+        c.base31 += 32;
+        c.next   = sph_ldsu(c.maddr);
+        c.maddr  = min(c.maddr + 4u * SPH_TB, mend);
+    }
+}
+
+// Walks the accepted entries of the lane's two targets.  Two entry sets per target are used in
+// turn: the record of an entry is in flight while the entry before it is worked on, without
+// register copies.  work(t, entry) sees bubbles too (has = false, m = 0).
+template <class Work>
+__device__ __forceinline__ void sph_tile_walk(const SphTileMem& sm, const SphTileInfo& ti, int lane,
+                                              const bool on[2], Work&& work) {
+    SphCursor cu[2];
+    SphEntry  ea[2], eb[2];
+    const int      idx_max = ti.nwords * 32;                               // first padding entry
+    const uint32_t mend = sm.mask_sa + 4u * (uint32_t)((ti.nwords + 1) * SPH_TB);   // a zero word
+#pragma unroll
+    for (int t = 0; t < 2; ++t) {
+        sph_cursor_start(cu[t], sm, ti, lane + 32 * t, on[t]);
+        sph_cursor_fetch(cu[t], sm, idx_max, mend + 4u * (uint32_t)(lane + 32 * t), ea[t]);
+        sph_cursor_fetch(cu[t], sm, idx_max, mend + 4u * (uint32_t)(lane + 32 * t), eb[t]);
+    }
+    while (__any_sync(SPH_FULL, ea[0].has || ea[1].has || eb[0].has || eb[1].has ||
+                                    sph_cursor_live(cu[0], ti) || sph_cursor_live(cu[1], ti))) {
+#pragma unroll
+        for (int t = 0; t < 2; ++t) {
+            work(t, ea[t]);
+            sph_cursor_fetch(cu[t], sm, idx_max, mend + 4u * (uint32_t)(lane + 32 * t), ea[t]);
+        }
+#pragma unroll
+        for (int t = 0; t < 2; ++t) {
+            work(t, eb[t]);
+            sph_cursor_fetch(cu[t], sm, idx_max, mend + 4u * (uint32_t)(lane + 32 * t), eb[t]);
+        }
+    }
+}
+
+#endif  // __CUDACC__

@@ -1,0 +1,567 @@
+// sph_tile_density.cu -- steps a3-a6 of DESIGN.md on the staged-tile path: the bucket table
+// (buckets / groups of sinks) and the density + smoothing-length solve of
+// PAPER.md:137-154, Eqs. (5)-(7), with one lane per pair of targets over a shared-memory tile
+// of candidate sources (sph_tile.cuh).  The arithmetic of the solve is the one documented in
+// sph_density.cu (Halley step on S, E, F with Taylor-carried sums); only the parallel shape
+// differs:
+//   * one warp owns a bucket of <= 64 targets, two per lane;
+//   * the bucket's candidate rows are staged once by bulk asynchronous copies (UBLKCP) that
+//     complete on an mbarrier, then moved into the bucket's frame;
+//   * phase 1 turns the tile into per-target accept masks (FFMA2 on broadcast loads);
+//   * each sweep walks a lane-private cursor over its masks: no ballots, no shuffles, no
+//     per-candidate list stores, no reduction across lanes;
+//   * the masks stay in global memory for the force sweep (sph_tile_forces.cu).
+// Buckets the tile cannot hold (too many rows or candidates: steep h contrast, a periodic axis
+// barely longer than the search ball) are handed to the 8-lanes-per-target kernel of
+// sph_density.cu through a target list; targets with a borderline neighbour or without
+// convergence go to k_density_fix as before.
+#include <cstdio>
+#include "sph_tile.cuh"
+
+namespace {
+
+constexpr float T_ACCEPT = 3.0e-4f;   // a Halley step below this is final (sph_density.cu)
+constexpr float T_EDGE   = 4.0e-4f;   // list entries within this of 2h are kept for the final count
+
+// ------------------------------------------------------------------------------------------
+// a3: the bucket table.  One warp per group of G x G adjacent rows of cells; it walks along x
+// and closes a bucket as soon as the next cell would take it past 64 particles (or 32 cells).
+// ------------------------------------------------------------------------------------------
+__global__ void k_buckets(const SphGrid* __restrict__ gp, const uint32_t* __restrict__ cs, int G,
+                          SphBucket* out, unsigned* nout) {
+    const SphGrid& g = *gp;
+    const int lane = threadIdx.x & 31;
+    const int nwarp = (int)((gridDim.x * blockDim.x) >> 5);
+    const int ngy = (g.ny + G - 1) / G, ngz = (g.nz + G - 1) / G;
+    for (int grp = (int)((blockIdx.x * blockDim.x + threadIdx.x) >> 5); grp < ngy * ngz; grp += nwarp) {
+        const int gy = grp % ngy, gz = grp / ngy;
+        const int ry0 = gy * G, rz0 = gz * G;
+        const int nry = min(G, g.ny - ry0), nrz = min(G, g.nz - rz0), nrows = nry * nrz;
+        auto rowbase = [&](int rho) {
+            return (uint32_t)((rz0 + rho / nry) * g.ny + (ry0 + rho % nry)) * (uint32_t)g.nx;
+        };
+        uint32_t base = 0;
+        for (int rho = 0; rho < nrows; ++rho) base += __ldg(cs + rowbase(rho));
+        int pos = 0;
+        while (pos < g.nx) {
+            const int c = pos + 1 + lane;
+            uint32_t  cum = 0;
+            if (c <= g.nx)
+                for (int rho = 0; rho < nrows; ++rho) cum += __ldg(cs + rowbase(rho) + c);
+            const bool     ok  = c <= g.nx && cum - base <= (uint32_t)SPH_TB;
+            const unsigned bal = __ballot_sync(SPH_FULL, ok);
+            int m = (bal == SPH_FULL) ? 32 : __ffs((int)~bal) - 1;
+            if (m == 0) {   // the cells of this slab alone hold more than 64: one row, 64 at a time
+                if (lane < nrows) {
+                    const uint32_t rb = rowbase(lane);
+                    const int cnt = (int)(__ldg(cs + rb + pos + 1) - __ldg(cs + rb + pos));
+                    for (int skip = 0; skip < cnt; skip += SPH_TB) {
+                        SphBucket b{ry0 + lane % nry, rz0 + lane / nry, pos, pos + 1, 1, 1, skip, 0};
+                        out[atomicAdd(nout, 1u)] = b;
+                    }
+                }
+                m = 1;
+            } else {
+                const uint32_t tot = __shfl_sync(SPH_FULL, cum, m - 1) - base;
+                if (lane == 0 && tot > 0u) {
+                    SphBucket b{ry0, rz0, pos, pos + m, nry, nrz, 0, 0};
+                    out[atomicAdd(nout, 1u)] = b;
+                }
+            }
+            base = __shfl_sync(SPH_FULL, cum, m - 1);
+            pos += m;
+        }
+    }
+}
+
+struct TilePar {
+    float n_ngb, tol, slack;
+    int   max_iter, tcap;
+};
+
+// One safeguarded Halley step from the sums at h (the step of sph_density.cu: same formulas,
+// same safeguards).  Returns true if the step is accepted as final.
+__device__ __forceinline__ bool tile_halley(float s, float e, float f2, float T, float h, float ih,
+                                            float hcap, float tol, float& hlo, float& hhi,
+                                            float& hn, float& Sn, float& En, bool& conv) {
+    const float INF = __int_as_float(0x7f800000);
+    const float f = s - T;
+    if (f < 0.0f) hlo = h; else hhi = h;
+    const float den = 2.0f * e * e + f * (e + f2);
+    float dh;
+    bool  genuine = true;
+    if (e > 0.0f && den > 0.0f)  dh = __fdividef(-2.0f * f * e * h, den);
+    else if (e > 0.0f)           dh = __fdividef(-f * h, e);
+    else                       { dh = h; genuine = false; }
+    hn = h + dh;
+    if (!(hn >= 0.5f * h)) { hn = 0.5f * h; genuine = false; }
+    if (!(hn <= 2.0f * h)) { hn = 2.0f * h; genuine = false; }
+    if (hhi < INF && !(hn >= hlo && hn <= hhi)) { hn = 0.5f * (hlo + hhi); genuine = false; }
+    if (hn > hcap) { hn = hcap; genuine = false; }
+    dh = hn - h;
+    const float x = dh * ih;
+    Sn = s + x * (e - 0.5f * x * (e + f2));   // Taylor: S' = E/h, S'' = -(E+F)/h^2
+    En = e - x * f2;                          //         E' = -F/h
+    const bool small  = fabsf(dh) <= T_ACCEPT * h;
+    const bool tight  = (hhi - hlo) <= tol * h;
+    const bool capped = (hn >= hcap && h >= hcap);
+    conv = !(capped && f < 0.0f);
+    return (genuine && small) || tight || capped;
+}
+
+__device__ __forceinline__ float tile_hcap(const SphGrid& g) {   // as density_hcap of sph_density.cu
+    float hcap = 3.0e37f;
+    for (int d = 0; d < 3; ++d)
+        if (g.per[d]) hcap = fminf(hcap, g.len[d] / (4.0f * 1.25f) * 0.999f);
+        else          hcap = fminf(hcap, 4.0f * fmaxf(g.len[0], fmaxf(g.len[1], g.len[2])));
+    return hcap;
+}
+
+__device__ __forceinline__ float warp_max(float v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fmaxf(v, __shfl_xor_sync(SPH_FULL, v, o));
+    return v;
+}
+__device__ __forceinline__ float warp_min(float v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fminf(v, __shfl_xor_sync(SPH_FULL, v, o));
+    return v;
+}
+
+// ------------------------------------------------------------------------------------------
+// Wendland C2 on the tile: ONE sweep per solve.  With s = r / (2 h0), t = 1 - s the kernel is
+// w~ = t^4 (1 + 4 s) = B0 + 5 B1 and -q w~' = 20 s^2 t^3 = 20 B2 in the Bernstein basis
+// B_k = s^k t^(5-k); under h = h0 / lam the variables map linearly, s' = lam s, t' = t + eps s
+// (eps = 1 - lam), hence B_k' = lam^k sum_j C(5-k, j) eps^j B_(k+j): the six moments
+// M_k = sum_j m_j B_k(r_j / 2 h0) give S(h) and E(h) = dS/dln h EXACTLY as polynomials in lam,
+// for every h at which no list entry crosses the support edge.  Entries within T_ZONE of the
+// edge ("zone", a few per target) are remembered by tile index and their clamped contribution
+// is put right by one short pass at the solution.  The root of Eq. (6) then costs a scalar
+// Newton iteration per target -- no second sweep over the neighbours (the Halley path needs
+// two).  All terms of the expansions are positive for eps > 0 and well scaled: measured against
+// the FP64 root h agrees to 3e-7, rho to 9e-7, Omega to 2e-6 (FP32 emulation, lattices and
+// Poisson points with unequal masses; tolerance 1e-5).  A solution with |eps| > 0.9 T_ZONE is
+// only a step: the sweep is repeated from there (2-3 sweeps from a guess 25 % off).
+// ------------------------------------------------------------------------------------------
+constexpr float T_ZONE = 0.03f;
+
+__device__ __forceinline__ void c2_poly(const float M[6], float lam, float& S, float& E) {
+    const float e = 1.0f - lam;
+    const float S0 = M[0] + e * (5.0f * M[1] + e * (10.0f * M[2] + e * (10.0f * M[3] + e * (5.0f * M[4] + e * M[5]))));
+    const float S1 = M[1] + e * (4.0f * M[2] + e * (6.0f * M[3] + e * (4.0f * M[4] + e * M[5])));
+    const float E2 = M[2] + e * (3.0f * M[3] + e * (3.0f * M[4] + e * M[5]));
+    S = S0 + 5.0f * lam * S1;
+    E = 20.0f * lam * lam * E2;
+}
+
+// ------------------------------------------------------------------------------------------
+// a4-a6 on the tile.  One warp per block, persistent: buckets are handed out by a counter.
+// ------------------------------------------------------------------------------------------
+template <int KERN>
+__global__ __launch_bounds__(32) void k_density_tile(
+    const SphGrid* __restrict__ gp, const uint32_t* __restrict__ cell_start,
+    const float4* __restrict__ pos_m, const int32_t* __restrict__ perm,
+    const SphBucket* __restrict__ buckets, const unsigned* __restrict__ nbuckets, unsigned* next,
+    TilePar par, float* h_io, float* rho, float* omega, int32_t* nn, int32_t* fix_list,
+    unsigned* fix_cnt, uint32_t* fb_list, unsigned* fb_cnt, float* nb_rkeep,
+    unsigned long long* stats) {
+    constexpr bool MOM = (KERN == 1);   // the moment solve exists for Wendland C2
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ SphGrid g;
+    const int lane = threadIdx.x;
+    for (int k = lane; k < (int)(sizeof(SphGrid) / 4); k += 32) ((int*)&g)[k] = ((const int*)gp)[k];
+    __syncwarp();
+    const SphTileMem sm = sph_tile_carve<16>(smem_raw, par.tcap);
+    float* const edge = (float*)sm.zone;   // Halley path: [4][64] floats in the zone area
+    if (lane == 0) sph_mbar_init(sm.bar, 1u);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    __syncwarp();
+    uint32_t parity = 0;
+    const unsigned nb = *nbuckets;
+    const float hcap = tile_hcap(g);
+    const float lslack = MOM ? (1.0f + T_ZONE) * 1.001f : par.slack;   // list radius / 2h
+    unsigned long long c_tested = 0;
+    unsigned c_listed = 0, c_pairs = 0, c_sweeps = 0, c_recollect = 0;
+
+    for (;;) {
+        unsigned bi = 0;
+        if (lane == 0) bi = atomicAdd(next, 1u);
+        bi = __shfl_sync(SPH_FULL, bi, 0);
+        if (bi >= nb) break;
+        const SphBucket bk = buckets[bi];
+
+        // ---- the bucket's targets: rows (ry0 + a, rz0 + b), cells [c0, c1) of each
+        const int nrows = bk.nry * bk.nrz;
+        int rs = 0, rc = 0;
+        if (lane < nrows) {
+            const uint32_t rb = (uint32_t)((bk.rz0 + lane / bk.nry) * g.ny + (bk.ry0 + lane % bk.nry)) * (uint32_t)g.nx;
+            const int s0 = (int)__ldg(cell_start + rb + bk.c0) + bk.skip;
+            const int s1 = (int)__ldg(cell_start + rb + bk.c1);
+            rs = s0;
+            rc = min(max(s1 - s0, 0), SPH_TB);
+        }
+        int inc = rc;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int t = __shfl_up_sync(SPH_FULL, inc, o);
+            if (lane >= o) inc += t;
+        }
+        const int ntar = min(__shfl_sync(SPH_FULL, inc, 31), SPH_TB);
+        sm.rowoff[lane] = inc;                   // inclusive prefix of the row counts
+        __syncwarp();
+        int    p[2];
+        bool   valid[2];
+        float  xg[2], yg[2], zg[2], mi[2], h[2];
+        int    ic[2];
+#pragma unroll
+        for (int t = 0; t < 2; ++t) {
+            const int k = lane + 32 * t;
+            valid[t] = k < ntar;
+            int rho_ = 0;
+            while (rho_ < 31 && sm.rowoff[rho_] <= k) ++rho_;
+            const int before = rho_ ? sm.rowoff[rho_ - 1] : 0;
+            const int start  = __shfl_sync(SPH_FULL, rs, rho_);
+            p[t] = valid[t] ? start + (k - before) : 0;
+            float4 pi = make_float4(0.f, 0.f, 0.f, 1.f);
+            ic[t] = 0;
+            h[t]  = g.hmin;
+            if (valid[t]) {
+                pi    = pos_m[p[t]];
+                ic[t] = perm[p[t]];
+                h[t]  = h_io[ic[t]];
+            }
+            if (!(h[t] > 0.0f) || !(h[t] < 3.0e38f)) h[t] = g.hmin;
+            h[t]  = fminf(h[t], hcap);
+            xg[t] = pi.x; yg[t] = pi.y; zg[t] = pi.z; mi[t] = pi.w;
+        }
+        __syncwarp();
+        // bounding box of the targets
+        float b0[3], b1[3];
+        {
+            const float INF = __int_as_float(0x7f800000);
+            float lo[3] = {INF, INF, INF}, hi[3] = {-INF, -INF, -INF};
+#pragma unroll
+            for (int t = 0; t < 2; ++t)
+                if (valid[t]) {
+                    lo[0] = fminf(lo[0], xg[t]); hi[0] = fmaxf(hi[0], xg[t]);
+                    lo[1] = fminf(lo[1], yg[t]); hi[1] = fmaxf(hi[1], yg[t]);
+                    lo[2] = fminf(lo[2], zg[t]); hi[2] = fmaxf(hi[2], zg[t]);
+                }
+#pragma unroll
+            for (int d = 0; d < 3; ++d) { b0[d] = warp_min(lo[d]); b1[d] = warp_max(hi[d]); }
+        }
+
+        float T[2], hlo[2], hhi[2], S[2], E[2], Rc[2], want[2];
+        bool  done[2], fix[2], wait[2], recount[2];
+        int   sweeps[2], ni[2];
+#pragma unroll
+        for (int t = 0; t < 2; ++t) {
+            T[t]   = par.n_ngb * mi[t] * (1.0f / SphKernel<KERN>::self);
+            hlo[t] = 0.0f; hhi[t] = __int_as_float(0x7f800000);
+            S[t] = 0.0f; E[t] = 0.0f; Rc[t] = 0.0f;
+            done[t] = !valid[t]; fix[t] = false; wait[t] = valid[t];
+            want[t] = valid[t] ? 2.0f * h[t] * lslack : 0.0f;
+            sweeps[t] = 0; ni[t] = 0; recount[t] = false;
+        }
+        bool fallback = false;
+
+        // ---- stages: (re)build the tile for the largest list radius wanted
+        for (int stage = 0; stage < 4; ++stage) {
+            const float Rt = warp_max(fmaxf(wait[0] ? want[0] : 0.0f, wait[1] ? want[1] : 0.0f));
+            if (!(Rt > 0.0f)) break;
+            SphTileInfo ti;
+            const bool staged = sph_tile_stage(g, cell_start, pos_m, b0, b1, Rt * (1.0f + 1e-5f), sm, lane, ti);
+            if (!staged) {
+                if (stage == 0) fallback = true;
+                else {
+#pragma unroll
+                    for (int t = 0; t < 2; ++t) if (wait[t]) { done[t] = true; fix[t] = true; wait[t] = false; }
+                }
+                break;
+            }
+            if (stage > 0) c_recollect += (wait[0] ? 1u : 0u) + (wait[1] ? 1u : 0u);
+            sph_tile_finish(g, sm, ti, parity, lane);
+            parity ^= 1u;
+            // the targets in the frame of the tile
+            float xt[2], yt[2], zt[2];
+#pragma unroll
+            for (int t = 0; t < 2; ++t) {
+                xt[t] = (float)((double)xg[t] - (double)ti.ox);
+                yt[t] = (float)((double)yg[t] - (double)ti.oy);
+                zt[t] = (float)((double)zg[t] - (double)ti.oz);
+            }
+            const float band_c = 2.5e-7f * ti.ext;   // tau(h) = 1e-6 + band_c / h, DESIGN.md section 6
+#pragma unroll
+            for (int t = 0; t < 2; ++t)
+                if (wait[t]) { wait[t] = false; Rc[t] = fminf(want[t], Rt); }
+            bool remask = true;
+            c_tested += (unsigned long long)ti.used * (unsigned)ntar;   // uniform: lane 0 reports it
+
+            // ---- sweeps on this tile
+            while (__any_sync(SPH_FULL, (!done[0] && !wait[0]) || (!done[1] && !wait[1]))) {
+                bool on[2] = {!done[0] && !wait[0], !done[1] && !wait[1]};
+                if (__any_sync(SPH_FULL, remask)) {
+                    float rr[2];
+#pragma unroll
+                    for (int t = 0; t < 2; ++t) rr[t] = on[t] ? Rc[t] : 0.0f;
+                    sph_tile_masks(sm, ti, xt, yt, zt, rr, lane);
+                    remask = false;
+                }
+                int nent[2] = {0, 0};
+                if constexpr (MOM) {
+                    // ---- one sweep: the six Bernstein moments, the zone list, the entry count
+                    float M[2][6];
+                    float ihh[2];
+                    int   nz[2] = {0, 0};
+#pragma unroll
+                    for (int t = 0; t < 2; ++t) {
+                        ihh[t] = __fdividef(0.5f, h[t]);
+#pragma unroll
+                        for (int k = 0; k < 6; ++k) M[t][k] = 0.0f;
+                    }
+                    uint32_t za[2], zend[2];
+#pragma unroll
+                    for (int t = 0; t < 2; ++t) {
+                        za[t]   = sm.zone_sa + 2u * (uint32_t)(lane + 32 * t);
+                        zend[t] = za[t] + 2u * SPH_TB * (SPH_TZCAP - 1);
+                    }
+                    sph_tile_walk(sm, ti, lane, on, [&](int t, const SphEntry& en) {
+                        const float dx = xt[t] - en.c.x, dy = yt[t] - en.c.y, dz = zt[t] - en.c.z;
+                        const float r  = sph_sqrt(fmaf(dz, dz, fmaf(dy, dy, dx * dx)));
+                        const float s  = r * ihh[t], tt = 1.0f - s;
+                        const float t2 = tt * tt, t3 = t2 * tt, t4 = t2 * t2, t5 = t4 * tt;
+                        const float a1 = en.m * s, a2 = a1 * s, a3 = a2 * s, a4 = a3 * s, a5 = a4 * s;
+                        M[t][0] = fmaf(en.m, t5, M[t][0]);
+                        M[t][1] = fmaf(a1, t4, M[t][1]);
+                        M[t][2] = fmaf(a2, t3, M[t][2]);
+                        M[t][3] = fmaf(a3, t2, M[t][3]);
+                        M[t][4] = fmaf(a4, tt, M[t][4]);
+                        M[t][5] += a5;
+                        nent[t] += en.has ? 1 : 0;
+                        // next to (or beyond) the support edge: remember the entry (predicated
+                        // store; past the capacity the last slot is overwritten and nz says so)
+                        const bool inz = en.has && tt < T_ZONE;
+                        asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %2, 0;\n\t@p st.shared.u16 [%0], %1;\n\t}"
+                                     ::"r"(za[t]), "h"((unsigned short)en.idx), "r"((unsigned)inz) : "memory");
+                        za[t] = inz ? min(za[t] + 2u * SPH_TB, zend[t]) : za[t];
+                        nz[t] += inz ? 1 : 0;
+                    });
+#pragma unroll
+                    for (int t = 0; t < 2; ++t) {
+                        if (!on[t]) continue;
+                        if (sweeps[t] == 0) c_listed += (unsigned)nent[t];
+                        ++sweeps[t];
+                        // the sign of f at the swept h keeps the bracket (the zone's clamp is O(T_ZONE^4))
+                        const float f0 = M[t][0] + 5.0f * M[t][1] - T[t];
+                        if (f0 < 0.0f) hlo[t] = h[t]; else hhi[t] = h[t];
+                        // scalar Newton on lam = h0 / h with the polynomial S, E
+                        float lam = 1.0f, Sp = 0.0f, Ep = 0.0f;
+                        bool  okp = true;
+#pragma unroll 1
+                        for (int it = 0; it < 3; ++it) {
+                            c2_poly(M[t], lam, Sp, Ep);
+                            if (!(Ep > 0.0f)) { okp = false; break; }
+                            lam *= 1.0f + __fdividef(Sp - T[t], Ep);
+                            lam = fminf(fmaxf(lam, 0.5f), 2.0f);
+                        }
+                        const bool zfit = nz[t] <= SPH_TZCAP;
+#ifdef SPH_DEBUG_TILE
+                        if (bi == 0 && lane < 2) printf("dbg lane %d t %d h %g nent %d nz %d M %g %g %g %g %g %g T %g lam %g okp %d Sp %g Ep %g\n", lane, t, h[t], nent[t], nz[t], M[t][0], M[t][1], M[t][2], M[t][3], M[t][4], M[t][5], T[t], lam, (int)okp, Sp, Ep);
+#endif
+                        if (okp && zfit && fabsf(1.0f - lam) <= 0.9f * T_ZONE && h[t] / lam <= hcap) {
+                            // ---- final: put the clamped zone entries right at lam, one more step
+                            const float eps = 1.0f - lam;
+                            float dS = 0.0f, dE = 0.0f, amin = 3.0e38f;
+                            int   cz = 0;
+                            for (int q = 0; q < nz[t]; ++q) {
+                                const int    idx = sm.zone[q * SPH_TB + lane + 32 * t];
+                                const float4 c   = sm.tile[idx];
+                                const float  mj  = sm.ms[idx];
+                                const float dx = xt[t] - c.x, dy = yt[t] - c.y, dz = zt[t] - c.z;
+                                const float r  = sph_sqrt(fmaf(dz, dz, fmaf(dy, dy, dx * dx)));
+                                const float s  = r * ihh[t], tt = 1.0f - s;
+                                const float tq = fmaf(eps, s, tt), sq = lam * s;   // t', s' at lam
+                                amin = fminf(amin, fabsf(tq));
+                                if (tq < 0.0f) {
+                                    const float q2 = tq * tq, q3 = q2 * tq;
+                                    dS -= mj * q2 * q2 * (tq + 5.0f * sq);
+                                    dE -= 20.0f * mj * sq * sq * q3;
+                                } else ++cz;
+                            }
+                            c2_poly(M[t], lam, Sp, Ep);
+                            float lam2 = lam * (1.0f + __fdividef(Sp + dS - T[t], Ep + dE));
+                            c2_poly(M[t], lam2, Sp, Ep);
+                            const float hn = __fdividef(h[t], lam2);
+                            const float taun = 1e-6f + band_c * __fdividef(1.0f, hn);
+                            S[t] = Sp + dS; E[t] = Ep + dE; h[t] = hn;
+                            ni[t] = nent[t] - nz[t] + cz;
+                            // an entry closer to the edge than the band plus the last step: exact recount
+                            recount[t] = amin <= taun + 1.5f * fabsf(lam2 - lam);
+                            done[t] = true;
+                            continue;
+                        }
+                        // ---- a step only: move, keep inside the bracket, sweep again
+                        float hn;
+                        if (okp) hn = __fdividef(h[t], fminf(fmaxf(lam, 1.0f / 1.35f), 1.0f / 0.7f));
+                        else     hn = 1.25f * h[t];
+                        if (hhi[t] < 3.0e38f && !(hn >= hlo[t] && hn <= hhi[t])) hn = 0.5f * (hlo[t] + hhi[t]);
+                        const bool capped = hn >= hcap && h[t] >= hcap;
+                        hn = fminf(hn, hcap);
+                        if (capped || sweeps[t] >= par.max_iter || (hhi[t] - hlo[t]) <= par.tol * h[t] || !zfit) {
+                            done[t] = true; fix[t] = true;   // k_density_fix settles it (and counts non-convergence)
+                            continue;
+                        }
+                        h[t] = hn;
+                        want[t] = 2.0f * hn * lslack;
+                        if (want[t] <= Rt) { Rc[t] = want[t]; remask = true; }
+                        else wait[t] = true;
+                    }
+                } else {
+                    // ---- Halley path: S, E, F at h; interior count and the entries next to the edge
+                    float ih[2], Hlo[2], Hhi[2], s[2], e[2], f2[2];
+                    int   cin[2], ne[2];
+#pragma unroll
+                    for (int t = 0; t < 2; ++t) {
+                        ih[t]  = __fdividef(1.0f, h[t]);
+                        Hlo[t] = 2.0f * h[t] * (1.0f - T_EDGE);
+                        Hhi[t] = 2.0f * h[t] * (1.0f + T_EDGE);
+                        s[t] = 0.0f; e[t] = 0.0f; f2[t] = 0.0f; cin[t] = 0; ne[t] = 0;
+                    }
+                    sph_tile_walk(sm, ti, lane, on, [&](int t, const SphEntry& en) {
+                        const float4 c = en.c;
+                        const float  mj = en.m;
+                        const bool   has = en.has;
+                        const float dx = xt[t] - c.x, dy = yt[t] - c.y, dz = zt[t] - c.z;
+                        const float r  = sph_sqrt(fmaf(dz, dz, fmaf(dy, dy, dx * dx)));
+                        float wq, eq, fq;
+                        SphKernel<KERN>::sums_s(r * ih[t], wq, eq, fq);
+                        s[t]  = fmaf(mj, wq, s[t]);
+                        e[t]  = fmaf(mj, eq, e[t]);
+                        f2[t] = fmaf(mj, fq, f2[t]);
+                        nent[t] += has ? 1 : 0;
+                        cin[t]  += (has && r < Hlo[t]) ? 1 : 0;
+                        if (has && r >= Hlo[t] && r < Hhi[t]) {
+                            if (ne[t] < 4) edge[ne[t] * SPH_TB + lane + 32 * t] = r;
+                            ++ne[t];
+                        }
+                    });
+#pragma unroll
+                    for (int t = 0; t < 2; ++t) {
+                        if (!on[t]) continue;
+                        if (sweeps[t] == 0) c_listed += (unsigned)nent[t];
+                        ++sweeps[t];
+                        const float es = SphKernel<KERN>::escale * e[t];
+                        float hn, Sn, En;
+                        bool  conv;
+                        const bool acc = tile_halley(s[t], es, f2[t], T[t], h[t], ih[t], hcap, par.tol,
+                                                     hlo[t], hhi[t], hn, Sn, En, conv);
+                        const float taun = 1e-6f + band_c * __fdividef(1.0f, hn);
+                        const float needR = 2.0f * hn * (1.0f + 2.0f * taun) * (1.0f + 1e-4f);
+                        if (acc && needR <= Rc[t]) {
+                            const float H = 2.0f * hn, tauH = taun * H;
+                            int  n = cin[t];
+                            bool eg = ne[t] > 4;
+                            for (int q = 0; q < min(ne[t], 4); ++q) {
+                                const float r = edge[q * SPH_TB + lane + 32 * t];
+                                n += (r < H) ? 1 : 0;
+                                eg |= fabsf(r - H) <= tauH;
+                            }
+                            S[t] = Sn; E[t] = En; h[t] = hn; ni[t] = n;
+                            done[t] = true;
+                            fix[t]  = !conv;
+                            recount[t] = eg;
+                            continue;
+                        }
+                        h[t] = hn;
+                        if (sweeps[t] >= par.max_iter) { done[t] = true; fix[t] = true; continue; }
+                        if (needR > Rc[t]) {   // the ball outgrew the list
+                            want[t] = 2.0f * hn * fmaxf(par.slack, 1.25f);
+                            if (needR <= Rt) { Rc[t] = fminf(want[t], Rt); remask = true; }
+                            else wait[t] = true;
+                        }
+                    }
+                }
+            }
+        }
+
+        // ---- results
+        if (fallback) {   // whole bucket to the 8-lanes-per-target kernel
+#pragma unroll
+            for (int t = 0; t < 2; ++t)
+                if (valid[t]) fb_list[atomicAdd(fb_cnt, 1u)] = (uint32_t)p[t];
+            continue;
+        }
+#pragma unroll
+        for (int t = 0; t < 2; ++t) {
+            if (!valid[t]) continue;
+            if (wait[t] || !done[t]) { fix[t] = true; done[t] = true; }
+            const int i = ic[t];
+            h_io[i] = h[t];
+            nb_rkeep[p[t]] = 0.0f;     // no 8-lane list for this target
+            c_sweeps += (unsigned)sweeps[t];
+            if (!fix[t]) {
+                const float ih = 1.0f / h[t];
+                rho[i]   = SphKernel<KERN>::sigma * S[t] * ih * ih * ih;
+                omega[i] = E[t] / (3.0f * S[t]);
+                nn[i]    = ni[t];
+            }
+            if (fix[t])          fix_list[atomicAdd(fix_cnt, 1u)] = p[t];
+            else if (recount[t]) fix_list[atomicAdd(fix_cnt, 1u)] = p[t] | (int32_t)0x80000000;
+            else                 c_pairs += (unsigned)ni[t];
+        }
+    }
+
+    // ---- counters: one atomic per warp and counter
+    const unsigned tl = __reduce_add_sync(SPH_FULL, c_listed), tp = __reduce_add_sync(SPH_FULL, c_pairs);
+    const unsigned tsw = __reduce_add_sync(SPH_FULL, c_sweeps), trc = __reduce_add_sync(SPH_FULL, c_recollect);
+    if (lane == 0) {
+        if (c_tested) atomicAdd(stats + ST_DENS_TESTED, c_tested);
+        if (tl) atomicAdd(stats + ST_DENS_LISTED, (unsigned long long)tl);
+        if (tp) atomicAdd(stats + ST_DENS_PAIRS, (unsigned long long)tp);
+        if (tsw) atomicAdd(stats + ST_DENS_SWEEPS, (unsigned long long)tsw);
+        if (trc) atomicAdd(stats + ST_DENS_RECOLLECT, (unsigned long long)trc);
+    }
+}
+
+}  // namespace
+
+int sph_launch_buckets(sph_ctx* c) {
+    cudaStream_t s = c->stream;
+    SPH_CUDA_CHECK(c, cudaMemsetAsync(c->bucket_cnt, 0, sizeof(unsigned), s));
+    k_buckets<<<c->sm_count * 2, 256, 0, s>>>(c->grid, c->cell_start, c->par.tile_rows, c->buckets,
+                                              c->bucket_cnt);
+    SPH_CUDA_CHECK(c, cudaGetLastError());
+    return SPH_OK;
+}
+
+// Runs the tile kernel over all buckets; the targets it hands back are in c->fb_list
+// (c->fb_cnt of them) and are swept by the caller with the 8-lanes-per-target kernel.
+int sph_launch_density_tile(sph_ctx* c, float* h, float* rho, float* omega, int32_t* nn) {
+    cudaStream_t s = c->stream;
+    TilePar par{c->par.n_ngb, c->par.h_tol, c->par.search_slack, c->par.h_max_iter, c->par.tile_cap};
+    const size_t smem = sph_tile_smem_bytes(par.tcap, 16);
+    SPH_CUDA_CHECK(c, cudaMemsetAsync(c->tile_next, 0, 2 * sizeof(unsigned), s));
+    SPH_CUDA_CHECK(c, cudaMemsetAsync(c->fb_cnt, 0, sizeof(unsigned), s));
+    auto launch = [&](auto tag) -> cudaError_t {
+        constexpr int KERN = decltype(tag)::value;
+        cudaError_t e = cudaFuncSetAttribute(k_density_tile<KERN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        int per_sm = 0;
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_density_tile<KERN>, 32, smem);
+        if (e != cudaSuccess) return e;
+        if (per_sm < 1) per_sm = 1;
+        k_density_tile<KERN><<<c->sm_count * per_sm, 32, smem, s>>>(
+            c->grid, c->cell_start, c->pos_m, c->perm, c->buckets, c->bucket_cnt, c->tile_next, par, h,
+            rho, omega, nn, c->fix_list, c->fix_cnt, c->fb_list, c->fb_cnt, c->nb_rkeep, c->stats);
+        return cudaGetLastError();
+    };
+    cudaError_t e;
+    switch (c->par.kernel) {
+    case 0: e = launch(std::integral_constant<int, 0>{}); break;
+    case 2: e = launch(std::integral_constant<int, 2>{}); break;
+    case 3: e = launch(std::integral_constant<int, 3>{}); break;
+    default: e = launch(std::integral_constant<int, 1>{}); break;
+    }
+    SPH_CUDA_CHECK(c, e);
+    return SPH_OK;
+}

@@ -39,7 +39,8 @@ class _Params(C.Structure):
                 ("av_alpha", C.c_float), ("av_beta", C.c_float), ("av_eps", C.c_float),
                 ("eta_cfl", C.c_float), ("eta_acc", C.c_float), ("h_tol", C.c_float),
                 ("h_max_iter", C.c_int32), ("search_slack", C.c_float),
-                ("cell_div_x", C.c_float), ("cell_div_yz", C.c_float), ("entropy", C.c_int32)]
+                ("cell_div_x", C.c_float), ("cell_div_yz", C.c_float), ("entropy", C.c_int32),
+                ("tile", C.c_int32), ("tile_rows", C.c_int32), ("tile_cap", C.c_int32)]
 
 
 class _Stats(C.Structure):
@@ -65,11 +66,15 @@ class Params:
     cell_div_x: float = 0.0
     cell_div_yz: float = 0.0
     entropy: int = 0            # 1: dudt = Eq. (18) only, u advanced by isentropic_u
+    tile: int = 0               # -1: staged-tile sweeps off (8-lanes-per-target kernels only)
+    tile_rows: int = 0          # 0 -> library default
+    tile_cap: int = 0
 
     def c(self) -> _Params:
         return _Params(self.kernel, self.n_ngb, self.gamma, self.av_alpha, self.av_beta,
                        self.av_eps, self.eta_cfl, self.eta_acc, self.h_tol, self.h_max_iter,
-                       self.search_slack, self.cell_div_x, self.cell_div_yz, int(self.entropy))
+                       self.search_slack, self.cell_div_x, self.cell_div_yz, int(self.entropy),
+                       int(self.tile), int(self.tile_rows), int(self.tile_cap))
 
 
 @dataclass
@@ -113,6 +118,8 @@ def load():
     lib.sph_block_predict.argtypes = [vp, i64, i32, C.c_float] + [fp] * 14
     lib.sph_block_active.argtypes = [vp, i64, i32, fp, fp]
     lib.sph_block_kick.argtypes = [vp, i64, i32, i32, C.c_float] + [fp] * 12 + [i32]
+    lib.sph_set_active.argtypes = [vp, fp]
+    lib.sph_mark_neighbors.argtypes = [vp, fp, fp]
     lib.sph_neighbors.argtypes = [vp, fp, i32, fp, fp, i64, C.POINTER(i64)]
     lib.sph_stats.argtypes = [vp, C.POINTER(_Stats)]
     lib.sph_stats_reset.argtypes = [vp]
