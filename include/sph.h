@@ -79,6 +79,12 @@ typedef struct {
                           /* default 3; at most 5)                                           */
     int32_t tile_cap;     /* candidates a tile holds (<= 0: default 1024); buckets that need  */
                           /* more fall back to the 8-lane kernels                            */
+    int32_t tile_warps;   /* warps that share a bucket's tile (<= 0: default 1; at most 4)    */
+    int32_t tile_forces;  /* 0 (default): the force sweep reads the neighbour lists the       */
+                          /* density sweep kept (8 lanes per target); 1: the force sweep runs  */
+                          /* on staged tiles too (measured slower)        */
+    int32_t tile_fcap;    /* tile_cap and tile_warps of the force sweep (<= 0: defaults 576   */
+    int32_t tile_fwarps;  /* and 1); its tile holds 52 B per candidate, the density tile 20   */
 } sph_params;
 
 /* 64-bit counters accumulated on the device since the last sph_stats_reset.             */

@@ -19,9 +19,16 @@ static void fill_defaults(sph_params& p) {
     if (!(p.cell_div_yz > 0.0f)) p.cell_div_yz = 1.5f;
     if (p.tile_rows <= 0) p.tile_rows = 3;
     if (p.tile_rows > 5) p.tile_rows = 5;
-    if (p.tile_cap <= 0) p.tile_cap = 1024;
+    if (p.tile_cap <= 0) p.tile_cap = 768;
     p.tile_cap = (p.tile_cap + 31) & ~31;
     if (p.tile_cap > 4096) p.tile_cap = 4096;
+    if (p.tile_warps <= 0) p.tile_warps = 1;
+    if (p.tile_warps > SPH_TWMAX) p.tile_warps = SPH_TWMAX;
+    if (p.tile_fcap <= 0) p.tile_fcap = 576;
+    p.tile_fcap = (p.tile_fcap + 31) & ~31;
+    if (p.tile_fcap > 4096) p.tile_fcap = 4096;
+    if (p.tile_fwarps <= 0) p.tile_fwarps = 1;
+    if (p.tile_fwarps > SPH_TWMAX) p.tile_fwarps = SPH_TWMAX;
 }
 
 template <class T>
@@ -82,7 +89,12 @@ extern "C" int sph_create(sph_ctx** out, const sph_params* params, const sph_box
     ok = ok && dalloc(&c->act_cnt, (size_t)2) == cudaSuccess;
     ok = ok && dalloc(&c->buckets, (size_t)n_max) == cudaSuccess;
     ok = ok && dalloc(&c->bucket_cnt, (size_t)1) == cudaSuccess;
-    ok = ok && dalloc(&c->tile_next, (size_t)2) == cudaSuccess;
+    ok = ok && dalloc(&c->tile_next, (size_t)4) == cudaSuccess;
+    ok = ok && dalloc(&c->big_list, (size_t)n_max) == cudaSuccess;
+    ok = ok && dalloc(&c->big_cnt, (size_t)2) == cudaSuccess;
+    ok = ok && dalloc(&c->list_next, (size_t)1) == cudaSuccess;
+    ok = ok && dalloc(&c->bucket_loff, (size_t)n_max) == cudaSuccess;
+    ok = ok && dalloc(&c->tl_rkeep, (size_t)n_max) == cudaSuccess;
     ok = ok && dalloc(&c->fb_list, (size_t)n_max) == cudaSuccess;
     ok = ok && dalloc(&c->fb_cnt, (size_t)2) == cudaSuccess;
     ok = ok && dalloc(&c->dt_part, (size_t)1024) == cudaSuccess;
@@ -113,6 +125,8 @@ extern "C" void sph_destroy(sph_ctx* c) {
     cudaFree(c->nb_j);      cudaFree(c->nb_cnt);   cudaFree(c->nb_rkeep);
     cudaFree(c->buckets);   cudaFree(c->bucket_cnt); cudaFree(c->tile_next);
     cudaFree(c->fb_list);   cudaFree(c->fb_cnt);
+    cudaFree(c->big_list);  cudaFree(c->big_cnt);
+    cudaFree(c->list_next); cudaFree(c->bucket_loff); cudaFree(c->tl_rkeep);
     delete c;
 }
 

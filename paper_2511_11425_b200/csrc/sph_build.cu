@@ -253,6 +253,8 @@ int sph_launch_build(sph_ctx* c, int64_t n, const float* x, const float* y, cons
     const int    gs = c->sm_count * 8;
     // new positions: the neighbour lists kept from the last density sweep are void
     SPH_CUDA_CHECK(c, cudaMemsetAsync(c->nb_rkeep, 0, (size_t)n * sizeof(float), s));
+    SPH_CUDA_CHECK(c, cudaMemsetAsync(c->bucket_loff, 0xff, (size_t)n * sizeof(uint32_t), s));
+    SPH_CUDA_CHECK(c, cudaMemsetAsync(c->tl_rkeep, 0, (size_t)n * sizeof(float), s));
     k_init_red<<<1, 1, 0, s>>>(c->red);
     k_reduce_h<<<min(nb, gs), TPB, 0, s>>>(n, x, y, z, h, c->red);
     k_grid_setup<<<1, 1, 0, s>>>(c->grid, c->red, c->box, c->par.search_slack, c->par.cell_div_x,

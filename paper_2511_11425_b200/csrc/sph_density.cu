@@ -107,7 +107,9 @@ __global__ __launch_bounds__(D_TPB, SPH_MINB) void k_density(
     const float4* __restrict__ pos_m, const int32_t* __restrict__ perm, DensPar par, float* h_io,
     float* rho, float* omega, int32_t* nn, int32_t* fix_list, unsigned* fix_cnt, uint32_t* nb_j,
     uint32_t* nb_cnt, float* nb_rkeep, const uint32_t* __restrict__ act_list,
-    const unsigned* __restrict__ act_cnt, unsigned long long* stats) {
+    const unsigned* __restrict__ act_cnt, int keep, unsigned long long* stats) {
+    // keep = 0: no neighbour lists are left behind (the staged-tile sweep owns the list memory,
+    // in its own layout; this kernel then only serves the buckets that sweep handed back)
     // targets: all n sorted positions, or the act_cnt entries of act_list (the active set)
     const int nt = act_list ? (int)*act_cnt : n;
     if (blockIdx.x * D_TARGETS >= nt) return;
@@ -188,7 +190,7 @@ __global__ __launch_bounds__(D_TPB, SPH_MINB) void k_density(
                         const uint32_t a = gb + 4u * f;
                         sph_sts<0>(a, sph_sqrt(r2));
                         sph_sts<D_MOFF>(a, pj.w);
-                        sph_stg(gj + f, j);
+                        if (keep) sph_stg(gj + f, j);
                     }
                 });
                 __syncwarp();
@@ -262,7 +264,7 @@ __global__ __launch_bounds__(D_TPB, SPH_MINB) void k_density(
             atomicAdd(&st_sh[1], (unsigned)cnt);
             atomicAdd(&st_sh[3], (unsigned)sweeps);
             h_io[i] = h;   // final, or the best iterate for the fix kernel to start from
-            nb_rkeep[p] = fix ? 0.0f : Rc;
+            nb_rkeep[p] = (fix || !keep) ? 0.0f : Rc;
             nb_cnt[p]   = cnt;
             if (!fix) {
                 const float ih = 1.0f / h;
@@ -423,7 +425,8 @@ int sph_launch_density(sph_ctx* c, const float* m, float* h, float* rho, float* 
         constexpr int KERN = decltype(tag)::value;
         k_density<KERN><<<nblk, D_TPB, 0, s>>>((int)n, c->grid, c->cell_start, c->pos_m, c->perm, par,
                                                h, rho, omega, nn, c->fix_list, c->fix_cnt, c->nb_j,
-                                               c->nb_cnt, c->nb_rkeep, tlist, tcnt, c->stats);
+                                               c->nb_cnt, c->nb_rkeep, tlist, tcnt,
+                                               (tiled && !c->par.tile_forces) ? 0 : 1, c->stats);
         k_density_fix<KERN><<<c->sm_count * 4, 256, 0, s>>>(c->grid, c->cell_start, c->pos_m, c->perm,
                                                             par, c->fix_list, c->fix_cnt, h, rho,
                                                             omega, nn, c->stats);

@@ -18,6 +18,7 @@
 //               for v_ij.d < 0, else 0;   gbar = (g_i + g_j)/2;  A = P/(Omega rho^2).
 #include <cstdio>
 #include "sph_internal.cuh"
+#include "sph_force_pair.cuh"
 
 namespace {
 
@@ -31,10 +32,6 @@ constexpr int F_TPB    = F_WARPS * 32;
 constexpr int F_QUADS  = 16;   // target quads per block, handed out dynamically
 constexpr int F_TARGETS = F_NT * F_QUADS;
 constexpr int F_SLOTS  = SPH_SLOTS;   // list entries per lane
-
-struct ForcePar {
-    float alpha, beta, eps;
-};
 
 struct FWarpList {
     uint32_t j[F_SLOTS][32];
@@ -117,47 +114,6 @@ __global__ void k_coarse_blocks(const SphGrid* __restrict__ g, unsigned* coarse)
 }
 
 __global__ void k_zero_hmax(SphGrid* g) { g->force_hmax_bits = 0u; }
-
-// Per-target constants and accumulators of the pair sum.
-struct Target {
-    float4 pi, vi;                       // (x, y, z, h), (vx, vy, vz, m)
-    float  rho, c, A, K, ih;
-};
-struct Accum {
-    float    ax = 0.f, ay = 0.f, az = 0.f, du = 0.f, mumin = 0.f;
-    unsigned pairs = 0, av = 0;
-};
-
-// One pair of Eqs. (13)-(18): source j at displacement d = x_i - x_j (minimum image).
-// ENT: the entropy-conserving variant drops the Eq. (14) term of du/dt.
-template <int KERN, bool ENT>
-__device__ __forceinline__ void force_pair(const Target& t, Accum& a, const ForcePar& par,
-                                           const float4 vj, const float4 rj, float dx,
-                                           float dy, float dz, float r2, float hj) {
-    const float r  = sph_sqrt(r2);
-    const float gi = t.K * SphKernel<KERN>::g_s(r * t.ih);   // K carries gscale
-    const float gj = rj.w * SphKernel<KERN>::g_s(__fdividef(r, hj));
-    const float vdx = t.vi.x - vj.x, vdy = t.vi.y - vj.y, vdz = t.vi.z - vj.z;
-    const float vr = vdx * dx + vdy * dy + vdz * dz;   // v_ij . r_ij
-    float pig = 0.0f;                                   // Pi_ij * gbar
-    if (vr < 0.0f) {
-        const float hb  = 0.5f * (t.pi.w + hj);
-        const float mu  = __fdividef(hb * vr, r2 + par.eps * hb * hb);
-        const float cb  = 0.5f * (t.c + rj.y);
-        const float rb  = 0.5f * (t.rho + rj.x);
-        const float Pij = __fdividef(mu * (par.beta * mu - par.alpha * cb), rb);
-        pig     = Pij * 0.5f * (gi + gj);
-        a.mumin = fminf(a.mumin, mu);
-        ++a.av;
-    }
-    const float Ag = t.A * gi;
-    const float ca = vj.w * (Ag + rj.z * gj + pig);
-    a.ax += ca * dx;
-    a.ay += ca * dy;
-    a.az += ca * dz;
-    a.du -= vj.w * (ENT ? 0.5f * pig : Ag + 0.5f * pig) * vr;   // Eq. (18) [+ Eq. (14)]
-    ++a.pairs;
-}
 
 template <int KERN, bool ENT>
 __global__ __launch_bounds__(F_TPB, SPH_FMINB) void k_forces(
@@ -414,15 +370,24 @@ int sph_launch_forces(sph_ctx* c, const float* m, const float* vx, const float* 
     k_coarse_blocks<<<c->sm_count, 256, 0, s>>>(c->grid, c->coarse_hmax);
     ForcePar par{c->par.av_alpha, c->par.av_beta, c->par.av_eps};
     const int nblk = (int)((n + F_TARGETS - 1) / F_TARGETS);
+    // the staged-tile kernel first; what it hands back goes through the 8-lane kernel's target list
+    // the buckets of the staged-tile density sweep first: from its kept lists (default) or on
+    // staged tiles; what is handed back goes through the 8-lane kernel's target list
+    const bool tiled = c->par.tile >= 0 && !c->act_on;
+    if (tiled) {
+        const int rc = c->par.tile_forces > 0 ? sph_launch_forces_tile(c, ax, ay, az, dudt, mu_min)
+                                              : sph_launch_forces_list(c, ax, ay, az, dudt, mu_min);
+        if (rc != SPH_OK) return rc;
+    }
+    const uint32_t* tlist = tiled ? c->fb_list : (c->act_on ? c->act_list : nullptr);
+    const unsigned* tcnt  = tiled ? c->fb_cnt + 1 : c->act_cnt;
     auto launch2 = [&](auto tag, auto etag) {
         constexpr int  KERN = decltype(tag)::value;
         constexpr bool ENT  = decltype(etag)::value;
         k_forces<KERN, ENT><<<nblk, F_TPB, 0, s>>>((int)n, c->grid, c->cell_start, c->pos_h, c->vel_m,
                                               c->rcak, c->perm, par, ax, ay, az, dudt, mu_min,
                                               c->fix_list, c->fix_cnt + 1, c->coarse_hmax, c->nb_j,
-                                              c->nb_cnt, c->nb_rkeep,
-                                              c->act_on ? c->act_list : nullptr, c->act_cnt,
-                                              c->stats);
+                                              c->nb_cnt, c->nb_rkeep, tlist, tcnt, c->stats);
         k_forces_fix<KERN, ENT><<<c->sm_count * 4, 256, 0, s>>>(c->grid, c->cell_start, c->pos_h, c->vel_m,
                                                            c->rcak, c->perm, par, c->fix_list,
                                                            c->fix_cnt + 1, ax, ay, az, dudt, mu_min,

@@ -1,0 +1,283 @@
+// sph_forces_list.cu -- steps a8, a9 of DESIGN.md for the buckets of the staged-tile density
+// sweep: the hydro force pass of PAPER.md:186-219 (Section 2.3.5), Eqs. (13)-(18), read from
+// the neighbour lists the density sweep kept (one list serves gather and
+// scatter as long as it covers the reach 2 max(h_i, h_j)).
+//
+// One warp per bucket, one lane per pair of targets, NO shared memory: the list of a bucket is
+// bucket-major, entry f of target t at [f][t], so the 32 lanes read their f-th entries with one
+// coalesced load; the f-th neighbours of adjacent targets are adjacent records of the sorted
+// arrays (the lists are in tile order: row by row, ascending inside a row), so the three
+// 16-byte gathers per pair -- (x, y, z, h), (v, m), (rho, c, A, K) -- coalesce as well and the
+// bucket's ~600 source records stay in L1.  The pair arithmetic is the branch-free form of
+// sph_force_pair.cuh, two entries of both targets per trip: four independent dependency chains.
+// Targets whose list does not cover their reach (a larger h_j nearby), and buckets without a
+// list, go to k_forces (8 lanes per target, own search) through a target list.
+#include <cstdio>
+#include "sph_tile.cuh"
+#include "sph_force_pair.cuh"
+
+namespace {
+
+constexpr int FL_WARPS = 4;
+
+__device__ __forceinline__ float lwarp_max(float v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fmaxf(v, __shfl_xor_sync(SPH_FULL, v, o));
+    return v;
+}
+__device__ __forceinline__ float lwarp_min(float v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fminf(v, __shfl_xor_sync(SPH_FULL, v, o));
+    return v;
+}
+
+// a6 for a box (the bound of sph_scatter_hmax, for the bucket's bounding box): the largest h_j
+// of any particle that can reach a point of [b0, b1].  Warp-collective.
+__device__ __forceinline__ float list_scatter_hmax(const SphGrid& g, const unsigned* __restrict__ coarse,
+                                                   const float b0[3], const float b1[3], float hown,
+                                                   float hglobal, int lane) {
+    float H = fmaxf(hglobal, hown);
+#pragma unroll 1
+    for (int pass = 0; pass < 3; ++pass) {
+        int  u0[3], nn[3];
+        bool inside = true;
+        const float R = 2.0f * H * (1.0f + 1e-5f);
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+            float a = floorf((b0[d] - g.lo[d] - R) * g.ics[d] - 1e-3f);
+            float b = floorf((b1[d] - g.lo[d] + R) * g.ics[d] + 1e-3f);
+            a = fminf(fmaxf(a, -1.0e9f), 1.0e9f);
+            b = fminf(fmaxf(b, -1.0e9f), 1.0e9f);
+            int lo = (int)a, hi = (int)b;
+            if (g.per[d]) {
+                inside = inside && lo >= 0 && hi <= g.cn[d] - 1;
+                if (hi - lo + 1 >= g.cn[d]) { lo = 0; hi = g.cn[d] - 1; }
+            } else {
+                lo = min(max(lo, 0), g.cn[d] - 1);
+                hi = min(max(hi, 0), g.cn[d] - 1);
+            }
+            u0[d] = lo;
+            nn[d] = hi - lo + 1;
+        }
+        const bool blocks = inside && nn[0] * nn[1] * nn[2] > 512;
+        int dx = g.cn[0], dy = g.cn[1], dz = g.cn[2];
+        const unsigned* map = coarse;
+        if (blocks) {
+#pragma unroll
+            for (int d = 0; d < 3; ++d) {
+                const int q0 = u0[d] >> 3, q1 = (u0[d] + nn[d] - 1) >> 3;
+                u0[d] = q0;
+                nn[d] = q1 - q0 + 1;
+            }
+            dx = g.sn[0]; dy = g.sn[1]; dz = g.sn[2];
+            map = coarse + SPH_COARSE_MAX;
+        }
+        const int cnt = nn[0] * nn[1] * nn[2];
+        unsigned  best = 0u;
+        for (int q = lane; q < cnt; q += 32) {
+            const int t  = q / nn[0], ix = q - t * nn[0];
+            const int iz = t / nn[1], iy = t - iz * nn[1];
+            int cx = u0[0] + ix, cy = u0[1] + iy, cz = u0[2] + iz;
+            cx -= (cx >= dx) ? dx : 0; cx += (cx < 0) ? dx : 0;
+            cy -= (cy >= dy) ? dy : 0; cy += (cy < 0) ? dy : 0;
+            cz -= (cz >= dz) ? dz : 0; cz += (cz < 0) ? dz : 0;
+            cx = min(max(cx, 0), dx - 1);
+            cy = min(max(cy, 0), dy - 1);
+            cz = min(max(cz, 0), dz - 1);
+            best = max(best, __ldg(map + (cz * dy + cy) * dx + cx));
+        }
+        best = __reduce_max_sync(SPH_FULL, best);
+        const float Hn = fmaxf(hown, fminf(H, __uint_as_float(best)));
+        if (Hn >= H * (1.0f - 1e-6f)) { H = Hn; break; }
+        H = Hn;
+    }
+    return H;
+}
+
+template <int KERN, bool ENT>
+__global__ __launch_bounds__(FL_WARPS * 32) void k_forces_list(
+    const SphGrid* __restrict__ gp, const uint32_t* __restrict__ cell_start,
+    const float4* __restrict__ pos_h, const float4* __restrict__ vel_m,
+    const float4* __restrict__ rcak, const int32_t* __restrict__ perm,
+    const SphBucket* __restrict__ buckets, const unsigned* __restrict__ nbuckets, ForcePar par,
+    const unsigned* __restrict__ coarse, const uint32_t* __restrict__ nb_j,
+    const uint32_t* __restrict__ bucket_loff, const uint32_t* __restrict__ nb_cnt,
+    const float* __restrict__ tl_rkeep, int nall, unsigned* next, float* ax, float* ay, float* az, float* dudt,
+    float* mu_min, uint32_t* fb_list, unsigned* fb_cnt, unsigned long long* stats) {
+    __shared__ SphGrid g;
+    __shared__ int     rowoff_s[FL_WARPS][32];
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    for (int k = tid; k < (int)(sizeof(SphGrid) / 4); k += blockDim.x) ((int*)&g)[k] = ((const int*)gp)[k];
+    __syncthreads();
+    const unsigned nb = *nbuckets;
+    const float hmax_all = __uint_as_float(g.force_hmax_bits);
+    const float iLx = g.per[0] ? 1.0f / g.len[0] : 0.0f, Lx = g.per[0] ? g.len[0] : 0.0f;
+    const float iLy = g.per[1] ? 1.0f / g.len[1] : 0.0f, Ly = g.per[1] ? g.len[1] : 0.0f;
+    const float iLz = g.per[2] ? 1.0f / g.len[2] : 0.0f, Lz = g.per[2] ? g.len[2] : 0.0f;
+    const bool  anyper = (g.per[0] | g.per[1] | g.per[2]) != 0;
+    unsigned c_pairs = 0, c_av = 0;
+
+    for (;;) {   // persistent warps: buckets are handed out by a counter
+    unsigned bi = 0;
+    if (lane == 0) bi = atomicAdd(next, 1u);
+    bi = __shfl_sync(SPH_FULL, bi, 0);
+    if (bi >= nb) break;
+    const SphBucket bk = buckets[bi];
+    __syncwarp();
+
+    // ---- the bucket's targets
+    const int nrows = bk.nry * bk.nrz;
+    int rs = 0, rc = 0;
+    if (lane < nrows) {
+        const uint32_t rb = (uint32_t)((bk.rz0 + lane / bk.nry) * g.ny + (bk.ry0 + lane % bk.nry)) * (uint32_t)g.nx;
+        const int s0 = (int)__ldg(cell_start + rb + bk.c0) + bk.skip;
+        const int s1 = (int)__ldg(cell_start + rb + bk.c1);
+        rs = s0;
+        rc = min(max(s1 - s0, 0), SPH_TB);
+    }
+    int inc = rc;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int t = __shfl_up_sync(SPH_FULL, inc, o);
+        if (lane >= o) inc += t;
+    }
+    const int ntar = min(__shfl_sync(SPH_FULL, inc, 31), SPH_TB);
+    int* const rowoff = rowoff_s[wid];
+    rowoff[lane] = inc;
+    __syncwarp();
+    int    p[2];
+    bool   valid[2];
+    Target tg[2];
+#pragma unroll
+    for (int t = 0; t < 2; ++t) {
+        const int k = lane + 32 * t;
+        valid[t] = k < ntar;
+        int rho_ = 0;
+        while (rho_ < 31 && rowoff[rho_] <= k) ++rho_;
+        const int before = rho_ ? rowoff[rho_ - 1] : 0;
+        const int start  = __shfl_sync(SPH_FULL, rs, rho_);
+        p[t] = valid[t] ? start + (k - before) : 0;
+        tg[t].pi = make_float4(0.f, 0.f, 0.f, 0.f);
+        tg[t].vi = make_float4(0.f, 0.f, 0.f, 0.f);
+        float4 ri = make_float4(1.f, 1.f, 0.f, 0.f);
+        if (valid[t]) {
+            tg[t].pi = pos_h[p[t]];
+            tg[t].vi = vel_m[p[t]];
+            ri       = rcak[p[t]];
+        }
+        tg[t].rho = ri.x; tg[t].c = ri.y; tg[t].A = ri.z; tg[t].K = ri.w;
+        tg[t].ih  = valid[t] ? __fdividef(1.0f, tg[t].pi.w) : 0.0f;
+    }
+    float b0[3], b1[3], hown;
+    {
+        const float INF = __int_as_float(0x7f800000);
+        float lo[3] = {INF, INF, INF}, hi[3] = {-INF, -INF, -INF}, hm = 0.0f;
+#pragma unroll
+        for (int t = 0; t < 2; ++t)
+            if (valid[t]) {
+                lo[0] = fminf(lo[0], tg[t].pi.x); hi[0] = fmaxf(hi[0], tg[t].pi.x);
+                lo[1] = fminf(lo[1], tg[t].pi.y); hi[1] = fmaxf(hi[1], tg[t].pi.y);
+                lo[2] = fminf(lo[2], tg[t].pi.z); hi[2] = fmaxf(hi[2], tg[t].pi.z);
+                hm = fmaxf(hm, tg[t].pi.w);
+            }
+#pragma unroll
+        for (int d = 0; d < 3; ++d) { b0[d] = lwarp_min(lo[d]); b1[d] = lwarp_max(hi[d]); }
+        hown = lwarp_max(hm);
+    }
+    // a6: the largest h that can reach the bucket sets the reach R = 2 max(h_i, H)
+    const float Hs = list_scatter_hmax(g, coarse, b0, b1, hown, hmax_all, lane);
+
+    // ---- which targets the kept lists serve
+    const uint32_t reg = bucket_loff[bi];
+    const uint32_t* const lb = nb_j + (size_t)(reg == 0xffffffffu ? 0u : reg) * (SPH_LCAP * SPH_TB);
+    bool cov[2];
+    int  cnt[2];
+#pragma unroll
+    for (int t = 0; t < 2; ++t) {
+        const float R   = 2.0f * (1.0f + 1e-5f) * fmaxf(tg[t].pi.w, Hs);
+        const float tau = 1e-6f + 2.5e-7f * g.xext * tg[t].ih;
+        const float rk  = valid[t] ? tl_rkeep[p[t]] : 0.0f;
+        cov[t] = valid[t] && reg != 0xffffffffu && R * (1.0f + 4.0f * tau) <= rk;
+        cnt[t] = cov[t] ? (int)nb_cnt[p[t]] : 0;
+        // not served: to the 8-lane kernel, which searches (or reads the [target][entry] list its
+        // own density kernel left: nb_rkeep, a different array)
+        if (valid[t] && !cov[t]) fb_list[atomicAdd(fb_cnt, 1u)] = (uint32_t)p[t];
+    }
+    const int maxcnt = __reduce_max_sync(SPH_FULL, max(cnt[0], cnt[1]));
+
+    Accum acc[2];
+    auto pair = [&](int t, int f) {
+        const bool     in = f < cnt[t];
+        uint32_t j  = in ? __ldg(lb + f * SPH_TB + lane + 32 * t) : (uint32_t)p[t];
+#ifdef SPH_DEBUG_TILE
+        if (j >= (uint32_t)nall) { printf("bad j %u bucket %u reg %u f %d cnt %d lane %d t %d p %d\n", j, bi, reg, f, cnt[t], lane, t, p[t]); j = p[t]; }
+#endif
+        const float4 pj = __ldg(pos_h + j), vj = __ldg(vel_m + j), rj = __ldg(rcak + j);
+        float dx = tg[t].pi.x - pj.x, dy = tg[t].pi.y - pj.y, dz = tg[t].pi.z - pj.z;
+        if (anyper) {   // minimum image
+            dx -= Lx * rintf(dx * iLx);
+            dy -= Ly * rintf(dy * iLy);
+            dz -= Lz * rintf(dz * iLz);
+        }
+        const float r2 = dx * dx + dy * dy + dz * dz;
+        const float hm = fmaxf(tg[t].pi.w, pj.w);
+        const bool  ok = in && r2 < 4.0f * hm * hm && r2 > 0.0f;
+        force_pair_nb<KERN, ENT>(tg[t], acc[t], par, ok, vj, rj, dx, dy, dz, r2, pj.w);
+    };
+    for (int f = 0; f < maxcnt; f += 2) {
+        pair(0, f);
+        pair(1, f);
+        pair(0, f + 1);
+        pair(1, f + 1);
+    }
+#pragma unroll
+    for (int t = 0; t < 2; ++t) {
+        if (!cov[t]) continue;
+        const int i = perm[p[t]];
+        ax[i] = acc[t].ax; ay[i] = acc[t].ay; az[i] = acc[t].az;
+        dudt[i]   = acc[t].du;
+        mu_min[i] = acc[t].mumin;
+        c_pairs += acc[t].pairs;
+        c_av    += acc[t].av;
+    }
+    }   // bucket loop
+    const unsigned tp = __reduce_add_sync(SPH_FULL, c_pairs), ta = __reduce_add_sync(SPH_FULL, c_av);
+    if (lane == 0) {
+        if (tp) atomicAdd(stats + ST_FORCE_PAIRS, (unsigned long long)tp);
+        if (ta) atomicAdd(stats + ST_FORCE_AV, (unsigned long long)ta);
+    }
+}
+
+}  // namespace
+
+// Sweeps the buckets whose targets have kept lists; the targets it hands back are in
+// c->fb_list (c->fb_cnt[1] of them) and are swept by the caller with the 8-lane kernel.
+int sph_launch_forces_list(sph_ctx* c, float* ax, float* ay, float* az, float* dudt, float* mu_min) {
+    cudaStream_t s = c->stream;
+    SPH_CUDA_CHECK(c, cudaMemsetAsync(c->fb_cnt + 1, 0, sizeof(unsigned), s));
+    ForcePar par{c->par.av_alpha, c->par.av_beta, c->par.av_eps};
+    SPH_CUDA_CHECK(c, cudaMemsetAsync(c->tile_next + 2, 0, sizeof(unsigned), s));
+    auto launch2 = [&](auto tag, auto etag) {
+        constexpr int  KERN = decltype(tag)::value;
+        constexpr bool ENT  = decltype(etag)::value;
+        int per_sm = 4;
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_forces_list<KERN, ENT>, FL_WARPS * 32, 0);
+        if (per_sm < 1) per_sm = 1;
+        k_forces_list<KERN, ENT><<<c->sm_count * per_sm, FL_WARPS * 32, 0, s>>>(
+            c->grid, c->cell_start, c->pos_h, c->vel_m, c->rcak, c->perm, c->buckets, c->bucket_cnt, par,
+            c->coarse_hmax, c->nb_j, c->bucket_loff, c->nb_cnt, c->tl_rkeep, (int)c->n, c->tile_next + 2, ax, ay, az,
+            dudt, mu_min, c->fb_list, c->fb_cnt + 1, c->stats);
+    };
+    auto launch = [&](auto tag) {
+        if (c->par.entropy) launch2(tag, std::true_type{});
+        else launch2(tag, std::false_type{});
+    };
+    switch (c->par.kernel) {
+    case 0: launch(std::integral_constant<int, 0>{}); break;
+    case 2: launch(std::integral_constant<int, 2>{}); break;
+    case 3: launch(std::integral_constant<int, 3>{}); break;
+    default: launch(std::integral_constant<int, 1>{}); break;
+    }
+    SPH_CUDA_CHECK(c, cudaGetLastError());
+    return SPH_OK;
+}

@@ -33,6 +33,7 @@ struct SphGrid {
 #define SPH_POS_PAD 64             // records of padding behind the sorted float4 arrays
 #define SPH_G 8                    // lanes per target in the sweeps
 #define SPH_SLOTS 24               // list entries per lane (24 x 8 = 192 per target)
+#define SPH_LCAP 128               // entries per target of a bucket-major list region (staged-tile path)
 
 enum {  // indices into the device counter block (uint64 each), mirrors sph_stats_t
     ST_DENS_TESTED = 0, ST_DENS_LISTED, ST_DENS_PAIRS, ST_DENS_SWEEPS, ST_DENS_RECOLLECT,
@@ -76,7 +77,13 @@ struct sph_ctx {
     bool         act_on;       // sph_set_active gave a mask since the last build
     struct SphBucket* buckets; // n_max: the bucket table of the staged-tile sweeps (sph_tile.cuh)
     unsigned*    bucket_cnt;   // [1]
-    unsigned*    tile_next;    // [2]: work counters of the persistent tile kernels
+    unsigned*    tile_next;    // [4]: work counters of the persistent tile kernels (density, forces; two passes)
+    unsigned*    big_list;     // n_max: buckets the first pass of a tile sweep left to the second (larger tile)
+    unsigned*    big_cnt;      // [2]: their number (density, forces)
+    unsigned*    list_next;    // [1]: next free region of nb_j (bucket-major lists of the tile sweep)
+    uint32_t*    bucket_loff;  // n_max: list region of a bucket (0xffffffff: none)
+    float*       tl_rkeep;     // n_max: radius inside which a target's bucket-major list is complete (0: none);
+                               // nb_rkeep stays the radius of the 8-lane kernels' [target][entry] lists
     uint32_t*    fb_list;      // n_max: targets the tile kernels hand to the 8-lane kernels
     unsigned*    fb_cnt;       // [2]: their number (density, forces)
     float*       dt_part;      // per-block minima of the time-step reduction
@@ -703,6 +710,8 @@ int sph_launch_rungs(sph_ctx* c, const float* dt_i, float dt0, int32_t max_rung,
 int sph_launch_coarse_map(sph_ctx* c);
 int sph_launch_buckets(sph_ctx* c);
 int sph_launch_density_tile(sph_ctx* c, float* h, float* rho, float* omega, int32_t* nn);
+int sph_launch_forces_tile(sph_ctx* c, float* ax, float* ay, float* az, float* dudt, float* mu_min);
+int sph_launch_forces_list(sph_ctx* c, float* ax, float* ay, float* az, float* dudt, float* mu_min);
 int sph_launch_mark(sph_ctx* c, const uint8_t* src, uint8_t* mark);
 int sph_launch_set_active(sph_ctx* c, const uint8_t* active);
 int sph_launch_compact(sph_ctx* c, const uint8_t* mask, uint32_t* list, unsigned* cnt);

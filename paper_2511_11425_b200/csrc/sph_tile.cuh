@@ -18,21 +18,28 @@
 #ifdef __CUDACC__
 
 #define SPH_TB 64        // targets per bucket: two per lane
-#define SPH_TROWS 128    // candidate rows of cells per bucket (cap)
+#define SPH_TROWS 96    // candidate rows of cells per bucket (cap)
 #define SPH_TSEGS (2 * SPH_TROWS)   // a row that crosses a periodic face has two segments
-#define SPH_TZCAP 32     // per-target slots for list entries next to the support edge (the "zone")
+#define SPH_TZCAP 28     // per-target slots for list entries next to the support edge (the "zone")
+#define SPH_TWMAX 4      // at most this many warps share a bucket
 
 // shared memory of one warp (bytes), tcap = tile capacity in candidates (multiple of 32)
 //   tile   float4[tcap]        (x', y', z', |x'|^2) in the bucket's frame
 //   ms     float[tcap]         m_j
+//   gidx   uint32[tcap]        sorted position of the candidate (density sweep: for the kept lists)
 //   mask   uint32[tcap/32][64] accept bits of the 64 targets, word-major
-//   seg    uint4[SPH_TSEGS]    (first sorted position, count, tile offset, image)
+//   seg    uint2[SPH_TSEGS]    (first sorted position, count | tile offset << 12 | image << 24)
 //   zone   uint16[SPH_TZCAP][64]  tile indices of the entries next to the support edge
 //   rowoff int[32]
 //   mbar   uint64
-__host__ __device__ inline size_t sph_tile_smem_bytes(int tcap, int rec_bytes) {
-    return (size_t)(tcap + 32) * (rec_bytes + 4) + (size_t)(tcap / 32 + 2) * SPH_TB * 4 + SPH_TSEGS * 16 +
-           SPH_TZCAP * SPH_TB * 2 + 32 * 4 + 16;
+// xbytes: size of the segment table's region, which doubles as the warps' exchange area
+__host__ __device__ inline size_t sph_tile_xbytes(int W, int words_per_target) {
+    const size_t x = W > 1 ? (size_t)W * words_per_target * SPH_TB * 4 : 0, s = SPH_TSEGS * 8;
+    return x > s ? x : s;
+}
+__host__ __device__ inline size_t sph_tile_smem_bytes(int tcap, int rec_bytes, size_t xbytes, int W) {
+    return (size_t)(tcap + 4) * (rec_bytes + 4 + 4) + (size_t)(tcap / 32 + 2 * W) * SPH_TB * 4 +
+           xbytes + SPH_TZCAP * SPH_TB * 2 + 16;
 }
 
 // ---- mbarrier / bulk-copy primitives (PTX; SASS: SYNCS.*, UBLKCP) -----------------------
@@ -114,30 +121,33 @@ struct SphTileMem {
     float4*   tile;
     float*    ms;
     uint32_t* mask;
-    uint4*    seg;
+    uint32_t* gidx;
+    uint2*    seg;
     uint16_t* zone;
-    int*      rowoff;
+    int*      rowoff;   // [W][32]: aliases the head of the mask area (used before the masks exist)
     uint32_t  bar;      // shared-window address of the mbarrier
     uint32_t  tile_sa;  // shared-window addresses of the tile, the masses, the masks, the zone list
-    uint32_t  ms_sa, mask_sa, zone_sa;
+    uint32_t  ms_sa, mask_sa, zone_sa, gidx_sa;
     int       tcap;
 };
 
 template <int REC>
-__device__ __forceinline__ SphTileMem sph_tile_carve(unsigned char* base, int tcap) {
+__device__ __forceinline__ SphTileMem sph_tile_carve(unsigned char* base, int tcap, size_t xbytes, int W) {
     SphTileMem t;
     t.tcap = tcap;
-    t.tile = (float4*)base;                 base += (size_t)(tcap + 32) * REC;
-    t.ms   = (float*)base;                  base += (size_t)(tcap + 32) * 4;
-    t.mask = (uint32_t*)base;               base += (size_t)(tcap / 32 + 2) * SPH_TB * 4;
-    t.seg  = (uint4*)base;                  base += SPH_TSEGS * 16;
+    t.tile = (float4*)base;                 base += (size_t)(tcap + 4) * REC;
+ t.ms   = (float*)base;                  base += (size_t)(tcap + 4) * 4;
+    t.gidx = (uint32_t*)base;               base += (size_t)(tcap + 4) * 4;
+    t.mask = (uint32_t*)base;               base += (size_t)(tcap / 32 + 2 * W) * SPH_TB * 4;
+ t.seg  = (uint2*)base;                  base += xbytes;
     t.zone = (uint16_t*)base;               base += SPH_TZCAP * SPH_TB * 2;
-    t.rowoff = (int*)base;                  base += 32 * 4;
+    t.rowoff = (int*)t.mask;
     t.bar  = (uint32_t)__cvta_generic_to_shared(base);
     t.tile_sa = (uint32_t)__cvta_generic_to_shared(t.tile);
     t.ms_sa   = (uint32_t)__cvta_generic_to_shared(t.ms);
     t.mask_sa = (uint32_t)__cvta_generic_to_shared(t.mask);
     t.zone_sa = (uint32_t)__cvta_generic_to_shared(t.zone);
+    t.gidx_sa = (uint32_t)__cvta_generic_to_shared(t.gidx);
     return t;
 }
 
@@ -147,6 +157,8 @@ struct SphTileInfo {
     float R;            // every source within R of any target of the bucket is in the tile
     float ext;          // largest |coordinate| in the frame: bounds the FP32 rounding of r^2
     int   nseg, nrow, used, nwords;
+    int   shifted;      // some segment is seen through a periodic image
+    int   ok;           // the bucket fits the tile
 };
 
 // Squared distance between the slab [u s, (u+1) s) + lo and the interval [b0, b1]; edge cells
@@ -191,7 +203,9 @@ __device__ __forceinline__ bool sph_axis_span(float b0, float b1, float R, float
 __device__ __forceinline__ bool sph_tile_stage(const SphGrid& g, const uint32_t* __restrict__ cell_start,
                                                const float4* __restrict__ rec, const float b0[3],
                                                const float b1[3], float R, const SphTileMem& sm,
-                                               int lane, SphTileInfo& ti) {
+                                               int lane, SphTileInfo& ti,
+                                               const float4* __restrict__ rec2 = nullptr, uint32_t dst2 = 0u,
+                                               const float4* __restrict__ rec3 = nullptr, uint32_t dst3 = 0u) {
     int x0, x1, y0, y1, z0, z1;
     bool ok = sph_axis_span(b0[1], b1[1], R, g.lo[1], g.len[1], g.isy, g.ny, g.per[1], y0, y1);
     ok = sph_axis_span(b0[2], b1[2], R, g.lo[2], g.len[2], g.isz, g.nz, g.per[2], z0, z1) && ok;
@@ -200,7 +214,8 @@ __device__ __forceinline__ bool sph_tile_stage(const SphGrid& g, const uint32_t*
     const int nyr = y1 - y0 + 1, nzr = z1 - z0 + 1, nrow = nyr * nzr;
     if (nrow > SPH_TROWS) return false;
     const float R2 = R * R * (1.0f + 1e-5f);
-    int base = 0;
+    int  base = 0;
+    bool shifted = false;
     for (int rb = 0; rb < nrow; rb += 32) {
         const int r  = rb + lane;
         bool      in = r < nrow;
@@ -234,6 +249,7 @@ __device__ __forceinline__ bool sph_tile_stage(const SphGrid& g, const uint32_t*
             }
         }
         const int na = (int)(a1 - a0), nb = (int)(c1 - c0);
+        shifted = shifted || (na > 0 && ka != 0x15) || nb > 0;
         int inc = na + nb;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
@@ -242,12 +258,14 @@ __device__ __forceinline__ bool sph_tile_stage(const SphGrid& g, const uint32_t*
         }
         const int off = base + inc - (na + nb);
         if (r < nrow) {
-            sm.seg[2 * r]     = make_uint4(a0, (uint32_t)na, (uint32_t)off, (uint32_t)ka);
-            sm.seg[2 * r + 1] = make_uint4(c0, (uint32_t)nb, (uint32_t)(off + na), (uint32_t)kb);
+            // counts and offsets stay below 4096 (tile_cap), the image code below 64
+            const uint32_t oa = (uint32_t)min(off, 4095), ob = (uint32_t)min(off + na, 4095);
+            sm.seg[2 * r]     = make_uint2(a0, (uint32_t)min(na, 4095) | (oa << 12) | ((uint32_t)ka << 24));
+            sm.seg[2 * r + 1] = make_uint2(c0, (uint32_t)min(nb, 4095) | (ob << 12) | ((uint32_t)kb << 24));
         }
         base += __shfl_sync(SPH_FULL, inc, 31);
     }
-    if (base + 32 > sm.tcap || base == 0) return false;
+    if (base > sm.tcap || base == 0) return false;
     ti.nrow = nrow;
     ti.nseg = 2 * nrow;
     ti.used = base;
@@ -258,49 +276,84 @@ __device__ __forceinline__ bool sph_tile_stage(const SphGrid& g, const uint32_t*
     ti.oz = 0.5f * (b0[2] + b1[2]);
     ti.ext = R + 0.5f * fmaxf(b1[0] - b0[0], fmaxf(b1[1] - b0[1], b1[2] - b0[2])) +
              fmaxf(g.sx, fmaxf(g.sy, g.sz));
+    ti.shifted = __any_sync(SPH_FULL, shifted) ? 1 : 0;
     // the tile's previous contents were read / written through the generic proxy
     sph_fence_async_smem();
     __syncwarp();
-    if (lane == 0) sph_mbar_expect_tx(sm.bar, (uint32_t)base * 16u);
+    const uint32_t narr = 1u + (rec2 ? 1u : 0u) + (rec3 ? 1u : 0u);
+    if (lane == 0) sph_mbar_expect_tx(sm.bar, (uint32_t)base * 16u * narr);
     __syncwarp();
     for (int s = lane; s < ti.nseg; s += 32) {
-        const uint4 sg = sm.seg[s];
-        if (sg.y) sph_bulk_g2s(sm.tile_sa + sg.z * 16u, rec + sg.x, sg.y * 16u, sm.bar);
+        const uint2    sg  = sm.seg[s];
+        const uint32_t cnt = sg.y & 4095u, off = (sg.y >> 12) & 4095u;
+        if (cnt) {
+            sph_bulk_g2s(sm.tile_sa + off * 16u, rec + sg.x, cnt * 16u, sm.bar);
+            if (rec2) sph_bulk_g2s(dst2 + off * 16u, rec2 + sg.x, cnt * 16u, sm.bar);
+            if (rec3) sph_bulk_g2s(dst3 + off * 16u, rec3 + sg.x, cnt * 16u, sm.bar);
+        }
+    }
+    if (sm.gidx) {   // sorted position of every tile entry, written while the copies are in flight
+        for (int s = lane; s < ti.nseg; s += 32) {
+            const uint2    sg  = sm.seg[s];
+            const uint32_t cnt = sg.y & 4095u, off = (sg.y >> 12) & 4095u;
+            for (uint32_t k = 0; k < cnt; ++k) sm.gidx[off + k] = sg.x + k;
+        }
     }
     return true;
 }
 
 // Completes the copies of sph_tile_stage and turns the raw records (x, y, z, w) into the
-// bucket's frame: (x', y', z', |x'|^2) with x' = fl((x_j + k L) - origin) evaluated in FP64
-// on the FP32 inputs, so that the displacement x_i' - x_j' of any pair -- through a periodic
-// image or not -- carries two roundings of 2^-25 |x'| and |x'| is a few h, not the box; the
-// fourth component goes to ms[].  Pads the tile to a multiple of 32 with far-away dummies.
+// bucket's frame: (x', y', z', |x'|^2) with x' = fl((x_j + k L) - origin); the fourth
+// component goes to ms[].  Without a periodic image the origin is a float and the FP32
+// subtraction is the correctly rounded difference; through an image the shifted origin is not
+// representable and the difference is taken in FP64 on the FP32 inputs.  Either way the
+// displacement x_i' - x_j' of a pair carries two roundings of 2^-25 |x'|, and |x'| is a few h,
+// not the box.  Pads the tile with far-away dummies to a full word and one more entry (the
+// record a cursor's bubble reads).
+// Called by all nthr threads of the block; ends with a block barrier.
 __device__ __forceinline__ void sph_tile_finish(const SphGrid& g, const SphTileMem& sm,
-                                                const SphTileInfo& ti, uint32_t parity, int lane) {
+                                                const SphTileInfo& ti, uint32_t parity, int tid,
+                                                int nthr, float pad_w) {
     sph_mbar_wait(sm.bar, parity);
-    int    s = -1;
-    int    send = 0;
-    double ox = 0.0, oy = 0.0, oz = 0.0;
-    for (int k = lane; k < ti.used; k += 32) {
-        while (k >= send) {   // the segments are in tile order; each lane only moves forward
-            ++s;
-            const uint4 sg = sm.seg[s];
-            send = (int)(sg.z + sg.y);
-            const int kx = (int)(sg.w & 3u) - 1, ky = (int)((sg.w >> 2) & 3u) - 1, kz = (int)((sg.w >> 4) & 3u) - 1;
-            ox = (double)ti.ox - (double)kx * (double)g.len[0];
-            oy = (double)ti.oy - (double)ky * (double)g.len[1];
-            oz = (double)ti.oz - (double)kz * (double)g.len[2];
+    if (!ti.shifted) {
+        for (int k = tid; k < ti.used; k += nthr) {
+            const float4 p = sm.tile[k];
+            const float  x = p.x - ti.ox, y = p.y - ti.oy, z = p.z - ti.oz;
+            sm.tile[k] = make_float4(x, y, z, fmaf(z, z, fmaf(y, y, x * x)));
+            sm.ms[k]   = p.w;
         }
-        const float4 p = sm.tile[k];
-        const float  x = (float)((double)p.x - ox), y = (float)((double)p.y - oy), z = (float)((double)p.z - oz);
-        sm.tile[k] = make_float4(x, y, z, fmaf(z, z, fmaf(y, y, x * x)));
-        sm.ms[k]   = p.w;
+    } else {
+        int    s = -1;
+        int    send = 0;
+        double ox = 0.0, oy = 0.0, oz = 0.0;
+        for (int k = tid; k < ti.used; k += nthr) {
+            while (k >= send) {   // the segments are in tile order; each thread only moves forward
+                ++s;
+                const uint2    sg = sm.seg[s];
+                const uint32_t kk = sg.y >> 24;
+                send = (int)(((sg.y >> 12) & 4095u) + (sg.y & 4095u));
+                const int kx = (int)(kk & 3u) - 1, ky = (int)((kk >> 2) & 3u) - 1, kz = (int)((kk >> 4) & 3u) - 1;
+                ox = (double)ti.ox - (double)kx * (double)g.len[0];
+                oy = (double)ti.oy - (double)ky * (double)g.len[1];
+                oz = (double)ti.oz - (double)kz * (double)g.len[2];
+            }
+            const float4 p = sm.tile[k];
+            const float  x = (float)((double)p.x - ox), y = (float)((double)p.y - oy), z = (float)((double)p.z - oz);
+            sm.tile[k] = make_float4(x, y, z, fmaf(z, z, fmaf(y, y, x * x)));
+            sm.ms[k]   = p.w;
+        }
     }
-    for (int k = ti.used + lane; k < ti.nwords * 32 + 32; k += 32) {
+    for (int k = ti.used + tid; k < ti.nwords * 32 + 1; k += nthr) {
         sm.tile[k] = make_float4(0.0f, 0.0f, 0.0f, 3.0e37f);
-        sm.ms[k]   = 0.0f;
+        sm.ms[k]   = pad_w;
     }
-    __syncwarp();
+    __syncthreads();
+}
+
+// The first mask word at or behind nwords that belongs to warp wid of W (words w = wid mod W).
+__device__ __forceinline__ int sph_first_pad_word(int nwords, int wid, int W) {
+    const int r = (wid - nwords % W + W) % W;
+    return nwords + r;
 }
 
 // Phase 1: the accept masks of the lane's two targets over the whole tile.  Target t of the
@@ -313,7 +366,8 @@ __device__ __forceinline__ void sph_tile_finish(const SphGrid& g, const SphTileM
 // the caller leaves between Rc and the ball it relies on.  Rc <= 0 switches a target off.
 __device__ __forceinline__ void sph_tile_masks(const SphTileMem& sm, const SphTileInfo& ti,
                                                const float xt[2], const float yt[2],
-                                               const float zt[2], const float Rc[2], int lane) {
+                                               const float zt[2], const float Rc[2], int lane,
+                                               int wid, int W) {
     float ci[2];
 #pragma unroll
     for (int t = 0; t < 2; ++t)
@@ -323,7 +377,7 @@ __device__ __forceinline__ void sph_tile_masks(const SphTileMem& sm, const SphTi
     const sph_f2 ay = sph_pk(-2.0f * yt[0], -2.0f * yt[1]);
     const sph_f2 az = sph_pk(-2.0f * zt[0], -2.0f * zt[1]);
     const sph_f2 cc = sph_pk(ci[0], ci[1]);
-    for (int w = 0; w < ti.nwords; ++w) {
+    for (int w = wid; w < ti.nwords; w += W) {
         uint32_t m0 = 0u, m1 = 0u;
         const float4* c = sm.tile + w * 32;
 #pragma unroll
@@ -339,8 +393,12 @@ __device__ __forceinline__ void sph_tile_masks(const SphTileMem& sm, const SphTi
         sm.mask[w * SPH_TB + lane]      = m0;
         sm.mask[w * SPH_TB + 32 + lane] = m1;
     }
-#pragma unroll
-    for (int k = 0; k < 4; ++k) sm.mask[ti.nwords * SPH_TB + 32 * k + lane] = 0u;   // the cursors read ahead
+    // the cursor reads two words of its own stride ahead: this warp's first two words at or
+    // behind nwords are zero
+    for (int k = 0, w = sph_first_pad_word(ti.nwords, wid, W); k < 2; ++k, w += W) {
+        sm.mask[w * SPH_TB + lane]      = 0u;
+        sm.mask[w * SPH_TB + 32 + lane] = 0u;
+    }
     __syncwarp();
 }
 
@@ -361,20 +419,23 @@ __device__ __forceinline__ uint32_t sph_ldsu(uint32_t a) {
     return v;
 }
 
-// A lane's private cursor over the accept bits of one target, in tile order.  The word after
-// the current one is held in a register (`next`), so a refill never waits for shared memory.
+// A lane's private cursor over the accept bits of one target, in tile order, over the mask
+// words wid, wid + W, wid + 2 W, ... (the W warps that share a bucket split the words).  The
+// word after the current one is held in a register (`next`), so a refill never waits.
 struct SphCursor {
     uint32_t bits, next;
     uint32_t maddr;    // shared address of the word after `next`
     int      base31;   // 32 w + 31 for the current word w
 };
 __device__ __forceinline__ void sph_cursor_start(SphCursor& c, const SphTileMem& sm,
-                                                 const SphTileInfo& ti, int t, bool on) {
-    const uint32_t a = sm.mask_sa + 4u * (uint32_t)t;
-    c.base31 = on ? 31 : ti.nwords * 32 + 31;
-    c.bits   = on ? sph_ldsu(a) : 0u;
-    c.next   = on ? sph_ldsu(a + 4u * SPH_TB) : 0u;     // two zero words follow the last mask word
-    c.maddr  = a + 8u * SPH_TB;
+                                                 const SphTileInfo& ti, int t, bool on, int wid, int W) {
+    const uint32_t a = sm.mask_sa + 4u * (uint32_t)(wid * SPH_TB + t);
+    c.base31 = on ? 32 * wid + 31 : ti.nwords * 32 + 31;
+    c.bits   = on ? sph_ldsu(a) : 0u;                      // zero words follow the last mask word
+    c.next   = on ? sph_ldsu(a + 4u * SPH_TB * (uint32_t)W) : 0u;
+    // a cursor that is off must stay empty: it only ever reads the zero word
+    const uint32_t zw = sm.mask_sa + 4u * (uint32_t)((sph_first_pad_word(ti.nwords, wid, W) + W) * SPH_TB + t);
+    c.maddr  = on ? min(a + 8u * SPH_TB * (uint32_t)W, zw) : zw;
 }
 __device__ __forceinline__ bool sph_cursor_live(const SphCursor& c, const SphTileInfo& ti) {
     return c.base31 < ti.nwords * 32;
@@ -389,7 +450,7 @@ struct SphEntry {
 // Takes the next entry of the cursor and starts the loads of its record.  Straight-line code:
 // the refill of an exhausted word is predicated, the index of a bubble points at the padding.
 __device__ __forceinline__ void sph_cursor_fetch(SphCursor& c, const SphTileMem& sm, int idx_max,
-                                                 uint32_t mend, SphEntry& e) {
+                                                 uint32_t mend, int W, SphEntry& e) {
     uint32_t flo, bit;
     asm("bfind.u32 %0, %1;" : "=r"(flo) : "r"(c.bits));            // 0xffffffff for an empty word
     e.has = c.bits != 0u;
@@ -400,39 +461,67 @@ __device__ __forceinline__ void sph_cursor_fetch(SphCursor& c, const SphTileMem&
     e.m = sph_lds1(sm.ms_sa + 4u * (uint32_t)e.idx);               // padding entries carry m = 0
     if (c.bits == 0u) {
         c.bits   = c.next;
-        c.base31 += 32;
+        c.base31 += 32 * W;
         c.next   = sph_ldsu(c.maddr);
-        c.maddr  = min(c.maddr + 4u * SPH_TB, mend);
+        c.maddr  = min(c.maddr + 4u * SPH_TB * (uint32_t)W, mend);
     }
 }
 
-// Walks the accepted entries of the lane's two targets.  Two entry sets per target are used in
-// turn: the record of an entry is in flight while the entry before it is worked on, without
-// register copies.  work(t, entry) sees bubbles too (has = false, m = 0).
+// Advances the cursor by one step without touching the records (the steps other warps take).
+__device__ __forceinline__ void sph_cursor_skip(SphCursor& c, uint32_t mend, int W) {
+    uint32_t flo, bit;
+    asm("bfind.u32 %0, %1;" : "=r"(flo) : "r"(c.bits));
+    asm("shl.b32 %0, %1, %2;" : "=r"(bit) : "r"(1u), "r"(flo));
+    c.bits ^= bit;
+    if (c.bits == 0u) {
+        c.bits   = c.next;
+        c.base31 += 32 * W;
+        c.next   = sph_ldsu(c.maddr);
+        c.maddr  = min(c.maddr + 4u * SPH_TB * (uint32_t)W, mend);
+    }
+}
+
+// Walks the accepted entries of the lane's two targets.  Two ways to share a bucket between
+// the W warps of a block:
+//   by words   (es = 1): this warp's cursor runs over the mask words wid, wid + W, ...;
+//   by entries (es = W): every warp's cursor runs over all words, and this warp takes the steps
+//                        ep, ep + es, ... of it (bubbles included), which balances the work
+//                        of a lane exactly when the per-entry work dominates the cursor's.
+// Two entry sets per target are used in turn: the record of an entry is in flight while the
+// entry before it is worked on, without register copies.  work(t, entry) sees bubbles too
+// (has = false; the padding record, m = pad_w of sph_tile_finish).
 template <class Work>
 __device__ __forceinline__ void sph_tile_walk(const SphTileMem& sm, const SphTileInfo& ti, int lane,
-                                              const bool on[2], Work&& work) {
+                                              int wid, int W, const bool on[2], Work&& work,
+                                              int ep = 0, int es = 1) {
     SphCursor cu[2];
     SphEntry  ea[2], eb[2];
-    const int      idx_max = ti.nwords * 32;                               // first padding entry
-    const uint32_t mend = sm.mask_sa + 4u * (uint32_t)((ti.nwords + 1) * SPH_TB);   // a zero word
+    const int idx_max = ti.nwords * 32;                               // first padding entry
+    // this warp's second zero word behind the masks
+    const uint32_t mend = sm.mask_sa + 4u * (uint32_t)((sph_first_pad_word(ti.nwords, wid, W) + W) * SPH_TB);
+    auto fetch = [&](int t, SphEntry& e) {
+        const uint32_t me = mend + 4u * (uint32_t)(lane + 32 * t);
+        for (int s = 0; s < ep; ++s) sph_cursor_skip(cu[t], me, W);
+        sph_cursor_fetch(cu[t], sm, idx_max, me, W, e);
+        for (int s = ep + 1; s < es; ++s) sph_cursor_skip(cu[t], me, W);
+    };
 #pragma unroll
     for (int t = 0; t < 2; ++t) {
-        sph_cursor_start(cu[t], sm, ti, lane + 32 * t, on[t]);
-        sph_cursor_fetch(cu[t], sm, idx_max, mend + 4u * (uint32_t)(lane + 32 * t), ea[t]);
-        sph_cursor_fetch(cu[t], sm, idx_max, mend + 4u * (uint32_t)(lane + 32 * t), eb[t]);
+        sph_cursor_start(cu[t], sm, ti, lane + 32 * t, on[t], wid, W);
+        fetch(t, ea[t]);
+        fetch(t, eb[t]);
     }
     while (__any_sync(SPH_FULL, ea[0].has || ea[1].has || eb[0].has || eb[1].has ||
                                     sph_cursor_live(cu[0], ti) || sph_cursor_live(cu[1], ti))) {
 #pragma unroll
         for (int t = 0; t < 2; ++t) {
             work(t, ea[t]);
-            sph_cursor_fetch(cu[t], sm, idx_max, mend + 4u * (uint32_t)(lane + 32 * t), ea[t]);
+            fetch(t, ea[t]);
         }
 #pragma unroll
         for (int t = 0; t < 2; ++t) {
             work(t, eb[t]);
-            sph_cursor_fetch(cu[t], sm, idx_max, mend + 4u * (uint32_t)(lane + 32 * t), eb[t]);
+            fetch(t, eb[t]);
         }
     }
 }

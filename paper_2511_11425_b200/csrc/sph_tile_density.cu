@@ -155,27 +155,42 @@ __device__ __forceinline__ void c2_poly(const float M[6], float lam, float& S, f
 }
 
 // ------------------------------------------------------------------------------------------
-// a4-a6 on the tile.  One warp per block, persistent: buckets are handed out by a counter.
+// a4-a6 on the tile.  Persistent blocks of W warps; a block takes one bucket at a time (handed
+// out by a counter).  Every warp holds the bucket's 64 targets (lane l: targets l and l + 32)
+// and works on its share of the tile -- the candidates for the frame transform, the mask words
+// w = wid, wid + W, ... for phase 1 and for the walk -- so W warps hide each other's latencies
+// on one tile's worth of shared memory.  The partial sums meet in shared memory; every warp
+// then runs the same scalar solve (identical state in all warps, no broadcast), warp 0 alone
+// finishes (zone pass, results).
 // ------------------------------------------------------------------------------------------
+constexpr int DT_NPART = 8;   // words per target and warp in the exchange area: 6 sums, entries, zone entries
+
 template <int KERN>
-__global__ __launch_bounds__(32) void k_density_tile(
+__global__ __launch_bounds__(SPH_TWMAX * 32) void k_density_tile(
     const SphGrid* __restrict__ gp, const uint32_t* __restrict__ cell_start,
     const float4* __restrict__ pos_m, const int32_t* __restrict__ perm,
-    const SphBucket* __restrict__ buckets, const unsigned* __restrict__ nbuckets, unsigned* next,
+    const SphBucket* __restrict__ buckets, const unsigned* __restrict__ nbuckets,
+    const uint32_t* __restrict__ blist, unsigned* big_list, unsigned* big_cnt, unsigned* next,
     TilePar par, float* h_io, float* rho, float* omega, int32_t* nn, int32_t* fix_list,
-    unsigned* fix_cnt, uint32_t* fb_list, unsigned* fb_cnt, float* nb_rkeep,
+    unsigned* fix_cnt, uint32_t* fb_list, unsigned* fb_cnt, uint32_t* nb_j, unsigned nb_regions,
+    unsigned* list_next, uint32_t* bucket_loff, uint32_t* nb_cnt, float* nb_rkeep, float* tl_rkeep,
     unsigned long long* stats) {
     constexpr bool MOM = (KERN == 1);   // the moment solve exists for Wendland C2
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    __shared__ SphGrid g;
-    const int lane = threadIdx.x;
-    for (int k = lane; k < (int)(sizeof(SphGrid) / 4); k += 32) ((int*)&g)[k] = ((const int*)gp)[k];
-    __syncwarp();
-    const SphTileMem sm = sph_tile_carve<16>(smem_raw, par.tcap);
-    float* const edge = (float*)sm.zone;   // Halley path: [4][64] floats in the zone area
-    if (lane == 0) sph_mbar_init(sm.bar, 1u);
+    __shared__ SphGrid     g;
+    __shared__ SphTileInfo ti;
+    __shared__ unsigned    bi_s;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5, W = blockDim.x >> 5, nthr = blockDim.x;
+    for (int k = tid; k < (int)(sizeof(SphGrid) / 4); k += nthr) ((int*)&g)[k] = ((const int*)gp)[k];
+    const SphTileMem sm = sph_tile_carve<16>(smem_raw, par.tcap, sph_tile_xbytes(W, DT_NPART), W);
+    // exchange area of the partial sums [W][DT_NPART][64]: the segment table's memory, which is
+    // dead once the tile is in place
+    float* const xch = (float*)sm.seg;
+    const int ZW = SPH_TZCAP / W;          // zone slots per warp: [wid * ZW, +ZW)
+    float* const edge = (float*)sm.zone;   // Halley path: [W][4][64] floats in the zone area
+    if (tid == 0) sph_mbar_init(sm.bar, 1u);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    __syncwarp();
+    __syncthreads();
     uint32_t parity = 0;
     const unsigned nb = *nbuckets;
     const float hcap = tile_hcap(g);
@@ -184,10 +199,12 @@ __global__ __launch_bounds__(32) void k_density_tile(
     unsigned c_listed = 0, c_pairs = 0, c_sweeps = 0, c_recollect = 0;
 
     for (;;) {
-        unsigned bi = 0;
-        if (lane == 0) bi = atomicAdd(next, 1u);
-        bi = __shfl_sync(SPH_FULL, bi, 0);
-        if (bi >= nb) break;
+        __syncthreads();                     // the last bucket's tile and tables are free
+        if (tid == 0) bi_s = atomicAdd(next, 1u);
+        __syncthreads();
+        if (bi_s >= nb) break;
+        // the buckets of the table, or (second pass, larger tile) the ones the first pass left
+        const unsigned  bi = blist ? blist[bi_s] : bi_s;
         const SphBucket bk = buckets[bi];
 
         // ---- the bucket's targets: rows (ry0 + a, rz0 + b), cells [c0, c1) of each
@@ -207,7 +224,8 @@ __global__ __launch_bounds__(32) void k_density_tile(
             if (lane >= o) inc += t;
         }
         const int ntar = min(__shfl_sync(SPH_FULL, inc, 31), SPH_TB);
-        sm.rowoff[lane] = inc;                   // inclusive prefix of the row counts
+        int* const rowoff = sm.rowoff + 32 * wid;   // in the mask area: free until phase 1
+        rowoff[lane] = inc;                      // inclusive prefix of the row counts
         __syncwarp();
         int    p[2];
         bool   valid[2];
@@ -218,8 +236,8 @@ __global__ __launch_bounds__(32) void k_density_tile(
             const int k = lane + 32 * t;
             valid[t] = k < ntar;
             int rho_ = 0;
-            while (rho_ < 31 && sm.rowoff[rho_] <= k) ++rho_;
-            const int before = rho_ ? sm.rowoff[rho_ - 1] : 0;
+            while (rho_ < 31 && rowoff[rho_] <= k) ++rho_;
+            const int before = rho_ ? rowoff[rho_ - 1] : 0;
             const int start  = __shfl_sync(SPH_FULL, rs, rho_);
             p[t] = valid[t] ? start + (k - before) : 0;
             float4 pi = make_float4(0.f, 0.f, 0.f, 1.f);
@@ -252,7 +270,7 @@ __global__ __launch_bounds__(32) void k_density_tile(
         }
 
         float T[2], hlo[2], hhi[2], S[2], E[2], Rc[2], want[2];
-        bool  done[2], fix[2], wait[2], recount[2];
+        bool  done[2], fix[2], wait[2], recount[2], mvalid[2];
         int   sweeps[2], ni[2];
 #pragma unroll
         for (int t = 0; t < 2; ++t) {
@@ -261,17 +279,39 @@ __global__ __launch_bounds__(32) void k_density_tile(
             S[t] = 0.0f; E[t] = 0.0f; Rc[t] = 0.0f;
             done[t] = !valid[t]; fix[t] = false; wait[t] = valid[t];
             want[t] = valid[t] ? 2.0f * h[t] * lslack : 0.0f;
-            sweeps[t] = 0; ni[t] = 0; recount[t] = false;
+            sweeps[t] = 0; ni[t] = 0; recount[t] = false; mvalid[t] = false;
         }
         bool fallback = false;
+        // The neighbour lists kept for the force sweep ("we keep the precomputed
+        // interaction list"): entry f of target t of this bucket at lbase[f * 64 + t], the
+        // sorted position of the source -- written from the sweep as the entries are met, so a
+        // warp's stores fall into a few 256-byte rows.  The bucket takes one region of
+        // SPH_LCAP x 64 words from the pool (none left: no lists, the force sweep searches).
+        uint32_t* lbase = nullptr;
+        if (nb_j != nullptr && W == 1) {
+            unsigned reg = 0xffffffffu;
+            if (lane == 0) {
+                reg = atomicAdd(list_next, 1u);
+                if (reg >= nb_regions) reg = 0xffffffffu;
+                bucket_loff[bi] = reg;
+            }
+            reg = __shfl_sync(SPH_FULL, reg, 0);
+            if (reg != 0xffffffffu) lbase = nb_j + (size_t)reg * (SPH_LCAP * SPH_TB);
+        }
+        int nlist[2] = {0, 0};
 
         // ---- stages: (re)build the tile for the largest list radius wanted
         for (int stage = 0; stage < 4; ++stage) {
             const float Rt = warp_max(fmaxf(wait[0] ? want[0] : 0.0f, wait[1] ? want[1] : 0.0f));
             if (!(Rt > 0.0f)) break;
-            SphTileInfo ti;
-            const bool staged = sph_tile_stage(g, cell_start, pos_m, b0, b1, Rt * (1.0f + 1e-5f), sm, lane, ti);
-            if (!staged) {
+            __syncthreads();                 // everybody is done with the old tile and the exchange area
+            if (wid == 0) {
+                SphTileInfo tl;
+                tl.ok = sph_tile_stage(g, cell_start, pos_m, b0, b1, Rt * (1.0f + 1e-5f), sm, lane, tl) ? 1 : 0;
+                if (lane == 0) ti = tl;
+            }
+            __syncthreads();
+            if (!ti.ok) {
                 if (stage == 0) fallback = true;
                 else {
 #pragma unroll
@@ -280,7 +320,8 @@ __global__ __launch_bounds__(32) void k_density_tile(
                 break;
             }
             if (stage > 0) c_recollect += (wait[0] ? 1u : 0u) + (wait[1] ? 1u : 0u);
-            sph_tile_finish(g, sm, ti, parity, lane);
+            mvalid[0] = mvalid[1] = false;   // a new tile: the masks of the old one are gone
+            sph_tile_finish(g, sm, ti, parity, tid, nthr, 0.0f);
             parity ^= 1u;
             // the targets in the frame of the tile
             float xt[2], yt[2], zt[2];
@@ -295,7 +336,7 @@ __global__ __launch_bounds__(32) void k_density_tile(
             for (int t = 0; t < 2; ++t)
                 if (wait[t]) { wait[t] = false; Rc[t] = fminf(want[t], Rt); }
             bool remask = true;
-            c_tested += (unsigned long long)ti.used * (unsigned)ntar;   // uniform: lane 0 reports it
+            c_tested += (unsigned long long)ti.used * (unsigned)ntar;   // uniform: thread 0 reports it
 
             // ---- sweeps on this tile
             while (__any_sync(SPH_FULL, (!done[0] && !wait[0]) || (!done[1] && !wait[1]))) {
@@ -304,28 +345,26 @@ __global__ __launch_bounds__(32) void k_density_tile(
                     float rr[2];
 #pragma unroll
                     for (int t = 0; t < 2; ++t) rr[t] = on[t] ? Rc[t] : 0.0f;
-                    sph_tile_masks(sm, ti, xt, yt, zt, rr, lane);
+                    sph_tile_masks(sm, ti, xt, yt, zt, rr, lane, wid, W);   // this warp's words only
                     remask = false;
+#pragma unroll
+                    for (int t = 0; t < 2; ++t) mvalid[t] = on[t];   // finished targets lost theirs
                 }
-                int nent[2] = {0, 0};
                 if constexpr (MOM) {
                     // ---- one sweep: the six Bernstein moments, the zone list, the entry count
                     float M[2][6];
                     float ihh[2];
-                    int   nz[2] = {0, 0};
+                    int   nz[2] = {0, 0}, nent[2] = {0, 0};
+                    uint32_t za[2], zend[2];
 #pragma unroll
                     for (int t = 0; t < 2; ++t) {
                         ihh[t] = __fdividef(0.5f, h[t]);
 #pragma unroll
                         for (int k = 0; k < 6; ++k) M[t][k] = 0.0f;
+                        za[t]   = sm.zone_sa + 2u * (uint32_t)(wid * ZW * SPH_TB + lane + 32 * t);
+                        zend[t] = za[t] + 2u * SPH_TB * (ZW - 1);
                     }
-                    uint32_t za[2], zend[2];
-#pragma unroll
-                    for (int t = 0; t < 2; ++t) {
-                        za[t]   = sm.zone_sa + 2u * (uint32_t)(lane + 32 * t);
-                        zend[t] = za[t] + 2u * SPH_TB * (SPH_TZCAP - 1);
-                    }
-                    sph_tile_walk(sm, ti, lane, on, [&](int t, const SphEntry& en) {
+                    sph_tile_walk(sm, ti, lane, wid, W, on, [&](int t, const SphEntry& en) {
                         const float dx = xt[t] - en.c.x, dy = yt[t] - en.c.y, dz = zt[t] - en.c.z;
                         const float r  = sph_sqrt(fmaf(dz, dz, fmaf(dy, dy, dx * dx)));
                         const float s  = r * ihh[t], tt = 1.0f - s;
@@ -337,6 +376,8 @@ __global__ __launch_bounds__(32) void k_density_tile(
                         M[t][3] = fmaf(a3, t2, M[t][3]);
                         M[t][4] = fmaf(a4, tt, M[t][4]);
                         M[t][5] += a5;
+                        if (lbase != nullptr && en.has && nent[t] < SPH_LCAP)   // the kept list (a set: any sweep of this mask writes the same)
+                            lbase[nent[t] * SPH_TB + lane + 32 * t] = sm.gidx[en.idx];
                         nent[t] += en.has ? 1 : 0;
                         // next to (or beyond) the support edge: remember the entry (predicated
                         // store; past the capacity the last slot is overwritten and nz says so)
@@ -346,11 +387,52 @@ __global__ __launch_bounds__(32) void k_density_tile(
                         za[t] = inz ? min(za[t] + 2u * SPH_TB, zend[t]) : za[t];
                         nz[t] += inz ? 1 : 0;
                     });
+                    // ---- the warps' partial sums meet in shared memory; fixed order of addition
+                    int  nzw[2][SPH_TWMAX];
+                    bool zfit[2];
+#pragma unroll
+                    for (int t = 0; t < 2; ++t) {
+#pragma unroll
+                        for (int w = 0; w < SPH_TWMAX; ++w) nzw[t][w] = 0;
+                        nzw[t][0] = nz[t];
+                        zfit[t]   = nz[t] <= ZW;
+                    }
+                    if (W > 1) {
+#pragma unroll
+                        for (int t = 0; t < 2; ++t) {
+                            float* x = xch + (wid * DT_NPART) * SPH_TB + lane + 32 * t;
+#pragma unroll
+                            for (int k = 0; k < 6; ++k) x[k * SPH_TB] = M[t][k];
+                            x[6 * SPH_TB] = __int_as_float(nent[t]);
+                            x[7 * SPH_TB] = __int_as_float(nz[t]);
+                        }
+                        __syncthreads();
+#pragma unroll
+                        for (int t = 0; t < 2; ++t) {
+                            nent[t] = 0; nz[t] = 0; zfit[t] = true;
+#pragma unroll
+                            for (int k = 0; k < 6; ++k) M[t][k] = 0.0f;
+#pragma unroll
+                            for (int w = 0; w < SPH_TWMAX; ++w) {
+                                nzw[t][w] = 0;
+                                if (w >= W) continue;
+                                const float* x = xch + (w * DT_NPART) * SPH_TB + lane + 32 * t;
+#pragma unroll
+                                for (int k = 0; k < 6; ++k) M[t][k] += x[k * SPH_TB];
+                                nent[t] += __float_as_int(x[6 * SPH_TB]);
+                                const int q = __float_as_int(x[7 * SPH_TB]);
+                                nzw[t][w] = q;
+                                nz[t] += q;
+                                zfit[t] = zfit[t] && q <= ZW;
+                            }
+                        }
+                    }
 #pragma unroll
                     for (int t = 0; t < 2; ++t) {
                         if (!on[t]) continue;
                         if (sweeps[t] == 0) c_listed += (unsigned)nent[t];
                         ++sweeps[t];
+                        nlist[t] = nent[t];
                         // the sign of f at the swept h keeps the bracket (the zone's clamp is O(T_ZONE^4))
                         const float f0 = M[t][0] + 5.0f * M[t][1] - T[t];
                         if (f0 < 0.0f) hlo[t] = h[t]; else hhi[t] = h[t];
@@ -364,30 +446,30 @@ __global__ __launch_bounds__(32) void k_density_tile(
                             lam *= 1.0f + __fdividef(Sp - T[t], Ep);
                             lam = fminf(fmaxf(lam, 0.5f), 2.0f);
                         }
-                        const bool zfit = nz[t] <= SPH_TZCAP;
-#ifdef SPH_DEBUG_TILE
-                        if (bi == 0 && lane < 2) printf("dbg lane %d t %d h %g nent %d nz %d M %g %g %g %g %g %g T %g lam %g okp %d Sp %g Ep %g\n", lane, t, h[t], nent[t], nz[t], M[t][0], M[t][1], M[t][2], M[t][3], M[t][4], M[t][5], T[t], lam, (int)okp, Sp, Ep);
-#endif
-                        if (okp && zfit && fabsf(1.0f - lam) <= 0.9f * T_ZONE && h[t] / lam <= hcap) {
+                        if (okp && zfit[t] && fabsf(1.0f - lam) <= 0.9f * T_ZONE && h[t] / lam <= hcap) {
+                            done[t] = true;
+                            if (wid != 0) continue;   // warp 0 finishes alone
                             // ---- final: put the clamped zone entries right at lam, one more step
                             const float eps = 1.0f - lam;
                             float dS = 0.0f, dE = 0.0f, amin = 3.0e38f;
                             int   cz = 0;
-                            for (int q = 0; q < nz[t]; ++q) {
-                                const int    idx = sm.zone[q * SPH_TB + lane + 32 * t];
-                                const float4 c   = sm.tile[idx];
-                                const float  mj  = sm.ms[idx];
-                                const float dx = xt[t] - c.x, dy = yt[t] - c.y, dz = zt[t] - c.z;
-                                const float r  = sph_sqrt(fmaf(dz, dz, fmaf(dy, dy, dx * dx)));
-                                const float s  = r * ihh[t], tt = 1.0f - s;
-                                const float tq = fmaf(eps, s, tt), sq = lam * s;   // t', s' at lam
-                                amin = fminf(amin, fabsf(tq));
-                                if (tq < 0.0f) {
-                                    const float q2 = tq * tq, q3 = q2 * tq;
-                                    dS -= mj * q2 * q2 * (tq + 5.0f * sq);
-                                    dE -= 20.0f * mj * sq * sq * q3;
-                                } else ++cz;
-                            }
+#pragma unroll
+                            for (int w = 0; w < SPH_TWMAX; ++w)
+                                for (int q = 0; q < nzw[t][w]; ++q) {
+                                    const int    idx = sm.zone[(w * ZW + q) * SPH_TB + lane + 32 * t];
+                                    const float4 c   = sm.tile[idx];
+                                    const float  mj  = sm.ms[idx];
+                                    const float dx = xt[t] - c.x, dy = yt[t] - c.y, dz = zt[t] - c.z;
+                                    const float r  = sph_sqrt(fmaf(dz, dz, fmaf(dy, dy, dx * dx)));
+                                    const float s  = r * ihh[t], tt = 1.0f - s;
+                                    const float tq = fmaf(eps, s, tt), sq = lam * s;   // t', s' at lam
+                                    amin = fminf(amin, fabsf(tq));
+                                    if (tq < 0.0f) {
+                                        const float q2 = tq * tq, q3 = q2 * tq;
+                                        dS -= mj * q2 * q2 * (tq + 5.0f * sq);
+                                        dE -= 20.0f * mj * sq * sq * q3;
+                                    } else ++cz;
+                                }
                             c2_poly(M[t], lam, Sp, Ep);
                             float lam2 = lam * (1.0f + __fdividef(Sp + dS - T[t], Ep + dE));
                             c2_poly(M[t], lam2, Sp, Ep);
@@ -397,7 +479,6 @@ __global__ __launch_bounds__(32) void k_density_tile(
                             ni[t] = nent[t] - nz[t] + cz;
                             // an entry closer to the edge than the band plus the last step: exact recount
                             recount[t] = amin <= taun + 1.5f * fabsf(lam2 - lam);
-                            done[t] = true;
                             continue;
                         }
                         // ---- a step only: move, keep inside the bracket, sweep again
@@ -407,7 +488,7 @@ __global__ __launch_bounds__(32) void k_density_tile(
                         if (hhi[t] < 3.0e38f && !(hn >= hlo[t] && hn <= hhi[t])) hn = 0.5f * (hlo[t] + hhi[t]);
                         const bool capped = hn >= hcap && h[t] >= hcap;
                         hn = fminf(hn, hcap);
-                        if (capped || sweeps[t] >= par.max_iter || (hhi[t] - hlo[t]) <= par.tol * h[t] || !zfit) {
+                        if (capped || sweeps[t] >= par.max_iter || (hhi[t] - hlo[t]) <= par.tol * h[t] || !zfit[t]) {
                             done[t] = true; fix[t] = true;   // k_density_fix settles it (and counts non-convergence)
                             continue;
                         }
@@ -419,7 +500,8 @@ __global__ __launch_bounds__(32) void k_density_tile(
                 } else {
                     // ---- Halley path: S, E, F at h; interior count and the entries next to the edge
                     float ih[2], Hlo[2], Hhi[2], s[2], e[2], f2[2];
-                    int   cin[2], ne[2];
+                    int   cin[2], ne[2], nent[2] = {0, 0};
+                    float* const myedge = edge + wid * 4 * SPH_TB;
 #pragma unroll
                     for (int t = 0; t < 2; ++t) {
                         ih[t]  = __fdividef(1.0f, h[t]);
@@ -427,7 +509,7 @@ __global__ __launch_bounds__(32) void k_density_tile(
                         Hhi[t] = 2.0f * h[t] * (1.0f + T_EDGE);
                         s[t] = 0.0f; e[t] = 0.0f; f2[t] = 0.0f; cin[t] = 0; ne[t] = 0;
                     }
-                    sph_tile_walk(sm, ti, lane, on, [&](int t, const SphEntry& en) {
+                    sph_tile_walk(sm, ti, lane, wid, W, on, [&](int t, const SphEntry& en) {
                         const float4 c = en.c;
                         const float  mj = en.m;
                         const bool   has = en.has;
@@ -438,18 +520,57 @@ __global__ __launch_bounds__(32) void k_density_tile(
                         s[t]  = fmaf(mj, wq, s[t]);
                         e[t]  = fmaf(mj, eq, e[t]);
                         f2[t] = fmaf(mj, fq, f2[t]);
+                        if (lbase != nullptr && has && nent[t] < SPH_LCAP) {
+#ifdef SPH_DEBUG_TILE
+                            if (sm.gidx[en.idx] > 100000000u) printf("bad gidx %u idx %d used %d nwords %d tcap %d stage %d bucket %u lane %d t %d f %d\n", sm.gidx[en.idx], en.idx, ti.used, ti.nwords, par.tcap, stage, bi, lane, t, nent[t]);
+#endif
+                            lbase[nent[t] * SPH_TB + lane + 32 * t] = sm.gidx[en.idx];
+                        }
                         nent[t] += has ? 1 : 0;
                         cin[t]  += (has && r < Hlo[t]) ? 1 : 0;
                         if (has && r >= Hlo[t] && r < Hhi[t]) {
-                            if (ne[t] < 4) edge[ne[t] * SPH_TB + lane + 32 * t] = r;
+                            if (ne[t] < 4) myedge[ne[t] * SPH_TB + lane + 32 * t] = r;
                             ++ne[t];
                         }
                     });
+                    int new_[2][SPH_TWMAX];
+#pragma unroll
+                    for (int t = 0; t < 2; ++t) {
+#pragma unroll
+                        for (int w = 0; w < SPH_TWMAX; ++w) new_[t][w] = 0;
+                        new_[t][0] = ne[t];
+                    }
+                    if (W > 1) {
+#pragma unroll
+                        for (int t = 0; t < 2; ++t) {
+                            float* x = xch + (wid * DT_NPART) * SPH_TB + lane + 32 * t;
+                            x[0] = s[t]; x[SPH_TB] = e[t]; x[2 * SPH_TB] = f2[t];
+                            x[3 * SPH_TB] = __int_as_float(cin[t]);
+                            x[4 * SPH_TB] = __int_as_float(ne[t]);
+                            x[5 * SPH_TB] = __int_as_float(nent[t]);
+                        }
+                        __syncthreads();
+#pragma unroll
+                        for (int t = 0; t < 2; ++t) {
+                            s[t] = 0.0f; e[t] = 0.0f; f2[t] = 0.0f; cin[t] = 0; nent[t] = 0;
+#pragma unroll
+                            for (int w = 0; w < SPH_TWMAX; ++w) {
+                                new_[t][w] = 0;
+                                if (w >= W) continue;
+                                const float* x = xch + (w * DT_NPART) * SPH_TB + lane + 32 * t;
+                                s[t] += x[0]; e[t] += x[SPH_TB]; f2[t] += x[2 * SPH_TB];
+                                cin[t] += __float_as_int(x[3 * SPH_TB]);
+                                new_[t][w] = __float_as_int(x[4 * SPH_TB]);
+                                nent[t] += __float_as_int(x[5 * SPH_TB]);
+                            }
+                        }
+                    }
 #pragma unroll
                     for (int t = 0; t < 2; ++t) {
                         if (!on[t]) continue;
                         if (sweeps[t] == 0) c_listed += (unsigned)nent[t];
                         ++sweeps[t];
+                        nlist[t] = nent[t];
                         const float es = SphKernel<KERN>::escale * e[t];
                         float hn, Sn, En;
                         bool  conv;
@@ -460,11 +581,15 @@ __global__ __launch_bounds__(32) void k_density_tile(
                         if (acc && needR <= Rc[t]) {
                             const float H = 2.0f * hn, tauH = taun * H;
                             int  n = cin[t];
-                            bool eg = ne[t] > 4;
-                            for (int q = 0; q < min(ne[t], 4); ++q) {
-                                const float r = edge[q * SPH_TB + lane + 32 * t];
-                                n += (r < H) ? 1 : 0;
-                                eg |= fabsf(r - H) <= tauH;
+                            bool eg = false;
+#pragma unroll
+                            for (int w = 0; w < SPH_TWMAX; ++w) {
+                                eg |= new_[t][w] > 4;
+                                for (int q = 0; q < min(new_[t][w], 4); ++q) {
+                                    const float r = edge[(w * 4 + q) * SPH_TB + lane + 32 * t];
+                                    n += (r < H) ? 1 : 0;
+                                    eg |= fabsf(r - H) <= tauH;
+                                }
                             }
                             S[t] = Sn; E[t] = En; h[t] = hn; ni[t] = n;
                             done[t] = true;
@@ -481,14 +606,22 @@ __global__ __launch_bounds__(32) void k_density_tile(
                         }
                     }
                 }
+                // the exchange area and the zone / edge slots are rewritten by the next sweep
+                if (W > 1 && __any_sync(SPH_FULL, (!done[0] && !wait[0]) || (!done[1] && !wait[1]))) __syncthreads();
             }
         }
 
-        // ---- results
-        if (fallback) {   // whole bucket to the 8-lanes-per-target kernel
+        // ---- results (warp 0; the state is the same in every warp)
+        if (wid != 0) continue;
+        if (fallback) {
+            if (lbase != nullptr && lane == 0) bucket_loff[bi] = 0xffffffffu;   // no tile-format list
+            if (big_list) {   // to the second pass, which has a larger tile
+                if (lane == 0) big_list[atomicAdd(big_cnt, 1u)] = bi;
+            } else {          // whole bucket to the 8-lanes-per-target kernel
 #pragma unroll
-            for (int t = 0; t < 2; ++t)
-                if (valid[t]) fb_list[atomicAdd(fb_cnt, 1u)] = (uint32_t)p[t];
+                for (int t = 0; t < 2; ++t)
+                    if (valid[t]) fb_list[atomicAdd(fb_cnt, 1u)] = (uint32_t)p[t];
+            }
             continue;
         }
 #pragma unroll
@@ -497,7 +630,11 @@ __global__ __launch_bounds__(32) void k_density_tile(
             if (wait[t] || !done[t]) { fix[t] = true; done[t] = true; }
             const int i = ic[t];
             h_io[i] = h[t];
-            nb_rkeep[p[t]] = 0.0f;     // no 8-lane list for this target
+            // the list is complete inside the radius of its mask (less the rounding margin of phase 1)
+            const bool lok = lbase != nullptr && !fix[t] && mvalid[t] && nlist[t] <= SPH_LCAP;
+            nb_rkeep[p[t]] = 0.0f;     // no [target][entry] list of the 8-lane kernels for this target
+            tl_rkeep[p[t]] = lok ? Rc[t] * (1.0f - 1e-4f) : 0.0f;
+            nb_cnt[p[t]]   = lok ? (uint32_t)nlist[t] : 0u;
             c_sweeps += (unsigned)sweeps[t];
             if (!fix[t]) {
                 const float ih = 1.0f / h[t];
@@ -511,15 +648,17 @@ __global__ __launch_bounds__(32) void k_density_tile(
         }
     }
 
-    // ---- counters: one atomic per warp and counter
-    const unsigned tl = __reduce_add_sync(SPH_FULL, c_listed), tp = __reduce_add_sync(SPH_FULL, c_pairs);
-    const unsigned tsw = __reduce_add_sync(SPH_FULL, c_sweeps), trc = __reduce_add_sync(SPH_FULL, c_recollect);
-    if (lane == 0) {
-        if (c_tested) atomicAdd(stats + ST_DENS_TESTED, c_tested);
-        if (tl) atomicAdd(stats + ST_DENS_LISTED, (unsigned long long)tl);
-        if (tp) atomicAdd(stats + ST_DENS_PAIRS, (unsigned long long)tp);
-        if (tsw) atomicAdd(stats + ST_DENS_SWEEPS, (unsigned long long)tsw);
-        if (trc) atomicAdd(stats + ST_DENS_RECOLLECT, (unsigned long long)trc);
+    // ---- counters (warp 0 holds them): one atomic per block and counter
+    if (wid == 0) {
+        const unsigned tl = __reduce_add_sync(SPH_FULL, c_listed), tp = __reduce_add_sync(SPH_FULL, c_pairs);
+        const unsigned tsw = __reduce_add_sync(SPH_FULL, c_sweeps), trc = __reduce_add_sync(SPH_FULL, c_recollect);
+        if (lane == 0) {
+            if (c_tested) atomicAdd(stats + ST_DENS_TESTED, c_tested);
+            if (tl) atomicAdd(stats + ST_DENS_LISTED, (unsigned long long)tl);
+            if (tp) atomicAdd(stats + ST_DENS_PAIRS, (unsigned long long)tp);
+            if (tsw) atomicAdd(stats + ST_DENS_SWEEPS, (unsigned long long)tsw);
+            if (trc) atomicAdd(stats + ST_DENS_RECOLLECT, (unsigned long long)trc);
+        }
     }
 }
 
@@ -534,26 +673,45 @@ int sph_launch_buckets(sph_ctx* c) {
     return SPH_OK;
 }
 
-// Runs the tile kernel over all buckets; the targets it hands back are in c->fb_list
-// (c->fb_cnt of them) and are swept by the caller with the 8-lanes-per-target kernel.
+// Runs the tile kernel over all buckets with a tile of tile_cap candidates (sized for the
+// occupancy), then over the buckets that did not fit with a tile of SPH_TCAP_BIG; the targets
+// left after that are in c->fb_list (c->fb_cnt of them) and are swept by the caller with the
+// 8-lanes-per-target kernel.
+#define SPH_TCAP_BIG 2560
 int sph_launch_density_tile(sph_ctx* c, float* h, float* rho, float* omega, int32_t* nn) {
     cudaStream_t s = c->stream;
-    TilePar par{c->par.n_ngb, c->par.h_tol, c->par.search_slack, c->par.h_max_iter, c->par.tile_cap};
-    const size_t smem = sph_tile_smem_bytes(par.tcap, 16);
-    SPH_CUDA_CHECK(c, cudaMemsetAsync(c->tile_next, 0, 2 * sizeof(unsigned), s));
+    const int W = c->par.tile_warps;
+    SPH_CUDA_CHECK(c, cudaMemsetAsync(c->tile_next, 0, 4 * sizeof(unsigned), s));
     SPH_CUDA_CHECK(c, cudaMemsetAsync(c->fb_cnt, 0, sizeof(unsigned), s));
+    SPH_CUDA_CHECK(c, cudaMemsetAsync(c->big_cnt, 0, sizeof(unsigned), s));
+    SPH_CUDA_CHECK(c, cudaMemsetAsync(c->list_next, 0, sizeof(unsigned), s));
+    SPH_CUDA_CHECK(c, cudaMemsetAsync(c->bucket_loff, 0xff, (size_t)c->n_max * sizeof(uint32_t), s));
     auto launch = [&](auto tag) -> cudaError_t {
         constexpr int KERN = decltype(tag)::value;
-        cudaError_t e = cudaFuncSetAttribute(k_density_tile<KERN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        int per_sm = 0;
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_density_tile<KERN>, 32, smem);
-        if (e != cudaSuccess) return e;
-        if (per_sm < 1) per_sm = 1;
-        k_density_tile<KERN><<<c->sm_count * per_sm, 32, smem, s>>>(
-            c->grid, c->cell_start, c->pos_m, c->perm, c->buckets, c->bucket_cnt, c->tile_next, par, h,
-            rho, omega, nn, c->fix_list, c->fix_cnt, c->fb_list, c->fb_cnt, c->nb_rkeep, c->stats);
-        return cudaGetLastError();
+        for (int pass = 0; pass < 2; ++pass) {
+            const int tcap = pass == 0 ? c->par.tile_cap : SPH_TCAP_BIG;
+            if (pass == 1 && c->par.tile_cap >= SPH_TCAP_BIG) break;
+            TilePar par{c->par.n_ngb, c->par.h_tol, c->par.search_slack, c->par.h_max_iter, tcap};
+            const size_t smem = sph_tile_smem_bytes(tcap, 16, sph_tile_xbytes(W, 8), W);
+            cudaError_t e = cudaFuncSetAttribute(k_density_tile<KERN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (e != cudaSuccess) return e;
+            int per_sm = 0;
+            e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_density_tile<KERN>, 32 * W, smem);
+            if (e != cudaSuccess) return e;
+            if (per_sm < 1) per_sm = 1;
+            const bool last = pass == 1 || c->par.tile_cap >= SPH_TCAP_BIG;
+            k_density_tile<KERN><<<c->sm_count * per_sm, 32 * W, smem, s>>>(
+                c->grid, c->cell_start, c->pos_m, c->perm, c->buckets,
+                pass == 0 ? c->bucket_cnt : c->big_cnt, pass == 0 ? nullptr : c->big_list,
+                last ? nullptr : c->big_list, c->big_cnt, c->tile_next + pass, par, h, rho, omega, nn,
+                c->fix_list, c->fix_cnt, c->fb_list, c->fb_cnt,
+                c->par.tile_forces ? nullptr : c->nb_j,
+                (unsigned)(((size_t)c->n_max * SPH_SLOTS * SPH_G) / (SPH_LCAP * SPH_TB)), c->list_next,
+                c->bucket_loff, c->nb_cnt, c->nb_rkeep, c->tl_rkeep, c->stats);
+            e = cudaGetLastError();
+            if (e != cudaSuccess) return e;
+        }
+        return cudaSuccess;
     };
     cudaError_t e;
     switch (c->par.kernel) {
