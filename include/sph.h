@@ -66,8 +66,9 @@ typedef struct {
     float   search_slack; /* density search radius = 2 h_guess x this (<= 1: default 1.1);  */
                           /* PAPER.md:152 "slightly larger kernel"; results do not depend   */
                           /* on it                                                         */
-    float   cell_div_x;   /* cells per minimum search radius along x (<= 0: default 4)     */
-    float   cell_div_yz;  /* ... along y and z (<= 0: default 1.5)                         */
+    float   cell_div_x;   /* cells per minimum search radius along x (<= 0: default 8 with  */
+                          /* the staged-tile sweeps, 4 without)                            */
+    float   cell_div_yz;  /* ... along y and z (<= 0: default 2, or 1.5 without tiles)      */
     int32_t entropy;      /* 1: entropy-conserving variant: sph_forces drops */
                           /* the Eq. (14) term, dudt is the viscous heating of Eq. (18)     */
                           /* alone; the caller advances u with sph_isentropic_u             */

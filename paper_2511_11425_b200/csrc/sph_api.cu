@@ -15,8 +15,8 @@ static void fill_defaults(sph_params& p) {
     if (!(p.h_tol > 0.0f)) p.h_tol = 1e-6f;
     if (p.h_max_iter <= 0) p.h_max_iter = 40;
     if (!(p.search_slack > 1.0f)) p.search_slack = 1.1f;
-    if (!(p.cell_div_x > 0.0f)) p.cell_div_x = 4.0f;
-    if (!(p.cell_div_yz > 0.0f)) p.cell_div_yz = 1.5f;
+    if (!(p.cell_div_x > 0.0f)) p.cell_div_x = p.tile >= 0 ? 8.0f : 4.0f;
+    if (!(p.cell_div_yz > 0.0f)) p.cell_div_yz = p.tile >= 0 ? 2.0f : 1.5f;
     if (p.tile_rows <= 0) p.tile_rows = 3;
     if (p.tile_rows > 5) p.tile_rows = 5;
     if (p.tile_cap <= 0) p.tile_cap = 768;

@@ -64,21 +64,29 @@ __device__ __forceinline__ void force_pair(const Target& t, Accum& a, const Forc
 // the compiler interleave the dependency chains of several pairs (the staged-tile sweep
 // evaluates four per trip); a source whose records are not meaningful (ok = false: a cursor
 // bubble, the self pair) may produce anything, the selects drop it.
-template <int KERN, bool ENT>
+// v_ij . r_ij of a pair (the sign decides Eq. 15)
+__device__ __forceinline__ float force_pair_vr(const Target& t, const float4 vj, float dx, float dy, float dz) {
+    return (t.vi.x - vj.x) * dx + (t.vi.y - vj.y) * dy + (t.vi.z - vj.z) * dz;
+}
+// AV = false: the caller knows that no pair it evaluates together is approaching (a warp-uniform
+// decision); the viscous terms are then exactly zero and are left out.
+template <int KERN, bool ENT, bool AV = true>
 __device__ __forceinline__ void force_pair_nb(const Target& t, Accum& a, const ForcePar& par, bool ok,
                                               const float4 vj, const float4 rj, float dx, float dy,
                                               float dz, float r2, float hj) {
     const float r  = sph_sqrt(r2);
     const float gi = t.K * SphKernel<KERN>::g_s(r * t.ih);   // K carries gscale
     const float gj = rj.w * SphKernel<KERN>::g_s(__fdividef(r, hj));
-    const float vdx = t.vi.x - vj.x, vdy = t.vi.y - vj.y, vdz = t.vi.z - vj.z;
-    const float vr = vdx * dx + vdy * dy + vdz * dz;   // v_ij . r_ij
-    const float hb  = 0.5f * (t.pi.w + hj);
-    const float mu  = fminf(__fdividef(hb * vr, r2 + par.eps * hb * hb), 0.0f);
-    const float cb  = 0.5f * (t.c + rj.y);
-    const float rb  = 0.5f * (t.rho + rj.x);
-    const float Pij = __fdividef(mu * (par.beta * mu - par.alpha * cb), rb);
-    const float pig = Pij * 0.5f * (gi + gj);           // Pi_ij * gbar
+    const float vr = force_pair_vr(t, vj, dx, dy, dz);   // v_ij . r_ij
+    float mu = 0.0f, pig = 0.0f;
+    if (AV) {
+        const float hb  = 0.5f * (t.pi.w + hj);
+        mu = fminf(__fdividef(hb * vr, r2 + par.eps * hb * hb), 0.0f);
+        const float cb  = 0.5f * (t.c + rj.y);
+        const float rb  = 0.5f * (t.rho + rj.x);
+        const float Pij = __fdividef(mu * (par.beta * mu - par.alpha * cb), rb);
+        pig = Pij * 0.5f * (gi + gj);           // Pi_ij * gbar
+    }
     const float Ag  = t.A * gi;
     const float ca  = ok ? vj.w * (Ag + rj.z * gj + pig) : 0.0f;
     const float du  = ok ? vj.w * (ENT ? 0.5f * pig : Ag + 0.5f * pig) * vr : 0.0f;   // Eq. (18) [+ Eq. (14)]

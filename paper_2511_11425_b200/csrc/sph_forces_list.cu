@@ -205,31 +205,68 @@ __global__ __launch_bounds__(FL_WARPS * 32) void k_forces_list(
     }
     const int maxcnt = __reduce_max_sync(SPH_FULL, max(cnt[0], cnt[1]));
 
-    Accum acc[2];
-    auto pair = [&](int t, int f) {
-        const bool     in = f < cnt[t];
-        uint32_t j  = in ? __ldg(lb + f * SPH_TB + lane + 32 * t) : (uint32_t)p[t];
-#ifdef SPH_DEBUG_TILE
-        if (j >= (uint32_t)nall) { printf("bad j %u bucket %u reg %u f %d cnt %d lane %d t %d p %d\n", j, bi, reg, f, cnt[t], lane, t, p[t]); j = p[t]; }
-#endif
-        const float4 pj = __ldg(pos_h + j), vj = __ldg(vel_m + j), rj = __ldg(rcak + j);
-        float dx = tg[t].pi.x - pj.x, dy = tg[t].pi.y - pj.y, dz = tg[t].pi.z - pj.z;
-        if (anyper) {   // minimum image
-            dx -= Lx * rintf(dx * iLx);
-            dy -= Ly * rintf(dy * iLy);
-            dz -= Lz * rintf(dz * iLz);
-        }
-        const float r2 = dx * dx + dy * dy + dz * dz;
-        const float hm = fmaxf(tg[t].pi.w, pj.w);
-        const bool  ok = in && r2 < 4.0f * hm * hm && r2 > 0.0f;
-        force_pair_nb<KERN, ENT>(tg[t], acc[t], par, ok, vj, rj, dx, dy, dz, r2, pj.w);
-    };
-    for (int f = 0; f < maxcnt; f += 2) {
-        pair(0, f);
-        pair(1, f);
-        pair(0, f + 1);
-        pair(1, f + 1);
+    // Does the bucket's reach cross a periodic face?  If not, no pair of it needs the minimum
+    // image (warp-uniform, decided once).
+    bool wraps = false;
+    {
+        const float Rb = 2.0f * (1.0f + 1e-4f) * Hs;
+#pragma unroll
+        for (int d = 0; d < 3; ++d)
+            wraps = wraps || (g.per[d] && (b0[d] - Rb < g.lo[d] || b1[d] + Rb > g.lo[d] + g.len[d]));
     }
+    Accum acc[2];
+    auto entry = [&](int t, int f) -> uint32_t {   // the sorted position of entry f (own record past the end)
+        return f < cnt[t] ? __ldg(lb + f * SPH_TB + lane + 32 * t) : (uint32_t)p[t];
+    };
+    // one pair, in two halves: fetch + geometry (is the pair there, is it approaching), then
+    // the arithmetic -- with or without the viscous terms, decided for the four pairs of a trip
+    // at once (warp-uniform: a flow at rest, or a receding one, never pays for Eq. 15)
+    struct PairIn { float4 vj, rj; float dx, dy, dz, r2, hj; bool ok; };
+    auto fetch = [&](int t, int f, uint32_t j, auto wrap_tag, PairIn& q) -> bool {
+        constexpr bool WRAP = decltype(wrap_tag)::value;
+        const float4 pj = __ldg(pos_h + j);
+        q.vj = __ldg(vel_m + j);
+        q.rj = __ldg(rcak + j);
+        q.dx = tg[t].pi.x - pj.x; q.dy = tg[t].pi.y - pj.y; q.dz = tg[t].pi.z - pj.z;
+        if (WRAP) {   // minimum image
+            q.dx -= Lx * rintf(q.dx * iLx);
+            q.dy -= Ly * rintf(q.dy * iLy);
+            q.dz -= Lz * rintf(q.dz * iLz);
+        }
+        q.r2 = q.dx * q.dx + q.dy * q.dy + q.dz * q.dz;
+        q.hj = pj.w;
+        const float hm = fmaxf(tg[t].pi.w, pj.w);
+        q.ok = f < cnt[t] && q.r2 < 4.0f * hm * hm && q.r2 > 0.0f;
+        return q.ok && force_pair_vr(tg[t], q.vj, q.dx, q.dy, q.dz) < 0.0f;
+    };
+    // two entries of both targets per trip (four independent chains); the list indices of the
+    // next trip are loaded before this trip's records are used, so the list stream (HBM) and
+    // the record gathers (L1 / L2) are not waited for one after the other
+    auto sweep = [&](auto wrap_tag) {
+        uint32_t jc[4] = {entry(0, 0), entry(1, 0), entry(0, 1), entry(1, 1)};
+        for (int f = 0; f < maxcnt; f += 2) {
+            const uint32_t jn[4] = {entry(0, f + 2), entry(1, f + 2), entry(0, f + 3), entry(1, f + 3)};
+            PairIn q[4];
+            bool   av = false;
+#pragma unroll
+            for (int k = 0; k < 4; ++k) av = fetch(k & 1, f + (k >> 1), jc[k], wrap_tag, q[k]) || av;
+            if (__any_sync(SPH_FULL, av)) {
+#pragma unroll
+                for (int k = 0; k < 4; ++k)
+                    force_pair_nb<KERN, ENT, true>(tg[k & 1], acc[k & 1], par, q[k].ok, q[k].vj, q[k].rj, q[k].dx,
+                                                   q[k].dy, q[k].dz, q[k].r2, q[k].hj);
+            } else {
+#pragma unroll
+                for (int k = 0; k < 4; ++k)
+                    force_pair_nb<KERN, ENT, false>(tg[k & 1], acc[k & 1], par, q[k].ok, q[k].vj, q[k].rj, q[k].dx,
+                                                    q[k].dy, q[k].dz, q[k].r2, q[k].hj);
+            }
+#pragma unroll
+            for (int k = 0; k < 4; ++k) jc[k] = jn[k];
+        }
+    };
+    if (wraps && anyper) sweep(std::true_type{});
+    else                 sweep(std::false_type{});
 #pragma unroll
     for (int t = 0; t < 2; ++t) {
         if (!cov[t]) continue;

@@ -364,6 +364,12 @@ __global__ __launch_bounds__(SPH_TWMAX * 32) void k_density_tile(
                         za[t]   = sm.zone_sa + 2u * (uint32_t)(wid * ZW * SPH_TB + lane + 32 * t);
                         zend[t] = za[t] + 2u * SPH_TB * (ZW - 1);
                     }
+                    uint32_t *lp[2], *lend[2];   // the target's column of the bucket's list region
+#pragma unroll
+                    for (int t = 0; t < 2; ++t) {
+                        lp[t]   = lbase ? lbase + lane + 32 * t : nullptr;
+                        lend[t] = lbase ? lp[t] + SPH_LCAP * SPH_TB : nullptr;
+                    }
                     sph_tile_walk(sm, ti, lane, wid, W, on, [&](int t, const SphEntry& en) {
                         const float dx = xt[t] - en.c.x, dy = yt[t] - en.c.y, dz = zt[t] - en.c.z;
                         const float r  = sph_sqrt(fmaf(dz, dz, fmaf(dy, dy, dx * dx)));
@@ -376,8 +382,13 @@ __global__ __launch_bounds__(SPH_TWMAX * 32) void k_density_tile(
                         M[t][3] = fmaf(a3, t2, M[t][3]);
                         M[t][4] = fmaf(a4, tt, M[t][4]);
                         M[t][5] += a5;
-                        if (lbase != nullptr && en.has && nent[t] < SPH_LCAP)   // the kept list (a set: any sweep of this mask writes the same)
-                            lbase[nent[t] * SPH_TB + lane + 32 * t] = sm.gidx[en.idx];
+                        {   // the kept list (a set: any sweep of this mask writes the same); predicated store
+                            const uint32_t gj = sph_ldsu(sm.gidx_sa + 4u * (uint32_t)en.idx);
+                            const bool st = en.has && lp[t] < lend[t];
+                            asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %2, 0;\n\t@p st.global.u32 [%0], %1;\n\t}"
+                                         ::"l"(lp[t]), "r"(gj), "r"((unsigned)st) : "memory");
+                            lp[t] += st ? SPH_TB : 0;
+                        }
                         nent[t] += en.has ? 1 : 0;
                         // next to (or beyond) the support edge: remember the entry (predicated
                         // store; past the capacity the last slot is overwritten and nz says so)
@@ -509,6 +520,12 @@ __global__ __launch_bounds__(SPH_TWMAX * 32) void k_density_tile(
                         Hhi[t] = 2.0f * h[t] * (1.0f + T_EDGE);
                         s[t] = 0.0f; e[t] = 0.0f; f2[t] = 0.0f; cin[t] = 0; ne[t] = 0;
                     }
+                    uint32_t *lp[2], *lend[2];
+#pragma unroll
+                    for (int t = 0; t < 2; ++t) {
+                        lp[t]   = lbase ? lbase + lane + 32 * t : nullptr;
+                        lend[t] = lbase ? lp[t] + SPH_LCAP * SPH_TB : nullptr;
+                    }
                     sph_tile_walk(sm, ti, lane, wid, W, on, [&](int t, const SphEntry& en) {
                         const float4 c = en.c;
                         const float  mj = en.m;
@@ -520,11 +537,12 @@ __global__ __launch_bounds__(SPH_TWMAX * 32) void k_density_tile(
                         s[t]  = fmaf(mj, wq, s[t]);
                         e[t]  = fmaf(mj, eq, e[t]);
                         f2[t] = fmaf(mj, fq, f2[t]);
-                        if (lbase != nullptr && has && nent[t] < SPH_LCAP) {
-#ifdef SPH_DEBUG_TILE
-                            if (sm.gidx[en.idx] > 100000000u) printf("bad gidx %u idx %d used %d nwords %d tcap %d stage %d bucket %u lane %d t %d f %d\n", sm.gidx[en.idx], en.idx, ti.used, ti.nwords, par.tcap, stage, bi, lane, t, nent[t]);
-#endif
-                            lbase[nent[t] * SPH_TB + lane + 32 * t] = sm.gidx[en.idx];
+                        {
+                            const uint32_t gj = sph_ldsu(sm.gidx_sa + 4u * (uint32_t)en.idx);
+                            const bool st = has && lp[t] < lend[t];
+                            asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %2, 0;\n\t@p st.global.u32 [%0], %1;\n\t}"
+                                         ::"l"(lp[t]), "r"(gj), "r"((unsigned)st) : "memory");
+                            lp[t] += st ? SPH_TB : 0;
                         }
                         nent[t] += has ? 1 : 0;
                         cin[t]  += (has && r < Hlo[t]) ? 1 : 0;
