@@ -31,18 +31,77 @@ if ROOT not in sys.path:
 METRIC = "particle-neighbour interactions/sec per density+force step"
 UNIT = "interactions/s"
 NOMINAL_FP32_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12   # SMs x FP32 lanes x 2 (FMA) x max clock
-KERNELS_PER_STEP = 11 + 3 + 6 + 2   # build_cells, density_h, forces, timestep kernel launches
+KERNELS_PER_STEP = 12 + 5 + 7 + 2   # build_cells, density_h, forces, timestep kernel launches
 # algorithmic FLOPs: per accepted density pair and Newton
 # sweep 27; per force pair 50 (AV branch not taken) or 70 (taken)
 FLOP_DENS, FLOP_FORCE, FLOP_FORCE_AV = 27.0, 50.0, 70.0
-# dram__bytes_read.sum + dram__bytes_write.sum per launch on sedov_128^3, from the ncu --set full
-# capture summarised in profiles/r1h_density_forces.md (k_density / k_forces)
-NCU_DRAM_BYTES = {"density_h": 158.0e6 + 783.7e6, "forces": 941.9e6 + 43.6e6}
-# executed FP32 lane-operations per cycle (fadd + fmul + 2 ffma, predicated-on threads) over the
-# 148 x 128 x 2 the chip can retire, same capture: what the kernel executes, rejected candidates,
-# culling and Taylor/Halley bookkeeping included -- printed beside the useful (reject-free) fraction
-NCU_EXECUTED_FP32_FRAC = {"density_h": (1013.1 + 1190.0 + 2 * 1101.9) / (148 * 128 * 2),
-                          "forces": (783.6 + 1742.4 + 2 * 1495.4) / (148 * 128 * 2)}
+# What ncu measured on the dominant kernels (DRAM bytes per launch, executed FP32 lane-operations)
+# lives in profiles/ncu_current.json together with a hash of the CUDA sources it was taken at;
+# the numbers are printed only while that hash matches the sources that run (else null + stale).
+NCU_JSON = os.path.join(ROOT, "profiles", "ncu_current.json")
+NCU_KERNEL_OF_CALL = {"density_h": "k_density_tile", "forces": "k_forces_list"}
+
+
+def csrc_hash():
+    """sha256 over the CUDA sources and the C header, in name order."""
+    import hashlib
+    d = os.path.join(ROOT, "paper_2511_11425_b200", "csrc")
+    hh = hashlib.sha256()
+    for f in sorted(os.listdir(d)) + ["../../include/sph.h"]:
+        with open(os.path.join(d, f), "rb") as fh:
+            hh.update(f.encode() + b"\0" + fh.read())
+    return hh.hexdigest()[:16]
+
+
+def ncu_numbers(call):
+    """(traffic bytes per launch, executed FP32 fraction, stale) of the kernel behind a call."""
+    try:
+        with open(NCU_JSON) as fh:
+            j = json.load(fh)
+    except Exception:
+        return None, None, None
+    k = j.get("kernels", {}).get(NCU_KERNEL_OF_CALL.get(call, ""), None)
+    if k is None:
+        return None, None, None
+    if j.get("csrc_hash") != csrc_hash():
+        return None, None, True
+    return k.get("dram_bytes"), k.get("executed_fp32_frac"), False
+
+
+def write_ncu_json(paths):
+    """--ncu-raw-csv: turns `ncu -i rep --page raw --csv` dumps (one launch each) into
+    profiles/ncu_current.json, stamped with the hash of the sources as they are now."""
+    import csv
+    out = dict(csrc_hash=csrc_hash(), workload="sedov_128^3", kernels={},
+               note="per launch; executed_fp32_frac = (fadd + fmul + 2 ffma predicated-on thread "
+                    "instructions per elapsed cycle, as ncu counts them) / (148 x 128 x 2)")
+    for path in paths:
+        rows = list(csv.reader(open(path)))
+        hdr, val = rows[0], rows[2]
+        g = lambda k: float(val[hdr.index(k)].replace(",", "")) if k in hdr else 0.0
+        name = val[hdr.index("Kernel Name")]
+        short = [k for k in NCU_KERNEL_OF_CALL.values() if k in name]
+        if not short:
+            continue
+        cyc = 1.0   # the --set full page gives the counters per elapsed cycle, summed over the chip
+        fl = (g("smsp__sass_thread_inst_executed_op_fadd_pred_on.sum.per_cycle_elapsed") +
+              g("smsp__sass_thread_inst_executed_op_fmul_pred_on.sum.per_cycle_elapsed") +
+              2.0 * g("smsp__sass_thread_inst_executed_op_ffma_pred_on.sum.per_cycle_elapsed"))
+        unit = {"Mbyte": 1e6, "Gbyte": 1e9, "Kbyte": 1e3, "byte": 1.0}
+        u = lambda k: unit.get(rows[1][hdr.index(k)], 1.0)
+        out["kernels"][short[0]] = dict(
+            dram_bytes=g("dram__bytes_read.sum") * u("dram__bytes_read.sum") +
+                       g("dram__bytes_write.sum") * u("dram__bytes_write.sum"),
+            executed_fp32_frac=fl / (cyc * 148 * 128 * 2) if cyc else None,
+            duration_ms=g("gpu__time_duration.sum") * {"ms": 1.0, "us": 1e-3, "ns": 1e-6}.get(
+                rows[1][hdr.index("gpu__time_duration.sum")], 1.0),
+            issue_active_pct=g("smsp__issue_active.avg.pct_of_peak_sustained_active"),
+            warp_inst=g("smsp__inst_executed.sum"),
+            registers=g("launch__registers_per_thread"))
+    with open(NCU_JSON, "w") as fh:
+        json.dump(out, fh, indent=1)
+    print(json.dumps(out))
+
 
 KERNEL_IDS = {"cubic_spline": 0, "wendland_c2": 1, "wendland_c4": 2, "wendland_c6": 3}
 
@@ -62,6 +121,11 @@ def parse():
     ap.add_argument("--ref-nside", type=int, default=96,
                     help="lattice side of the bounded sample the CPU oracle is timed on")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-cpu-legs", dest="cpu_legs", action="store_false",
+                    help="skip the oracle legs of BASELINE.md section 3 (brute force on C1 with 1 "
+                         "and all threads, cell list with 1 thread: 15 s)")
+    ap.add_argument("--ncu-raw-csv", nargs="+", default=None,
+                    help="write profiles/ncu_current.json from `ncu --page raw --csv` dumps and exit")
     ap.add_argument("--workload", default="sedov", choices=sorted(workloads_names()),
                     help="sedov (BASELINE.json's metric configuration, the default) or another of "
                          "the five configurations at its full size, for the per-configuration table")
@@ -105,6 +169,44 @@ def oracle_sample(nside, v_sigma=0.0):
                 sample=f"sedov {nside}^3 = {w['n']} particles, one density+force+dt pass, "
                        f"FP64 cell-list oracle (oracle/sph_oracle.c), {dt:.2f} s",
                 particles_per_s=w["n"] / dt, seconds=dt, n=int(w["n"]))
+
+
+def oracle_legs():
+    """The other oracle timings BASELINE.md section 3 lists, each in a subprocess so that the
+    thread count (OMP_NUM_THREADS) can differ: brute force O(N^2) on C1 (4096 particles) with one
+    and with all threads, the cell-list oracle on a 40^3 Sedov lattice with one thread."""
+    code = (
+        "import sys, json, time, numpy as np\n"
+        "sys.path.insert(0, %r)\n"
+        "from oracle import sph_oracle as orc\n"
+        "from paper_2511_11425_b200 import workloads\n"
+        "orc.build()\n"
+        "kind = sys.argv[1]\n"
+        "w = workloads.uniform_cube() if kind == 'brute' else workloads.sedov(nside=40)\n"
+        "op = orc.Params(gamma=float(np.float32(w['gamma'])), av_alpha=w['av_alpha'], av_beta=w['av_beta'])\n"
+        "ob = orc.Box(w['box_lo'], w['box_len'], w['periodic'])\n"
+        "c = kind != 'brute'\n"
+        "t0 = time.perf_counter()\n"
+        "h, rho, om, nn = orc.density(w['x'], w['y'], w['z'], w['m'], w['h'], ob, op, cells=c)\n"
+        "o = orc.forces(w['x'], w['y'], w['z'], w['m'], w['vx'], w['vy'], w['vz'], w['u'], rho, h, om, ob, op, cells=c)\n"
+        "dt = time.perf_counter() - t0\n"
+        "print(json.dumps(dict(value=(int(nn.sum()) + int(o['n_pairs'].sum())) / dt, unit='interactions/s',\n"
+        "      cores=orc.num_threads(), seconds=dt, n=int(w['n']))))\n") % ROOT
+    legs = {}
+    for name, kind, threads in (("brute_force_c1_1_thread", "brute", "1"), ("brute_force_c1_all_threads", "brute", None),
+                                ("cell_list_sedov40_1_thread", "fast", "1")):
+        env = dict(os.environ)
+        if threads:
+            env["OMP_NUM_THREADS"] = threads
+        else:
+            env.pop("OMP_NUM_THREADS", None)
+        try:
+            r = subprocess.run([sys.executable, "-c", code, kind], env=env, capture_output=True, text=True,
+                               timeout=300)
+            legs[name] = json.loads(r.stdout.strip().splitlines()[-1])
+        except Exception as e:   # a leg that cannot run is reported, not fatal
+            legs[name] = dict(error=str(e)[:200])
+    return legs
 
 
 def run_reference(a):
@@ -271,6 +373,32 @@ def run_gpu(a):
         dist.all_reduce(total_ms, op=dist.ReduceOp.MAX)
     total_s = float(total_ms.item()) * 1e-3
 
+    # ---- the same steps with random velocities (Sedov variant C3v of SURVEY.md 8(d)): half of the
+    # pairs are approaching and take the viscosity of Eqs. (15)-(18); reported beside the headline
+    av_line = None
+    if a.workload == "sedov" and a.v_sigma == 0.0 and not custom:
+        gsd = torch.Generator(device="cuda").manual_seed(114253)
+        keep = {k: d[k].clone() for k in ("vx", "vy", "vz")}
+        for k in keep:
+            d[k].normal_(0.0, 0.01, generator=gsd)
+        one_step(); one_step()
+        ctx.stats_reset()
+        ev2 = [[torch.cuda.Event(enable_timing=True) for _ in range(5)] for _ in range(a.steps)]
+        for k in range(a.steps):
+            one_step(ev2[k])
+            flush.fill_(k & 0xff)
+        torch.cuda.synchronize()
+        st2 = ctx.stats()
+        per2 = np.array([[e[i].elapsed_time(e[i + 1]) for i in range(4)] for e in ev2]).mean(axis=0)
+        av_line = dict(workload=wname + "_v (v ~ N(0, 0.01))", ms_per_step=float(per2.sum()),
+                       ms_forces=float(per2[2]), force_av_pairs=st2["force_av_pairs"] / a.steps,
+                       force_pairs=st2["force_pairs"] / a.steps,
+                       value=(st2["dens_pairs"] + st2["force_pairs"]) / a.steps / (float(per2.sum()) * 1e-3))
+        for k in keep:
+            d[k].copy_(keep[k])
+        one_step()
+        ctx.stats_reset()
+
     # ---- end to end: host (pinned) inputs in, all outputs back, every step ----------------
     outs_host = {k: torch.empty(v.shape, dtype=v.dtype).pin_memory() for k, v in out.t.items()}
     h_host = torch.empty(n, dtype=torch.float32).pin_memory()
@@ -345,6 +473,9 @@ def run_gpu(a):
     dom_flops = {1: f_dens, 2: f_force}.get(dom, 0.0)
     ach = dom_flops / (call_ms[dom] * 1e-3) / 1e12
     fma_peak = sph.fp32_peak(1.0)
+    default_cfg = wname == "sedov_128^3" and not custom
+    traffic, exe_frac, stale = ncu_numbers(names[dom]) if default_cfg else (None, None, None)
+    frac_of = lambda fl, ms: fl / (ms * 1e-3) / 1e12 / NOMINAL_FP32_TFLOPS
     line = dict(
         metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=K, warmup=max(a.warmup, 3),
         ms_per_step=float(step_ms.mean()), higher_is_better=True, scaling="weak",
@@ -365,14 +496,17 @@ def run_gpu(a):
         newton_sweeps_per_particle=sweeps, grid_dims=st["grid_dims"],
         roofline=dict(bound="alu", kernel=names[dom], achieved=ach, peak=NOMINAL_FP32_TFLOPS,
                       unit="TFLOP/s", frac=ach / NOMINAL_FP32_TFLOPS,
-                      traffic=(NCU_DRAM_BYTES.get(names[dom]) if wname == "sedov_128^3" else None),
-                      traffic_source="profiles/r1h_density_forces.md (ncu --set full, bytes per launch)",
+                      traffic=traffic,
+                      traffic_source="profiles/ncu_current.json (ncu --set full, dram bytes per launch of "
+                                     + NCU_KERNEL_OF_CALL.get(names[dom], "-") + "; null when the CUDA "
+                                     "sources changed since the capture)",
+                      ncu_stale=stale,
                       peak_source="derived: 148 SM x 128 FP32 lanes x 2 x 1.965 GHz",
                       measured_fma_peak=fma_peak, frac_of_measured_fma=ach / fma_peak,
                       useful_frac=ach / NOMINAL_FP32_TFLOPS,
-                      executed_fp32_frac=(NCU_EXECUTED_FP32_FRAC.get(names[dom])
-                                          if wname == "sedov_128^3" else None),
+                      executed_fp32_frac=exe_frac,
                       algorithmic_flops_per_launch=dom_flops,
+                      frac_density_h=frac_of(f_dens, call_ms[1]), frac_forces=frac_of(f_force, call_ms[2]),
                       step_frac=(f_dens + f_force) / (float(step_ms.mean()) * 1e-3) / 1e12 /
                                 NOMINAL_FP32_TFLOPS),
         e2e=dict(value=e2e_val, unit=UNIT, h2d_bytes_per_step=h2d, d2h_bytes_per_step=d2h,
@@ -380,11 +514,15 @@ def run_gpu(a):
                  overlap="copies of steps k+1 / k-1 overlap the kernels of step k (two device "
                          "buffer sets, one copy stream per direction)"),
         gpu_launches=KERNELS_PER_STEP * K, clocks=clocks)
+    if av_line:
+        line["av_variant"] = av_line
     if world == 1 and not a.no_cpu_baseline and not custom:   # the oracle sample is wendland_c2 / 64
         cb = oracle_sample(a.ref_nside, a.v_sigma)
         for k in ("seconds", "n"):
             cb.pop(k, None)
         line["cpu_baseline"] = cb
+        if a.cpu_legs:
+            line["cpu_baseline_legs"] = oracle_legs()
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
@@ -392,7 +530,9 @@ def run_gpu(a):
 
 if __name__ == "__main__":
     args = parse()
-    if args.impl == "reference":
+    if args.ncu_raw_csv:
+        write_ncu_json(args.ncu_raw_csv)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_gpu(args)

@@ -19,6 +19,9 @@
 namespace {
 
 constexpr int FL_WARPS = 4;
+#ifndef FL_MINB
+#define FL_MINB 4
+#endif
 
 __device__ __forceinline__ float lwarp_max(float v) {
 #pragma unroll
@@ -95,7 +98,7 @@ __device__ __forceinline__ float list_scatter_hmax(const SphGrid& g, const unsig
 }
 
 template <int KERN, bool ENT>
-__global__ __launch_bounds__(FL_WARPS * 32) void k_forces_list(
+__global__ __launch_bounds__(FL_WARPS * 32, FL_MINB) void k_forces_list(
     const SphGrid* __restrict__ gp, const uint32_t* __restrict__ cell_start,
     const float4* __restrict__ pos_h, const float4* __restrict__ vel_m,
     const float4* __restrict__ rcak, const int32_t* __restrict__ perm,
