@@ -17,6 +17,11 @@
  *     unless stated (sph_stats, sph_neighbors, sph_fp32_peak do).
  *   - Return value: SPH_OK (0) or a negative error code.  No exceptions, no exit, no
  *     printing.  sph_last_error gives a text for the last failure of a context.
+ *   - Positions on a periodic axis must lie in [lo, lo + len) (sph_drift wraps them); a
+ *     coordinate outside is binned into the edge cell and its neighbours across the face
+ *     are missed.  On an open axis any coordinate is fine (edge cells extend to infinity).
+ *   - Device memory of a context: about 1 KB per particle of n_max (768 B of it the neighbour
+ *     lists kept between sph_density_h and sph_forces) plus 4 B per cell of the index.
  *   - Call order: sph_build_cells -> sph_density_h -> sph_forces -> sph_timestep.
  *     sph_forces / sph_neighbors may be fed rho, h, Omega from elsewhere as long as
  *     sph_build_cells ran on the same positions (else SPH_ESTALE).

@@ -76,8 +76,9 @@ extern "C" int sph_create(sph_ctx** out, const sph_params* params, const sph_box
     ok = ok && dalloc(&c->scan_part, (size_t)SPH_SCAN_BLOCKS + 1) == cudaSuccess;
     ok = ok && dalloc(&c->pos_h, (size_t)n_max + SPH_POS_PAD) == cudaSuccess;
     ok = ok && dalloc(&c->pos_m, (size_t)n_max + SPH_POS_PAD) == cudaSuccess;
-    ok = ok && dalloc(&c->vel_m, (size_t)n_max) == cudaSuccess;
-    ok = ok && dalloc(&c->rcak, (size_t)n_max) == cudaSuccess;
+    // every array handed to sph_group_collect carries the padding its window loads rely on
+    ok = ok && dalloc(&c->vel_m, (size_t)n_max + SPH_POS_PAD) == cudaSuccess;
+    ok = ok && dalloc(&c->rcak, (size_t)n_max + SPH_POS_PAD) == cudaSuccess;
     ok = ok && dalloc(&c->stats, (size_t)ST_NCOUNTERS) == cudaSuccess;
     ok = ok && dalloc(&c->coarse_hmax, (size_t)2 * SPH_COARSE_MAX) == cudaSuccess;
     ok = ok && dalloc(&c->nb_j, (size_t)n_max * SPH_SLOTS * SPH_G) == cudaSuccess;

@@ -39,7 +39,7 @@ __global__ void k_ic_prep(int64_t n, const int32_t* __restrict__ inv_perm,
 template <int KERN, int PASS>
 __global__ __launch_bounds__(I_TPB, SPH_MINB) void k_interface(
     int n, const SphGrid* __restrict__ gp, const uint32_t* __restrict__ cell_start,
-    const float4* __restrict__ ica, const float4* __restrict__ icb, const float* __restrict__ expI,
+    const float4* __restrict__ ica, const float4* __restrict__ icb, const float* expI,
     const int32_t* __restrict__ perm, const uint32_t* __restrict__ nb_j,
     const uint32_t* __restrict__ nb_cnt, const float* __restrict__ nb_rkeep, float alpha,
     float gamma, float* imbalance, float* expI_out, float* rho_corr, float* P_corr) {

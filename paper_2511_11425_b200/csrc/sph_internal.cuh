@@ -514,7 +514,9 @@ __device__ __forceinline__ void sph_group_collect(const SphGrid& g,
                         constexpr int NW = decltype(nw_tag)::value;
                         float4 pp[NW];
 #pragma unroll
-                        for (int u = 0; u < NW; ++u) pp[u] = __ldg(pos + c + u * G);
+                        // (a group whose own row is short walks as many windows as the longest
+                        // row of the warp: the index is clamped to the row's padded end)
+                        for (int u = 0; u < NW; ++u) pp[u] = __ldg(pos + min(c + u * G, re + (uint32_t)(G - 1)));
 #pragma unroll
                         for (int u = 0; u < NW; ++u) {
                             float dx = sxx - pp[u].x, dy = rsy - pp[u].y, dz = rsz - pp[u].z;

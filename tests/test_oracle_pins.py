@@ -316,12 +316,17 @@ def test_two_particle_hand_values():
     assert f["ax"][0] < 0 < f["ax"][1]                      # positive pressure repels
     assert abs(f["dudt"][0] - g["dudt0_noav"]) < 1e-13      # compression heats
     assert f["ay"][0] == 0 and f["az"][0] == 0
+    # the normalisers of the force tolerance (sum of the pair-term magnitudes): with one pair
+    # they ARE the magnitudes of the results -- Sa = |a|, Su = |du/dt| (m_j = 1, |r^| = 1)
+    assert abs(f["Sa"][0] - abs(g["a0x_noav"])) < 1e-13 and abs(f["Sa"][1] - abs(g["a0x_noav"])) < 1e-13
+    assert abs(f["Su"][0] - abs(g["dudt0_noav"])) < 1e-13 and abs(f["Su"][1] - abs(g["dudt0_noav"])) < 1e-13
     f = orc.forces(x, zero, zero, one, vx, zero, zero, 3 * one, 2 * one, one, one, box,
                    orc.Params(av_alpha=1.0, av_beta=2.0, av_eps=0.01, **common))
     assert abs(f["mu_min"][0] - g["mu"]) < 1e-13 and abs(f["mu_min"][1] - g["mu"]) < 1e-13
     assert abs(f["ax"][0] - g["a0x_av"]) < 1e-12
     assert abs(f["dudt"][0] - g["dudt0_av"]) < 1e-12
     assert abs(f["dudt"][1] - g["dudt0_av"]) < 1e-12        # both heat equally (equal A here)
+    assert abs(f["Sa"][0] - abs(g["a0x_av"])) < 1e-12 and abs(f["Su"][0] - abs(g["dudt0_av"])) < 1e-12
     # receding pair: Pi = 0 exactly (Eq. 15 "otherwise" branch), mu_min stays 0
     f = orc.forces(x, zero, zero, one, -vx, zero, zero, 3 * one, 2 * one, one, one, box,
                    orc.Params(av_alpha=1.0, av_beta=2.0, **common))
@@ -339,6 +344,35 @@ def test_two_particle_hand_values():
     f = orc.forces(zero, zero, zero, one, vx, zero, zero, 3 * one, 2 * one, one, one, box,
                    orc.Params(**common))
     assert f["n_pairs"][0] == 0 and f["ax"][0] == 0.0
+
+
+def test_force_normalisers_bound_the_results_and_scale_with_the_source_mass():
+    """Sa_i = sum_j m_j |C_ij| and Su_i = sum_j m_j |(A_i F_i + Pi F/2)(v_ij . r^)| (SURVEY.md 8(c)
+    O6) define the 1e-4 force tolerance, so they are pinned like results: by the triangle
+    inequality |a_i| <= Sa_i and |du_i/dt| <= Su_i for every particle, with equality for a
+    particle that has a single partner; doubling every mass at fixed rho, u, h doubles a, du/dt,
+    Sa and Su alike (each is linear in the m_j), and a three-particle line gives the sums by hand:
+    the middle particle's two pair terms cancel in a but add up in Sa."""
+    w = W.uniform_cube(nside=8)
+    box = orc.Box(w["box_lo"], w["box_len"], w["periodic"])
+    par = _par(w)
+    h, rho, om, nn = orc.density(w["x"], w["y"], w["z"], w["m"], w["h"], box, par)
+    f = orc.forces(w["x"], w["y"], w["z"], w["m"], w["vx"], w["vy"], w["vz"], w["u"], rho, h, om, box, par)
+    amag = np.sqrt(f["ax"] ** 2 + f["ay"] ** 2 + f["az"] ** 2)
+    assert (amag <= f["Sa"] * (1 + 1e-12)).all() and (np.abs(f["dudt"]) <= f["Su"] * (1 + 1e-12)).all()
+    assert (f["Sa"] > 0).all() and (amag < 0.9 * f["Sa"]).any()      # cancellation does occur
+    f2 = orc.forces(w["x"], w["y"], w["z"], 2 * w["m"].astype(np.float64), w["vx"], w["vy"], w["vz"], w["u"],
+                    rho, h, om, box, par)
+    for k in ("ax", "dudt", "Sa", "Su"):
+        assert np.allclose(f2[k], 2 * f[k], rtol=1e-13, atol=0), k
+    # three particles on a line, symmetric: a = 0 in the middle, Sa = 2 x one pair term
+    big = orc.Box((-10, -10, -10), (20, 20, 20), (0, 0, 0))
+    x = np.array([-1.0, 0.0, 1.0]); z3 = np.zeros(3); o3 = np.ones(3)
+    p0 = orc.Params(kernel=1, gamma=5.0 / 3.0, av_alpha=0.0, av_beta=0.0)
+    f3 = orc.forces(x, z3, z3, o3, z3, z3, z3, 3 * o3, 2 * o3, o3, o3, big, p0)
+    fp = orc.forces(x[:2], z3[:2], z3[:2], o3[:2], z3[:2], z3[:2], z3[:2], 3 * o3[:2], 2 * o3[:2], o3[:2], o3[:2], big, p0)
+    assert abs(f3["ax"][1]) < 1e-15 and abs(f3["Sa"][1] - 2 * abs(fp["ax"][0])) < 1e-13
+    assert f3["Su"][1] == 0.0                                          # v = 0: no work terms
 
 
 def test_two_particle_density():
