@@ -135,6 +135,7 @@ def parse():
     ap.add_argument("--tile", type=int, default=0, help="sph_params.tile (-1: 8-lane kernels only)")
     ap.add_argument("--tile-rows", type=int, default=0, help="sph_params.tile_rows (0: default)")
     ap.add_argument("--tile-cap", type=int, default=0, help="sph_params.tile_cap (0: default)")
+    ap.add_argument("--tile-cap2", type=int, default=0, help="sph_params.tile_cap2 (0: default; 1: no second pass)")
     ap.add_argument("--tile-warps", type=int, default=0, help="sph_params.tile_warps (0: default)")
     ap.add_argument("--tile-forces", type=int, default=0, help="sph_params.tile_forces (1: force sweep on staged tiles)")
     ap.add_argument("--tile-fcap", type=int, default=0, help="sph_params.tile_fcap (0: default)")
@@ -323,7 +324,7 @@ def run_gpu(a):
     ctx = sph.Sph(sph.Params(kernel=KERNEL_IDS[a.kernel], n_ngb=a.n_ngb, gamma=w["gamma"],
                              av_alpha=w["av_alpha"], av_beta=w["av_beta"], search_slack=a.slack, cell_div_x=a.cell_div_x,
                              cell_div_yz=a.cell_div_yz, tile=a.tile, tile_rows=a.tile_rows,
-                             tile_cap=a.tile_cap, tile_warps=a.tile_warps,
+                             tile_cap=a.tile_cap, tile_cap2=a.tile_cap2, tile_warps=a.tile_warps,
                              tile_forces=a.tile_forces,
                              tile_fcap=a.tile_fcap, tile_fwarps=a.tile_fwarps),
                   sph.Box(w["box_lo"], w["box_len"], w["periodic"]), n)

@@ -85,6 +85,8 @@ typedef struct {
                           /* default 3; at most 5)                                           */
     int32_t tile_cap;     /* candidates a tile holds (<= 0: default 1024); buckets that need  */
                           /* more fall back to the 8-lane kernels                            */
+    int32_t tile_cap2;    /* tile of the second pass over the buckets the first tile could not  */
+                          /* hold (<= 0: default 2560; below tile_cap + 32: no second pass)    */
     int32_t tile_warps;   /* warps that share a bucket's tile (<= 0: default 1; at most 4)    */
     int32_t tile_forces;  /* 0 (default): the force sweep reads the neighbour lists the       */
                           /* density sweep kept (8 lanes per target); 1: the force sweep runs  */

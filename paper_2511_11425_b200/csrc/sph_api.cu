@@ -15,13 +15,16 @@ static void fill_defaults(sph_params& p) {
     if (!(p.h_tol > 0.0f)) p.h_tol = 1e-6f;
     if (p.h_max_iter <= 0) p.h_max_iter = 40;
     if (!(p.search_slack > 1.0f)) p.search_slack = 1.1f;
-    if (!(p.cell_div_x > 0.0f)) p.cell_div_x = p.tile >= 0 ? 8.0f : 4.0f;
-    if (!(p.cell_div_yz > 0.0f)) p.cell_div_yz = p.tile >= 0 ? 2.0f : 1.5f;
+    // cell_div_x / cell_div_yz <= 0 stay "automatic": sph_build_cells picks 8 x 2 for the staged-
+    // tile sweeps and 4 x 1.5 for the 8-lane kernels (sph_tile_on, the grid's steep-h flag)
     if (p.tile_rows <= 0) p.tile_rows = 3;
     if (p.tile_rows > 5) p.tile_rows = 5;
     if (p.tile_cap <= 0) p.tile_cap = 768;
     p.tile_cap = (p.tile_cap + 31) & ~31;
     if (p.tile_cap > 4096) p.tile_cap = 4096;
+    if (p.tile_cap2 <= 0) p.tile_cap2 = 2560;
+    p.tile_cap2 = (p.tile_cap2 + 31) & ~31;
+    if (p.tile_cap2 > 4064) p.tile_cap2 = 4064;
     if (p.tile_warps <= 0) p.tile_warps = 1;
     if (p.tile_warps > SPH_TWMAX) p.tile_warps = SPH_TWMAX;
     if (p.tile_fcap <= 0) p.tile_fcap = 576;

@@ -45,11 +45,19 @@ __global__ void k_reduce_h(int64_t n, const float* __restrict__ x, const float* 
 // One thread: derive the grid from min(h).  Cell sides: the smallest density search radius
 // R_min = 2 h_min slack, divided by cell_div_x along x (rows are contiguous, so fine cells
 // along x cost nothing and trim the row ends) and by cell_div_yz along y and z.
+// steep_check: automatic tile mode -- a contrast of h above 3 sets SPH_GRID_STEEP and takes the
+// cell sides of the 8-lane kernels (divx_s, divyz_s) instead of the tile sweeps' (divx, divyz).
 __global__ void k_grid_setup(SphGrid* g, const unsigned* red, sph_box box, float slack, float divx,
-                             float divyz, long long cap_cells) {
+                             float divyz, float divx_s, float divyz_s, int steep_check,
+                             long long cap_cells) {
     float hmin = __uint_as_float(red[0]), hmax = __uint_as_float(red[1]);
     float xm = __uint_as_float(red[2]);
     int   flags = 0;
+    if (steep_check && hmax > 3.0f * hmin) {
+        flags |= SPH_GRID_STEEP;
+        divx = divx_s;
+        divyz = divyz_s;
+    }
     float lmax = fmaxf(box.len[0], fmaxf(box.len[1], box.len[2]));
     if (!(hmin < 3.0e38f) || !(hmin > 0.0f)) {  // no valid h at all: one coarse grid
         hmin = hmax = lmax * 0.05f;
@@ -257,8 +265,13 @@ int sph_launch_build(sph_ctx* c, int64_t n, const float* x, const float* y, cons
     SPH_CUDA_CHECK(c, cudaMemsetAsync(c->tl_rkeep, 0, (size_t)n * sizeof(float), s));
     k_init_red<<<1, 1, 0, s>>>(c->red);
     k_reduce_h<<<min(nb, gs), TPB, 0, s>>>(n, x, y, z, h, c->red);
-    k_grid_setup<<<1, 1, 0, s>>>(c->grid, c->red, c->box, c->par.search_slack, c->par.cell_div_x,
-                                 c->par.cell_div_yz, (long long)c->cap_cells);
+    c->n_build = n;
+    const bool  tl = sph_tile_on(c);
+    const float ux = c->par.cell_div_x, uyz = c->par.cell_div_yz;   // > 0: the caller's choice
+    k_grid_setup<<<1, 1, 0, s>>>(c->grid, c->red, c->box, c->par.search_slack,
+                                 ux > 0.0f ? ux : (tl ? 8.0f : 4.0f), uyz > 0.0f ? uyz : (tl ? 2.0f : 1.5f),
+                                 ux > 0.0f ? ux : 4.0f, uyz > 0.0f ? uyz : 1.5f,
+                                 (tl && c->par.tile == 0) ? 1 : 0, (long long)c->cap_cells);
     k_zero_cells<<<gs, TPB, 0, s>>>(c->grid, c->cell_cnt);
     k_bin<<<nb, TPB, 0, s>>>(n, c->grid, x, y, z, c->cell_cnt, c->key, c->rank);
     k_scan_sum<<<SPH_SCAN_BLOCKS, TPB, 0, s>>>(c->grid, c->cell_cnt, c->scan_part);
@@ -269,6 +282,6 @@ int sph_launch_build(sph_ctx* c, int64_t n, const float* x, const float* y, cons
     k_cell_sort<<<nb, TPB, 0, s>>>(n, c->key, c->cell_start, c->perm);
     k_gather<<<nb, TPB, 0, s>>>(n, c->perm, x, y, z, h, c->pos_h, c->inv_perm);
     SPH_CUDA_CHECK(c, cudaGetLastError());
-    if (c->par.tile >= 0) return sph_launch_buckets(c);   // a3: the bucket table
+    if (sph_tile_on(c)) return sph_launch_buckets(c);   // a3: the bucket table
     return SPH_OK;
 }

@@ -106,10 +106,16 @@ __global__ __launch_bounds__(D_TPB, SPH_MINB) void k_density(
     int n, const SphGrid* __restrict__ gp, const uint32_t* __restrict__ cell_start,
     const float4* __restrict__ pos_m, const int32_t* __restrict__ perm, DensPar par, float* h_io,
     float* rho, float* omega, int32_t* nn, int32_t* fix_list, unsigned* fix_cnt, uint32_t* nb_j,
-    uint32_t* nb_cnt, float* nb_rkeep, const uint32_t* __restrict__ act_list,
-    const unsigned* __restrict__ act_cnt, int keep, unsigned long long* stats) {
+    uint32_t* nb_cnt, float* nb_rkeep, const uint32_t* __restrict__ act_list_,
+    const unsigned* __restrict__ act_cnt_, int keep, int all_if_steep, unsigned long long* stats) {
     // keep = 0: no neighbour lists are left behind (the staged-tile sweep owns the list memory,
     // in its own layout; this kernel then only serves the buckets that sweep handed back)
+    // all_if_steep: the target list is the tile sweep's hand-back list; under SPH_GRID_STEEP that
+    // sweep stands back, this kernel takes every particle and keeps its lists as without tiles
+    const bool steep = all_if_steep && (gp->flags & SPH_GRID_STEEP);
+    const uint32_t* __restrict__ act_list = steep ? nullptr : act_list_;
+    const unsigned* __restrict__ act_cnt  = act_cnt_;
+    if (steep) keep = 1;
     // targets: all n sorted positions, or the act_cnt entries of act_list (the active set)
     const int nt = act_list ? (int)*act_cnt : n;
     if (blockIdx.x * D_TARGETS >= nt) return;
@@ -414,7 +420,7 @@ int sph_launch_density(sph_ctx* c, const float* m, float* h, float* rho, float* 
     const int nblk = (int)((n + D_TARGETS - 1) / D_TARGETS);
     // the staged-tile kernel first (all particles as targets only); what it hands back --
     // buckets its tile cannot hold -- is swept by the 8-lane kernel through a target list
-    const bool tiled = c->par.tile >= 0 && !c->act_on;
+    const bool tiled = sph_tile_on(c) && !c->act_on;
     if (tiled) {
         const int rc = sph_launch_density_tile(c, h, rho, omega, nn);
         if (rc != SPH_OK) return rc;
@@ -426,7 +432,7 @@ int sph_launch_density(sph_ctx* c, const float* m, float* h, float* rho, float* 
         k_density<KERN><<<nblk, D_TPB, 0, s>>>((int)n, c->grid, c->cell_start, c->pos_m, c->perm, par,
                                                h, rho, omega, nn, c->fix_list, c->fix_cnt, c->nb_j,
                                                c->nb_cnt, c->nb_rkeep, tlist, tcnt,
-                                               (tiled && !c->par.tile_forces) ? 0 : 1, c->stats);
+                                               (tiled && !c->par.tile_forces) ? 0 : 1, tiled ? 1 : 0, c->stats);
         k_density_fix<KERN><<<c->sm_count * 4, 256, 0, s>>>(c->grid, c->cell_start, c->pos_m, c->perm,
                                                             par, c->fix_list, c->fix_cnt, h, rho,
                                                             omega, nn, c->stats);

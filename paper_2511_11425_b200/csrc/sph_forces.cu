@@ -123,8 +123,11 @@ __global__ __launch_bounds__(F_TPB, SPH_FMINB) void k_forces(
     float* ay, float* az, float* dudt, float* mu_min, int32_t* fix_list, unsigned* fix_cnt,
     const unsigned* __restrict__ coarse, const uint32_t* __restrict__ nb_j,
     const uint32_t* __restrict__ nb_cnt, const float* __restrict__ nb_rkeep,
-    const uint32_t* __restrict__ act_list, const unsigned* __restrict__ act_cnt,
+    const uint32_t* __restrict__ act_list_, const unsigned* __restrict__ act_cnt, int all_if_steep,
     unsigned long long* stats) {
+    // all_if_steep: the target list is the hand-back list of the tile / list sweeps; under
+    // SPH_GRID_STEEP those stand back and this kernel takes every particle
+    const uint32_t* __restrict__ act_list = (all_if_steep && (gp->flags & SPH_GRID_STEEP)) ? nullptr : act_list_;
     // targets: all n sorted positions, or the act_cnt entries of act_list (the active set)
     const int nt = act_list ? (int)*act_cnt : n;
     if (blockIdx.x * F_TARGETS >= nt) return;
@@ -373,7 +376,7 @@ int sph_launch_forces(sph_ctx* c, const float* m, const float* vx, const float* 
     // the staged-tile kernel first; what it hands back goes through the 8-lane kernel's target list
     // the buckets of the staged-tile density sweep first: from its kept lists (default) or on
     // staged tiles; what is handed back goes through the 8-lane kernel's target list
-    const bool tiled = c->par.tile >= 0 && !c->act_on;
+    const bool tiled = sph_tile_on(c) && !c->act_on;
     if (tiled) {
         const int rc = c->par.tile_forces > 0 ? sph_launch_forces_tile(c, ax, ay, az, dudt, mu_min)
                                               : sph_launch_forces_list(c, ax, ay, az, dudt, mu_min);
@@ -387,7 +390,7 @@ int sph_launch_forces(sph_ctx* c, const float* m, const float* vx, const float* 
         k_forces<KERN, ENT><<<nblk, F_TPB, 0, s>>>((int)n, c->grid, c->cell_start, c->pos_h, c->vel_m,
                                               c->rcak, c->perm, par, ax, ay, az, dudt, mu_min,
                                               c->fix_list, c->fix_cnt + 1, c->coarse_hmax, c->nb_j,
-                                              c->nb_cnt, c->nb_rkeep, tlist, tcnt, c->stats);
+                                              c->nb_cnt, c->nb_rkeep, tlist, tcnt, tiled ? 1 : 0, c->stats);
         k_forces_fix<KERN, ENT><<<c->sm_count * 4, 256, 0, s>>>(c->grid, c->cell_start, c->pos_h, c->vel_m,
                                                            c->rcak, c->perm, par, c->fix_list,
                                                            c->fix_cnt + 1, ax, ay, az, dudt, mu_min,

@@ -112,6 +112,7 @@ __global__ __launch_bounds__(FL_WARPS * 32, FL_MINB) void k_forces_list(
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     for (int k = tid; k < (int)(sizeof(SphGrid) / 4); k += blockDim.x) ((int*)&g)[k] = ((const int*)gp)[k];
     __syncthreads();
+    if (g.flags & SPH_GRID_STEEP) return;   // steep h contrast: the 8-lane kernels take every target
     const unsigned nb = *nbuckets;
     const float hmax_all = __uint_as_float(g.force_hmax_bits);
     const float iLx = g.per[0] ? 1.0f / g.len[0] : 0.0f, Lx = g.per[0] ? g.len[0] : 0.0f;

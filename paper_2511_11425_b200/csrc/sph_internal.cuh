@@ -22,7 +22,9 @@ struct SphGrid {
     int   per[3];
     float hmin, hmax;          // of the h given to sph_build_cells
     float xext;                // largest |coordinate| that enters a displacement
-    int   flags;               // bit0: periodic side too short; bit1: cell table clipped
+    int   flags;               // bit0: periodic side too short; bit1: cell table clipped; bit2: no valid h;
+                               // bit3: steep h contrast (max h > 3 min h): the staged-tile sweeps stand
+                               // back and every target takes the 8-lane kernels (set only in automatic mode)
     unsigned force_hmax_bits;  // max h given to sph_forces (float bits, atomicMax)
     int   cn[3];               // coarse grid (max-h map for the scatter reach of the force search)
     float ics[3];              // inverse coarse cell sides
@@ -45,6 +47,7 @@ struct sph_ctx {
     sph_params   par;
     sph_box      box;
     int64_t      n_max, n;
+    int64_t      n_build;      // n of the sph_build_cells call in progress / last
     int64_t      cap_cells;
     cudaStream_t stream;
     bool         built;
@@ -92,6 +95,15 @@ struct sph_ctx {
 };
 
 #define SPH_SCAN_BLOCKS 1024
+#define SPH_GRID_STEEP 8           // SphGrid.flags bit 3
+#define SPH_TILE_MIN_N (1 << 19)   // automatic mode: fewer particles than this cannot fill the GPU with
+                                   // one warp per bucket of 64 (148 SMs x 7 warps x a few buckets each)
+
+// The staged-tile sweeps are in use for this index: forced (tile > 0), or automatic (tile = 0) with
+// enough particles.  (In automatic mode the device may still stand them down: SPH_GRID_STEEP.)
+static inline bool sph_tile_on(const sph_ctx* c) {
+    return c->par.tile > 0 || (c->par.tile == 0 && c->n_build >= SPH_TILE_MIN_N);
+}
 
 #define SPH_CUDA_CHECK(ctx, call)                                                          \
     do {                                                                                   \

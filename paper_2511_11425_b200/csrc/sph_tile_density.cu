@@ -192,6 +192,7 @@ __global__ __launch_bounds__(SPH_TWMAX * 32) void k_density_tile(
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     __syncthreads();
     uint32_t parity = 0;
+    if (g.flags & SPH_GRID_STEEP) return;   // steep h contrast: the 8-lane kernels take every target
     const unsigned nb = *nbuckets;
     const float hcap = tile_hcap(g);
     const float lslack = MOM ? (1.0f + T_ZONE) * 1.001f : par.slack;   // list radius / 2h
@@ -695,7 +696,6 @@ int sph_launch_buckets(sph_ctx* c) {
 // occupancy), then over the buckets that did not fit with a tile of SPH_TCAP_BIG; the targets
 // left after that are in c->fb_list (c->fb_cnt of them) and are swept by the caller with the
 // 8-lanes-per-target kernel.
-#define SPH_TCAP_BIG 2560
 int sph_launch_density_tile(sph_ctx* c, float* h, float* rho, float* omega, int32_t* nn) {
     cudaStream_t s = c->stream;
     const int W = c->par.tile_warps;
@@ -707,8 +707,9 @@ int sph_launch_density_tile(sph_ctx* c, float* h, float* rho, float* omega, int3
     auto launch = [&](auto tag) -> cudaError_t {
         constexpr int KERN = decltype(tag)::value;
         for (int pass = 0; pass < 2; ++pass) {
-            const int tcap = pass == 0 ? c->par.tile_cap : SPH_TCAP_BIG;
-            if (pass == 1 && c->par.tile_cap >= SPH_TCAP_BIG) break;
+            const int  tcap = pass == 0 ? c->par.tile_cap : c->par.tile_cap2;
+            const bool two  = c->par.tile_cap2 >= c->par.tile_cap + 32;
+            if (pass == 1 && !two) break;
             TilePar par{c->par.n_ngb, c->par.h_tol, c->par.search_slack, c->par.h_max_iter, tcap};
             const size_t smem = sph_tile_smem_bytes(tcap, 16, sph_tile_xbytes(W, 8), W);
             cudaError_t e = cudaFuncSetAttribute(k_density_tile<KERN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -717,7 +718,7 @@ int sph_launch_density_tile(sph_ctx* c, float* h, float* rho, float* omega, int3
             e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_density_tile<KERN>, 32 * W, smem);
             if (e != cudaSuccess) return e;
             if (per_sm < 1) per_sm = 1;
-            const bool last = pass == 1 || c->par.tile_cap >= SPH_TCAP_BIG;
+            const bool last = pass == 1 || !two;
             k_density_tile<KERN><<<c->sm_count * per_sm, 32 * W, smem, s>>>(
                 c->grid, c->cell_start, c->pos_m, c->perm, c->buckets,
                 pass == 0 ? c->bucket_cnt : c->big_cnt, pass == 0 ? nullptr : c->big_list,

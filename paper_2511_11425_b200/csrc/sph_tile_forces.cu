@@ -150,6 +150,7 @@ __global__ __launch_bounds__(SPH_TWMAX * 32) void k_forces_tile(
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     __syncthreads();
     uint32_t parity = 0;
+    if (g.flags & SPH_GRID_STEEP) return;   // steep h contrast: the 8-lane kernels take every target
     const unsigned nb = *nbuckets;
     const float hmax_all = __uint_as_float(g.force_hmax_bits);
     unsigned long long c_tested = 0;
@@ -339,8 +340,9 @@ int sph_launch_forces_tile(sph_ctx* c, float* ax, float* ay, float* az, float* d
         constexpr int  KERN = decltype(tag)::value;
         constexpr bool ENT  = decltype(etag)::value;
         for (int pass = 0; pass < 2; ++pass) {
-            const int tcap = pass == 0 ? c->par.tile_fcap : SPH_FTCAP_BIG;
-            if (pass == 1 && c->par.tile_fcap >= SPH_FTCAP_BIG) break;
+            const int  tcap = pass == 0 ? c->par.tile_fcap : SPH_FTCAP_BIG;
+            const bool two  = c->par.tile_fcap < SPH_FTCAP_BIG && c->par.tile_cap2 >= c->par.tile_cap + 32;
+            if (pass == 1 && !two) break;
             FTilePar par{{c->par.av_alpha, c->par.av_beta, c->par.av_eps}, tcap};
             const size_t smem = ftile_smem_bytes(tcap, W);
             cudaError_t e = cudaFuncSetAttribute(k_forces_tile<KERN, ENT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -349,7 +351,7 @@ int sph_launch_forces_tile(sph_ctx* c, float* ax, float* ay, float* az, float* d
             e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_forces_tile<KERN, ENT>, 32 * W, smem);
             if (e != cudaSuccess) return e;
             if (per_sm < 1) per_sm = 1;
-            const bool last = pass == 1 || c->par.tile_fcap >= SPH_FTCAP_BIG;
+            const bool last = pass == 1 || !two;
             k_forces_tile<KERN, ENT><<<c->sm_count * per_sm, 32 * W, smem, s>>>(
                 c->grid, c->cell_start, c->pos_h, c->vel_m, c->rcak, c->perm, c->buckets,
                 pass == 0 ? c->bucket_cnt : c->big_cnt + 1, pass == 0 ? nullptr : c->big_list,

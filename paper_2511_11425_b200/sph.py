@@ -41,7 +41,7 @@ class _Params(C.Structure):
                 ("h_max_iter", C.c_int32), ("search_slack", C.c_float),
                 ("cell_div_x", C.c_float), ("cell_div_yz", C.c_float), ("entropy", C.c_int32),
                 ("tile", C.c_int32), ("tile_rows", C.c_int32), ("tile_cap", C.c_int32),
-                ("tile_warps", C.c_int32), ("tile_forces", C.c_int32), ("tile_fcap", C.c_int32),
+                ("tile_cap2", C.c_int32), ("tile_warps", C.c_int32), ("tile_forces", C.c_int32), ("tile_fcap", C.c_int32),
                 ("tile_fwarps", C.c_int32)]
 
 
@@ -71,6 +71,7 @@ class Params:
     tile: int = 0               # -1: staged-tile sweeps off (8-lanes-per-target kernels only)
     tile_rows: int = 0          # 0 -> library default
     tile_cap: int = 0
+    tile_cap2: int = 0
     tile_warps: int = 0
     tile_forces: int = 0        # 1: force sweep on staged tiles (default: kept neighbour lists)
     tile_fcap: int = 0          # the force sweep's tile capacity and warps per bucket
@@ -80,7 +81,7 @@ class Params:
         return _Params(self.kernel, self.n_ngb, self.gamma, self.av_alpha, self.av_beta,
                        self.av_eps, self.eta_cfl, self.eta_acc, self.h_tol, self.h_max_iter,
                        self.search_slack, self.cell_div_x, self.cell_div_yz, int(self.entropy),
-                       int(self.tile), int(self.tile_rows), int(self.tile_cap), int(self.tile_warps),
+                       int(self.tile), int(self.tile_rows), int(self.tile_cap), int(self.tile_cap2), int(self.tile_warps),
                        int(self.tile_forces), int(self.tile_fcap), int(self.tile_fwarps))
 
 

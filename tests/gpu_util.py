@@ -18,6 +18,9 @@ def to_device(w):
 
 
 def make_params(w, **kw):
+    # the staged-tile sweeps are forced on unless a test says otherwise: in automatic mode
+    # (tile = 0) the small test cases would all take the 8-lanes-per-target kernels
+    kw.setdefault("tile", 1)
     gp = sph.Params(gamma=float(w["gamma"]), av_alpha=float(w["av_alpha"]),
                     av_beta=float(w["av_beta"]), **kw)
     op = orc.Params(kernel=gp.kernel, n_ngb=float(np.float32(gp.n_ngb)),

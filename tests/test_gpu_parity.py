@@ -403,11 +403,11 @@ def test_c4_kelvin_helmholtz_full_size_sampled(gu):
     assert st["force_av_pairs"] > 0          # the shear takes the viscosity branch
 
 
-def _impact_case(gu, n_target, n_impactor, k):
+def _impact_case(gu, n_target, n_impactor, k, **kw):
     w = workloads.impact(n_target=n_target, n_impactor=n_impactor, h_start="warm")
     _, op = gu.make_params(w)
     _, ob = gu.make_boxes(w)
-    ctx, d, out, h = _full_step(gu, w)
+    ctx, d, out, h = _full_step(gu, w, **kw)
     st = ctx.stats()
     assert st["dens_nonconv"] == 0, st
     # free surfaces: half of the sample from the 2 % of particles with the largest h
@@ -422,13 +422,30 @@ def _impact_case(gu, n_target, n_impactor, k):
 def test_c5_impact_reduced_size_free_surfaces(gu):
     """Config 5's shape at 1/10 of its size (two n=1 polytropes in vacuum, ~1.3 M particles):
     open box, one-sided neighbourhoods at the surfaces, h varying by an order of magnitude."""
-    _impact_case(gu, 1_200_000, 150_000, 1024)
+    st = _impact_case(gu, 1_200_000, 150_000, 1024)       # staged tiles forced: hand-backs exercised
+    assert st["grid_flags"] & 8 == 0 and st["dens_tested"] > 300 * 1_000_000
 
 
 def test_c5_impact_full_size_sampled(gu):
     """Config 5 at BASELINE.json's full size: 12 M + 1.5 M lattice points before the surface
     truncation (about 13.4 M particles), sampled like the reduced case (~25 s on a B200 box)."""
-    _impact_case(gu, 12_000_000, 1_500_000, 256)
+    st = _impact_case(gu, 12_000_000, 1_500_000, 256, tile=0)
+    assert st["grid_flags"] & 8                            # automatic mode saw the h contrast: 8-lane kernels
+
+
+def test_automatic_mode_picks_the_sweep_by_size_and_h_contrast(gu):
+    """sph_params.tile = 0: the staged-tile sweeps run when there are at least 2^19 particles and
+    max h <= 3 min h (decided on the device, SphGrid flag bit 3); results are within tolerance of
+    the oracle either way (the other tests), here: which path ran."""
+    for nside, tiled in ((64, False), (96, True)):
+        w = workloads.sedov(nside=nside, h_start="warm")
+        ctx, d, out, h = _full_step(gu, w, tile=0)
+        st = ctx.stats()
+        assert st["grid_flags"] & 8 == 0
+        # the tile sweep tests every staged candidate for every target (~700), the 8-lane kernel ~210
+        assert (st["dens_tested"] > 500 * w["n"]) == tiled, (nside, st["dens_tested"] / w["n"])
+        assert st["dens_nonconv"] == 0
+        ctx.close()
 
 
 # ------------------------------------------------------------------------------------------
