@@ -3,14 +3,15 @@
 // PAPER.md:137-154, Eqs. (5)-(7), with one lane per pair of targets over a shared-memory tile
 // of candidate sources (sph_tile.cuh).  The arithmetic of the solve is the one documented in
 // sph_density.cu (Halley step on S, E, F with Taylor-carried sums); only the parallel shape
-// differs:
+// differs (Wendland C2 solves Eq. (6) from the moments of ONE sweep, see below):
 //   * one warp owns a bucket of <= 64 targets, two per lane;
 //   * the bucket's candidate rows are staged once by bulk asynchronous copies (UBLKCP) that
 //     complete on an mbarrier, then moved into the bucket's frame;
 //   * phase 1 turns the tile into per-target accept masks (FFMA2 on broadcast loads);
 //   * each sweep walks a lane-private cursor over its masks: no ballots, no shuffles, no
 //     per-candidate list stores, no reduction across lanes;
-//   * the masks stay in global memory for the force sweep (sph_tile_forces.cu).
+//   * the accepted entries' sorted positions go to a bucket-major list in global memory, from
+//     the sweep itself: the neighbour lists the force sweep reads (sph_forces_list.cu).
 // Buckets the tile cannot hold (too many rows or candidates: steep h contrast, a periodic axis
 // barely longer than the search ball) are handed to the 8-lanes-per-target kernel of
 // sph_density.cu through a target list; targets with a borderline neighbour or without
