@@ -71,26 +71,30 @@ typedef struct {
     float   search_slack; /* density search radius = 2 h_guess x this (<= 1: default 1.1);  */
                           /* PAPER.md:152 "slightly larger kernel"; results do not depend   */
                           /* on it                                                         */
-    float   cell_div_x;   /* cells per minimum search radius along x (<= 0: default 8 with  */
-                          /* the staged-tile sweeps, 4 without)                            */
-    float   cell_div_yz;  /* ... along y and z (<= 0: default 2, or 1.5 without tiles)      */
+    float   cell_div_x;   /* cells per minimum search radius along x (<= 0: automatic: 8     */
+                          /* when the staged-tile sweeps run, 4 otherwise)                   */
+    float   cell_div_yz;  /* ... along y and z (<= 0: automatic: 2 with tiles, else 1.5)     */
     int32_t entropy;      /* 1: entropy-conserving variant: sph_forces drops */
                           /* the Eq. (14) term, dudt is the viscous heating of Eq. (18)     */
                           /* alone; the caller advances u with sph_isentropic_u             */
     int32_t tile;         /* staged-tile sweeps (buckets of 64 targets over a shared-memory   */
-                          /* tile of sources): 0 = on (default), -1 =    */
-                          /* off: every target takes the 8-lanes-per-target kernels.  Results */
-                          /* do not depend on it beyond rounding                             */
+                          /* tile of sources).  0 (default) = automatic: */
+                          /* on for n >= 2^19 particles unless max h > 3 min h at build time  */
+                          /* (decided on the device); 1 = on whatever the size or h contrast; */
+                          /* -1 = off: every target takes the 8-lanes-per-target kernels.     */
+                          /* Results do not depend on it beyond rounding                      */
     int32_t tile_rows;    /* a bucket spans tile_rows x tile_rows rows of cells (<= 0:        */
                           /* default 3; at most 5)                                           */
-    int32_t tile_cap;     /* candidates a tile holds (<= 0: default 1024); buckets that need  */
-                          /* more fall back to the 8-lane kernels                            */
-    int32_t tile_cap2;    /* tile of the second pass over the buckets the first tile could not  */
-                          /* hold (<= 0: default 2560; below tile_cap + 32: no second pass)    */
+    int32_t tile_cap;     /* candidates a tile holds (<= 0: default 768); buckets that need   */
+                          /* more go to the second pass                                      */
+    int32_t tile_cap2;    /* tile of the second pass (<= 0: default 2560; below tile_cap + 32: */
+                          /* no second pass); buckets it cannot hold either fall back to the  */
+                          /* 8-lane kernels                                                   */
     int32_t tile_warps;   /* warps that share a bucket's tile (<= 0: default 1; at most 4)    */
-    int32_t tile_forces;  /* 0 (default): the force sweep reads the neighbour lists the       */
-                          /* density sweep kept (8 lanes per target); 1: the force sweep runs  */
-                          /* on staged tiles too (measured slower)        */
+    int32_t tile_forces;  /* 0 (default): the force sweep reads the bucket-major neighbour    */
+                          /* lists the tile density sweep kept (one warp per bucket); 1: the  */
+                          /* force sweep runs on staged tiles too (measured slower, DESIGN.md */
+                          /* section 7)                                                       */
     int32_t tile_fcap;    /* tile_cap and tile_warps of the force sweep (<= 0: defaults 576   */
     int32_t tile_fwarps;  /* and 1); its tile holds 52 B per candidate, the density tile 20   */
 } sph_params;

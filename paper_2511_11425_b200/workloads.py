@@ -100,7 +100,7 @@ def sod_tube(ncross=38, seed=114252, h_start="warm", jitter=0.0):
 
 def sedov(nside=128, jitter=0.01, seed=114253, h_start="warm", v_sigma=0.0):
     """C3: unit periodic cube, rho=1, u_bg=1e-5, E=1 spread smoothly over the particles within
-    2.4694 lattice spacings of the centre (PAPER.md:311 uses a top-hat of radius 0.02).
+    2.5 lattice spacings of the centre (PAPER.md:311 uses a top-hat of radius 0.02).
     v_sigma > 0 gives the throughput variant C3v with random velocities."""
     rng = np.random.default_rng(seed)
     dx = 1.0 / nside
@@ -110,10 +110,11 @@ def sedov(nside=128, jitter=0.01, seed=114253, h_start="warm", v_sigma=0.0):
     y = (y + rng.uniform(-jitter, jitter, n) * dx) % 1.0
     z = (z + rng.uniform(-jitter, jitter, n) * dx) % 1.0
     m = 1.0 / n
-    # initial-condition profile of the deposited energy: a smooth bump of radius R
-    R = 2.0 * H_OVER_DELTA * dx
-    s = np.sqrt((x - 0.5) ** 2 + (y - 0.5) ** 2 + (z - 0.5) ** 2) / R
-    bump = np.where(s < 1.0, (1.0 - s) ** 4 * (1.0 + 4.0 * s), 0.0)
+    # initial-condition profile of the deposited energy: a smooth bump (1 - s^2)^2 of radius
+    # 2.5 lattice spacings -- a recipe of this generator, not a formula of the method
+    R = 2.5 * dx
+    s2 = ((x - 0.5) ** 2 + (y - 0.5) ** 2 + (z - 0.5) ** 2) / R ** 2
+    bump = np.where(s2 < 1.0, (1.0 - s2) ** 2, 0.0)
     u = 1e-5 + 1.0 * bump / (m * bump.sum())
     vel = (lambda: rng.normal(0, v_sigma, n)) if v_sigma > 0 else (lambda: 0.0)
     w = dict(name="sedov" if v_sigma == 0 else "sedov_v", x=x, y=y, z=z, m=m,
