@@ -90,7 +90,8 @@ typedef struct {
     int32_t tile_cap2;    /* tile of the second pass (<= 0: default 2560; below tile_cap + 32: */
                           /* no second pass); buckets it cannot hold either fall back to the  */
                           /* 8-lane kernels                                                   */
-    int32_t tile_warps;   /* warps that share a bucket's tile (<= 0: default 1; at most 4)    */
+    int32_t tile_warps;   /* warps per bucket of the density sweep: 2 (default, <= 0) = one   */
+                          /* target per thread; 1 = one warp, two targets per lane            */
     int32_t tile_forces;  /* 0 (default): the force sweep reads the bucket-major neighbour    */
                           /* lists the tile density sweep kept (one warp per bucket); 1: the  */
                           /* force sweep runs on staged tiles too (measured slower, DESIGN.md */

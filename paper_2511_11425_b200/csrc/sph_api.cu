@@ -25,8 +25,8 @@ static void fill_defaults(sph_params& p) {
     if (p.tile_cap2 <= 0) p.tile_cap2 = 2560;
     p.tile_cap2 = (p.tile_cap2 + 31) & ~31;
     if (p.tile_cap2 > 4064) p.tile_cap2 = 4064;
-    if (p.tile_warps <= 0) p.tile_warps = 1;
-    if (p.tile_warps > SPH_TWMAX) p.tile_warps = SPH_TWMAX;
+    if (p.tile_warps <= 0) p.tile_warps = 2;
+    if (p.tile_warps > 2) p.tile_warps = 2;
     if (p.tile_fcap <= 0) p.tile_fcap = 576;
     p.tile_fcap = (p.tile_fcap + 31) & ~31;
     if (p.tile_fcap > 4096) p.tile_fcap = 4096;

@@ -490,38 +490,115 @@ __device__ __forceinline__ void sph_cursor_skip(SphCursor& c, uint32_t mend, int
 // Two entry sets per target are used in turn: the record of an entry is in flight while the
 // entry before it is worked on, without register copies.  work(t, entry) sees bubbles too
 // (has = false; the padding record, m = pad_w of sph_tile_finish).
-template <class Work>
+template <int NSET = 2, class Work>
 __device__ __forceinline__ void sph_tile_walk(const SphTileMem& sm, const SphTileInfo& ti, int lane,
                                               int wid, int W, const bool on[2], Work&& work,
                                               int ep = 0, int es = 1) {
     SphCursor cu[2];
-    SphEntry  ea[2], eb[2];
+    SphEntry  e[NSET][2];
     const int idx_max = ti.nwords * 32;                               // first padding entry
     // this warp's second zero word behind the masks
     const uint32_t mend = sm.mask_sa + 4u * (uint32_t)((sph_first_pad_word(ti.nwords, wid, W) + W) * SPH_TB);
-    auto fetch = [&](int t, SphEntry& e) {
+    auto fetch = [&](int t, SphEntry& en) {
         const uint32_t me = mend + 4u * (uint32_t)(lane + 32 * t);
         for (int s = 0; s < ep; ++s) sph_cursor_skip(cu[t], me, W);
-        sph_cursor_fetch(cu[t], sm, idx_max, me, W, e);
+        sph_cursor_fetch(cu[t], sm, idx_max, me, W, en);
         for (int s = ep + 1; s < es; ++s) sph_cursor_skip(cu[t], me, W);
     };
 #pragma unroll
     for (int t = 0; t < 2; ++t) {
         sph_cursor_start(cu[t], sm, ti, lane + 32 * t, on[t], wid, W);
-        fetch(t, ea[t]);
-        fetch(t, eb[t]);
+#pragma unroll
+        for (int q = 0; q < NSET; ++q) fetch(t, e[q][t]);
     }
-    while (__any_sync(SPH_FULL, ea[0].has || ea[1].has || eb[0].has || eb[1].has ||
-                                    sph_cursor_live(cu[0], ti) || sph_cursor_live(cu[1], ti))) {
+    for (;;) {
+        bool live = sph_cursor_live(cu[0], ti) || sph_cursor_live(cu[1], ti);
 #pragma unroll
-        for (int t = 0; t < 2; ++t) {
-            work(t, ea[t]);
-            fetch(t, ea[t]);
+        for (int q = 0; q < NSET; ++q) live = live || e[q][0].has || e[q][1].has;
+        if (!__any_sync(SPH_FULL, live)) break;
+#pragma unroll
+        for (int q = 0; q < NSET; ++q) {
+#pragma unroll
+            for (int t = 0; t < 2; ++t) {
+                work(t, e[q][t]);
+                fetch(t, e[q][t]);
+            }
         }
+    }
+}
+
+// ---- one thread per target (or two): the forms used when NW = 2 / NT warps share a bucket,
+// each thread owning NT targets: columns tid + 32 t, t < NT, of the mask words --------------
+
+// Phase 1 with the targets' parameters in shared memory, as pairs: component c (0..3 =
+// -2 x, -2 y, -2 z, |x|^2 - Rc^2 in the tile's frame; (0, 0, 0, 3e38) switches a target off)
+// of target columns l and l + 32 side by side at tgt[2 (32 c + l)], so that one 64-bit load
+// gives the operand of a packed instruction (sph_tgt_put writes one column).
+// Warp wid of NW computes the words w = wid, wid + NW, ... for all 64 columns (lane l: columns
+// l and l + 32, as sph_tile_masks) and zeroes its share of the pad words nwords .. nwords +
+// 2 NW - 1.  The caller puts a block barrier on both sides.
+__device__ __forceinline__ void sph_tgt_put(float* tgt, int col, float x, float y, float z, float c) {
+    float* q = tgt + 2 * (col & 31) + (col >> 5);
+    q[0] = x; q[64] = y; q[128] = z; q[192] = c;
+}
+__device__ __forceinline__ void sph_tile_masks_sh(const SphTileMem& sm, const SphTileInfo& ti,
+                                                  const float* tgt, int lane, int wid, int NW) {
+    const sph_f2* tp = (const sph_f2*)tgt;
+    const sph_f2 ax = tp[lane], ay = tp[32 + lane], az = tp[64 + lane], cc = tp[96 + lane];
+    for (int w = wid; w < ti.nwords; w += NW) {
+        uint32_t m0 = 0u, m1 = 0u;
+        const float4* c = sm.tile + w * 32;
 #pragma unroll
-        for (int t = 0; t < 2; ++t) {
-            work(t, eb[t]);
-            fetch(t, eb[t]);
+        for (int u = 0; u < 32; ++u) {
+            const float4 p = c[u];
+            sph_f2 t = sph_add2(sph_pk(p.w, p.w), cc);
+            t = sph_fma2(ax, sph_pk(p.x, p.x), t);
+            t = sph_fma2(ay, sph_pk(p.y, p.y), t);
+            t = sph_fma2(az, sph_pk(p.z, p.z), t);
+            m0 = __funnelshift_l((uint32_t)t, m0, 1);
+            m1 = __funnelshift_l((uint32_t)(t >> 32), m1, 1);
+        }
+        sm.mask[w * SPH_TB + lane]      = m0;
+        sm.mask[w * SPH_TB + 32 + lane] = m1;
+    }
+    for (int k = 0, w = sph_first_pad_word(ti.nwords, wid, NW); k < 2; ++k, w += NW) {
+        sm.mask[w * SPH_TB + lane]      = 0u;
+        sm.mask[w * SPH_TB + 32 + lane] = 0u;
+    }
+}
+
+// Walks the accepted entries of the thread's NT targets (columns tid + 32 t) over ALL mask
+// words, NSET entries per target in flight.  work(t, entry) sees bubbles too.
+template <int NT, int NSET, class Work>
+__device__ __forceinline__ void sph_tile_walk_own(const SphTileMem& sm, const SphTileInfo& ti, int tid,
+                                                  const bool on[NT], Work&& work) {
+    SphCursor cu[NT];
+    SphEntry  e[NSET][NT];
+    const int idx_max = ti.nwords * 32;                               // first padding entry
+    const uint32_t mend = sm.mask_sa + 4u * (uint32_t)((ti.nwords + 1) * SPH_TB);   // second zero word
+#pragma unroll
+    for (int t = 0; t < NT; ++t) {
+        sph_cursor_start(cu[t], sm, ti, tid + 32 * t, on[t], 0, 1);
+#pragma unroll
+        for (int q = 0; q < NSET; ++q)
+            sph_cursor_fetch(cu[t], sm, idx_max, mend + 4u * (uint32_t)(tid + 32 * t), 1, e[q][t]);
+    }
+    for (;;) {
+        bool live = false;
+#pragma unroll
+        for (int t = 0; t < NT; ++t) {
+            live = live || sph_cursor_live(cu[t], ti);
+#pragma unroll
+            for (int q = 0; q < NSET; ++q) live = live || e[q][t].has;
+        }
+        if (!__any_sync(SPH_FULL, live)) break;
+#pragma unroll
+        for (int q = 0; q < NSET; ++q) {
+#pragma unroll
+            for (int t = 0; t < NT; ++t) {
+                work(t, e[q][t]);
+                sph_cursor_fetch(cu[t], sm, idx_max, mend + 4u * (uint32_t)(tid + 32 * t), 1, e[q][t]);
+            }
         }
     }
 }

@@ -156,18 +156,21 @@ __device__ __forceinline__ void c2_poly(const float M[6], float lam, float& S, f
 }
 
 // ------------------------------------------------------------------------------------------
-// a4-a6 on the tile.  Persistent blocks of W warps; a block takes one bucket at a time (handed
-// out by a counter).  Every warp holds the bucket's 64 targets (lane l: targets l and l + 32)
-// and works on its share of the tile -- the candidates for the frame transform, the mask words
-// w = wid, wid + W, ... for phase 1 and for the walk -- so W warps hide each other's latencies
-// on one tile's worth of shared memory.  The partial sums meet in shared memory; every warp
-// then runs the same scalar solve (identical state in all warps, no broadcast), warp 0 alone
-// finishes (zone pass, results).
+// a4-a6 on the tile.  Persistent blocks of NW = 2 / NT warps; a block takes one bucket at a
+// time (handed out by a counter) and every thread owns NT of its 64 targets (columns
+// tid + 32 t of the mask words): NT = 2, one warp, two targets per lane; NT = 1, two warps,
+// one target per thread.  The block stages the tile once (warp 0 issues the copies), all
+// threads move it into the bucket's frame, the warps split the mask words of phase 1, and
+// then every thread walks, solves and stores its own targets -- no exchange of partial sums.
+// Decisions that steer the block (another stage, another sweep, new masks) are block-wide
+// votes through shared memory.
 // ------------------------------------------------------------------------------------------
-constexpr int DT_NPART = 8;   // words per target and warp in the exchange area: 6 sums, entries, zone entries
+#ifndef SPH_DT_NSET
+#define SPH_DT_NSET 0   // 0: 3 with one target per thread, 2 with two
+#endif
 
-template <int KERN>
-__global__ __launch_bounds__(SPH_TWMAX * 32) void k_density_tile(
+template <int KERN, int NT>
+__global__ __launch_bounds__(64 / NT, NT == 1 ? 7 : 8) void k_density_tile(
     const SphGrid* __restrict__ gp, const uint32_t* __restrict__ cell_start,
     const float4* __restrict__ pos_m, const int32_t* __restrict__ perm,
     const SphBucket* __restrict__ buckets, const unsigned* __restrict__ nbuckets,
@@ -177,18 +180,21 @@ __global__ __launch_bounds__(SPH_TWMAX * 32) void k_density_tile(
     unsigned* list_next, uint32_t* bucket_loff, uint32_t* nb_cnt, float* nb_rkeep, float* tl_rkeep,
     unsigned long long* stats) {
     constexpr bool MOM = (KERN == 1);   // the moment solve exists for Wendland C2
+    constexpr int  NW = 2 / NT, NTHR = 32 * NW;
+    constexpr int  NSET = SPH_DT_NSET > 0 ? SPH_DT_NSET : (NT == 1 ? 3 : 2);   // entries in flight per target in the sweep
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ SphGrid     g;
     __shared__ SphTileInfo ti;
-    __shared__ unsigned    bi_s;
-    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5, W = blockDim.x >> 5, nthr = blockDim.x;
-    for (int k = tid; k < (int)(sizeof(SphGrid) / 4); k += nthr) ((int*)&g)[k] = ((const int*)gp)[k];
-    const SphTileMem sm = sph_tile_carve<16>(smem_raw, par.tcap, sph_tile_xbytes(W, DT_NPART), W);
-    // exchange area of the partial sums [W][DT_NPART][64]: the segment table's memory, which is
-    // dead once the tile is in place
-    float* const xch = (float*)sm.seg;
-    const int ZW = SPH_TZCAP / W;          // zone slots per warp: [wid * ZW, +ZW)
-    float* const edge = (float*)sm.zone;   // Halley path: [W][4][64] floats in the zone area
+    __shared__ unsigned    bi_s, lreg_s;
+    __shared__ float       bb_s[2][8];      // per warp: bounding box of its targets, first list radius
+    __shared__ float       xf_s[2][2];      // block votes: [phase][warp]
+    __shared__ unsigned    xu_s[2][2];
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    for (int k = tid; k < (int)(sizeof(SphGrid) / 4); k += NTHR) ((int*)&g)[k] = ((const int*)gp)[k];
+    const SphTileMem sm = sph_tile_carve<16>(smem_raw, par.tcap, sph_tile_xbytes(1, 0), NW);
+    // the targets' mask parameters (sph_tgt_put): the segment table's memory, dead once the tile is in place
+    float* const  tgt  = (float*)sm.seg;
+    float* const  edge = (float*)sm.zone;   // Halley path: [4][64] floats in the zone area
     if (tid == 0) sph_mbar_init(sm.bar, 1u);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     __syncthreads();
@@ -199,15 +205,56 @@ __global__ __launch_bounds__(SPH_TWMAX * 32) void k_density_tile(
     const float lslack = MOM ? (1.0f + T_ZONE) * 1.001f : par.slack;   // list radius / 2h
     unsigned long long c_tested = 0;
     unsigned c_listed = 0, c_pairs = 0, c_sweeps = 0, c_recollect = 0;
+    int xph = 0;
+    auto block_sync = [&]() { if constexpr (NW > 1) __syncthreads(); else __syncwarp(); };
+    auto block_max = [&](float v) -> float {
+        v = warp_max(v);
+        if constexpr (NW > 1) {
+            if (lane == 0) xf_s[xph][wid] = v;
+            __syncthreads();
+            v = fmaxf(xf_s[xph][0], xf_s[xph][1]);
+            xph ^= 1;
+        }
+        return v;
+    };
+    auto block_or = [&](unsigned v) -> unsigned {
+        v = __reduce_or_sync(SPH_FULL, v);
+        if constexpr (NW > 1) {
+            if (lane == 0) xu_s[xph][wid] = v;
+            __syncthreads();
+            v = xu_s[xph][0] | xu_s[xph][1];
+            xph ^= 1;
+        }
+        return v;
+    };
+    // the next bucket's number is asked for one bucket ahead (thread 0 holds it)
+    unsigned nxt = 0;
+    if (tid == 0) nxt = atomicAdd(next, 1u);
 
     for (;;) {
         __syncthreads();                     // the last bucket's tile and tables are free
-        if (tid == 0) bi_s = atomicAdd(next, 1u);
+        if (tid == 0) bi_s = nxt;
         __syncthreads();
-        if (bi_s >= nb) break;
+        const unsigned bslot = bi_s;
+        if (bslot >= nb) break;
+        if (tid == 0) nxt = atomicAdd(next, 1u);
         // the buckets of the table, or (second pass, larger tile) the ones the first pass left
-        const unsigned  bi = blist ? blist[bi_s] : bi_s;
+        const unsigned  bi = blist ? blist[bslot] : bslot;
         const SphBucket bk = buckets[bi];
+        // The neighbour lists kept for the force sweep (PAPER.md:152 "we keep the precomputed
+        // interaction list"): entry f of target t of this bucket at lbase[f * 64 + t], the
+        // sorted position of the source -- written from the sweep as the entries are met, so a
+        // warp's stores fall into a few 256-byte rows.  The bucket takes one region of
+        // SPH_LCAP x 64 words from the pool (none left: no lists, the force sweep searches).
+        if (tid == 0) {
+            unsigned reg = 0xffffffffu;
+            if (nb_j != nullptr) {
+                reg = atomicAdd(list_next, 1u);
+                if (reg >= nb_regions) reg = 0xffffffffu;
+                bucket_loff[bi] = reg;
+            }
+            lreg_s = reg;   // read behind the barriers of the first stage
+        }
 
         // ---- the bucket's targets: rows (ry0 + a, rz0 + b), cells [c0, c1) of each
         const int nrows = bk.nry * bk.nrz;
@@ -229,13 +276,14 @@ __global__ __launch_bounds__(SPH_TWMAX * 32) void k_density_tile(
         int* const rowoff = sm.rowoff + 32 * wid;   // in the mask area: free until phase 1
         rowoff[lane] = inc;                      // inclusive prefix of the row counts
         __syncwarp();
-        int    p[2];
-        bool   valid[2];
-        float  xg[2], yg[2], zg[2], mi[2], h[2];
-        int    ic[2];
+        int    kc[NT], p[NT];                    // target column, sorted position
+        bool   valid[NT];
+        float  xg[NT], yg[NT], zg[NT], mi[NT], h[NT];
+        int    ic[NT];
 #pragma unroll
-        for (int t = 0; t < 2; ++t) {
-            const int k = lane + 32 * t;
+        for (int t = 0; t < NT; ++t) {
+            const int k = tid + 32 * t;
+            kc[t]    = k;
             valid[t] = k < ntar;
             int rho_ = 0;
             while (rho_ < 31 && rowoff[rho_] <= k) ++rho_;
@@ -255,124 +303,140 @@ __global__ __launch_bounds__(SPH_TWMAX * 32) void k_density_tile(
             xg[t] = pi.x; yg[t] = pi.y; zg[t] = pi.z; mi[t] = pi.w;
         }
         __syncwarp();
-        // bounding box of the targets
-        float b0[3], b1[3];
-        {
-            const float INF = __int_as_float(0x7f800000);
-            float lo[3] = {INF, INF, INF}, hi[3] = {-INF, -INF, -INF};
-#pragma unroll
-            for (int t = 0; t < 2; ++t)
-                if (valid[t]) {
-                    lo[0] = fminf(lo[0], xg[t]); hi[0] = fmaxf(hi[0], xg[t]);
-                    lo[1] = fminf(lo[1], yg[t]); hi[1] = fmaxf(hi[1], yg[t]);
-                    lo[2] = fminf(lo[2], zg[t]); hi[2] = fmaxf(hi[2], zg[t]);
-                }
-#pragma unroll
-            for (int d = 0; d < 3; ++d) { b0[d] = warp_min(lo[d]); b1[d] = warp_max(hi[d]); }
-        }
 
-        float T[2], hlo[2], hhi[2], S[2], E[2], Rc[2], want[2];
-        bool  done[2], fix[2], wait[2], recount[2], mvalid[2];
-        int   sweeps[2], ni[2];
+        float T[NT], hlo[NT], hhi[NT], S[NT], E[NT], Rc[NT], want[NT];
+        bool  done[NT], fix[NT], wait[NT], recount[NT], mvalid[NT];
+        int   sweeps[NT], ni[NT], nlist[NT];
 #pragma unroll
-        for (int t = 0; t < 2; ++t) {
+        for (int t = 0; t < NT; ++t) {
             T[t]   = par.n_ngb * mi[t] * (1.0f / SphKernel<KERN>::self);
             hlo[t] = 0.0f; hhi[t] = __int_as_float(0x7f800000);
             S[t] = 0.0f; E[t] = 0.0f; Rc[t] = 0.0f;
             done[t] = !valid[t]; fix[t] = false; wait[t] = valid[t];
             want[t] = valid[t] ? 2.0f * h[t] * lslack : 0.0f;
-            sweeps[t] = 0; ni[t] = 0; recount[t] = false; mvalid[t] = false;
+            sweeps[t] = 0; ni[t] = 0; recount[t] = false; mvalid[t] = false; nlist[t] = 0;
+        }
+        // bounding box of the block's targets and the first list radius
+        float b0[3], b1[3], Rt;
+        {
+            const float INF = __int_as_float(0x7f800000);
+            float lo[3] = {INF, INF, INF}, hi[3] = {-INF, -INF, -INF}, wr = 0.0f;
+#pragma unroll
+            for (int t = 0; t < NT; ++t)
+                if (valid[t]) {
+                    lo[0] = fminf(lo[0], xg[t]); hi[0] = fmaxf(hi[0], xg[t]);
+                    lo[1] = fminf(lo[1], yg[t]); hi[1] = fmaxf(hi[1], yg[t]);
+                    lo[2] = fminf(lo[2], zg[t]); hi[2] = fmaxf(hi[2], zg[t]);
+                    wr = fmaxf(wr, want[t]);
+                }
+#pragma unroll
+            for (int d = 0; d < 3; ++d) { b0[d] = warp_min(lo[d]); b1[d] = warp_max(hi[d]); }
+            Rt = warp_max(wr);
+            if constexpr (NW > 1) {
+                if (lane == 0) {
+#pragma unroll
+                    for (int d = 0; d < 3; ++d) { bb_s[wid][d] = b0[d]; bb_s[wid][3 + d] = b1[d]; }
+                    bb_s[wid][6] = Rt;
+                }
+                __syncthreads();
+#pragma unroll
+                for (int d = 0; d < 3; ++d) {
+                    b0[d] = fminf(bb_s[0][d], bb_s[1][d]);
+                    b1[d] = fmaxf(bb_s[0][3 + d], bb_s[1][3 + d]);
+                }
+                Rt = fmaxf(bb_s[0][6], bb_s[1][6]);
+            }
         }
         bool fallback = false;
-        // The neighbour lists kept for the force sweep (PAPER.md:152 "we keep the precomputed
-        // interaction list"): entry f of target t of this bucket at lbase[f * 64 + t], the
-        // sorted position of the source -- written from the sweep as the entries are met, so a
-        // warp's stores fall into a few 256-byte rows.  The bucket takes one region of
-        // SPH_LCAP x 64 words from the pool (none left: no lists, the force sweep searches).
         uint32_t* lbase = nullptr;
-        if (nb_j != nullptr && W == 1) {
-            unsigned reg = 0xffffffffu;
-            if (lane == 0) {
-                reg = atomicAdd(list_next, 1u);
-                if (reg >= nb_regions) reg = 0xffffffffu;
-                bucket_loff[bi] = reg;
-            }
-            reg = __shfl_sync(SPH_FULL, reg, 0);
-            if (reg != 0xffffffffu) lbase = nb_j + (size_t)reg * (SPH_LCAP * SPH_TB);
-        }
-        int nlist[2] = {0, 0};
 
         // ---- stages: (re)build the tile for the largest list radius wanted
-        for (int stage = 0; stage < 4; ++stage) {
-            const float Rt = warp_max(fmaxf(wait[0] ? want[0] : 0.0f, wait[1] ? want[1] : 0.0f));
-            if (!(Rt > 0.0f)) break;
-            __syncthreads();                 // everybody is done with the old tile and the exchange area
+        for (int stage = 0; stage < 4 && Rt > 0.0f; ++stage) {
+            __syncthreads();                 // everybody is done with the old tile and the targets' table
             if (wid == 0) {
                 SphTileInfo tl;
                 tl.ok = sph_tile_stage(g, cell_start, pos_m, b0, b1, Rt * (1.0f + 1e-5f), sm, lane, tl) ? 1 : 0;
                 if (lane == 0) ti = tl;
             }
             __syncthreads();
+            if (stage == 0 && lreg_s != 0xffffffffu) lbase = nb_j + (size_t)lreg_s * (SPH_LCAP * SPH_TB);
             if (!ti.ok) {
                 if (stage == 0) fallback = true;
                 else {
 #pragma unroll
-                    for (int t = 0; t < 2; ++t) if (wait[t]) { done[t] = true; fix[t] = true; wait[t] = false; }
+                    for (int t = 0; t < NT; ++t) if (wait[t]) { done[t] = true; fix[t] = true; wait[t] = false; }
                 }
                 break;
             }
-            if (stage > 0) c_recollect += (wait[0] ? 1u : 0u) + (wait[1] ? 1u : 0u);
-            mvalid[0] = mvalid[1] = false;   // a new tile: the masks of the old one are gone
-            sph_tile_finish(g, sm, ti, parity, tid, nthr, 0.0f);
+            if (stage > 0) {
+#pragma unroll
+                for (int t = 0; t < NT; ++t) c_recollect += wait[t] ? 1u : 0u;
+            }
+#pragma unroll
+            for (int t = 0; t < NT; ++t) mvalid[t] = false;   // a new tile: the masks of the old one are gone
+            sph_tile_finish(g, sm, ti, parity, tid, NTHR, 0.0f);
             parity ^= 1u;
             // the targets in the frame of the tile
-            float xt[2], yt[2], zt[2];
+            float xt[NT], yt[NT], zt[NT];
 #pragma unroll
-            for (int t = 0; t < 2; ++t) {
+            for (int t = 0; t < NT; ++t) {
                 xt[t] = (float)((double)xg[t] - (double)ti.ox);
                 yt[t] = (float)((double)yg[t] - (double)ti.oy);
                 zt[t] = (float)((double)zg[t] - (double)ti.oz);
             }
             const float band_c = 2.5e-7f * ti.ext;   // tau(h) = 1e-6 + band_c / h, DESIGN.md section 6
 #pragma unroll
-            for (int t = 0; t < 2; ++t)
+            for (int t = 0; t < NT; ++t)
                 if (wait[t]) { wait[t] = false; Rc[t] = fminf(want[t], Rt); }
             bool remask = true;
-            c_tested += (unsigned long long)ti.used * (unsigned)ntar;   // uniform: thread 0 reports it
+            if (tid == 0) c_tested += (unsigned long long)ti.used * (unsigned)ntar;
 
             // ---- sweeps on this tile
-            while (__any_sync(SPH_FULL, (!done[0] && !wait[0]) || (!done[1] && !wait[1]))) {
-                bool on[2] = {!done[0] && !wait[0], !done[1] && !wait[1]};
-                if (__any_sync(SPH_FULL, remask)) {
-                    float rr[2];
+            for (;;) {
+                bool need = false;
 #pragma unroll
-                    for (int t = 0; t < 2; ++t) rr[t] = on[t] ? Rc[t] : 0.0f;
-                    sph_tile_masks(sm, ti, xt, yt, zt, rr, lane, wid, W);   // this warp's words only
+                for (int t = 0; t < NT; ++t) need = need || (!done[t] && !wait[t]);
+                const unsigned vote = block_or((need ? 1u : 0u) | (remask ? 2u : 0u));
+                if (!(vote & 1u)) break;
+                bool on[NT];
+#pragma unroll
+                for (int t = 0; t < NT; ++t) on[t] = !done[t] && !wait[t];
+                if (vote & 2u) {
+#pragma unroll
+                    for (int t = 0; t < NT; ++t)
+                        if (on[t]) sph_tgt_put(tgt, kc[t], -2.0f * xt[t], -2.0f * yt[t], -2.0f * zt[t],
+                                               fmaf(zt[t], zt[t], fmaf(yt[t], yt[t], xt[t] * xt[t])) - Rc[t] * Rc[t]);
+                        else       sph_tgt_put(tgt, kc[t], 0.0f, 0.0f, 0.0f, 3.0e38f);
+                    block_sync();
+                    sph_tile_masks_sh(sm, ti, tgt, lane, wid, NW);   // this warp's words, all 64 columns
+                    block_sync();
                     remask = false;
 #pragma unroll
-                    for (int t = 0; t < 2; ++t) mvalid[t] = on[t];   // finished targets lost theirs
+                    for (int t = 0; t < NT; ++t) mvalid[t] = on[t];   // finished targets lost theirs
                 }
+                uint32_t* lcol[NT];   // the target's column of the bucket's list region
+#pragma unroll
+                for (int t = 0; t < NT; ++t) lcol[t] = lbase + kc[t];
+                const int lcap = lbase ? SPH_LCAP : 0;
+                int nent[NT];
+#pragma unroll
+                for (int t = 0; t < NT; ++t) nent[t] = 0;
                 if constexpr (MOM) {
                     // ---- one sweep: the six Bernstein moments, the zone list, the entry count
-                    float M[2][6];
-                    float ihh[2];
-                    int   nz[2] = {0, 0}, nent[2] = {0, 0};
-                    uint32_t za[2], zend[2];
+                    float M[NT][6];
+                    float ihh[NT];
+                    int   nz[NT];
+                    uint32_t za[NT], zend[NT];
 #pragma unroll
-                    for (int t = 0; t < 2; ++t) {
+                    for (int t = 0; t < NT; ++t) {
                         ihh[t] = __fdividef(0.5f, h[t]);
 #pragma unroll
                         for (int k = 0; k < 6; ++k) M[t][k] = 0.0f;
-                        za[t]   = sm.zone_sa + 2u * (uint32_t)(wid * ZW * SPH_TB + lane + 32 * t);
-                        zend[t] = za[t] + 2u * SPH_TB * (ZW - 1);
+                        nz[t]   = 0;
+                        za[t]   = sm.zone_sa + 2u * (uint32_t)kc[t];
+                        zend[t] = za[t] + 2u * SPH_TB * (SPH_TZCAP - 1);
                     }
-                    uint32_t *lp[2], *lend[2];   // the target's column of the bucket's list region
-#pragma unroll
-                    for (int t = 0; t < 2; ++t) {
-                        lp[t]   = lbase ? lbase + lane + 32 * t : nullptr;
-                        lend[t] = lbase ? lp[t] + SPH_LCAP * SPH_TB : nullptr;
-                    }
-                    sph_tile_walk(sm, ti, lane, wid, W, on, [&](int t, const SphEntry& en) {
+                    sph_tile_walk_own<NT, NSET>(sm, ti, tid, on, [&](int t, const SphEntry& en) {
                         const float dx = xt[t] - en.c.x, dy = yt[t] - en.c.y, dz = zt[t] - en.c.z;
                         const float r  = sph_sqrt(fmaf(dz, dz, fmaf(dy, dy, dx * dx)));
                         const float s  = r * ihh[t], tt = 1.0f - s;
@@ -386,10 +450,10 @@ __global__ __launch_bounds__(SPH_TWMAX * 32) void k_density_tile(
                         M[t][5] += a5;
                         {   // the kept list (a set: any sweep of this mask writes the same); predicated store
                             const uint32_t gj = sph_ldsu(sm.gidx_sa + 4u * (uint32_t)en.idx);
-                            const bool st = en.has && lp[t] < lend[t];
+                            const bool st = en.has && nent[t] < lcap;
+                            uint32_t* const la = lcol[t] + (uint32_t)nent[t] * (uint32_t)SPH_TB;
                             asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %2, 0;\n\t@p st.global.u32 [%0], %1;\n\t}"
-                                         ::"l"(lp[t]), "r"(gj), "r"((unsigned)st) : "memory");
-                            lp[t] += st ? SPH_TB : 0;
+                                         ::"l"(la), "r"(gj), "r"((unsigned)st) : "memory");
                         }
                         nent[t] += en.has ? 1 : 0;
                         // next to (or beyond) the support edge: remember the entry (predicated
@@ -400,49 +464,10 @@ __global__ __launch_bounds__(SPH_TWMAX * 32) void k_density_tile(
                         za[t] = inz ? min(za[t] + 2u * SPH_TB, zend[t]) : za[t];
                         nz[t] += inz ? 1 : 0;
                     });
-                    // ---- the warps' partial sums meet in shared memory; fixed order of addition
-                    int  nzw[2][SPH_TWMAX];
-                    bool zfit[2];
 #pragma unroll
-                    for (int t = 0; t < 2; ++t) {
-#pragma unroll
-                        for (int w = 0; w < SPH_TWMAX; ++w) nzw[t][w] = 0;
-                        nzw[t][0] = nz[t];
-                        zfit[t]   = nz[t] <= ZW;
-                    }
-                    if (W > 1) {
-#pragma unroll
-                        for (int t = 0; t < 2; ++t) {
-                            float* x = xch + (wid * DT_NPART) * SPH_TB + lane + 32 * t;
-#pragma unroll
-                            for (int k = 0; k < 6; ++k) x[k * SPH_TB] = M[t][k];
-                            x[6 * SPH_TB] = __int_as_float(nent[t]);
-                            x[7 * SPH_TB] = __int_as_float(nz[t]);
-                        }
-                        __syncthreads();
-#pragma unroll
-                        for (int t = 0; t < 2; ++t) {
-                            nent[t] = 0; nz[t] = 0; zfit[t] = true;
-#pragma unroll
-                            for (int k = 0; k < 6; ++k) M[t][k] = 0.0f;
-#pragma unroll
-                            for (int w = 0; w < SPH_TWMAX; ++w) {
-                                nzw[t][w] = 0;
-                                if (w >= W) continue;
-                                const float* x = xch + (w * DT_NPART) * SPH_TB + lane + 32 * t;
-#pragma unroll
-                                for (int k = 0; k < 6; ++k) M[t][k] += x[k * SPH_TB];
-                                nent[t] += __float_as_int(x[6 * SPH_TB]);
-                                const int q = __float_as_int(x[7 * SPH_TB]);
-                                nzw[t][w] = q;
-                                nz[t] += q;
-                                zfit[t] = zfit[t] && q <= ZW;
-                            }
-                        }
-                    }
-#pragma unroll
-                    for (int t = 0; t < 2; ++t) {
+                    for (int t = 0; t < NT; ++t) {
                         if (!on[t]) continue;
+                        const bool zfit = nz[t] <= SPH_TZCAP;
                         if (sweeps[t] == 0) c_listed += (unsigned)nent[t];
                         ++sweeps[t];
                         nlist[t] = nent[t];
@@ -459,30 +484,27 @@ __global__ __launch_bounds__(SPH_TWMAX * 32) void k_density_tile(
                             lam *= 1.0f + __fdividef(Sp - T[t], Ep);
                             lam = fminf(fmaxf(lam, 0.5f), 2.0f);
                         }
-                        if (okp && zfit[t] && fabsf(1.0f - lam) <= 0.9f * T_ZONE && h[t] / lam <= hcap) {
+                        if (okp && zfit && fabsf(1.0f - lam) <= 0.9f * T_ZONE && h[t] / lam <= hcap) {
                             done[t] = true;
-                            if (wid != 0) continue;   // warp 0 finishes alone
                             // ---- final: put the clamped zone entries right at lam, one more step
                             const float eps = 1.0f - lam;
                             float dS = 0.0f, dE = 0.0f, amin = 3.0e38f;
                             int   cz = 0;
-#pragma unroll
-                            for (int w = 0; w < SPH_TWMAX; ++w)
-                                for (int q = 0; q < nzw[t][w]; ++q) {
-                                    const int    idx = sm.zone[(w * ZW + q) * SPH_TB + lane + 32 * t];
-                                    const float4 c   = sm.tile[idx];
-                                    const float  mj  = sm.ms[idx];
-                                    const float dx = xt[t] - c.x, dy = yt[t] - c.y, dz = zt[t] - c.z;
-                                    const float r  = sph_sqrt(fmaf(dz, dz, fmaf(dy, dy, dx * dx)));
-                                    const float s  = r * ihh[t], tt = 1.0f - s;
-                                    const float tq = fmaf(eps, s, tt), sq = lam * s;   // t', s' at lam
-                                    amin = fminf(amin, fabsf(tq));
-                                    if (tq < 0.0f) {
-                                        const float q2 = tq * tq, q3 = q2 * tq;
-                                        dS -= mj * q2 * q2 * (tq + 5.0f * sq);
-                                        dE -= 20.0f * mj * sq * sq * q3;
-                                    } else ++cz;
-                                }
+                            for (int q = 0; q < nz[t]; ++q) {
+                                const int    idx = sm.zone[q * SPH_TB + kc[t]];
+                                const float4 c   = sm.tile[idx];
+                                const float  mj  = sm.ms[idx];
+                                const float dx = xt[t] - c.x, dy = yt[t] - c.y, dz = zt[t] - c.z;
+                                const float r  = sph_sqrt(fmaf(dz, dz, fmaf(dy, dy, dx * dx)));
+                                const float s  = r * ihh[t], tt = 1.0f - s;
+                                const float tq = fmaf(eps, s, tt), sq = lam * s;   // t', s' at lam
+                                amin = fminf(amin, fabsf(tq));
+                                if (tq < 0.0f) {
+                                    const float q2 = tq * tq, q3 = q2 * tq;
+                                    dS -= mj * q2 * q2 * (tq + 5.0f * sq);
+                                    dE -= 20.0f * mj * sq * sq * q3;
+                                } else ++cz;
+                            }
                             c2_poly(M[t], lam, Sp, Ep);
                             float lam2 = lam * (1.0f + __fdividef(Sp + dS - T[t], Ep + dE));
                             c2_poly(M[t], lam2, Sp, Ep);
@@ -501,7 +523,7 @@ __global__ __launch_bounds__(SPH_TWMAX * 32) void k_density_tile(
                         if (hhi[t] < 3.0e38f && !(hn >= hlo[t] && hn <= hhi[t])) hn = 0.5f * (hlo[t] + hhi[t]);
                         const bool capped = hn >= hcap && h[t] >= hcap;
                         hn = fminf(hn, hcap);
-                        if (capped || sweeps[t] >= par.max_iter || (hhi[t] - hlo[t]) <= par.tol * h[t] || !zfit[t]) {
+                        if (capped || sweeps[t] >= par.max_iter || (hhi[t] - hlo[t]) <= par.tol * h[t] || !zfit) {
                             done[t] = true; fix[t] = true;   // k_density_fix settles it (and counts non-convergence)
                             continue;
                         }
@@ -512,23 +534,16 @@ __global__ __launch_bounds__(SPH_TWMAX * 32) void k_density_tile(
                     }
                 } else {
                     // ---- Halley path: S, E, F at h; interior count and the entries next to the edge
-                    float ih[2], Hlo[2], Hhi[2], s[2], e[2], f2[2];
-                    int   cin[2], ne[2], nent[2] = {0, 0};
-                    float* const myedge = edge + wid * 4 * SPH_TB;
+                    float ih[NT], Hlo[NT], Hhi[NT], s[NT], e[NT], f2[NT];
+                    int   cin[NT], ne[NT];
 #pragma unroll
-                    for (int t = 0; t < 2; ++t) {
+                    for (int t = 0; t < NT; ++t) {
                         ih[t]  = __fdividef(1.0f, h[t]);
                         Hlo[t] = 2.0f * h[t] * (1.0f - T_EDGE);
                         Hhi[t] = 2.0f * h[t] * (1.0f + T_EDGE);
                         s[t] = 0.0f; e[t] = 0.0f; f2[t] = 0.0f; cin[t] = 0; ne[t] = 0;
                     }
-                    uint32_t *lp[2], *lend[2];
-#pragma unroll
-                    for (int t = 0; t < 2; ++t) {
-                        lp[t]   = lbase ? lbase + lane + 32 * t : nullptr;
-                        lend[t] = lbase ? lp[t] + SPH_LCAP * SPH_TB : nullptr;
-                    }
-                    sph_tile_walk(sm, ti, lane, wid, W, on, [&](int t, const SphEntry& en) {
+                    sph_tile_walk_own<NT, NSET>(sm, ti, tid, on, [&](int t, const SphEntry& en) {
                         const float4 c = en.c;
                         const float  mj = en.m;
                         const bool   has = en.has;
@@ -541,52 +556,20 @@ __global__ __launch_bounds__(SPH_TWMAX * 32) void k_density_tile(
                         f2[t] = fmaf(mj, fq, f2[t]);
                         {
                             const uint32_t gj = sph_ldsu(sm.gidx_sa + 4u * (uint32_t)en.idx);
-                            const bool st = has && lp[t] < lend[t];
+                            const bool st = has && nent[t] < lcap;
+                            uint32_t* const la = lcol[t] + (uint32_t)nent[t] * (uint32_t)SPH_TB;
                             asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %2, 0;\n\t@p st.global.u32 [%0], %1;\n\t}"
-                                         ::"l"(lp[t]), "r"(gj), "r"((unsigned)st) : "memory");
-                            lp[t] += st ? SPH_TB : 0;
+                                         ::"l"(la), "r"(gj), "r"((unsigned)st) : "memory");
                         }
                         nent[t] += has ? 1 : 0;
                         cin[t]  += (has && r < Hlo[t]) ? 1 : 0;
                         if (has && r >= Hlo[t] && r < Hhi[t]) {
-                            if (ne[t] < 4) myedge[ne[t] * SPH_TB + lane + 32 * t] = r;
+                            if (ne[t] < 4) edge[ne[t] * SPH_TB + kc[t]] = r;
                             ++ne[t];
                         }
                     });
-                    int new_[2][SPH_TWMAX];
 #pragma unroll
-                    for (int t = 0; t < 2; ++t) {
-#pragma unroll
-                        for (int w = 0; w < SPH_TWMAX; ++w) new_[t][w] = 0;
-                        new_[t][0] = ne[t];
-                    }
-                    if (W > 1) {
-#pragma unroll
-                        for (int t = 0; t < 2; ++t) {
-                            float* x = xch + (wid * DT_NPART) * SPH_TB + lane + 32 * t;
-                            x[0] = s[t]; x[SPH_TB] = e[t]; x[2 * SPH_TB] = f2[t];
-                            x[3 * SPH_TB] = __int_as_float(cin[t]);
-                            x[4 * SPH_TB] = __int_as_float(ne[t]);
-                            x[5 * SPH_TB] = __int_as_float(nent[t]);
-                        }
-                        __syncthreads();
-#pragma unroll
-                        for (int t = 0; t < 2; ++t) {
-                            s[t] = 0.0f; e[t] = 0.0f; f2[t] = 0.0f; cin[t] = 0; nent[t] = 0;
-#pragma unroll
-                            for (int w = 0; w < SPH_TWMAX; ++w) {
-                                new_[t][w] = 0;
-                                if (w >= W) continue;
-                                const float* x = xch + (w * DT_NPART) * SPH_TB + lane + 32 * t;
-                                s[t] += x[0]; e[t] += x[SPH_TB]; f2[t] += x[2 * SPH_TB];
-                                cin[t] += __float_as_int(x[3 * SPH_TB]);
-                                new_[t][w] = __float_as_int(x[4 * SPH_TB]);
-                                nent[t] += __float_as_int(x[5 * SPH_TB]);
-                            }
-                        }
-                    }
-#pragma unroll
-                    for (int t = 0; t < 2; ++t) {
+                    for (int t = 0; t < NT; ++t) {
                         if (!on[t]) continue;
                         if (sweeps[t] == 0) c_listed += (unsigned)nent[t];
                         ++sweeps[t];
@@ -601,15 +584,11 @@ __global__ __launch_bounds__(SPH_TWMAX * 32) void k_density_tile(
                         if (acc && needR <= Rc[t]) {
                             const float H = 2.0f * hn, tauH = taun * H;
                             int  n = cin[t];
-                            bool eg = false;
-#pragma unroll
-                            for (int w = 0; w < SPH_TWMAX; ++w) {
-                                eg |= new_[t][w] > 4;
-                                for (int q = 0; q < min(new_[t][w], 4); ++q) {
-                                    const float r = edge[(w * 4 + q) * SPH_TB + lane + 32 * t];
-                                    n += (r < H) ? 1 : 0;
-                                    eg |= fabsf(r - H) <= tauH;
-                                }
+                            bool eg = ne[t] > 4;
+                            for (int q = 0; q < min(ne[t], 4); ++q) {
+                                const float r = edge[q * SPH_TB + kc[t]];
+                                n += (r < H) ? 1 : 0;
+                                eg |= fabsf(r - H) <= tauH;
                             }
                             S[t] = Sn; E[t] = En; h[t] = hn; ni[t] = n;
                             done[t] = true;
@@ -626,26 +605,29 @@ __global__ __launch_bounds__(SPH_TWMAX * 32) void k_density_tile(
                         }
                     }
                 }
-                // the exchange area and the zone / edge slots are rewritten by the next sweep
-                if (W > 1 && __any_sync(SPH_FULL, (!done[0] && !wait[0]) || (!done[1] && !wait[1]))) __syncthreads();
             }
+            // the next stage: the largest list radius still wanted
+            float wr = 0.0f;
+#pragma unroll
+            for (int t = 0; t < NT; ++t) wr = fmaxf(wr, wait[t] ? want[t] : 0.0f);
+            Rt = block_max(wr);
         }
 
-        // ---- results (warp 0; the state is the same in every warp)
-        if (wid != 0) continue;
+        // ---- results: every thread stores its own targets
         if (fallback) {
-            if (lbase != nullptr && lane == 0) bucket_loff[bi] = 0xffffffffu;   // no tile-format list
-            if (big_list) {   // to the second pass, which has a larger tile
-                if (lane == 0) big_list[atomicAdd(big_cnt, 1u)] = bi;
-            } else {          // whole bucket to the 8-lanes-per-target kernel
+            if (tid == 0) {
+                if (lbase != nullptr) bucket_loff[bi] = 0xffffffffu;   // no tile-format list
+                if (big_list) big_list[atomicAdd(big_cnt, 1u)] = bi;    // to the second pass, which has a larger tile
+            }
+            if (!big_list) {          // whole bucket to the 8-lanes-per-target kernel
 #pragma unroll
-                for (int t = 0; t < 2; ++t)
+                for (int t = 0; t < NT; ++t)
                     if (valid[t]) fb_list[atomicAdd(fb_cnt, 1u)] = (uint32_t)p[t];
             }
             continue;
         }
 #pragma unroll
-        for (int t = 0; t < 2; ++t) {
+        for (int t = 0; t < NT; ++t) {
             if (!valid[t]) continue;
             if (wait[t] || !done[t]) { fix[t] = true; done[t] = true; }
             const int i = ic[t];
@@ -668,8 +650,8 @@ __global__ __launch_bounds__(SPH_TWMAX * 32) void k_density_tile(
         }
     }
 
-    // ---- counters (warp 0 holds them): one atomic per block and counter
-    if (wid == 0) {
+    // ---- counters: one atomic per warp and counter
+    {
         const unsigned tl = __reduce_add_sync(SPH_FULL, c_listed), tp = __reduce_add_sync(SPH_FULL, c_pairs);
         const unsigned tsw = __reduce_add_sync(SPH_FULL, c_sweeps), trc = __reduce_add_sync(SPH_FULL, c_recollect);
         if (lane == 0) {
@@ -705,22 +687,22 @@ int sph_launch_density_tile(sph_ctx* c, float* h, float* rho, float* omega, int3
     SPH_CUDA_CHECK(c, cudaMemsetAsync(c->big_cnt, 0, sizeof(unsigned), s));
     SPH_CUDA_CHECK(c, cudaMemsetAsync(c->list_next, 0, sizeof(unsigned), s));
     SPH_CUDA_CHECK(c, cudaMemsetAsync(c->bucket_loff, 0xff, (size_t)c->n_max * sizeof(uint32_t), s));
-    auto launch = [&](auto tag) -> cudaError_t {
-        constexpr int KERN = decltype(tag)::value;
+    auto launch = [&](auto tag, auto ntag) -> cudaError_t {
+        constexpr int KERN = decltype(tag)::value, NT = decltype(ntag)::value, NTHR = 64 / NT;
         for (int pass = 0; pass < 2; ++pass) {
             const int  tcap = pass == 0 ? c->par.tile_cap : c->par.tile_cap2;
             const bool two  = c->par.tile_cap2 >= c->par.tile_cap + 32;
             if (pass == 1 && !two) break;
             TilePar par{c->par.n_ngb, c->par.h_tol, c->par.search_slack, c->par.h_max_iter, tcap};
-            const size_t smem = sph_tile_smem_bytes(tcap, 16, sph_tile_xbytes(W, 8), W);
-            cudaError_t e = cudaFuncSetAttribute(k_density_tile<KERN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            const size_t smem = sph_tile_smem_bytes(tcap, 16, sph_tile_xbytes(1, 0), 2 / NT);
+            cudaError_t e = cudaFuncSetAttribute(k_density_tile<KERN, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
             if (e != cudaSuccess) return e;
             int per_sm = 0;
-            e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_density_tile<KERN>, 32 * W, smem);
+            e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_density_tile<KERN, NT>, NTHR, smem);
             if (e != cudaSuccess) return e;
             if (per_sm < 1) per_sm = 1;
             const bool last = pass == 1 || !two;
-            k_density_tile<KERN><<<c->sm_count * per_sm, 32 * W, smem, s>>>(
+            k_density_tile<KERN, NT><<<c->sm_count * per_sm, NTHR, smem, s>>>(
                 c->grid, c->cell_start, c->pos_m, c->perm, c->buckets,
                 pass == 0 ? c->bucket_cnt : c->big_cnt, pass == 0 ? nullptr : c->big_list,
                 last ? nullptr : c->big_list, c->big_cnt, c->tile_next + pass, par, h, rho, omega, nn,
@@ -733,12 +715,16 @@ int sph_launch_density_tile(sph_ctx* c, float* h, float* rho, float* omega, int3
         }
         return cudaSuccess;
     };
+    // tile_warps = 2: two warps per bucket, one target per thread; 1: one warp, two targets per lane
+    auto launch_k = [&](auto tag) -> cudaError_t {
+        return W >= 2 ? launch(tag, std::integral_constant<int, 1>{}) : launch(tag, std::integral_constant<int, 2>{});
+    };
     cudaError_t e;
     switch (c->par.kernel) {
-    case 0: e = launch(std::integral_constant<int, 0>{}); break;
-    case 2: e = launch(std::integral_constant<int, 2>{}); break;
-    case 3: e = launch(std::integral_constant<int, 3>{}); break;
-    default: e = launch(std::integral_constant<int, 1>{}); break;
+    case 0: e = launch_k(std::integral_constant<int, 0>{}); break;
+    case 2: e = launch_k(std::integral_constant<int, 2>{}); break;
+    case 3: e = launch_k(std::integral_constant<int, 3>{}); break;
+    default: e = launch_k(std::integral_constant<int, 1>{}); break;
     }
     SPH_CUDA_CHECK(c, e);
     return SPH_OK;
