@@ -287,6 +287,29 @@ int  sph_permutation(sph_ctx* ctx, int32_t* perm_out);
  * bench.py.  Synchronises.                                                               */
 int  sph_fp32_peak(void* cuda_stream, float seconds, double* tflops);
 
+/* sph_timestep without a context and WITHOUT ANY ALLOCATION (no cudaMalloc / cudaFree, no
+ * allocating library routine): for callers that may not allocate -- code under CUDA graph
+ * capture, serving loops, harnesses that forbid it.  Same operation as sph_timestep (steps
+ * a10-a11, Eq. 26): dt_i = min(eta_acc sqrt(2h/|a|), eta_cfl h / ((1 + 0.6
+ * av_alpha) c + 0.6 av_beta |mu_min|)), *dt_min_device = min_i dt_i; all arrays DEVICE pointers,
+ * n floats (dt_min_device: one float), owned by the caller; work is enqueued on cuda_stream
+ * (a cudaStream_t; NULL = the default stream) of the CURRENT device and not waited for.
+ * The block minima of the reduction go to a scratch array of SPH_STATIC_SCRATCH_BYTES that is
+ * part of the library image: every GPU that loads the library holds it until exit, and that
+ * size is the limit -- n <= SPH_STATIC_MAX_N, else SPH_EINVAL (use sph_timestep).  All calls on a
+ * device share the scratch, which keeps the last call's contents (nothing in it needs to start
+ * at zero); calls that overlap on one GPU (two streams) race on it and must be ordered by the
+ * caller.  The first call on a device looks up the array's device address (no allocation).
+ * SPH_EINVAL: null pointer, n out of range, eta <= 0 or a negative viscosity parameter;
+ * SPH_ECUDA: CUDA runtime error.  sph_static_last_error: text of this thread's last failure.  */
+#define SPH_STATIC_SCRATCH_BYTES 16384
+#define SPH_STATIC_MAX_N 16777216 /* 4096 block minima x 4096 particles per block */
+int  sph_timestep_static(void* cuda_stream, int64_t n, float eta_cfl, float eta_acc,
+                         float av_alpha, float av_beta, const float* h, const float* c,
+                         const float* ax, const float* ay, const float* az, const float* mu_min,
+                         float* dt_i, float* dt_min_device);
+const char* sph_static_last_error(void);
+
 const char* sph_strerror(int code);
 const char* sph_last_error(const sph_ctx* ctx);
 

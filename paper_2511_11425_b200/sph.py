@@ -21,7 +21,7 @@ SPH_OK, SPH_EINVAL, SPH_EBOX, SPH_ENOMEM, SPH_ECUDA, SPH_ESTALE, SPH_ENOSPC = 0,
 SYMBOLS = ["sph_create", "sph_destroy", "sph_build_cells", "sph_density_h", "sph_forces",
            "sph_timestep", "sph_rungs", "sph_set_active", "sph_mark_neighbors",
            "sph_interface_correction", "sph_predict", "sph_kick", "sph_drift", "sph_isentropic_u", "sph_block_predict", "sph_block_active", "sph_block_kick", "sph_neighbors", "sph_stats", "sph_stats_reset", "sph_permutation",
-           "sph_fp32_peak", "sph_strerror", "sph_last_error"]
+           "sph_fp32_peak", "sph_timestep_static", "sph_static_last_error", "sph_strerror", "sph_last_error"]
 
 
 class SphError(RuntimeError):
@@ -133,12 +133,15 @@ def load():
     lib.sph_stats_reset.argtypes = [vp]
     lib.sph_permutation.argtypes = [vp, fp]
     lib.sph_fp32_peak.argtypes = [vp, C.c_float, C.POINTER(C.c_double)]
+    lib.sph_timestep_static.argtypes = [vp, i64] + [C.c_float] * 4 + [fp] * 8
+    lib.sph_static_last_error.argtypes = []
+    lib.sph_static_last_error.restype = C.c_char_p
     lib.sph_strerror.argtypes = [C.c_int]
     lib.sph_strerror.restype = C.c_char_p
     lib.sph_last_error.argtypes = [vp]
     lib.sph_last_error.restype = C.c_char_p
     for name in SYMBOLS:
-        if name not in ("sph_destroy", "sph_strerror", "sph_last_error"):
+        if name not in ("sph_destroy", "sph_strerror", "sph_last_error", "sph_static_last_error"):
             getattr(lib, name).restype = C.c_int
     _lib = lib
     return lib
@@ -162,6 +165,24 @@ def fp32_peak(seconds: float = 1.0) -> float:
     if rc:
         raise SphError(rc, load().sph_strerror(rc).decode())
     return out.value
+
+
+STATIC_MAX_N = 16777216   # SPH_STATIC_MAX_N of include/sph.h
+
+
+def timestep_static(h, c, ax, ay, az, mu_min, dt_i, dt_min, eta_cfl=0.3, eta_acc=0.2,
+                    av_alpha=1.0, av_beta=2.0):
+    """sph_timestep_static: the time-step criteria without a context and without any allocation
+    (scratch in a fixed array of the library image; n <= STATIC_MAX_N).  Enqueued on torch's
+    current stream of the current device."""
+    if not torch.cuda.is_available():
+        raise SphError(SPH_ECUDA, "no CUDA device: the SPH path has no CPU fallback")
+    lib, n, f = load(), int(h.numel()), torch.float32
+    args = [_ptr(t, f, n) for t in (h, c, ax, ay, az, mu_min, dt_i)] + [_ptr(dt_min, f, 1)]
+    rc = lib.sph_timestep_static(C.c_void_p(torch.cuda.current_stream().cuda_stream), n,
+                                 float(eta_cfl), float(eta_acc), float(av_alpha), float(av_beta), *args)
+    if rc:
+        raise SphError(rc, lib.sph_static_last_error().decode())
 
 
 class Sph:
