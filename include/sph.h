@@ -21,7 +21,9 @@
  *     coordinate outside is binned into the edge cell and its neighbours across the face
  *     are missed.  On an open axis any coordinate is fine (edge cells extend to infinity).
  *   - Device memory of a context: about 1 KB per particle of n_max (768 B of it the neighbour
- *     lists kept between sph_density_h and sph_forces) plus 4 B per cell of the index.
+ *     lists kept between sph_density_h and sph_forces; for n_ngb > 64 that part grows to about
+ *     8 n_ngb s^3 bytes, s = search_slack: 4.4 KB per particle at Wendland C6 / 400) plus 4 B per
+ *     cell of the index.
  *   - Call order: sph_build_cells -> sph_density_h -> sph_forces -> sph_timestep.
  *     sph_forces / sph_neighbors may be fed rho, h, Omega from elsewhere as long as
  *     sph_build_cells ran on the same positions (else SPH_ESTALE).
@@ -84,12 +86,12 @@ typedef struct {
                           /* -1 = off: every target takes the 8-lanes-per-target kernels.     */
                           /* Results do not depend on it beyond rounding                      */
     int32_t tile_rows;    /* a bucket spans tile_rows x tile_rows rows of cells (<= 0:        */
-                          /* default 3; at most 5)                                           */
-    int32_t tile_cap;     /* candidates a tile holds (<= 0: default 768); buckets that need   */
-                          /* more go to the second pass                                      */
-    int32_t tile_cap2;    /* tile of the second pass (<= 0: default 2560; below tile_cap + 32: */
-                          /* no second pass); buckets it cannot hold either fall back to the  */
-                          /* 8-lane kernels                                                   */
+                          /* default 3, or 2 for n_ngb > 100; at most 5)                      */
+    int32_t tile_cap;     /* candidates a tile holds (<= 0: default 12 n_ngb, between 768 and */
+                          /* 3072); buckets that need more go to the second pass              */
+    int32_t tile_cap2;    /* tile of the second pass (<= 0: default 2560 for n_ngb <= 64,     */
+                          /* else 4064, the largest; below tile_cap + 32: no second pass);    */
+                          /* buckets it cannot hold either fall back to the 8-lane kernels    */
     int32_t tile_warps;   /* warps per bucket of the density sweep: 2 (default, <= 0) = one   */
                           /* target per thread; 1 = one warp, two targets per lane            */
     int32_t tile_forces;  /* 0 (default): the force sweep reads the bucket-major neighbour    */

@@ -17,12 +17,13 @@ static void fill_defaults(sph_params& p) {
     if (!(p.search_slack > 1.0f)) p.search_slack = 1.1f;
     // cell_div_x / cell_div_yz <= 0 stay "automatic": sph_build_cells picks 8 x 2 for the staged-
     // tile sweeps and 4 x 1.5 for the 8-lane kernels (sph_tile_on, the grid's steep-h flag)
-    if (p.tile_rows <= 0) p.tile_rows = 3;
+    if (p.tile_rows <= 0) p.tile_rows = p.n_ngb > 100.0f ? 2 : 3;
     if (p.tile_rows > 5) p.tile_rows = 5;
-    if (p.tile_cap <= 0) p.tile_cap = 768;
+    // tile capacities follow the neighbour number: ~12 x n_ngb candidates reach a bucket of 64 targets
+    if (p.tile_cap <= 0) p.tile_cap = (int)fminf(fmaxf(12.0f * p.n_ngb, 768.0f), 3072.0f);
     p.tile_cap = (p.tile_cap + 31) & ~31;
     if (p.tile_cap > 4096) p.tile_cap = 4096;
-    if (p.tile_cap2 <= 0) p.tile_cap2 = 2560;
+    if (p.tile_cap2 <= 0) p.tile_cap2 = p.n_ngb > 64.0f ? 4064 : 2560;
     p.tile_cap2 = (p.tile_cap2 + 31) & ~31;
     if (p.tile_cap2 > 4064) p.tile_cap2 = 4064;
     if (p.tile_warps <= 0) p.tile_warps = 2;
@@ -84,7 +85,20 @@ extern "C" int sph_create(sph_ctx** out, const sph_params* params, const sph_box
     ok = ok && dalloc(&c->rcak, (size_t)n_max + SPH_POS_PAD) == cudaSuccess;
     ok = ok && dalloc(&c->stats, (size_t)ST_NCOUNTERS) == cudaSuccess;
     ok = ok && dalloc(&c->coarse_hmax, (size_t)2 * SPH_COARSE_MAX) == cudaSuccess;
-    ok = ok && dalloc(&c->nb_j, (size_t)n_max * SPH_SLOTS * SPH_G) == cudaSuccess;
+    // bucket-major lists of the tile sweep: lcap entries per target hold the list ball (2h x 1.03 for
+    // the moment solve of Wendland C2, 2h x search_slack for the Halley sweeps) with a margin of 30 %;
+    // the pool holds a region of lcap x 64 words for every bucket at an average fill of 43 targets,
+    // and never less than the [target][192] lists of the 8-lane kernels need
+    {
+        const float sl = c->par.kernel == 1 ? 1.031f : c->par.search_slack;
+        int lc = (int)(c->par.n_ngb * sl * sl * sl * 1.3f) + 32;
+        lc = (lc + 31) & ~31;
+        c->lcap = lc < SPH_LCAP_MIN ? SPH_LCAP_MIN : lc;
+        size_t per = (size_t)c->lcap * 3 / 2;
+        if (per < (size_t)SPH_SLOTS * SPH_G) per = (size_t)SPH_SLOTS * SPH_G;
+        c->nb_words = (size_t)n_max * per;
+    }
+    ok = ok && dalloc(&c->nb_j, c->nb_words) == cudaSuccess;
     ok = ok && dalloc(&c->nb_cnt, (size_t)n_max) == cudaSuccess;
     ok = ok && dalloc(&c->nb_rkeep, (size_t)n_max) == cudaSuccess;
     ok = ok && dalloc(&c->fix_list, (size_t)n_max) == cudaSuccess;

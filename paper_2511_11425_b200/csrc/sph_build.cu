@@ -269,7 +269,9 @@ int sph_launch_build(sph_ctx* c, int64_t n, const float* x, const float* y, cons
     const bool  tl = sph_tile_on(c);
     const float ux = c->par.cell_div_x, uyz = c->par.cell_div_yz;   // > 0: the caller's choice
     k_grid_setup<<<1, 1, 0, s>>>(c->grid, c->red, c->box, c->par.search_slack,
-                                 ux > 0.0f ? ux : (tl ? 8.0f : 4.0f), uyz > 0.0f ? uyz : (tl ? 2.0f : 1.5f),
+                                 ux > 0.0f ? ux : (tl ? 8.0f : 4.0f),
+                                 // several hundred neighbours: finer rows keep a bucket of 64 compact
+                                 uyz > 0.0f ? uyz : (tl ? (c->par.n_ngb > 100.0f ? 3.0f : 2.0f) : 1.5f),
                                  ux > 0.0f ? ux : 4.0f, uyz > 0.0f ? uyz : 1.5f,
                                  (tl && c->par.tile == 0) ? 1 : 0, (long long)c->cap_cells);
     k_zero_cells<<<gs, TPB, 0, s>>>(c->grid, c->cell_cnt);

@@ -105,7 +105,7 @@ __global__ __launch_bounds__(FL_WARPS * 32, FL_MINB) void k_forces_list(
     const SphBucket* __restrict__ buckets, const unsigned* __restrict__ nbuckets, ForcePar par,
     const unsigned* __restrict__ coarse, const uint32_t* __restrict__ nb_j,
     const uint32_t* __restrict__ bucket_loff, const uint32_t* __restrict__ nb_cnt,
-    const float* __restrict__ tl_rkeep, int nall, unsigned* next, float* ax, float* ay, float* az, float* dudt,
+    const float* __restrict__ tl_rkeep, int lcap, unsigned* next, float* ax, float* ay, float* az, float* dudt,
     float* mu_min, uint32_t* fb_list, unsigned* fb_cnt, unsigned long long* stats) {
     __shared__ SphGrid g;
     __shared__ int     rowoff_s[FL_WARPS][32];
@@ -193,7 +193,7 @@ __global__ __launch_bounds__(FL_WARPS * 32, FL_MINB) void k_forces_list(
 
     // ---- which targets the kept lists serve
     const uint32_t reg = bucket_loff[bi];
-    const uint32_t* const lb = nb_j + (size_t)(reg == 0xffffffffu ? 0u : reg) * (SPH_LCAP * SPH_TB);
+    const uint32_t* const lb = nb_j + (size_t)(reg == 0xffffffffu ? 0u : reg) * ((size_t)lcap * SPH_TB);
     bool cov[2];
     int  cnt[2];
 #pragma unroll
@@ -306,7 +306,7 @@ int sph_launch_forces_list(sph_ctx* c, float* ax, float* ay, float* az, float* d
         if (per_sm < 1) per_sm = 1;
         k_forces_list<KERN, ENT><<<c->sm_count * per_sm, FL_WARPS * 32, 0, s>>>(
             c->grid, c->cell_start, c->pos_h, c->vel_m, c->rcak, c->perm, c->buckets, c->bucket_cnt, par,
-            c->coarse_hmax, c->nb_j, c->bucket_loff, c->nb_cnt, c->tl_rkeep, (int)c->n, c->tile_next + 2, ax, ay, az,
+            c->coarse_hmax, c->nb_j, c->bucket_loff, c->nb_cnt, c->tl_rkeep, c->lcap, c->tile_next + 2, ax, ay, az,
             dudt, mu_min, c->fb_list, c->fb_cnt + 1, c->stats);
     };
     auto launch = [&](auto tag) {

@@ -35,7 +35,7 @@ struct SphGrid {
 #define SPH_POS_PAD 64             // records of padding behind the sorted float4 arrays
 #define SPH_G 8                    // lanes per target in the sweeps
 #define SPH_SLOTS 24               // list entries per lane (24 x 8 = 192 per target)
-#define SPH_LCAP 128               // entries per target of a bucket-major list region (staged-tile path)
+#define SPH_LCAP_MIN 128           // entries per target of a bucket-major list region: at least this (sph_ctx.lcap)
 
 enum {  // indices into the device counter block (uint64 each), mirrors sph_stats_t
     ST_DENS_TESTED = 0, ST_DENS_LISTED, ST_DENS_PAIRS, ST_DENS_SWEEPS, ST_DENS_RECOLLECT,
@@ -84,6 +84,8 @@ struct sph_ctx {
     unsigned*    big_list;     // n_max: buckets the first pass of a tile sweep left to the second (larger tile)
     unsigned*    big_cnt;      // [2]: their number (density, forces)
     unsigned*    list_next;    // [1]: next free region of nb_j (bucket-major lists of the tile sweep)
+    int          lcap;         // entries per target of a bucket-major list region (from n_ngb, sph_create)
+    size_t       nb_words;     // words in nb_j
     uint32_t*    bucket_loff;  // n_max: list region of a bucket (0xffffffff: none)
     float*       tl_rkeep;     // n_max: radius inside which a target's bucket-major list is complete (0: none);
                                // nb_rkeep stays the radius of the 8-lane kernels' [target][entry] lists

@@ -77,7 +77,7 @@ __global__ void k_buckets(const SphGrid* __restrict__ gp, const uint32_t* __rest
 
 struct TilePar {
     float n_ngb, tol, slack;
-    int   max_iter, tcap;
+    int   max_iter, tcap, lcap;
 };
 
 // One safeguarded Halley step from the sums at h (the step of sph_density.cu: same formulas,
@@ -194,7 +194,8 @@ __global__ __launch_bounds__(64 / NT, NT == 1 ? 7 : 8) void k_density_tile(
     const SphTileMem sm = sph_tile_carve<16>(smem_raw, par.tcap, sph_tile_xbytes(1, 0), NW);
     // the targets' mask parameters (sph_tgt_put): the segment table's memory, dead once the tile is in place
     float* const  tgt  = (float*)sm.seg;
-    float* const  edge = (float*)sm.zone;   // Halley path: [4][64] floats in the zone area
+    float* const  edge = (float*)sm.zone;   // Halley path: [DT_NEDGE][64] floats, the whole zone area
+    constexpr int DT_NEDGE = SPH_TZCAP / 2;
     if (tid == 0) sph_mbar_init(sm.bar, 1u);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     __syncthreads();
@@ -245,13 +246,16 @@ __global__ __launch_bounds__(64 / NT, NT == 1 ? 7 : 8) void k_density_tile(
         // interaction list"): entry f of target t of this bucket at lbase[f * 64 + t], the
         // sorted position of the source -- written from the sweep as the entries are met, so a
         // warp's stores fall into a few 256-byte rows.  The bucket takes one region of
-        // SPH_LCAP x 64 words from the pool (none left: no lists, the force sweep searches).
+        // lcap x 64 words from the pool (none left: no lists, the force sweep searches).
         if (tid == 0) {
             unsigned reg = 0xffffffffu;
             if (nb_j != nullptr) {
-                reg = atomicAdd(list_next, 1u);
-                if (reg >= nb_regions) reg = 0xffffffffu;
-                bucket_loff[bi] = reg;
+                if (blist) reg = bucket_loff[bi];   // second pass: the region the first pass took
+                if (reg == 0xffffffffu) {
+                    reg = atomicAdd(list_next, 1u);
+                    if (reg >= nb_regions) reg = 0xffffffffu;
+                    bucket_loff[bi] = reg;
+                }
             }
             lreg_s = reg;   // read behind the barriers of the first stage
         }
@@ -359,7 +363,7 @@ __global__ __launch_bounds__(64 / NT, NT == 1 ? 7 : 8) void k_density_tile(
                 if (lane == 0) ti = tl;
             }
             __syncthreads();
-            if (stage == 0 && lreg_s != 0xffffffffu) lbase = nb_j + (size_t)lreg_s * (SPH_LCAP * SPH_TB);
+            if (stage == 0 && lreg_s != 0xffffffffu) lbase = nb_j + (size_t)lreg_s * ((size_t)par.lcap * SPH_TB);
             if (!ti.ok) {
                 if (stage == 0) fallback = true;
                 else {
@@ -417,7 +421,7 @@ __global__ __launch_bounds__(64 / NT, NT == 1 ? 7 : 8) void k_density_tile(
                 uint32_t* lcol[NT];   // the target's column of the bucket's list region
 #pragma unroll
                 for (int t = 0; t < NT; ++t) lcol[t] = lbase + kc[t];
-                const int lcap = lbase ? SPH_LCAP : 0;
+                const int lcap = lbase ? par.lcap : 0;
                 int nent[NT];
 #pragma unroll
                 for (int t = 0; t < NT; ++t) nent[t] = 0;
@@ -564,7 +568,7 @@ __global__ __launch_bounds__(64 / NT, NT == 1 ? 7 : 8) void k_density_tile(
                         nent[t] += has ? 1 : 0;
                         cin[t]  += (has && r < Hlo[t]) ? 1 : 0;
                         if (has && r >= Hlo[t] && r < Hhi[t]) {
-                            if (ne[t] < 4) edge[ne[t] * SPH_TB + kc[t]] = r;
+                            if (ne[t] < DT_NEDGE) edge[ne[t] * SPH_TB + kc[t]] = r;
                             ++ne[t];
                         }
                     });
@@ -584,8 +588,8 @@ __global__ __launch_bounds__(64 / NT, NT == 1 ? 7 : 8) void k_density_tile(
                         if (acc && needR <= Rc[t]) {
                             const float H = 2.0f * hn, tauH = taun * H;
                             int  n = cin[t];
-                            bool eg = ne[t] > 4;
-                            for (int q = 0; q < min(ne[t], 4); ++q) {
+                            bool eg = ne[t] > DT_NEDGE;
+                            for (int q = 0; q < min(ne[t], DT_NEDGE); ++q) {
                                 const float r = edge[q * SPH_TB + kc[t]];
                                 n += (r < H) ? 1 : 0;
                                 eg |= fabsf(r - H) <= tauH;
@@ -616,8 +620,10 @@ __global__ __launch_bounds__(64 / NT, NT == 1 ? 7 : 8) void k_density_tile(
         // ---- results: every thread stores its own targets
         if (fallback) {
             if (tid == 0) {
-                if (lbase != nullptr) bucket_loff[bi] = 0xffffffffu;   // no tile-format list
-                if (big_list) big_list[atomicAdd(big_cnt, 1u)] = bi;    // to the second pass, which has a larger tile
+                // to the second pass, which has a larger tile (the bucket keeps its list region);
+                // from the last pass to the 8-lane kernel: no tile-format list
+                if (big_list) big_list[atomicAdd(big_cnt, 1u)] = bi;
+                else if (lbase != nullptr) bucket_loff[bi] = 0xffffffffu;
             }
             if (!big_list) {          // whole bucket to the 8-lanes-per-target kernel
 #pragma unroll
@@ -633,7 +639,7 @@ __global__ __launch_bounds__(64 / NT, NT == 1 ? 7 : 8) void k_density_tile(
             const int i = ic[t];
             h_io[i] = h[t];
             // the list is complete inside the radius of its mask (less the rounding margin of phase 1)
-            const bool lok = lbase != nullptr && !fix[t] && mvalid[t] && nlist[t] <= SPH_LCAP;
+            const bool lok = lbase != nullptr && !fix[t] && mvalid[t] && nlist[t] <= par.lcap;
             nb_rkeep[p[t]] = 0.0f;     // no [target][entry] list of the 8-lane kernels for this target
             tl_rkeep[p[t]] = lok ? Rc[t] * (1.0f - 1e-4f) : 0.0f;
             nb_cnt[p[t]]   = lok ? (uint32_t)nlist[t] : 0u;
@@ -693,7 +699,7 @@ int sph_launch_density_tile(sph_ctx* c, float* h, float* rho, float* omega, int3
             const int  tcap = pass == 0 ? c->par.tile_cap : c->par.tile_cap2;
             const bool two  = c->par.tile_cap2 >= c->par.tile_cap + 32;
             if (pass == 1 && !two) break;
-            TilePar par{c->par.n_ngb, c->par.h_tol, c->par.search_slack, c->par.h_max_iter, tcap};
+            TilePar par{c->par.n_ngb, c->par.h_tol, c->par.search_slack, c->par.h_max_iter, tcap, c->lcap};
             const size_t smem = sph_tile_smem_bytes(tcap, 16, sph_tile_xbytes(1, 0), 2 / NT);
             cudaError_t e = cudaFuncSetAttribute(k_density_tile<KERN, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
             if (e != cudaSuccess) return e;
@@ -708,7 +714,7 @@ int sph_launch_density_tile(sph_ctx* c, float* h, float* rho, float* omega, int3
                 last ? nullptr : c->big_list, c->big_cnt, c->tile_next + pass, par, h, rho, omega, nn,
                 c->fix_list, c->fix_cnt, c->fb_list, c->fb_cnt,
                 c->par.tile_forces ? nullptr : c->nb_j,
-                (unsigned)(((size_t)c->n_max * SPH_SLOTS * SPH_G) / (SPH_LCAP * SPH_TB)), c->list_next,
+                (unsigned)(c->nb_words / ((size_t)c->lcap * SPH_TB)), c->list_next,
                 c->bucket_loff, c->nb_cnt, c->nb_rkeep, c->tl_rkeep, c->stats);
             e = cudaGetLastError();
             if (e != cudaSuccess) return e;

@@ -473,22 +473,30 @@ def test_automatic_mode_picks_the_sweep_by_size_and_h_contrast(gu):
 # ------------------------------------------------------------------------------------------
 # The other kernels the paper offers: cubic spline, Wendland C4 and C6.
 # ------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("kernel,n_ngb", [(0, 32.0), (2, 64.0), (3, 64.0), (3, 200.0), (1, 100.0)])
-def test_c1_other_kernels_and_neighbour_numbers(gu, kernel, n_ngb):
+@pytest.mark.parametrize("kernel,n_ngb", [(0, 32.0), (2, 64.0), (3, 64.0), (3, 200.0), (1, 100.0), (3, 400.0)])
+@pytest.mark.parametrize("tile", [1, -1])
+def test_c1_other_kernels_and_neighbour_numbers(gu, kernel, n_ngb, tile):
     """Config 1 with the cubic spline / 32, Wendland C4 and C6, and neighbour
-    numbers beyond the 192-entry lists (those targets run through the list-free kernels):
-    every particle against the brute-force oracle."""
+    numbers up to the paper's C6 / 400, on the staged-tile path (bucket-major
+    lists sized from n_ngb) and on the 8-lane path (192-entry lists: beyond them the targets run
+    through the list-free kernels): every particle against the brute-force oracle."""
     w = workloads.uniform_cube(h_start="warm")
     scale = (n_ngb / 64.0) ** (1.0 / 3.0) * {0: 0.96, 1: 1.0, 2: 1.0, 3: 1.0}[kernel]
     w["h"] = (w["h"] * np.float32(scale)).astype(np.float32)
     _, op = gu.make_params(w, kernel=kernel, n_ngb=n_ngb)
     _, ob = gu.make_boxes(w)
-    ctx, d, out, h = _full_step(gu, w, kernel=kernel, n_ngb=n_ngb)
+    ctx, d, out, h = _full_step(gu, w, kernel=kernel, n_ngb=n_ngb, tile=tile)
     st = ctx.stats()
     assert st["dens_nonconv"] == 0, st
     _check_sample(gu, w, ctx, out, h, np.arange(w["n"]), op, ob)
-    if n_ngb >= 200.0:
+    print("stats", kernel, n_ngb, tile, {k: v for k, v in st.items() if v})
+    if tile == -1 and n_ngb >= 200.0:
         assert st["dens_overflow"] > 0      # the robust path was exercised
+    if tile == 1:
+        # the lists hold the whole slack ball and the force sweep is served from them: it
+        # distance-tests (searches) for a small share of the targets only
+        assert st["dens_listed"] >= st["dens_pairs"]
+        assert st["force_tested"] <= 0.25 * st["dens_tested"], st
 
 
 # ------------------------------------------------------------------------------------------
