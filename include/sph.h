@@ -75,7 +75,8 @@ typedef struct {
                           /* on it                                                         */
     float   cell_div_x;   /* cells per minimum search radius along x (<= 0: automatic: 8     */
                           /* when the staged-tile sweeps run, 4 otherwise)                   */
-    float   cell_div_yz;  /* ... along y and z (<= 0: automatic: 2 with tiles, else 1.5)     */
+    float   cell_div_yz;  /* ... along y and z (<= 0: automatic: 2 with tiles (3 for n_ngb >  */
+                          /* 100), else 1.5, or 1 where max h > 3 min h)                     */
     int32_t entropy;      /* 1: entropy-conserving variant: sph_forces drops */
                           /* the Eq. (14) term, dudt is the viscous heating of Eq. (18)     */
                           /* alone; the caller advances u with sph_isentropic_u             */

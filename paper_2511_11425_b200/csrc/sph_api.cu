@@ -16,7 +16,7 @@ static void fill_defaults(sph_params& p) {
     if (p.h_max_iter <= 0) p.h_max_iter = 40;
     if (!(p.search_slack > 1.0f)) p.search_slack = 1.1f;
     // cell_div_x / cell_div_yz <= 0 stay "automatic": sph_build_cells picks 8 x 2 for the staged-
-    // tile sweeps and 4 x 1.5 for the 8-lane kernels (sph_tile_on, the grid's steep-h flag)
+    // tile sweeps and 4 x 1.5 for the 8-lane kernels (4 x 1 under the grid's steep-h flag)
     if (p.tile_rows <= 0) p.tile_rows = p.n_ngb > 100.0f ? 2 : 3;
     if (p.tile_rows > 5) p.tile_rows = 5;
     // tile capacities follow the neighbour number: ~12 x n_ngb candidates reach a bucket of 64 targets

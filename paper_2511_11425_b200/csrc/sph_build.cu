@@ -272,7 +272,8 @@ int sph_launch_build(sph_ctx* c, int64_t n, const float* x, const float* y, cons
                                  ux > 0.0f ? ux : (tl ? 8.0f : 4.0f),
                                  // several hundred neighbours: finer rows keep a bucket of 64 compact
                                  uyz > 0.0f ? uyz : (tl ? (c->par.n_ngb > 100.0f ? 3.0f : 2.0f) : 1.5f),
-                                 ux > 0.0f ? ux : 4.0f, uyz > 0.0f ? uyz : 1.5f,
+                                 // steep h contrast: coarser rows (fewer near-empty rows around large-h targets)
+                                 ux > 0.0f ? ux : 4.0f, uyz > 0.0f ? uyz : 1.0f,
                                  (tl && c->par.tile == 0) ? 1 : 0, (long long)c->cap_cells);
     k_zero_cells<<<gs, TPB, 0, s>>>(c->grid, c->cell_cnt);
     k_bin<<<nb, TPB, 0, s>>>(n, c->grid, x, y, z, c->cell_cnt, c->key, c->rank);
