@@ -19,15 +19,25 @@ __global__ void k_reduce_h(int64_t n, const float* __restrict__ x, const float* 
                            const float* __restrict__ z, const float* __restrict__ h,
                            unsigned* red) {
     float hmin = __int_as_float(0x7f800000), hmax = 0.0f, xm = 0.0f;
-    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < n;
-         i += (int64_t)gridDim.x * blockDim.x) {
-        float hi = h[i];
-        if (hi > 0.0f && hi < 3.0e38f) {
-            hmin = fminf(hmin, hi);
-            hmax = fmaxf(hmax, hi);
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    // four particles per trip: sixteen independent loads in flight per thread
+    for (int64_t i0 = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i0 < n; i0 += 4 * stride) {
+        float hv[4], av[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const int64_t i = i0 + k * stride;
+            const bool in = i < n;
+            hv[k] = in ? h[i] : 0.0f;
+            av[k] = in ? fmaxf(fabsf(x[i]), fmaxf(fabsf(y[i]), fabsf(z[i]))) : 0.0f;
         }
-        float a = fmaxf(fabsf(x[i]), fmaxf(fabsf(y[i]), fabsf(z[i])));
-        if (a < 3.0e38f) xm = fmaxf(xm, a);
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            if (hv[k] > 0.0f && hv[k] < 3.0e38f) {
+                hmin = fminf(hmin, hv[k]);
+                hmax = fmaxf(hmax, hv[k]);
+            }
+            if (av[k] < 3.0e38f) xm = fmaxf(xm, av[k]);
+        }
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
@@ -35,7 +45,16 @@ __global__ void k_reduce_h(int64_t n, const float* __restrict__ x, const float* 
         hmax = fmaxf(hmax, __shfl_xor_sync(SPH_FULL, hmax, o));
         xm   = fmaxf(xm, __shfl_xor_sync(SPH_FULL, xm, o));
     }
-    if ((threadIdx.x & 31) == 0) {  // positive floats order like their bit patterns
+    // one set of atomics per block (they all hit the same three words)
+    __shared__ float sh[3][TPB / 32];
+    if ((threadIdx.x & 31) == 0) {
+        sh[0][threadIdx.x >> 5] = hmin; sh[1][threadIdx.x >> 5] = hmax; sh[2][threadIdx.x >> 5] = xm;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {  // positive floats order like their bit patterns
+        for (int w = 1; w < (int)(blockDim.x >> 5); ++w) {
+            hmin = fminf(hmin, sh[0][w]); hmax = fmaxf(hmax, sh[1][w]); xm = fmaxf(xm, sh[2][w]);
+        }
         atomicMin(red + 0, __float_as_uint(hmin));
         atomicMax(red + 1, __float_as_uint(hmax));
         atomicMax(red + 2, __float_as_uint(xm));

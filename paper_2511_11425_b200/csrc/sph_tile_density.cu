@@ -27,51 +27,90 @@ constexpr float T_EDGE   = 4.0e-4f;   // list entries within this of 2h are kept
 // ------------------------------------------------------------------------------------------
 // a3: the bucket table.  One warp per group of G x G adjacent rows of cells; it walks along x
 // and closes a bucket as soon as the next cell would take it past 64 particles (or 32 cells).
+// The group's cumulative counts along x are summed over the rows a chunk of cells at a time
+// (independent loads, all lanes busy) into shared memory; the cuts, which are sequential, then
+// run on shared memory alone.
 // ------------------------------------------------------------------------------------------
-__global__ void k_buckets(const SphGrid* __restrict__ gp, const uint32_t* __restrict__ cs, int G,
-                          SphBucket* out, unsigned* nout) {
+constexpr int BK_WARPS = 8;
+constexpr int BK_CHUNK = 2048;   // cells of a group held in shared memory at a time
+
+__global__ __launch_bounds__(BK_WARPS * 32) void k_buckets(const SphGrid* __restrict__ gp,
+                                                          const uint32_t* __restrict__ cs, int G,
+                                                          SphBucket* out, unsigned* nout) {
+    __shared__ uint32_t  cum[BK_CHUNK + 1];
+    __shared__ SphBucket stage[32];
+    __shared__ int       q_s;
     const SphGrid& g = *gp;
-    const int lane = threadIdx.x & 31;
-    const int nwarp = (int)((gridDim.x * blockDim.x) >> 5);
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int ngy = (g.ny + G - 1) / G, ngz = (g.nz + G - 1) / G;
-    for (int grp = (int)((blockIdx.x * blockDim.x + threadIdx.x) >> 5); grp < ngy * ngz; grp += nwarp) {
+    int nst = 0;   // warp 0: staged buckets (uniform); the table's counter is asked for 32 at a time
+    auto flush = [&]() {
+        __syncwarp();
+        unsigned at = 0;
+        if (lane == 0 && nst > 0) at = atomicAdd(nout, (unsigned)nst);
+        at = __shfl_sync(SPH_FULL, at, 0);
+        if (lane < nst) out[at + lane] = stage[lane];
+        __syncwarp();
+        nst = 0;
+    };
+    for (int grp = (int)blockIdx.x; grp < ngy * ngz; grp += (int)gridDim.x) {   // one block per group
         const int gy = grp % ngy, gz = grp / ngy;
         const int ry0 = gy * G, rz0 = gz * G;
         const int nry = min(G, g.ny - ry0), nrz = min(G, g.nz - rz0), nrows = nry * nrz;
         auto rowbase = [&](int rho) {
             return (uint32_t)((rz0 + rho / nry) * g.ny + (ry0 + rho % nry)) * (uint32_t)g.nx;
         };
-        uint32_t base = 0;
-        for (int rho = 0; rho < nrows; ++rho) base += __ldg(cs + rowbase(rho));
         int pos = 0;
         while (pos < g.nx) {
-            const int c = pos + 1 + lane;
-            uint32_t  cum = 0;
-            if (c <= g.nx)
-                for (int rho = 0; rho < nrows; ++rho) cum += __ldg(cs + rowbase(rho) + c);
-            const bool     ok  = c <= g.nx && cum - base <= (uint32_t)SPH_TB;
-            const unsigned bal = __ballot_sync(SPH_FULL, ok);
-            int m = (bal == SPH_FULL) ? 32 : __ffs((int)~bal) - 1;
-            if (m == 0) {   // the cells of this slab alone hold more than 64: one row, 64 at a time
-                if (lane < nrows) {
-                    const uint32_t rb = rowbase(lane);
-                    const int cnt = (int)(__ldg(cs + rb + pos + 1) - __ldg(cs + rb + pos));
-                    for (int skip = 0; skip < cnt; skip += SPH_TB) {
-                        SphBucket b{ry0 + lane % nry, rz0 + lane / nry, pos, pos + 1, 1, 1, skip, 0};
-                        out[atomicAdd(nout, 1u)] = b;
-                    }
+            // cum[k] = particles of the group's rows in the cells before pos + k (all threads)
+            const int len = min(BK_CHUNK, g.nx - pos);
+            __syncthreads();
+            for (int k = tid; k <= len; k += BK_WARPS * 32) {
+                uint32_t v = 0;
+                for (int r0 = 0; r0 < nrows; r0 += 5) {
+                    uint32_t t[5];
+#pragma unroll
+                    for (int u = 0; u < 5; ++u) t[u] = (r0 + u < nrows) ? __ldg(cs + rowbase(r0 + u) + pos + k) : 0u;
+                    v += (t[0] + t[1]) + (t[2] + t[3]) + t[4];
                 }
-                m = 1;
-            } else {
-                const uint32_t tot = __shfl_sync(SPH_FULL, cum, m - 1) - base;
-                if (lane == 0 && tot > 0u) {
-                    SphBucket b{ry0, rz0, pos, pos + m, nry, nrz, 0, 0};
-                    out[atomicAdd(nout, 1u)] = b;
-                }
+                cum[k] = v;
             }
-            base = __shfl_sync(SPH_FULL, cum, m - 1);
-            pos += m;
+            __syncthreads();
+            if (wid == 0) {   // the cuts are sequential: one warp, on shared memory alone
+                const bool tail = pos + len >= g.nx;   // the chunk ends where the rows end
+                int q = 0;
+                while (q < len && (q + 32 <= len || tail)) {
+                    const uint32_t base = cum[q];
+                    const int      c    = q + 1 + lane;
+                    const uint32_t cu   = c <= len ? cum[c] : 0u;
+                    const bool     ok   = c <= len && cu - base <= (uint32_t)SPH_TB;
+                    const unsigned bal  = __ballot_sync(SPH_FULL, ok);
+                    int m = (bal == SPH_FULL) ? 32 : __ffs((int)~bal) - 1;
+                    if (m == 0) {   // the cells of this slab alone hold more than 64: one row, 64 at a time
+                        if (lane < nrows) {
+                            const uint32_t rb = rowbase(lane);
+                            const int cnt = (int)(__ldg(cs + rb + pos + q + 1) - __ldg(cs + rb + pos + q));
+                            for (int skip = 0; skip < cnt; skip += SPH_TB) {
+                                SphBucket b{ry0 + lane % nry, rz0 + lane / nry, pos + q, pos + q + 1, 1, 1, skip, 0};
+                                out[atomicAdd(nout, 1u)] = b;
+                            }
+                        }
+                        m = 1;
+                    } else {
+                        const uint32_t tot = cum[q + m] - base;
+                        if (tot > 0u) {
+                            if (lane == 0) stage[nst] = SphBucket{ry0, rz0, pos + q, pos + q + m, nry, nrz, 0, 0};
+                            if (++nst == 32) flush();
+                        }
+                    }
+                    q += m;
+                }
+                if (lane == 0) q_s = q;
+            }
+            __syncthreads();
+            pos += q_s;
         }
+        if (wid == 0) flush();
     }
 }
 
@@ -675,7 +714,7 @@ __global__ __launch_bounds__(64 / NT, NT == 1 ? 7 : 8) void k_density_tile(
 int sph_launch_buckets(sph_ctx* c) {
     cudaStream_t s = c->stream;
     SPH_CUDA_CHECK(c, cudaMemsetAsync(c->bucket_cnt, 0, sizeof(unsigned), s));
-    k_buckets<<<c->sm_count * 2, 256, 0, s>>>(c->grid, c->cell_start, c->par.tile_rows, c->buckets,
+    k_buckets<<<c->sm_count * 4, BK_WARPS * 32, 0, s>>>(c->grid, c->cell_start, c->par.tile_rows, c->buckets,
                                               c->bucket_cnt);
     SPH_CUDA_CHECK(c, cudaGetLastError());
     return SPH_OK;
