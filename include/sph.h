@@ -76,13 +76,13 @@ typedef struct {
     float   cell_div_x;   /* cells per minimum search radius along x (<= 0: automatic: 8     */
                           /* when the staged-tile sweeps run, 4 otherwise)                   */
     float   cell_div_yz;  /* ... along y and z (<= 0: automatic: 2 with tiles (3 for n_ngb >  */
-                          /* 100), else 1.5, or 1 where max h > 3 min h)                     */
+                          /* 100), else 1.5, or 1 where max h > 3 min h)                      */
     int32_t entropy;      /* 1: entropy-conserving variant: sph_forces drops */
                           /* the Eq. (14) term, dudt is the viscous heating of Eq. (18)     */
                           /* alone; the caller advances u with sph_isentropic_u             */
     int32_t tile;         /* staged-tile sweeps (buckets of 64 targets over a shared-memory   */
                           /* tile of sources).  0 (default) = automatic: */
-                          /* on for n >= 2^19 particles unless max h > 3 min h at build time  */
+                          /* on for n >= 2^17 particles unless max h > 1.6 min h at build time */
                           /* (decided on the device); 1 = on whatever the size or h contrast; */
                           /* -1 = off: every target takes the 8-lanes-per-target kernels.     */
                           /* Results do not depend on it beyond rounding                      */

@@ -67,15 +67,16 @@ __global__ void k_reduce_h(int64_t n, const float* __restrict__ x, const float* 
 // steep_check: automatic tile mode -- a contrast of h above 3 sets SPH_GRID_STEEP and takes the
 // cell sides of the 8-lane kernels (divx_s, divyz_s) instead of the tile sweeps' (divx, divyz).
 __global__ void k_grid_setup(SphGrid* g, const unsigned* red, sph_box box, float slack, float divx,
-                             float divyz, float divx_s, float divyz_s, int steep_check,
+                             float divyz, float divx_s, float divyz_m, float divyz_s, int steep_check,
                              long long cap_cells) {
     float hmin = __uint_as_float(red[0]), hmax = __uint_as_float(red[1]);
     float xm = __uint_as_float(red[2]);
     int   flags = 0;
-    if (steep_check && hmax > 3.0f * hmin) {
+    if (steep_check && hmax > SPH_STEEP_RATIO * hmin) {
         flags |= SPH_GRID_STEEP;
         divx = divx_s;
-        divyz = divyz_s;
+        // the 8-lane kernels' cells; coarser rows only where h really spreads (measured on C5)
+        divyz = hmax > 3.0f * hmin ? divyz_s : divyz_m;
     }
     float lmax = fmaxf(box.len[0], fmaxf(box.len[1], box.len[2]));
     if (!(hmin < 3.0e38f) || !(hmin > 0.0f)) {  // no valid h at all: one coarse grid
@@ -292,7 +293,7 @@ int sph_launch_build(sph_ctx* c, int64_t n, const float* x, const float* y, cons
                                  // several hundred neighbours: finer rows keep a bucket of 64 compact
                                  uyz > 0.0f ? uyz : (tl ? (c->par.n_ngb > 100.0f ? 3.0f : 2.0f) : 1.5f),
                                  // steep h contrast: coarser rows (fewer near-empty rows around large-h targets)
-                                 ux > 0.0f ? ux : 4.0f, uyz > 0.0f ? uyz : 1.0f,
+                                 ux > 0.0f ? ux : 4.0f, uyz > 0.0f ? uyz : 1.5f, uyz > 0.0f ? uyz : 1.0f,
                                  (tl && c->par.tile == 0) ? 1 : 0, (long long)c->cap_cells);
     k_zero_cells<<<gs, TPB, 0, s>>>(c->grid, c->cell_cnt);
     k_bin<<<nb, TPB, 0, s>>>(n, c->grid, x, y, z, c->cell_cnt, c->key, c->rank);

@@ -23,7 +23,7 @@ struct SphGrid {
     float hmin, hmax;          // of the h given to sph_build_cells
     float xext;                // largest |coordinate| that enters a displacement
     int   flags;               // bit0: periodic side too short; bit1: cell table clipped; bit2: no valid h;
-                               // bit3: steep h contrast (max h > 3 min h): the staged-tile sweeps stand
+                               // bit3: steep h contrast (max h > 1.6 min h): the staged-tile sweeps stand
                                // back and every target takes the 8-lane kernels (set only in automatic mode)
     unsigned force_hmax_bits;  // max h given to sph_forces (float bits, atomicMax)
     int   cn[3];               // coarse grid (max-h map for the scatter reach of the force search)
@@ -98,8 +98,10 @@ struct sph_ctx {
 
 #define SPH_SCAN_BLOCKS 1024
 #define SPH_GRID_STEEP 8           // SphGrid.flags bit 3
-#define SPH_TILE_MIN_N (1 << 19)   // automatic mode: fewer particles than this cannot fill the GPU with
-                                   // one warp per bucket of 64 (148 SMs x 7 warps x a few buckets each)
+#define SPH_TILE_MIN_N (1 << 17)   // automatic mode: fewer particles than this cannot fill the GPU with
+                                   // one block per bucket of 64 (148 SMs x 7 blocks x a few buckets each);
+                                   // measured: the tile sweeps win from about 10^5 particles up
+#define SPH_STEEP_RATIO 1.6f       // automatic mode: max h beyond this x min h stands the tile sweeps down
 
 // The staged-tile sweeps are in use for this index: forced (tile > 0), or automatic (tile = 0) with
 // enough particles.  (In automatic mode the device may still stand them down: SPH_GRID_STEEP.)

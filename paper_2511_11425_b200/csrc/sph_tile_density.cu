@@ -41,6 +41,7 @@ __global__ __launch_bounds__(BK_WARPS * 32) void k_buckets(const SphGrid* __rest
     __shared__ SphBucket stage[32];
     __shared__ int       q_s;
     const SphGrid& g = *gp;
+    if (g.flags & SPH_GRID_STEEP) return;   // the tile sweeps stand down: nobody reads the table
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
     const int ngy = (g.ny + G - 1) / G, ngz = (g.nz + G - 1) / G;
     int nst = 0;   // warp 0: staged buckets (uniform); the table's counter is asked for 32 at a time

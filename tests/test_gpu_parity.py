@@ -456,10 +456,10 @@ def test_c5_impact_full_size_sampled(gu):
 
 
 def test_automatic_mode_picks_the_sweep_by_size_and_h_contrast(gu):
-    """sph_params.tile = 0: the staged-tile sweeps run when there are at least 2^19 particles and
-    max h <= 3 min h (decided on the device, SphGrid flag bit 3); results are within tolerance of
+    """sph_params.tile = 0: the staged-tile sweeps run when there are at least 2^17 particles and
+    max h <= 1.6 min h (decided on the device, SphGrid flag bit 3); results are within tolerance of
     the oracle either way (the other tests), here: which path ran."""
-    for nside, tiled in ((64, False), (96, True)):
+    for nside, tiled in ((40, False), (64, True)):
         w = workloads.sedov(nside=nside, h_start="warm")
         ctx, d, out, h = _full_step(gu, w, tile=0)
         st = ctx.stats()
@@ -468,6 +468,13 @@ def test_automatic_mode_picks_the_sweep_by_size_and_h_contrast(gu):
         assert (st["dens_tested"] > 500 * w["n"]) == tiled, (nside, st["dens_tested"] / w["n"])
         assert st["dens_nonconv"] == 0
         ctx.close()
+    # the Sod tube (246 924 particles, h twice as large on the thin side): the flag stands the tiles down
+    w = workloads.make("sod_tube", h_start="warm")
+    ctx, d, out, h = _full_step(gu, w, tile=0)
+    st = ctx.stats()
+    assert st["grid_flags"] & 8
+    assert st["dens_tested"] < 500 * w["n"] and st["dens_nonconv"] == 0
+    ctx.close()
 
 
 # ------------------------------------------------------------------------------------------
