@@ -134,8 +134,15 @@ class BlockSimulation(Simulation):
     One substep s, in the paper's order (Figure 2):
       1. density pass for all particles (with `fastgas`, on the substeps that do not start a
          step of rung 0: marking pass, then the density of the marked particles only,
-         PAPER.md:276)                                      sph_build_cells, sph_density_h
+         PAPER.md:276; with the interface correction a second marking pass from the marked
+         particles, and the density of the particles with either mark)
+                                                            sph_build_cells, sph_mark_neighbors,
+                                                            sph_density_h
       2. prediction of v, u of every particle to the time of the substep   sph_block_predict
+      3. interface correction (`interface_alpha`; Eqs. 8-12) from the predicted u:
+         the corrected density replaces rho in the force pass.  The pass runs over all particles
+         (the paper restricts it to the first mark; the values it needs -- of the active
+         particles' neighbours -- are the same)             sph_interface_correction
       4. forces of the particles whose step ends now        sph_block_active, sph_set_active,
                                                             sph_forces
          their new desired rungs (Eq. 27 + limiter)         sph_timestep, sph_rungs
@@ -147,8 +154,6 @@ class BlockSimulation(Simulation):
         """fastgas: 0 / False = off; a fraction in (0, 1] = use the marking pass on a substep when
         the share of particles on its active rungs (rung histogram read once per big step, a
         performance heuristic only: the results do not depend on it) is below it; True = 1."""
-        if params.get("interface_alpha") is not None:
-            raise NotImplementedError("the interface correction is wired into the global-step driver only")
         super().__init__(w, **params)
         if not 0 <= int(max_rung) <= 24:
             raise ValueError("max_rung must be in 0..24")
@@ -163,6 +168,7 @@ class BlockSimulation(Simulation):
         self.hk = torch.zeros(n, dtype=torch.float32, device="cuda")
         self.active = torch.empty(n, dtype=torch.uint8, device="cuda")
         self.mark = torch.empty(n, dtype=torch.uint8, device="cuda")
+        self.mark2 = torch.empty(n, dtype=torch.uint8, device="cuda") if self.interface_alpha is not None else None
         self.fastgas = float(fastgas)
         self.rung_share = None                  # share of particles on rungs >= r, per r
         self.s = 0                              # substep counter (host integer, plumbing)
@@ -187,7 +193,14 @@ class BlockSimulation(Simulation):
                 use_fastgas = bool(self.rung_share[fl] < self.fastgas)
         if use_fastgas:
             c.mark_neighbors(self.active, self.mark)          # index holds the last pass's h
-            c.set_active(self.mark)
+            if self.interface_alpha is not None:
+                # the corrected density of a marked particle needs the densities of ITS
+                # neighbours: second marking pass, density for either mark
+                c.mark_neighbors(self.mark, self.mark2)
+                torch.maximum(self.mark, self.mark2, out=self.mark2)
+                c.set_active(self.mark2)
+            else:
+                c.set_active(self.mark)
         c.density_h(d["m"], d["h"], o["rho"], o["omega"], o["n_ngb"])
         self.have_density = True
         if self.entropy:
@@ -201,8 +214,13 @@ class BlockSimulation(Simulation):
         p = self.pred
         c.block_predict(s, self.delta, self.tnext, self.hk, d["vx"], d["vy"], d["vz"], d["u"],
                         o["ax"], o["ay"], o["az"], o["dudt"], p["vx"], p["vy"], p["vz"], p["u"])
+        rho = o["rho"]
+        if self.interface_alpha is not None:      # step 3
+            c.interface_correction(d["m"], p["u"], o["rho"], d["h"], self.mat, self.interface_alpha,
+                                   self.imbalance, self.rho_corr)
+            rho = self.rho_corr
         c.set_active(self.active)
-        c.forces(d["m"], p["vx"], p["vy"], p["vz"], p["u"], o["rho"], d["h"], o["omega"], o["ax"],
+        c.forces(d["m"], p["vx"], p["vy"], p["vz"], p["u"], rho, d["h"], o["omega"], o["ax"],
                  o["ay"], o["az"], o["dudt"], o["mu_min"], o["P"], o["c"])
         c.timestep(d["h"], o["c"], o["ax"], o["ay"], o["az"], o["mu_min"], o["dt_i"], self.dt_new)
         c.rungs(o["dt_i"], self.dt0, self.max_rung, self.rung_des)

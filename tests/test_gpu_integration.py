@@ -486,3 +486,95 @@ def test_driver_with_the_interface_correction_pass(gu):
     w2["u"] = np.where(w["x"] < 0.5, 4.0, 1.0).astype(np.float32)
     r2, dv2 = check(run(w2, None), run(w2, 1.5))
     assert r2 > r1 and dv2 > dv1, (r1, r2, dv1, dv2)
+
+
+def _two_material_cube(v_sigma):
+    """Config 1 on 24^3 particles, two materials split at x = 0.5 (and at the periodic face), a
+    4:1 jump of u across it: the imbalance and the density correction are not small there."""
+    w = workloads.uniform_cube(nside=24, h_start="warm", v_sigma=v_sigma)
+    w["mat"] = (w["x"] >= 0.5).astype(np.int32)
+    w["u"] = np.where(w["x"] < 0.5, 4.0, 1.0).astype(np.float32)
+    return w
+
+
+def test_block_driver_with_the_interface_correction_on_one_rung_is_the_global_step_driver(gu):
+    """Step 3 inside the block-step driver: with max_rung = 0 it must reproduce the
+    global-step driver with the correction bit for bit (same passes in the same order), and the
+    correction must matter (the run without it differs near the material boundary)."""
+    from paper_2511_11425_b200.integrate import BlockSimulation, Simulation
+    w = _two_material_cube(0.05)
+    dt0 = 1.0e-3
+    a = Simulation(w, interface_alpha=1.5, tile=-1)
+    b = BlockSimulation(w, dt0=dt0, max_rung=0, interface_alpha=1.5, tile=-1)
+    plain = BlockSimulation(w, dt0=dt0, max_rung=0, tile=-1)
+    for _ in range(4):
+        a.step(dt_cap=dt0)
+        b.step()
+        plain.step()
+    assert float(a.out["dt_min"].item()) == float(np.float32(dt0))   # the cap was the step
+    for k in ("x", "y", "z", "vx", "vy", "vz", "u", "h"):
+        assert torch.equal(a.d[k], b.d[k]), k
+    assert torch.equal(a.rho_corr, b.rho_corr) and torch.equal(a.imbalance, b.imbalance)
+    near = torch.from_numpy(np.abs(w["x"] - 0.5) < 0.03).cuda()
+    dv = (b.d["vx"] - plain.d["vx"]).abs()
+    assert float(dv[near].max()) > 1e-4 * float(b.d["vx"].abs().max())
+    assert float((b.rho_corr / b.out["rho"] - 1).abs()[near].max()) > 1e-3
+
+
+def test_block_steps_with_the_interface_correction_do_not_depend_on_fastgas(gu):
+    """Mixed rungs with the interface correction: FastGas (first marking pass from the active
+    particles, second from the marked ones, density for either mark) must give the
+    flow of the run that updates every density on every substep -- the same rungs and step ends,
+    the state to rounding (the sweeps of a subset sum in the same order; a density that is not
+    refreshed belongs to a particle no active particle interacts with)."""
+    from paper_2511_11425_b200.integrate import BlockSimulation
+    w = _two_material_cube(0.3)
+    R, dt0 = 2, float(np.float32(0.008))
+    a = BlockSimulation(w, dt0=dt0, max_rung=R, interface_alpha=1.5)
+    b = BlockSimulation(w, dt0=dt0, max_rung=R, interface_alpha=1.5, fastgas=1.0)
+    seen = set()
+    for _ in range(2 * (1 << R)):
+        a.step()
+        b.step()
+        seen |= set(a.rung.cpu().numpy().tolist())
+        assert torch.equal(a.rung, b.rung) and torch.equal(a.tnext, b.tnext)
+    assert len(seen) >= 2, seen
+    a.synchronise()
+    b.synchronise()
+    for k in ("x", "y", "z"):
+        assert np.abs(_wrapdiff(gu.np64(a.d[k]), gu.np64(b.d[k]), 1.0, 1)).max() <= 1e-6
+    vscale = max(float(a.d[k].abs().max()) for k in ("vx", "vy", "vz"))
+    for k in ("vx", "vy", "vz"):
+        assert float((a.d[k] - b.d[k]).abs().max()) <= 2e-5 * vscale, k
+    assert float((a.d["u"] / b.d["u"] - 1).abs().max()) <= 2e-5
+
+
+def test_block_substep_with_the_interface_correction_against_the_oracle(gu):
+    """The first substep of the block driver with the correction, driven through the FP64 oracle:
+    density, prediction (no kick pending), imbalance (Eq. 8) and corrected density (Eqs. 9-12) from
+    the predicted u, forces with the corrected density, Eq. (26), Eq. (27) + limiter."""
+    from paper_2511_11425_b200.integrate import BlockSimulation
+    w = _two_material_cube(0.3)
+    _, op = gu.make_params(w)
+    _, ob = gu.make_boxes(w)
+    R, dt0, alpha = 2, float(np.float32(0.008)), 1.5
+    sim = BlockSimulation(w, dt0=dt0, max_rung=R, interface_alpha=alpha)
+    sim.step()
+    s = {k: w[k].astype(np.float64) for k in ("x", "y", "z", "m", "vx", "vy", "vz", "u", "h")}
+    h, rho, om, _ = orc.density(s["x"], s["y"], s["z"], s["m"], s["h"], ob, op, cells=True)
+    imb = orc.imbalance(s["x"], s["y"], s["z"], s["m"], h, w["mat"], ob, op, alpha)
+    rho_c = orc.interface_correction(s["x"], s["y"], s["z"], h, s["u"], rho, imb, ob, op)
+    rho_c = rho_c[0] if isinstance(rho_c, tuple) else rho_c
+    assert np.abs(gu.np64(sim.imbalance) - imb).max() <= 1e-4 * max(imb.max(), 1.0)
+    assert np.abs(gu.np64(sim.rho_corr) / rho_c - 1).max() <= 2e-5
+    o = orc.forces(s["x"], s["y"], s["z"], s["m"], s["vx"], s["vy"], s["vz"], s["u"], rho_c, h, om, ob, op)
+    ea, eu = gu.force_errors(sim.out.t, o)
+    assert ea.max() <= 1e-4 and eu.max() <= 1e-4, (ea.max(), eu.max())
+    _, c = orc.eos(rho_c, s["u"], op.gamma)
+    dt_i, _ = orc.timestep(h, c, o["ax"], o["ay"], o["az"], o["mu_min"], op)
+    des = orc.rung_limiter(s["x"], s["y"], s["z"], h, orc.rungs(dt_i, dt0, R), ob)
+    got = sim.rung.cpu().numpy()
+    # a dt_i within rounding of a rung boundary may fall either way; the rest must agree
+    edge = np.abs(np.log2(dt0 / dt_i) - np.round(np.log2(dt0 / dt_i))) < 1e-4
+    assert np.array_equal(got[~edge], des[~edge]) and edge.mean() < 0.01
+    assert len(set(des.tolist())) >= 2
