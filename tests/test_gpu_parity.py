@@ -506,6 +506,34 @@ def test_c1_other_kernels_and_neighbour_numbers(gu, kernel, n_ngb, tile):
         assert st["force_tested"] <= 0.25 * st["dens_tested"], st
 
 
+def test_c6_400_on_the_bench_configuration_sampled(gu):
+    """The paper's Wendland C6 with 400 neighbours in the configuration bench.py
+    times it on (`--kernel wendland_c6 --n-ngb 400 --nside 96`: 884 736 particles with random
+    velocities here, automatic sweep choice = staged tiles, lists and tiles sized from n_ngb):
+    1024 seeded targets against the brute-force oracle over all particles, the pair counts of
+    every particle against the cell-list oracle, and the force sweep served from the kept lists."""
+    w = workloads.sedov(nside=96, h_start="warm", v_sigma=0.05)
+    scale = np.float32((400.0 / 64.0) ** (1.0 / 3.0))
+    w["h"] = (w["h"] * scale).astype(np.float32)
+    _, op = gu.make_params(w, kernel=3, n_ngb=400.0)
+    _, ob = gu.make_boxes(w)
+    ctx, d, out, h = _full_step(gu, w, kernel=3, n_ngb=400.0, tile=0)
+    st = ctx.stats()
+    assert st["dens_nonconv"] == 0 and st["grid_flags"] & 8 == 0
+    assert st["dens_tested"] > 1500 * w["n"]                 # the tile sweep ran (about 2300 candidates per target)
+    assert st["dens_overflow"] <= 0.05 * w["n"], st          # few targets left to the list-free kernels
+    assert st["force_tested"] <= 0.05 * st["dens_tested"]    # the force sweep searched for few targets only
+    sel = _sample(w["n"], 1024, 97)
+    _check_sample(gu, w, ctx, out, h, sel, op, ob)
+    hg = h.cpu().numpy()
+    _, _, onn, _ = orc.density_at_h(w["x"], w["y"], w["z"], w["m"], hg, ob, op, targets=sel)
+    assert 390 <= onn.mean() <= 520
+    assert int(out["n_ngb"].sum().item()) == st["dens_pairs"]
+    m = w["m"].astype(np.float64)
+    a = np.stack([gu.np64(out[k]) for k in ("ax", "ay", "az")])
+    assert np.abs((m * a).sum(axis=1)).max() <= 1e-5 * (m * np.linalg.norm(a, axis=0)).sum()
+
+
 # ------------------------------------------------------------------------------------------
 # Interface correction, PAPER.md:158-182, Eqs. (8)-(12)
 # ------------------------------------------------------------------------------------------
