@@ -96,9 +96,11 @@ typedef struct {
     int32_t tile_warps;   /* warps per bucket of the density sweep: 2 (default, <= 0) = one   */
                           /* target per thread; 1 = one warp, two targets per lane            */
     int32_t tile_forces;  /* 0 (default): the force sweep reads the bucket-major neighbour    */
-                          /* lists the tile density sweep kept (one warp per bucket); 1: the  */
-                          /* force sweep runs on staged tiles too (measured slower, DESIGN.md */
-                          /* section 7)                                                       */
+                          /* lists the tile density sweep kept and gathers the source records */
+                          /* from global memory (one warp per bucket); 2: the same lists as   */
+                          /* tile indices, the bucket's records staged in shared memory; 1:   */
+                          /* no lists, the force sweep runs on staged tiles with its own      */
+                          /* accept masks (1 and 2 measured slower)      */
     int32_t tile_fcap;    /* tile_cap and tile_warps of the force sweep (<= 0: defaults 576   */
     int32_t tile_fwarps;  /* and 1); its tile holds 52 B per candidate, the density tile 20   */
 } sph_params;

@@ -16,7 +16,7 @@ _CSRC = os.path.join(_HERE, "csrc")
 _OBJ = os.path.join(_HERE, "build")
 LIB = os.path.join(_HERE, "libsph_b200.so")
 SOURCES = ["sph_api.cu", "sph_build.cu", "sph_density.cu", "sph_forces.cu", "sph_misc.cu",
-           "sph_integrate.cu", "sph_interface.cu", "sph_rungs.cu", "sph_active.cu", "sph_tile_density.cu", "sph_tile_forces.cu", "sph_forces_list.cu", "sph_static.cu"]
+           "sph_integrate.cu", "sph_interface.cu", "sph_rungs.cu", "sph_active.cu", "sph_tile_density.cu", "sph_tile_forces.cu", "sph_forces_list.cu", "sph_forces_tlist.cu", "sph_static.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-ftz=true",
               "--expt-extended-lambda", "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 

@@ -111,6 +111,7 @@ extern "C" int sph_create(sph_ctx** out, const sph_params* params, const sph_box
     ok = ok && dalloc(&c->big_list, (size_t)n_max) == cudaSuccess;
     ok = ok && dalloc(&c->big_cnt, (size_t)2) == cudaSuccess;
     ok = ok && dalloc(&c->list_next, (size_t)1) == cudaSuccess;
+    ok = ok && dalloc(&c->bucket_rt, (size_t)n_max) == cudaSuccess;
     ok = ok && dalloc(&c->bucket_loff, (size_t)n_max) == cudaSuccess;
     ok = ok && dalloc(&c->tl_rkeep, (size_t)n_max) == cudaSuccess;
     ok = ok && dalloc(&c->fb_list, (size_t)n_max) == cudaSuccess;
@@ -144,7 +145,7 @@ extern "C" void sph_destroy(sph_ctx* c) {
     cudaFree(c->buckets);   cudaFree(c->bucket_cnt); cudaFree(c->tile_next);
     cudaFree(c->fb_list);   cudaFree(c->fb_cnt);
     cudaFree(c->big_list);  cudaFree(c->big_cnt);
-    cudaFree(c->list_next); cudaFree(c->bucket_loff); cudaFree(c->tl_rkeep);
+    cudaFree(c->list_next); cudaFree(c->bucket_loff); cudaFree(c->tl_rkeep); cudaFree(c->bucket_rt);
     delete c;
 }
 

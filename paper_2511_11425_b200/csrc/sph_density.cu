@@ -432,7 +432,7 @@ int sph_launch_density(sph_ctx* c, const float* m, float* h, float* rho, float* 
         k_density<KERN><<<nblk, D_TPB, 0, s>>>((int)n, c->grid, c->cell_start, c->pos_m, c->perm, par,
                                                h, rho, omega, nn, c->fix_list, c->fix_cnt, c->nb_j,
                                                c->nb_cnt, c->nb_rkeep, tlist, tcnt,
-                                               (tiled && !c->par.tile_forces) ? 0 : 1, tiled ? 1 : 0, c->stats);
+                                               (tiled && c->par.tile_forces != 1) ? 0 : 1, tiled ? 1 : 0, c->stats);
         k_density_fix<KERN><<<c->sm_count * 4, 256, 0, s>>>(c->grid, c->cell_start, c->pos_m, c->perm,
                                                             par, c->fix_list, c->fix_cnt, h, rho,
                                                             omega, nn, c->stats);

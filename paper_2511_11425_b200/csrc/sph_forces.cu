@@ -378,7 +378,8 @@ int sph_launch_forces(sph_ctx* c, const float* m, const float* vx, const float* 
     // staged tiles; what is handed back goes through the 8-lane kernel's target list
     const bool tiled = sph_tile_on(c) && !c->act_on;
     if (tiled) {
-        const int rc = c->par.tile_forces > 0 ? sph_launch_forces_tile(c, ax, ay, az, dudt, mu_min)
+        const int rc = c->par.tile_forces == 2 ? sph_launch_forces_tlist(c, ax, ay, az, dudt, mu_min)
+                     : c->par.tile_forces > 0 ? sph_launch_forces_tile(c, ax, ay, az, dudt, mu_min)
                                               : sph_launch_forces_list(c, ax, ay, az, dudt, mu_min);
         if (rc != SPH_OK) return rc;
     }

@@ -84,6 +84,7 @@ struct sph_ctx {
     unsigned*    big_list;     // n_max: buckets the first pass of a tile sweep left to the second (larger tile)
     unsigned*    big_cnt;      // [2]: their number (density, forces)
     unsigned*    list_next;    // [1]: next free region of nb_j (bucket-major lists of the tile sweep)
+    float*       bucket_rt;    // n_max: radius of the tile a bucket's lists index (tile_forces = 2), 0: none
     int          lcap;         // entries per target of a bucket-major list region (from n_ngb, sph_create)
     size_t       nb_words;     // words in nb_j
     uint32_t*    bucket_loff;  // n_max: list region of a bucket (0xffffffff: none)
@@ -729,6 +730,7 @@ int sph_launch_coarse_map(sph_ctx* c);
 int sph_launch_buckets(sph_ctx* c);
 int sph_launch_density_tile(sph_ctx* c, float* h, float* rho, float* omega, int32_t* nn);
 int sph_launch_forces_tile(sph_ctx* c, float* ax, float* ay, float* az, float* dudt, float* mu_min);
+int sph_launch_forces_tlist(sph_ctx* c, float* ax, float* ay, float* az, float* dudt, float* mu_min);
 int sph_launch_forces_list(sph_ctx* c, float* ax, float* ay, float* az, float* dudt, float* mu_min);
 int sph_launch_mark(sph_ctx* c, const uint8_t* src, uint8_t* mark);
 int sph_launch_set_active(sph_ctx* c, const uint8_t* active);

@@ -527,6 +527,69 @@ __device__ __forceinline__ void sph_tile_walk(const SphTileMem& sm, const SphTil
     }
 }
 
+// a6 for a box (the bound of sph_scatter_hmax, for the bucket's bounding box): the largest h_j
+// of any particle that can reach a point of [b0, b1].  Warp-collective.
+__device__ __forceinline__ float sph_box_scatter_hmax(const SphGrid& g, const unsigned* __restrict__ coarse,
+                                                   const float b0[3], const float b1[3], float hown,
+                                                   float hglobal, int lane) {
+    float H = fmaxf(hglobal, hown);
+#pragma unroll 1
+    for (int pass = 0; pass < 3; ++pass) {
+        int  u0[3], nn[3];
+        bool inside = true;
+        const float R = 2.0f * H * (1.0f + 1e-5f);
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+            float a = floorf((b0[d] - g.lo[d] - R) * g.ics[d] - 1e-3f);
+            float b = floorf((b1[d] - g.lo[d] + R) * g.ics[d] + 1e-3f);
+            a = fminf(fmaxf(a, -1.0e9f), 1.0e9f);
+            b = fminf(fmaxf(b, -1.0e9f), 1.0e9f);
+            int lo = (int)a, hi = (int)b;
+            if (g.per[d]) {
+                inside = inside && lo >= 0 && hi <= g.cn[d] - 1;
+                if (hi - lo + 1 >= g.cn[d]) { lo = 0; hi = g.cn[d] - 1; }
+            } else {
+                lo = min(max(lo, 0), g.cn[d] - 1);
+                hi = min(max(hi, 0), g.cn[d] - 1);
+            }
+            u0[d] = lo;
+            nn[d] = hi - lo + 1;
+        }
+        const bool blocks = inside && nn[0] * nn[1] * nn[2] > 512;
+        int dx = g.cn[0], dy = g.cn[1], dz = g.cn[2];
+        const unsigned* map = coarse;
+        if (blocks) {
+#pragma unroll
+            for (int d = 0; d < 3; ++d) {
+                const int q0 = u0[d] >> 3, q1 = (u0[d] + nn[d] - 1) >> 3;
+                u0[d] = q0;
+                nn[d] = q1 - q0 + 1;
+            }
+            dx = g.sn[0]; dy = g.sn[1]; dz = g.sn[2];
+            map = coarse + SPH_COARSE_MAX;
+        }
+        const int cnt = nn[0] * nn[1] * nn[2];
+        unsigned  best = 0u;
+        for (int q = lane; q < cnt; q += 32) {
+            const int t  = q / nn[0], ix = q - t * nn[0];
+            const int iz = t / nn[1], iy = t - iz * nn[1];
+            int cx = u0[0] + ix, cy = u0[1] + iy, cz = u0[2] + iz;
+            cx -= (cx >= dx) ? dx : 0; cx += (cx < 0) ? dx : 0;
+            cy -= (cy >= dy) ? dy : 0; cy += (cy < 0) ? dy : 0;
+            cz -= (cz >= dz) ? dz : 0; cz += (cz < 0) ? dz : 0;
+            cx = min(max(cx, 0), dx - 1);
+            cy = min(max(cy, 0), dy - 1);
+            cz = min(max(cz, 0), dz - 1);
+            best = max(best, __ldg(map + (cz * dy + cy) * dx + cx));
+        }
+        best = __reduce_max_sync(SPH_FULL, best);
+        const float Hn = fmaxf(hown, fminf(H, __uint_as_float(best)));
+        if (Hn >= H * (1.0f - 1e-6f)) { H = Hn; break; }
+        H = Hn;
+    }
+    return H;
+}
+
 // ---- one thread per target (or two): the forms used when NW = 2 / NT warps share a bucket,
 // each thread owning NT targets: columns tid + 32 t, t < NT, of the mask words --------------
 

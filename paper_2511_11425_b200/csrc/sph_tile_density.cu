@@ -118,6 +118,8 @@ __global__ __launch_bounds__(BK_WARPS * 32) void k_buckets(const SphGrid* __rest
 struct TilePar {
     float n_ngb, tol, slack;
     int   max_iter, tcap, lcap;
+    int   lmode;   // what a kept-list entry is: 0 the sorted position of the source, 1 its index in the
+                   // bucket's tile (the force sweep stages the same tile again: sph_forces_tlist.cu)
 };
 
 // One safeguarded Halley step from the sums at h (the step of sph_density.cu: same formulas,
@@ -218,7 +220,7 @@ __global__ __launch_bounds__(64 / NT, NT == 1 ? 7 : 8) void k_density_tile(
     TilePar par, float* h_io, float* rho, float* omega, int32_t* nn, int32_t* fix_list,
     unsigned* fix_cnt, uint32_t* fb_list, unsigned* fb_cnt, uint32_t* nb_j, unsigned nb_regions,
     unsigned* list_next, uint32_t* bucket_loff, uint32_t* nb_cnt, float* nb_rkeep, float* tl_rkeep,
-    unsigned long long* stats) {
+    float* bucket_rt, unsigned long long* stats) {
     constexpr bool MOM = (KERN == 1);   // the moment solve exists for Wendland C2
     constexpr int  NW = 2 / NT, NTHR = 32 * NW;
     constexpr int  NSET = SPH_DT_NSET > 0 ? SPH_DT_NSET : (NT == 1 ? 3 : 2);   // entries in flight per target in the sweep
@@ -393,6 +395,8 @@ __global__ __launch_bounds__(64 / NT, NT == 1 ? 7 : 8) void k_density_tile(
         }
         bool fallback = false;
         uint32_t* lbase = nullptr;
+        int   ntiles = 0;        // tiles staged for this bucket (uniform)
+        float rt_used = 0.0f;    // radius of the last one
 
         // ---- stages: (re)build the tile for the largest list radius wanted
         for (int stage = 0; stage < 4 && Rt > 0.0f; ++stage) {
@@ -416,6 +420,8 @@ __global__ __launch_bounds__(64 / NT, NT == 1 ? 7 : 8) void k_density_tile(
 #pragma unroll
                 for (int t = 0; t < NT; ++t) c_recollect += wait[t] ? 1u : 0u;
             }
+            ++ntiles;
+            rt_used = Rt;
 #pragma unroll
             for (int t = 0; t < NT; ++t) mvalid[t] = false;   // a new tile: the masks of the old one are gone
             sph_tile_finish(g, sm, ti, parity, tid, NTHR, 0.0f);
@@ -493,7 +499,7 @@ __global__ __launch_bounds__(64 / NT, NT == 1 ? 7 : 8) void k_density_tile(
                         M[t][4] = fmaf(a4, tt, M[t][4]);
                         M[t][5] += a5;
                         {   // the kept list (a set: any sweep of this mask writes the same); predicated store
-                            const uint32_t gj = sph_ldsu(sm.gidx_sa + 4u * (uint32_t)en.idx);
+                            const uint32_t gj = par.lmode ? (uint32_t)en.idx : sph_ldsu(sm.gidx_sa + 4u * (uint32_t)en.idx);
                             const bool st = en.has && nent[t] < lcap;
                             uint32_t* const la = lcol[t] + (uint32_t)nent[t] * (uint32_t)SPH_TB;
                             asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %2, 0;\n\t@p st.global.u32 [%0], %1;\n\t}"
@@ -599,7 +605,7 @@ __global__ __launch_bounds__(64 / NT, NT == 1 ? 7 : 8) void k_density_tile(
                         e[t]  = fmaf(mj, eq, e[t]);
                         f2[t] = fmaf(mj, fq, f2[t]);
                         {
-                            const uint32_t gj = sph_ldsu(sm.gidx_sa + 4u * (uint32_t)en.idx);
+                            const uint32_t gj = par.lmode ? (uint32_t)en.idx : sph_ldsu(sm.gidx_sa + 4u * (uint32_t)en.idx);
                             const bool st = has && nent[t] < lcap;
                             uint32_t* const la = lcol[t] + (uint32_t)nent[t] * (uint32_t)SPH_TB;
                             asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %2, 0;\n\t@p st.global.u32 [%0], %1;\n\t}"
@@ -672,6 +678,7 @@ __global__ __launch_bounds__(64 / NT, NT == 1 ? 7 : 8) void k_density_tile(
             }
             continue;
         }
+        if (par.lmode && tid == 0) bucket_rt[bi] = (lbase != nullptr && ntiles == 1) ? rt_used : 0.0f;
 #pragma unroll
         for (int t = 0; t < NT; ++t) {
             if (!valid[t]) continue;
@@ -679,7 +686,9 @@ __global__ __launch_bounds__(64 / NT, NT == 1 ? 7 : 8) void k_density_tile(
             const int i = ic[t];
             h_io[i] = h[t];
             // the list is complete inside the radius of its mask (less the rounding margin of phase 1)
-            const bool lok = lbase != nullptr && !fix[t] && mvalid[t] && nlist[t] <= par.lcap;
+            // (tile indices, lmode 1, mean something only if the bucket had one tile)
+            const bool lok = lbase != nullptr && !fix[t] && mvalid[t] && nlist[t] <= par.lcap &&
+                             (!par.lmode || ntiles == 1);
             nb_rkeep[p[t]] = 0.0f;     // no [target][entry] list of the 8-lane kernels for this target
             tl_rkeep[p[t]] = lok ? Rc[t] * (1.0f - 1e-4f) : 0.0f;
             nb_cnt[p[t]]   = lok ? (uint32_t)nlist[t] : 0u;
@@ -739,7 +748,8 @@ int sph_launch_density_tile(sph_ctx* c, float* h, float* rho, float* omega, int3
             const int  tcap = pass == 0 ? c->par.tile_cap : c->par.tile_cap2;
             const bool two  = c->par.tile_cap2 >= c->par.tile_cap + 32;
             if (pass == 1 && !two) break;
-            TilePar par{c->par.n_ngb, c->par.h_tol, c->par.search_slack, c->par.h_max_iter, tcap, c->lcap};
+            TilePar par{c->par.n_ngb, c->par.h_tol, c->par.search_slack, c->par.h_max_iter, tcap, c->lcap,
+                        c->par.tile_forces == 2 ? 1 : 0};
             const size_t smem = sph_tile_smem_bytes(tcap, 16, sph_tile_xbytes(1, 0), 2 / NT);
             cudaError_t e = cudaFuncSetAttribute(k_density_tile<KERN, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
             if (e != cudaSuccess) return e;
@@ -753,9 +763,9 @@ int sph_launch_density_tile(sph_ctx* c, float* h, float* rho, float* omega, int3
                 pass == 0 ? c->bucket_cnt : c->big_cnt, pass == 0 ? nullptr : c->big_list,
                 last ? nullptr : c->big_list, c->big_cnt, c->tile_next + pass, par, h, rho, omega, nn,
                 c->fix_list, c->fix_cnt, c->fb_list, c->fb_cnt,
-                c->par.tile_forces ? nullptr : c->nb_j,
+                c->par.tile_forces == 1 ? nullptr : c->nb_j,
                 (unsigned)(c->nb_words / ((size_t)c->lcap * SPH_TB)), c->list_next,
-                c->bucket_loff, c->nb_cnt, c->nb_rkeep, c->tl_rkeep, c->stats);
+                c->bucket_loff, c->nb_cnt, c->nb_rkeep, c->tl_rkeep, c->bucket_rt, c->stats);
             e = cudaGetLastError();
             if (e != cudaSuccess) return e;
         }

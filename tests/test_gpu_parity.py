@@ -325,15 +325,17 @@ def test_c3v_sedov_with_random_velocities_full_size(gu):
 
 
 def test_force_sweep_results_do_not_depend_on_the_list_path(gu):
-    """The three force sweeps -- from the density sweep's kept lists (default), on staged tiles
-    (tile_forces = 1), 8 lanes per target with their own search (tile = -1) -- agree to rounding
+    """The four force sweeps -- from the density sweep's kept lists with the records gathered
+    from global memory (tile_forces = 0) or from the bucket's tile staged in shared memory
+    (tile_forces = 2), on staged tiles with their own accept masks (tile_forces = 1), 8 lanes
+    per target with their own search (tile = -1) -- agree to rounding
     on a configuration with a 2:1 jump of h (the lists of the targets next to the jump do not
     cover their reach, so the hand-over to the searching kernel is exercised)."""
     w = workloads.sod_tube(ncross=24, h_start="warm")
     _, op = gu.make_params(w)
     _, ob = gu.make_boxes(w)
     res = []
-    for kw in (dict(), dict(tile_forces=1), dict(tile=-1)):
+    for kw in (dict(tile_forces=0), dict(tile_forces=2), dict(tile_forces=1), dict(tile=-1)):
         ctx, d, out, h = _full_step(gu, w, **kw)
         st = ctx.stats()
         _check_all_vs_cell_list(gu, w, out, h, op, ob, st)      # each of them against the oracle
