@@ -368,3 +368,38 @@ def step(ctx: Sph, w: dict, out: StepBuffers, h: torch.Tensor):
                out["ax"], out["ay"], out["az"], out["dudt"], out["mu_min"], out["P"], out["c"])
     ctx.timestep(h, out["c"], out["ax"], out["ay"], out["az"], out["mu_min"], out["dt_i"],
                  out["dt_min"])
+
+
+class StepGraph:
+    """The whole hot path -- build_cells -> density_h -> forces -> timestep, about 26 kernel
+    launches and a dozen memsets -- captured once in a CUDA graph and replayed with one launch:
+    for problems so small that the launches, not the kernels, set the time of a step (config 1:
+    4096 particles).  The context must live on a stream of its own (not the default stream):
+
+        s = torch.cuda.Stream(); ctx = Sph(params, box, n, stream=s)
+        g = StepGraph(ctx, w, out, h); g.replay()
+
+    The graph holds the addresses of the tensors it was captured with: `w`, `out` and `h` must stay
+    alive and are read / written in place by every replay (h: in the guess, out the solution).
+    replay() enqueues on torch's current stream.  Argument marshalling only, like step()."""
+
+    def __init__(self, ctx: Sph, w: dict, out: StepBuffers, h: torch.Tensor, warmup: int = 2):
+        if ctx.stream.cuda_stream == torch.cuda.default_stream().cuda_stream:
+            raise SphError(SPH_EINVAL, "StepGraph: create the context on a non-default stream")
+        self.ctx, self.w, self.out, self.h = ctx, w, out, h
+        cur = torch.cuda.current_stream()
+        ctx.stream.wait_stream(cur)
+        with torch.cuda.stream(ctx.stream):
+            h0 = h.clone()
+            for _ in range(max(int(warmup), 1)):      # module loading, function attributes
+                h.copy_(h0)
+                step(ctx, w, out, h)
+            h.copy_(h0)
+        ctx.stream.synchronize()
+        self.graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(self.graph, stream=ctx.stream):
+            step(ctx, w, out, h)
+        h.copy_(h0)                                    # the capture itself runs nothing
+
+    def replay(self):
+        self.graph.replay()
